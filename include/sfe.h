@@ -1,0 +1,164 @@
+/*
+ * sfe.h -- C ABI of libsfe: B200 (sm_100a) speculative Y-drop gapped extension.
+ *
+ * The hot path of arxiv/paper_2606_06811: the gapped-extension (Y-drop) phase of a LASTZ-style
+ * seed-filter-extend pipeline run as speculative batches (Algorithm 3), then
+ * resolved so that exactly the alignments of the serial in-order loop (PAPER.md:41-72,
+ * Algorithm 1) are kept.  The paper names the operations only; the exact recurrence, threshold
+ * and tie-break rules are the readings R1..R29 of SURVEY.md 8(c), restated in DESIGN.md.
+ *
+ * Conventions
+ *  - Every function returns int: SFE_OK (0) or a negative SFE_E* code.  No exceptions, no exit(),
+ *    nothing printed.
+ *  - Pointers named *_dev are DEVICE pointers owned by the caller; *_host are HOST pointers.
+ *    Inputs are read-only and must not alias outputs.  The ctx owns only scratch.
+ *  - All device work is enqueued on the ctx's CUDA stream.  sfe_pack and sfe_resolve do not
+ *    synchronise; sfe_ydrop_batch synchronises the stream once before returning when
+ *    SFE_WANT_CIGAR is set (it must read the traceback-overflow counter), otherwise not.
+ *  - Coordinates are 0-based corner positions (between bases), int64.  For strand -1 the query
+ *    coordinate refers to the reverse-complemented query (R15).
+ *  - There is no CPU fallback anywhere in this library.
+ */
+#ifndef SFE_H
+#define SFE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    SFE_OK = 0,
+    SFE_EINVAL = -1,   /* bad argument (NULL, negative size, unsupported prune_lag, ...)        */
+    SFE_ENOMEM = -2,   /* device or host allocation failed                                      */
+    SFE_ECUDA = -3,    /* a CUDA runtime call or kernel launch failed                           */
+    SFE_ELIMIT = -4    /* value outside the supported range (see sfe_scoring)                   */
+};
+
+#define SFE_YDROP_INF 0x7fffffff      /* R27: no pruning                                        */
+#define SFE_PRUNE_LAG 32              /* R4: the row lag the systolic kernel implements exactly  */
+
+/* flags of sfe_ydrop_batch */
+#define SFE_WANT_CIGAR 1u             /* spill traceback pointers to HBM and emit CIGARs         */
+#define SFE_SCORE_ONLY 0u             /* scores, boxes and cell counts only                      */
+#define SFE_NO_BINNING 2u             /* tickets in anchor order (default: longest-first bins)   */
+
+/* per-anchor status bits (sfe_result.status) */
+#define SFE_ST_TB_OVERFLOW 1u         /* traceback arena exhausted even when run alone: no CIGAR */
+#define SFE_ST_CIGAR_OVERFLOW 2u      /* cigar pool too small: ops not written (n_ops is valid)   */
+#define SFE_ST_WIDE 4u                /* a half took the wide-band (global-memory ring) path     */
+#define SFE_ST_SCORE_LIMIT 8u         /* R25: |score| would exceed 2^29                           */
+#define SFE_ST_BAD_ANCHOR 16u         /* anchor outside its pair's limits: nothing computed      */
+
+/* CIGAR op word: (length << 4) | code ; M = aligned pair, I = query base vs gap, D = target base
+ * vs gap (R12). */
+#define SFE_OP_M 0u
+#define SFE_OP_I 1u
+#define SFE_OP_D 2u
+
+typedef struct sfe_ctx sfe_ctx;       /* opaque: stream, scratch arenas, queue counters          */
+
+/* Scoring (R1, R2, R5, R13, R16).  Supported range: every sub[][] entry and n_score in
+ * [-128, 127] (the kernel keeps a query row's scores as packed int8), gap_open >= 0,
+ * gap_extend >= 1, gap_open + gap_extend <= 65535, 0 <= ydrop < 2^28 or SFE_YDROP_INF,
+ * prune_lag == SFE_PRUNE_LAG; anything else is SFE_ELIMIT / SFE_EINVAL. */
+typedef struct {
+    int32_t sub[4][4];                /* [query base][target base], A,C,G,T                      */
+    int32_t n_score;                  /* any pair involving N                                    */
+    int32_t gap_open, gap_extend;     /* a gap of length k costs gap_open + k * gap_extend       */
+    int32_t ydrop;
+    int32_t prune_lag;                /* Lambda of R4                                            */
+    int32_t min_score;                /* tau; used by sfe_resolve             */
+} sfe_scoring;
+
+typedef struct { int64_t tpos, qpos; int32_t pair; int32_t strand; /* +1 / -1 */ } sfe_anchor;
+
+/* extension limits: [t_begin, t_end) x [q_begin, q_end) in the FORWARD query frame; for a
+ * strand -1 anchor the query interval is mirrored into the reverse-complement frame. */
+typedef struct { int64_t t_begin, t_end, q_begin, q_end; } sfe_pair;
+
+typedef struct {
+    int32_t score, score_fwd, score_bwd;
+    uint32_t status;
+    int64_t tstart, tend, qstart, qend;   /* bounding box, corner coordinates, strand frame      */
+    int64_t cigar_off;                    /* index of the first op in the cigar pool, -1 if none  */
+    int32_t n_ops, n_ops_back;            /* ops = backward half (n_ops_back), then forward half  */
+    uint64_t cells;                       /* R28: cells inside the live column bounds, both halves */
+} sfe_result;
+
+typedef struct { int64_t tstart, tend, qstart, qend; int32_t strand; int32_t reserved; } sfe_box;
+
+/* counters accumulated by sfe_resolve (R29) */
+typedef struct sfe_stats {
+    int64_t n_anchors, n_kept, n_covered, n_below;
+    uint64_t cells_total, cells_covered;  /* cells of all anchors / of covered ones (shadow work) */
+} sfe_stats;
+
+/* Create a context on `device` that enqueues on `cuda_stream` (a cudaStream_t, may be NULL for
+ * the default stream).  scratch_bytes sizes the traceback arena (HBM); 0 selects 1 GiB. */
+int sfe_create(sfe_ctx **ctx, int device, void *cuda_stream, size_t scratch_bytes);
+int sfe_destroy(sfe_ctx *ctx);
+const char *sfe_strerror(int code);
+/* file:line and CUDA runtime message of the most recent SFE_ECUDA (process-wide, for diagnosis) */
+const char *sfe_last_error_detail(void);
+
+/* a1 Pack (R13, R14): ASCII (device) -> 2-bit code plane (base k in byte k/4, bits 2(k%4)..; A0 C1
+ * G2 T3, N stored as 0) and 1-bit N-mask plane (base k in byte k/8, bit k%8).  If rc_codes2_dev
+ * is non-NULL also the reverse-complement planes (3 - code, reversed order).  Output buffers
+ * hold (len+3)/4 and (len+7)/8 bytes, rounded up to a multiple of 16 bytes. */
+int sfe_pack(sfe_ctx *ctx, const char *ascii_dev, int64_t len, uint8_t *codes2_dev, uint8_t *nmask_dev,
+             uint8_t *rc_codes2_dev, uint8_t *rc_nmask_dev);
+
+/* a2-a8 Speculative batch of two-sided Y-drop extensions (Alg. 3 phase 2;
+ * one-sided rules: SURVEY 8(c), R1..R12).  For each anchor: one forward and one backward
+ * affine-gap extension on one warp each, joined at the anchor.  results_dev[n_anchors] is
+ * always written.  With SFE_WANT_CIGAR the ops of anchor i are written to
+ * cigar_pool_dev[cigar_off .. cigar_off + n_ops) (anchor order, deterministic offsets) and
+ * *cigar_pool_used_dev receives the total; anchors whose ops do not fit get
+ * SFE_ST_CIGAR_OVERFLOW.  qrc_* may be NULL if no anchor has strand -1. */
+int sfe_ydrop_batch(sfe_ctx *ctx, const uint8_t *t_codes2_dev, const uint8_t *t_nmask_dev, int64_t t_len,
+                    const uint8_t *q_codes2_dev, const uint8_t *q_nmask_dev,
+                    const uint8_t *qrc_codes2_dev, const uint8_t *qrc_nmask_dev, int64_t q_len,
+                    const sfe_pair *pairs_dev, int32_t n_pairs,
+                    const sfe_anchor *anchors_dev, int64_t n_anchors,
+                    const sfe_scoring *scoring_host, uint32_t flags,
+                    sfe_result *results_dev,
+                    uint32_t *cigar_pool_dev, int64_t cigar_pool_cap, int64_t *cigar_pool_used_dev);
+
+/* a9 Resolve (Alg. 3 phase 3; R17, R18, R26): in anchor order,
+ *   covered(i) = exists accepted box of the same strand containing (tpos_i, qpos_i),
+ *   kept(i)    = !covered(i) && score_i >= min_score  -> its box is appended to accepted.
+ * keep_dev[i] = 0 covered, 1 kept, 2 below min_score.  accepted_dev / *n_accepted_dev carry the
+ * boxes kept in earlier windows in and the extended list out.  With results_dev == NULL this
+ * is the phase-1 "is masked" filter: keep_dev[i] = 0 covered, 1 not covered,
+ * nothing appended.  stats_dev (may be NULL) is accumulated, not reset. */
+int sfe_resolve(sfe_ctx *ctx, const sfe_anchor *anchors_dev, const sfe_result *results_dev, int64_t n,
+                int32_t min_score, sfe_box *accepted_dev, int64_t accepted_cap, int64_t *n_accepted_dev,
+                uint8_t *keep_dev, sfe_stats *stats_dev);
+
+/* End-to-end convenience with HOST buffers (bench.py's e2e leg): copies the ASCII sequences and
+ * anchors to the device, packs, extends (flags as above), resolves in one window, copies
+ * results / keep / ops / stats back and synchronises.  cigar_host may be NULL. */
+int sfe_extend_host(sfe_ctx *ctx, const char *t_ascii_host, int64_t t_len, const char *q_ascii_host, int64_t q_len,
+                    const sfe_pair *pairs_host, int32_t n_pairs, const sfe_anchor *anchors_host, int64_t n_anchors,
+                    const sfe_scoring *scoring_host, uint32_t flags,
+                    sfe_result *results_host, uint8_t *keep_host,
+                    uint32_t *cigar_host, int64_t cigar_cap, int64_t *cigar_used_host, sfe_stats *stats_host);
+
+/* Measurement helpers.  sfe_probe_int_issue runs a register-only microbenchmark
+ * of the Y-drop kernel's own integer opcode mix on every SM and reports sustained
+ * lane-instructions per clock per SM (the R of the integer-issue roofline).  mix: 0 = the
+ * kernel's mix (ALU + DPX + IMAD), 1 = ALU-pipe only (IADD3/LOP3), 2 = DPX only
+ * (VIADDMNMX/VIMNMX3), 3 = IMAD only.  sfe_last_batch_info returns counters of the most recent
+ * sfe_ydrop_batch on this ctx: [0] kernel launches, [1] halves run, [2] halves re-run after a
+ * traceback overflow, [3] traceback bytes written, [4] DP steps (warp wavefronts) executed,
+ * [5] halves that took the wide path. */
+int sfe_probe_int_issue(sfe_ctx *ctx, int mix, int iters, double *lane_ops_per_clk_per_sm, double *elapsed_ms);
+int sfe_last_batch_info(sfe_ctx *ctx, int64_t info[8]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SFE_H */

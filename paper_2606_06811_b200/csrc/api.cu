@@ -1,0 +1,329 @@
+// api.cu -- the C ABI of include/sfe.h: argument validation, scratch management, launch order.
+// Every step of the path runs in the kernels of this directory; there is no CPU fallback.
+#include <new>
+#include <stdio.h>
+#include <string.h>
+#include "sfe_internal.cuh"
+
+#define ST_PASS_OVERFLOW 0x100u
+
+// launchers defined next to their kernels
+int sfe_launch_ydrop(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st);
+int sfe_launch_join(const sfe_anchor *anchors, const sfe_half *halves, long long n, const long long *sel, long long n_sel,
+                    const uint32_t *pool, const int32_t *chunk_prev, int want_cigar, sfe_result *results, cudaStream_t st);
+int sfe_launch_scan_emit(const sfe_half *halves, long long n, const long long *sel, long long n_sel, const uint32_t *pool,
+                         const int32_t *chunk_prev, sfe_result *results, uint32_t *cigar_pool, long long cap,
+                         long long *pool_used, cudaStream_t st);
+int sfe_launch_pack(const char *ascii, long long len, uint8_t *codes2, uint8_t *nmask, uint8_t *rc_codes2,
+                    uint8_t *rc_nmask, cudaStream_t st);
+int sfe_launch_resolve(const sfe_anchor *anchors, const sfe_result *results, long long n, int min_score, sfe_box *accepted,
+                       long long accepted_cap, long long *n_accepted_io, uint8_t *keep, sfe_stats *stats, long long *blkmin,
+                       sfe_box *act, cudaStream_t st);
+int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe_pair *pairs, int n_pairs, long long q_len,
+                       bool binned, unsigned int *hist, int32_t *tickets, cudaStream_t st);
+int sfe_launch_select_overflow(const sfe_half *halves, long long n_anchors, long long *sel, int32_t *tickets,
+                               unsigned long long *n_sel, cudaStream_t st);
+int sfe_launch_probe(int mix, int iters, int blocks, int *sink, cudaStream_t st);
+
+struct DevBuf {                       // grow-only device scratch
+    void *p = nullptr; size_t cap = 0;
+    int ensure(size_t bytes)
+    {
+        if (bytes <= cap) return SFE_OK;
+        if (p) cudaFree(p);
+        p = nullptr; cap = 0;
+        size_t want = bytes + bytes / 4 + 256;
+        if (cudaMalloc(&p, want) != cudaSuccess) { cudaGetLastError(); return SFE_ENOMEM; }
+        cap = want;
+        return SFE_OK;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+};
+
+struct sfe_ctx {
+    int device; cudaStream_t stream; int n_sm; int clock_khz;
+    uint32_t *pool; int32_t *chunk_prev; int n_chunks;
+    unsigned long long *counters;     // device, CNT_N
+    unsigned long long *counters_host;  // pinned
+    DevBuf halves, tickets, sel, hist, blkmin, act, misc;
+    // host-API staging
+    DevBuf h_tascii, h_qascii, h_t2, h_tm, h_q2, h_qm, h_r2, h_rm, h_pairs, h_anchors, h_results, h_keep, h_cigar, h_acc, h_small;
+    long long info[8];
+};
+
+static char g_err_detail[512] = "";
+void sfe_note_cuda_error(cudaError_t e, const char *file, int line)
+{
+    snprintf(g_err_detail, sizeof g_err_detail, "%s:%d: %s", file, line, cudaGetErrorString(e));
+    cudaGetLastError();
+}
+extern "C" const char *sfe_last_error_detail(void) { return g_err_detail; }
+
+static const char *const k_errs[] = {"ok", "invalid argument", "out of memory", "CUDA error", "value outside supported range"};
+
+extern "C" const char *sfe_strerror(int code)
+{
+    const int k = -code;
+    return (k >= 0 && k <= 4) ? k_errs[k] : "unknown error";
+}
+
+extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t scratch_bytes)
+{
+    if (!out || device < 0) return SFE_EINVAL;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { cudaGetLastError(); return SFE_ECUDA; }
+    SFE_CUDA_CHECK(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    SFE_CUDA_CHECK(cudaGetDeviceProperties(&prop, device));
+    if (prop.major < 10) return SFE_ECUDA;                     // sm_100a only
+    sfe_ctx *c = new (std::nothrow) sfe_ctx();
+    if (!c) return SFE_ENOMEM;
+    c->device = device; c->stream = (cudaStream_t)cuda_stream; c->n_sm = prop.multiProcessorCount;
+    int khz = 0; cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, device); c->clock_khz = khz;
+    if (scratch_bytes == 0) scratch_bytes = (size_t)1 << 30;
+    long long nch = (long long)(scratch_bytes / SFE_CHUNK_BYTES);
+    if (nch < 4) nch = 4;
+    if (nch > 0x7ffffff0LL / SFE_CHUNK_RECS) nch = 0x7ffffff0LL / SFE_CHUNK_RECS;   // record indices are int32
+    c->n_chunks = (int)nch;
+    c->pool = nullptr; c->chunk_prev = nullptr; c->counters = nullptr; c->counters_host = nullptr;
+    memset(c->info, 0, sizeof c->info);
+    if (cudaMalloc((void **)&c->pool, (size_t)nch * SFE_CHUNK_BYTES) != cudaSuccess ||
+        cudaMalloc((void **)&c->chunk_prev, (size_t)nch * sizeof(int32_t)) != cudaSuccess ||
+        cudaMalloc((void **)&c->counters, CNT_N * sizeof(unsigned long long)) != cudaSuccess ||
+        cudaMallocHost((void **)&c->counters_host, CNT_N * sizeof(unsigned long long)) != cudaSuccess) {
+        cudaGetLastError();
+        sfe_destroy(c);
+        return SFE_ENOMEM;
+    }
+    *out = c;
+    return SFE_OK;
+}
+
+extern "C" int sfe_destroy(sfe_ctx *c)
+{
+    if (!c) return SFE_EINVAL;
+    cudaSetDevice(c->device);
+    if (c->pool) cudaFree(c->pool);
+    if (c->chunk_prev) cudaFree(c->chunk_prev);
+    if (c->counters) cudaFree(c->counters);
+    if (c->counters_host) cudaFreeHost(c->counters_host);
+    DevBuf *bufs[] = {&c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
+                      &c->h_t2, &c->h_tm, &c->h_q2, &c->h_qm, &c->h_r2, &c->h_rm, &c->h_pairs, &c->h_anchors, &c->h_results,
+                      &c->h_keep, &c->h_cigar, &c->h_acc, &c->h_small};
+    for (DevBuf *b : bufs) b->release();
+    delete c;
+    return SFE_OK;
+}
+
+extern "C" int sfe_pack(sfe_ctx *c, const char *ascii_dev, int64_t len, uint8_t *codes2_dev, uint8_t *nmask_dev,
+                        uint8_t *rc_codes2_dev, uint8_t *rc_nmask_dev)
+{
+    if (!c || len < 0 || (len > 0 && (!ascii_dev || !codes2_dev || !nmask_dev))) return SFE_EINVAL;
+    if ((rc_codes2_dev == nullptr) != (rc_nmask_dev == nullptr)) return SFE_EINVAL;
+    SFE_CUDA_CHECK(cudaSetDevice(c->device));
+    return sfe_launch_pack(ascii_dev, len, codes2_dev, nmask_dev, rc_codes2_dev, rc_nmask_dev, c->stream);
+}
+
+extern "C" int sfe_probe_int_issue(sfe_ctx *c, int mix, int iters, double *lane_ops_per_clk_per_sm, double *elapsed_ms)
+{
+    if (!c || iters < 1 || mix < 0 || mix > 3 || !lane_ops_per_clk_per_sm) return SFE_EINVAL;
+    SFE_CUDA_CHECK(cudaSetDevice(c->device));
+    int rc = c->misc.ensure(256);
+    if (rc) return rc;
+    const int blocks = c->n_sm * 8;                            // 8 x 256 threads = 64 warps per SM
+    cudaEvent_t e0, e1;
+    SFE_CUDA_CHECK(cudaEventCreate(&e0)); SFE_CUDA_CHECK(cudaEventCreate(&e1));
+    rc = sfe_launch_probe(mix, iters / 8 + 1, blocks, (int *)c->misc.p, c->stream);   // warm-up
+    if (rc) return rc;
+    SFE_CUDA_CHECK(cudaEventRecord(e0, c->stream));
+    rc = sfe_launch_probe(mix, iters, blocks, (int *)c->misc.p, c->stream);
+    if (rc) return rc;
+    SFE_CUDA_CHECK(cudaEventRecord(e1, c->stream));
+    SFE_CUDA_CHECK(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    SFE_CUDA_CHECK(cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    // 16 instructions per thread per iteration (8 chains x 2 ops); the clock is sampled by the
+    // caller (nvidia-smi) -- here we report per max-clock cycle and the elapsed time.
+    const double lane_ops = (double)blocks * 256.0 * (double)iters * 16.0;
+    const double cycles = (double)ms * 1e-3 * (double)c->clock_khz * 1e3;
+    *lane_ops_per_clk_per_sm = lane_ops / cycles / (double)c->n_sm;
+    if (elapsed_ms) *elapsed_ms = ms;
+    return SFE_OK;
+}
+
+extern "C" int sfe_last_batch_info(sfe_ctx *c, int64_t info[8])
+{
+    if (!c || !info) return SFE_EINVAL;
+    for (int k = 0; k < 8; k++) info[k] = c->info[k];
+    return SFE_OK;
+}
+
+static int check_scoring(const sfe_scoring *s)
+{
+    if (!s) return SFE_EINVAL;
+    if (s->prune_lag != SFE_PRUNE_LAG) return SFE_EINVAL;
+    for (int a = 0; a < 4; a++)
+        for (int b = 0; b < 4; b++)
+            if (s->sub[a][b] < -128 || s->sub[a][b] > 127) return SFE_ELIMIT;
+    if (s->n_score < -128 || s->n_score > 127) return SFE_ELIMIT;
+    if (s->gap_open < 0 || s->gap_extend < 1 || s->gap_open + (long long)s->gap_extend > 65535) return SFE_ELIMIT;
+    if (s->ydrop != SFE_YDROP_INF && (s->ydrop < 0 || s->ydrop >= (1 << 28))) return SFE_ELIMIT;
+    return SFE_OK;
+}
+
+extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *t_nmask, int64_t t_len,
+                               const uint8_t *q_codes2, const uint8_t *q_nmask, const uint8_t *qrc_codes2,
+                               const uint8_t *qrc_nmask, int64_t q_len, const sfe_pair *pairs_dev, int32_t n_pairs,
+                               const sfe_anchor *anchors_dev, int64_t n_anchors, const sfe_scoring *sc, uint32_t flags,
+                               sfe_result *results_dev, uint32_t *cigar_pool_dev, int64_t cigar_pool_cap,
+                               int64_t *cigar_pool_used_dev)
+{
+    if (!c || n_anchors < 0 || t_len < 0 || q_len < 0 || n_pairs < 0) return SFE_EINVAL;
+    int rc = check_scoring(sc);
+    if (rc) return rc;
+    const bool want_tb = (flags & SFE_WANT_CIGAR) != 0;
+    if (n_anchors > 0 && (!t_codes2 || !t_nmask || !q_codes2 || !q_nmask || !pairs_dev || !anchors_dev || !results_dev)) return SFE_EINVAL;
+    if ((qrc_codes2 == nullptr) != (qrc_nmask == nullptr)) return SFE_EINVAL;
+    if (want_tb && (!cigar_pool_dev || cigar_pool_cap < 0 || !cigar_pool_used_dev)) return SFE_EINVAL;
+    if (2 * n_anchors > 0x7ffffff0LL) return SFE_ELIMIT;
+    SFE_CUDA_CHECK(cudaSetDevice(c->device));
+    memset(c->info, 0, sizeof c->info);
+    if (cigar_pool_used_dev) SFE_CUDA_CHECK(cudaMemsetAsync(cigar_pool_used_dev, 0, sizeof(int64_t), c->stream));
+    if (n_anchors == 0) return SFE_OK;
+
+    if ((rc = c->halves.ensure((size_t)(2 * n_anchors) * sizeof(sfe_half)))) return rc;
+    if ((rc = c->tickets.ensure((size_t)(2 * n_anchors) * sizeof(int32_t)))) return rc;
+    if ((rc = c->hist.ensure(64 * sizeof(unsigned int)))) return rc;
+    if (want_tb && (rc = c->sel.ensure((size_t)n_anchors * sizeof(long long)))) return rc;
+
+    YdParams p;
+    memset(&p, 0, sizeof p);
+    p.t_codes = t_codes2; p.t_nmask = t_nmask; p.q_codes = q_codes2; p.q_nmask = q_nmask;
+    p.qrc_codes = qrc_codes2; p.qrc_nmask = qrc_nmask; p.t_len = t_len; p.q_len = q_len;
+    p.pairs = pairs_dev; p.anchors = anchors_dev; p.tickets = (const int32_t *)c->tickets.p; p.n_tickets = 2 * n_anchors;
+    p.counters = c->counters; p.halves = (sfe_half *)c->halves.p; p.pool = c->pool; p.chunk_prev = c->chunk_prev;
+    p.n_chunks = want_tb ? c->n_chunks : 0; p.n_pairs = n_pairs;
+    p.OX = sc->gap_open + sc->gap_extend; p.X = sc->gap_extend;
+    p.ydrop_inf = sc->ydrop == SFE_YDROP_INF; p.Y = p.ydrop_inf ? 0 : sc->ydrop;
+    for (int a = 0; a < 4; a++) {
+        uint32_t w = 0;
+        for (int b = 0; b < 4; b++) w |= ((uint32_t)(uint8_t)(int8_t)sc->sub[a][b]) << (8 * b);
+        p.srow[a] = w;
+    }
+    p.srow[4] = 0x01010101u * (uint32_t)(uint8_t)(int8_t)sc->n_score;
+    p.srow_hi = (uint32_t)(uint8_t)(int8_t)sc->n_score | (0xE0u << 16);
+
+    SFE_CUDA_CHECK(cudaMemsetAsync(c->counters, 0, CNT_N * sizeof(unsigned long long), c->stream));
+    if ((rc = sfe_launch_tickets(anchors_dev, n_anchors, pairs_dev, n_pairs, q_len, !(flags & SFE_NO_BINNING),
+                                 (unsigned int *)c->hist.p, (int32_t *)c->tickets.p, c->stream))) return rc;
+    if ((rc = sfe_launch_ydrop(p, want_tb, c->n_sm, c->stream))) return rc;
+    c->info[0] += 1; c->info[1] += 2 * n_anchors;
+    if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, nullptr, n_anchors, c->pool, c->chunk_prev, want_tb,
+                              results_dev, c->stream))) return rc;
+    if (!want_tb) return SFE_OK;
+    if ((rc = sfe_launch_scan_emit(p.halves, n_anchors, nullptr, n_anchors, c->pool, c->chunk_prev, results_dev,
+                                   cigar_pool_dev, cigar_pool_cap, (long long *)cigar_pool_used_dev, c->stream))) return rc;
+
+    // traceback-arena overflow: re-run the anchors that did not fit, with the arena emptied
+    long long prev_overflow = -1;
+    for (;;) {
+        SFE_CUDA_CHECK(cudaMemcpyAsync(c->counters_host, c->counters, CNT_N * sizeof(unsigned long long),
+                                       cudaMemcpyDeviceToHost, c->stream));
+        SFE_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+        c->info[3] += (long long)c->counters_host[CNT_TBBYTES];
+        c->info[4] += (long long)c->counters_host[CNT_STEPS];
+        c->info[5] += (long long)c->counters_host[CNT_WIDE];
+        const long long n_over = (long long)c->counters_host[CNT_OVERFLOW];
+        if (n_over == 0) break;
+        // no progress possible: the anchors that overflowed were already running alone
+        if (prev_overflow >= 0 && n_over >= prev_overflow) break;
+        prev_overflow = n_over;
+        SFE_CUDA_CHECK(cudaMemsetAsync(c->counters, 0, CNT_N * sizeof(unsigned long long), c->stream));
+        if ((rc = sfe_launch_select_overflow(p.halves, n_anchors, (long long *)c->sel.p, (int32_t *)c->tickets.p,
+                                             &c->counters[CNT_RERUN], c->stream))) return rc;
+        SFE_CUDA_CHECK(cudaMemcpyAsync(c->counters_host, c->counters, CNT_N * sizeof(unsigned long long),
+                                       cudaMemcpyDeviceToHost, c->stream));
+        SFE_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+        const long long n_sel = (long long)c->counters_host[CNT_RERUN];
+        if (n_sel <= 0) break;
+        p.n_tickets = 2 * n_sel;
+        if ((rc = sfe_launch_ydrop(p, true, c->n_sm, c->stream))) return rc;
+        c->info[0] += 1; c->info[1] += 2 * n_sel; c->info[2] += 2 * n_sel;
+        if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, (const long long *)c->sel.p, n_sel, c->pool,
+                                  c->chunk_prev, 1, results_dev, c->stream))) return rc;
+        if ((rc = sfe_launch_scan_emit(p.halves, n_anchors, (const long long *)c->sel.p, n_sel, c->pool, c->chunk_prev,
+                                       results_dev, cigar_pool_dev, cigar_pool_cap, (long long *)cigar_pool_used_dev,
+                                       c->stream))) return rc;
+    }
+    return SFE_OK;
+}
+
+extern "C" int sfe_resolve(sfe_ctx *c, const sfe_anchor *anchors_dev, const sfe_result *results_dev, int64_t n,
+                           int32_t min_score, sfe_box *accepted_dev, int64_t accepted_cap, int64_t *n_accepted_dev,
+                           uint8_t *keep_dev, sfe_stats *stats_dev)
+{
+    if (!c || n < 0 || accepted_cap < 0) return SFE_EINVAL;
+    if (n == 0) return SFE_OK;
+    if (!anchors_dev || !keep_dev || !accepted_dev || !n_accepted_dev) return SFE_EINVAL;
+    SFE_CUDA_CHECK(cudaSetDevice(c->device));
+    int rc;
+    if ((rc = c->blkmin.ensure((size_t)((n + 31) / 32 + 32) * sizeof(long long)))) return rc;
+    if ((rc = c->act.ensure((size_t)(accepted_cap + 1) * sizeof(sfe_box)))) return rc;
+    return sfe_launch_resolve(anchors_dev, results_dev, n, min_score, accepted_dev, accepted_cap, (long long *)n_accepted_dev,
+                              keep_dev, stats_dev, (long long *)c->blkmin.p, (sfe_box *)c->act.p, c->stream);
+}
+
+extern "C" int sfe_extend_host(sfe_ctx *c, const char *t_ascii, int64_t t_len, const char *q_ascii, int64_t q_len,
+                               const sfe_pair *pairs, int32_t n_pairs, const sfe_anchor *anchors, int64_t n_anchors,
+                               const sfe_scoring *sc, uint32_t flags, sfe_result *results_host, uint8_t *keep_host,
+                               uint32_t *cigar_host, int64_t cigar_cap, int64_t *cigar_used_host, sfe_stats *stats_host)
+{
+    if (!c || !t_ascii || !q_ascii || !pairs || !anchors || !sc || !results_host || !keep_host) return SFE_EINVAL;
+    if (t_len <= 0 || q_len <= 0 || n_pairs <= 0 || n_anchors <= 0) return SFE_EINVAL;
+    const bool want_tb = (flags & SFE_WANT_CIGAR) != 0;
+    if (want_tb && (!cigar_host || cigar_cap <= 0 || !cigar_used_host)) return SFE_EINVAL;
+    SFE_CUDA_CHECK(cudaSetDevice(c->device));
+    cudaStream_t st = c->stream;
+    int rc;
+    const size_t tb2 = ((size_t)(t_len + 3) / 4 + 15) & ~(size_t)15, tbm = ((size_t)(t_len + 7) / 8 + 15) & ~(size_t)15;
+    const size_t qb2 = ((size_t)(q_len + 3) / 4 + 15) & ~(size_t)15, qbm = ((size_t)(q_len + 7) / 8 + 15) & ~(size_t)15;
+    if ((rc = c->h_tascii.ensure((size_t)t_len + 16)) || (rc = c->h_qascii.ensure((size_t)q_len + 16)) ||
+        (rc = c->h_t2.ensure(tb2)) || (rc = c->h_tm.ensure(tbm)) || (rc = c->h_q2.ensure(qb2)) || (rc = c->h_qm.ensure(qbm)) ||
+        (rc = c->h_r2.ensure(qb2)) || (rc = c->h_rm.ensure(qbm)) || (rc = c->h_pairs.ensure((size_t)n_pairs * sizeof(sfe_pair))) ||
+        (rc = c->h_anchors.ensure((size_t)n_anchors * sizeof(sfe_anchor))) ||
+        (rc = c->h_results.ensure((size_t)n_anchors * sizeof(sfe_result))) || (rc = c->h_keep.ensure((size_t)n_anchors)) ||
+        (rc = c->h_acc.ensure((size_t)(n_anchors + 1) * sizeof(sfe_box))) ||
+        (rc = c->h_small.ensure(256)) || (want_tb && (rc = c->h_cigar.ensure((size_t)cigar_cap * sizeof(uint32_t)))))
+        return rc;
+    SFE_CUDA_CHECK(cudaMemcpyAsync(c->h_tascii.p, t_ascii, (size_t)t_len, cudaMemcpyHostToDevice, st));
+    SFE_CUDA_CHECK(cudaMemcpyAsync(c->h_qascii.p, q_ascii, (size_t)q_len, cudaMemcpyHostToDevice, st));
+    SFE_CUDA_CHECK(cudaMemcpyAsync(c->h_pairs.p, pairs, (size_t)n_pairs * sizeof(sfe_pair), cudaMemcpyHostToDevice, st));
+    SFE_CUDA_CHECK(cudaMemcpyAsync(c->h_anchors.p, anchors, (size_t)n_anchors * sizeof(sfe_anchor), cudaMemcpyHostToDevice, st));
+    SFE_CUDA_CHECK(cudaMemsetAsync(c->h_small.p, 0, 256, st));
+    long long *d_used = (long long *)c->h_small.p;              // [0] cigar used, [1] n_accepted
+    sfe_stats *d_stats = (sfe_stats *)((char *)c->h_small.p + 64);
+    if ((rc = sfe_pack(c, (const char *)c->h_tascii.p, t_len, (uint8_t *)c->h_t2.p, (uint8_t *)c->h_tm.p, nullptr, nullptr))) return rc;
+    if ((rc = sfe_pack(c, (const char *)c->h_qascii.p, q_len, (uint8_t *)c->h_q2.p, (uint8_t *)c->h_qm.p, (uint8_t *)c->h_r2.p,
+                       (uint8_t *)c->h_rm.p))) return rc;
+    if ((rc = sfe_ydrop_batch(c, (uint8_t *)c->h_t2.p, (uint8_t *)c->h_tm.p, t_len, (uint8_t *)c->h_q2.p, (uint8_t *)c->h_qm.p,
+                              (uint8_t *)c->h_r2.p, (uint8_t *)c->h_rm.p, q_len, (sfe_pair *)c->h_pairs.p, n_pairs,
+                              (sfe_anchor *)c->h_anchors.p, n_anchors, sc, flags, (sfe_result *)c->h_results.p,
+                              (uint32_t *)c->h_cigar.p, cigar_cap, (int64_t *)d_used))) return rc;
+    if ((rc = sfe_resolve(c, (sfe_anchor *)c->h_anchors.p, (sfe_result *)c->h_results.p, n_anchors, sc->min_score,
+                          (sfe_box *)c->h_acc.p, n_anchors, (int64_t *)(d_used + 1), (uint8_t *)c->h_keep.p, d_stats))) return rc;
+    SFE_CUDA_CHECK(cudaMemcpyAsync(results_host, c->h_results.p, (size_t)n_anchors * sizeof(sfe_result), cudaMemcpyDeviceToHost, st));
+    SFE_CUDA_CHECK(cudaMemcpyAsync(keep_host, c->h_keep.p, (size_t)n_anchors, cudaMemcpyDeviceToHost, st));
+    long long used = 0;
+    if (want_tb) {
+        SFE_CUDA_CHECK(cudaMemcpyAsync(&used, d_used, sizeof used, cudaMemcpyDeviceToHost, st));
+        SFE_CUDA_CHECK(cudaStreamSynchronize(st));
+        const long long ncopy = used < cigar_cap ? used : cigar_cap;
+        if (ncopy > 0) SFE_CUDA_CHECK(cudaMemcpyAsync(cigar_host, c->h_cigar.p, (size_t)ncopy * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+        *cigar_used_host = used;
+    }
+    if (stats_host) SFE_CUDA_CHECK(cudaMemcpyAsync(stats_host, d_stats, sizeof(sfe_stats), cudaMemcpyDeviceToHost, st));
+    SFE_CUDA_CHECK(cudaStreamSynchronize(st));
+    return SFE_OK;
+}

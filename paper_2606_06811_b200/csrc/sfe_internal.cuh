@@ -1,0 +1,81 @@
+// sfe_internal.cuh -- shared declarations of the CUDA side of libsfe (sm_100a only).
+// Nothing here is shared with oracle/: the oracle defines its own structs and rules.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/sfe.h"
+
+#define SFE_NEG (-(1 << 30))            // "minus infinity" of the DP (R6)
+#define SFE_T_INF (-(1 << 29))          // threshold used for SFE_YDROP_INF (R27): every real cell is above it
+#define SFE_OOB_SCORE 0xE0000000u       // substitution "score" of a column beyond the target end (-2^29)
+
+// ---- shared-memory geometry of one warp -------------------------
+// A strip is 32 consecutive DP rows, one per lane, swept left to right; lane l is one column
+// behind lane l-1.  Messages (H-(O+X) gated by alive, E) travel lane l -> l+1 through a tiny
+// exchange area; the last lane's messages go to the boundary ring that lane 0 of the NEXT strip
+// reads.  Everything is laid out in 8 "rows", one per step of an unrolled group of 8 steps, so
+// that every access in the unrolled loop is base + immediate.
+#define SFE_RING 1024                               // boundary-ring capacity in columns
+#define SFE_EXCH_BYTES 256                          // 32 lanes x 8 B
+#define SFE_ROW_STRIDE (SFE_EXCH_BYTES + SFE_RING)  // bytes: exchange area + RING/8 segments x 8 B
+#define SFE_SELRING 1024                            // selector ring capacity in columns
+#define SFE_WARP_SMEM (8 * SFE_ROW_STRIDE + (SFE_SELRING + 8) * 2)
+#define SFE_MAX_STEPS (SFE_RING - 160)              // a strip wider than this takes the wide path
+
+// ---- traceback arena --------------------------------------------------------------------------
+// Record = 32 lanes x one 32-bit word (8 cells x 4 bits) = 128 B, written coalesced by one warp
+// per group of 8 steps.  Records live in 64 KiB chunks handed out by an atomic counter; a half's
+// chunks form a backward-linked list (chunk_prev).
+#define SFE_CHUNK_RECS 512
+#define SFE_CHUNK_BYTES (SFE_CHUNK_RECS * 128)
+
+struct sfe_half {                 // result of one one-sided extension (a7)
+    int32_t score;
+    int32_t end_i, end_j;         // argbest, rows / columns relative to the anchor
+    uint32_t status;
+    unsigned long long cells;     // R28
+    int32_t last_hdr;             // record index of the last strip's header record, -1 if none
+    int32_t last_chunk;           // chunk id holding the last record, -1 if none
+    int32_t n_strips;
+    int32_t n_rec;                // records written
+    int32_t steps;                // warp wavefronts executed
+    int32_t max_steps;            // widest strip
+};
+
+enum { CNT_TICKET = 0, CNT_CHUNK, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_N = 8 };
+
+struct YdParams {
+    const uint8_t *t_codes, *t_nmask;
+    const uint8_t *q_codes, *q_nmask, *qrc_codes, *qrc_nmask;
+    long long t_len, q_len;
+    const sfe_pair *pairs;
+    const sfe_anchor *anchors;
+    const int32_t *tickets;       // half ids (2*anchor + dir), in issue order
+    long long n_tickets;
+    unsigned long long *counters; // CNT_*
+    sfe_half *halves;             // [2 * n_anchors]
+    uint32_t *pool;               // traceback arena
+    int32_t *chunk_prev;
+    int32_t n_chunks;
+    int32_t n_pairs;
+    int32_t OX, X, Y, ydrop_inf;
+    uint32_t srow[5];             // packed int8 scores of a query base A,C,G,T,N against A,C,G,T
+    uint32_t srow_hi;             // bytes: n_score, 0x00, 0xE0 (OOB), 0x00
+    int32_t *wide_ring;           // global-memory boundary rings for the wide path (per warp), or NULL
+    int32_t wide_cols;
+};
+
+static __device__ __forceinline__ int sfe_lane() { return threadIdx.x & 31; }
+
+// base k of a packed sequence: code 0..3, or 4 if the N-mask bit is set
+static __device__ __forceinline__ int sfe_base(const uint8_t *codes2, const uint8_t *nmask, long long k)
+{
+    const int c = (codes2[k >> 2] >> ((k & 3) * 2)) & 3;
+    const int n = (nmask[k >> 3] >> (k & 7)) & 1;
+    return n ? 4 : c;
+}
+
+// last CUDA failure (file:line + runtime message), readable through sfe_last_error_detail()
+void sfe_note_cuda_error(cudaError_t e, const char *file, int line);
+#define SFE_CUDA_CHECK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { sfe_note_cuda_error(e_, __FILE__, __LINE__); return SFE_ECUDA; } } while (0)
+#define SFE_LAUNCH_CHECK() do { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) { sfe_note_cuda_error(e_, __FILE__, __LINE__); return SFE_ECUDA; } return SFE_OK; } while (0)
