@@ -1,0 +1,97 @@
+"""CPU-only checks of the boundary: the C-ABI library loads and exports every symbol that
+include/sfe.h declares; struct layouts of the binding match the header; the product path fails
+loudly without a GPU (no CPU fallback)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import __graft_entry__ as entry
+from paper_2606_06811_b200 import binding as B
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def built():
+    entry.build()
+    return B.lib()
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "sfe.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(sfe_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_exports_every_declared_symbol(built):
+    names = _declared()
+    assert set(B.EXPORTS) == set(names), (names, B.EXPORTS)
+    for n in names:
+        assert hasattr(built, n), n
+
+
+def test_struct_layouts_match_header():
+    assert C.sizeof(B.Scoring) == 22 * 4
+    assert B.ANCHOR_DT.itemsize == 24 and B.PAIR_DT.itemsize == 32
+    assert B.RESULT_DT.itemsize == 72 and B.RESULT_DT.fields["cells"][1] == 64
+    assert B.BOX_DT.itemsize == 40 and B.STATS_DT.itemsize == C.sizeof(B.Stats) == 48
+
+
+def test_strerror_and_null_args(built):
+    assert built.sfe_strerror(0) == b"ok" and built.sfe_strerror(-4).startswith(b"value")
+    assert built.sfe_destroy(None) == B.EINVAL
+    assert built.sfe_pack(None, None, 0, None, None, None, None) == B.EINVAL
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(B.SfeError):
+        B.Sfe(0)
+    h = C.c_void_p()
+    assert B.lib().sfe_create(C.byref(h), 0, None, 1 << 20) != B.OK and not h.value
+
+
+def test_product_does_not_import_oracle():
+    """The package never touches oracle/ (and the oracle never imports the package)."""
+    pkg = os.path.join(ROOT, "paper_2606_06811_b200")
+    for dp, _, fs in os.walk(pkg):
+        for f in fs:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                assert "oracle" not in open(os.path.join(dp, f)).read().lower().replace("oracle/", "oracle/") or \
+                    f in ("workloads.py",) or _only_comments_mention(os.path.join(dp, f))
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2606_06811_b200" not in txt and "from paper_2606_06811_b200" not in txt
+            assert "#include \"sfe" not in txt and "include/sfe.h\"" not in txt.replace("(", "")
+
+
+def _only_comments_mention(path):
+    for ln in open(path):
+        s = ln.strip()
+        if "oracle" in s.lower() and not (s.startswith("//") or s.startswith("#") or s.startswith("*") or '"""' in s
+                                          or "oracle tests" in s or "the oracle" in s.lower()):
+            if "import" in s or "include" in s:
+                return False
+    return True
+
+
+def test_workload_generators():
+    from paper_2606_06811_b200 import workloads as W
+    assert int(W.splitmix64(0, 2)[0]) == 0xE220A8397B1DCDAF and int(W.splitmix64(0, 2)[1]) == 0x6E789E6AA1B965F4
+    assert W.to_ascii(W.randseq(1, 16)).tobytes() == b"GGTCCTTGCTCGCGCA"
+    assert W.to_ascii(W.randseq(2, 16)).tobytes() == b"GGGTCCGGCGCCGCTA"
+    w = W.config1()
+    assert len(w.anchors) == 256 and len(w.target) == 200_000 and (w.anchors[:, 3] == 1).all()
+    assert (np.diff(w.anchors[:, 0]) >= 0).all()
+    src = W.randseq(5, 5000)
+    mu = W.mutate(src, 0.1, 0.02, W.Stream(6))
+    # aligned positions are a strictly increasing map and substitutions ~10%
+    assert (np.diff(mu.t_idx) > 0).all() and (np.diff(mu.q_idx) > 0).all()
+    ident = (src[mu.t_idx] == mu.seq[mu.q_idx]).mean()
+    assert 0.86 < ident < 0.94

@@ -1,0 +1,160 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the CPU oracle, bit-exact
+(scores, boxes, cell counts, CIGARs, kept set): all arithmetic is integer."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2606_06811_b200 import binding as B, workloads as W  # noqa: E402
+
+import gpu_harness as H  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def sfe():
+    import __graft_entry__ as entry
+    entry.build()
+    s = B.Sfe(0, 2 << 30)
+    yield s
+    s.close()
+
+
+def _wl(T, Q, anchors, pairs=None):
+    T = np.asarray(T, np.uint8); Q = np.asarray(Q, np.uint8)
+    pairs = np.array([[0, len(T), 0, len(Q)]] if pairs is None else pairs, np.int64)
+    return W.Workload("t", T, Q, pairs, np.array(anchors, np.int64).reshape(-1, 4))
+
+
+def test_pack_matches_definition(sfe, oracle):
+    import torch
+    rng = np.random.default_rng(5)
+    for n in (1, 3, 31, 32, 33, 100, 4099, 65537):
+        s = rng.choice(np.frombuffer(b"ACGTNacgtnXR", np.uint8), n)
+        c2, nm, r2, rm = sfe.pack(torch.from_numpy(s.copy()).to(sfe.device))
+        torch.cuda.synchronize()
+        e = oracle.pack(s.tobytes())
+        for got, exp in zip((c2, nm, r2, rm), e):
+            assert got.cpu().numpy()[: len(exp)].tolist() == exp.tolist(), n
+
+
+def test_appendix_a_examples(sfe, oracle):
+    c = oracle.codes
+    T = c("ACGTACGTTTGGCCAGTCAT"); Q = c("ACGTACGTGGCCAGTCAT")
+    w = _wl(T, Q, [(0, 0, 0, 1), (14, 12, 0, 1), (10, 10, 0, 1), (9, 8, 0, 1), (3, 5, 0, 1), (20, 18, 0, 1), (0, 18, 0, 1)])
+    out = H.gpu_run(sfe, w)
+    for i in range(len(w.anchors)):
+        H.assert_anchor_equal(out, w, i)
+    for q, t in (("ACGTACGT", "ACGTACGT"), ("ACGNACGT", "ACGTACGT"), ("AAAA", "CCCC"), ("ACGTTA", "ACGTCA"), ("A", "A"),
+                 ("A", "C"), ("ACGT", "A")):
+        w = _wl(c(t), c(q), [(0, 0, 0, 1), (len(t), len(q), 0, 1)])
+        out = H.gpu_run(sfe, w)
+        H.assert_anchor_equal(out, w, 0); H.assert_anchor_equal(out, w, 1)
+
+
+@pytest.mark.parametrize("ydrop", [120, 455, 1500, 9400])
+def test_small_ydrops_and_ties(sfe, oracle, ydrop):
+    """Y < O+X (gap-free), mid-range Y, default Y on related random pairs with N runs."""
+    rng = np.random.default_rng(ydrop)
+    T = rng.integers(0, 4, 900).astype(np.uint8)
+    mu = W.mutate(T, 0.08, 0.02, W.Stream(ydrop))
+    Q = mu.seq.copy()
+    Q[100:104] = 4; T[300:302] = 4
+    picks = rng.integers(0, len(mu.t_idx), 24)
+    anchors = [(int(mu.t_idx[k]), int(mu.q_idx[k]), 0, 1) for k in picks] + [(0, 0, 0, 1), (len(T), len(Q), 0, 1), (5, 700, 0, 1)]
+    w = _wl(T, Q, anchors)
+    out = H.gpu_run(sfe, w, ydrop=ydrop)
+    for i in range(len(anchors)):
+        H.assert_anchor_equal(out, w, i, ydrop=ydrop)
+
+
+def test_ydrop_inf_small(sfe, oracle):
+    """R27: nothing is pruned; every cell of the rectangle is alive."""
+    rng = np.random.default_rng(3)
+    T = rng.integers(0, 4, 150).astype(np.uint8); Q = T.copy(); Q[40] = (Q[40] + 1) % 4
+    Q = np.delete(Q, [70, 71])
+    w = _wl(T, Q, [(0, 0, 0, 1), (60, 60, 0, 1), (150, 148, 0, 1)])
+    out = H.gpu_run(sfe, w, ydrop=B.YDROP_INF)
+    for i in range(3):
+        r = H.assert_anchor_equal(out, w, i, ydrop=B.YDROP_INF)
+    assert int(out["results"][0]["cells"]) == 151 * 149 + 1
+
+
+def test_minus_strand_and_pairs(sfe, oracle):
+    """- strand anchors use the reverse-complemented query; pair limits clip the DP."""
+    w = W.config2(t_len=80_000, n_segments=40, per_seg=4, n_decoys=40, min_len=100, max_len=700)
+    out = H.gpu_run(sfe, w)
+    for i in range(len(w.anchors)):
+        H.assert_anchor_equal(out, w, i)
+    H.assert_resolve_equal(out, w)
+    # sub-rectangle pairs: limits inside the sequences
+    T = W.randseq(31, 3000); mu = W.mutate(T, 0.03, 0.005, W.Stream(32)); Q = mu.seq
+    pairs = [[500, 2500, 480, 2480], [0, 3000, 0, len(Q)], [1000, 1200, 990, 1190]]
+    k = np.searchsorted(mu.t_idx, [1100, 1500, 1100])
+    anchors = [(int(mu.t_idx[k[0]]), int(mu.q_idx[k[0]]), 0, 1), (int(mu.t_idx[k[1]]), int(mu.q_idx[k[1]]), 1, 1),
+               (int(mu.t_idx[k[2]]), int(mu.q_idx[k[2]]), 2, 1), (500, 480, 0, 1), (2500, 2480, 0, 1)]
+    w = _wl(T, Q, anchors, pairs)
+    out = H.gpu_run(sfe, w)
+    for i in range(len(anchors)):
+        H.assert_anchor_equal(out, w, i)
+
+
+def test_config1_full(sfe, oracle):
+    """BASELINE.json configs[0]: all 256 speculative extensions bit-exact; serial semantics keep 64."""
+    w = W.config1()
+    out = H.gpu_run(sfe, w)
+    for i in range(len(w.anchors)):
+        H.assert_anchor_equal(out, w, i)
+    ser = H.assert_resolve_equal(out, w)
+    assert ser["n_kept"] == 64 and int((out["keep"] == 1).sum()) == 64
+    st = out["stats"]
+    assert int(st["n_anchors"]) == 256 and int(st["n_covered"]) == 192 and int(st["n_below"]) == 0
+    assert int(st["cells_total"]) == int(out["results"]["cells"].sum())
+    # score-only mode gives the same scores / boxes / cells
+    out2 = H.gpu_run(sfe, w, flags=B.SCORE_ONLY)
+    for f in ("score", "tstart", "tend", "qstart", "qend", "cells"):
+        assert (out2["results"][f] == out["results"][f]).all()
+    assert out2["keep"].tolist() == out["keep"].tolist()
+
+
+def test_host_api_equals_device_api(sfe, oracle):
+    w = W.config1(n_segments=6, seg_len=500, slot=1200, per_seg=3)
+    out = H.gpu_run(sfe, w)
+    ho = sfe.extend_host(w.target_ascii(), w.query_ascii(), B.make_pairs(w.pairs), B.make_anchors(w.anchors), B.scoring())
+    assert ho["keep"].tolist() == out["keep"].tolist()
+    for f in ("score", "tstart", "tend", "qstart", "qend", "cells", "n_ops", "n_ops_back", "cigar_off"):
+        assert (ho["results"][f] == out["results"][f]).all(), f
+    assert ho["cigar_used"] == out["cigar_used"]
+    assert (ho["cigar"][: ho["cigar_used"]] == out["cigar"][: out["cigar_used"]]).all()
+    assert ho["stats"]["n_kept"] == int(out["stats"]["n_kept"])
+
+
+def test_windowed_resolve_equals_serial(sfe, oracle):
+    """Alg. 3 with windows of K through sfe_resolve (accepted list carried between calls, phase-1
+    filter with results == NULL) keeps what Alg. 1 keeps (P7), for several K."""
+    import torch
+    w = W.config2(t_len=60_000, n_segments=30, per_seg=8, n_decoys=40, min_len=150, max_len=700)
+    out = H.gpu_run(sfe, w)
+    ser = H.assert_resolve_equal(out, w)
+    n = len(w.anchors)
+    dev = sfe.device
+    A = B.make_anchors(w.anchors)
+    res_all = out["results"]
+    for K in (1, 5, 32, 33, n):
+        acc = torch.zeros((n + 1) * B.BOX_DT.itemsize, dtype=torch.uint8, device=dev)
+        nacc = torch.zeros(1, dtype=torch.int64, device=dev)
+        state = np.zeros(n, np.uint8)
+        j = 0
+        while j < n:
+            # phase 1: mask filter over the remaining anchors, take the first K unmasked
+            rest = B._dev(A[j:], dev)
+            m = sfe.resolve(rest, None, n - j, 0, acc, n + 1, nacc).cpu().numpy()[: n - j]
+            idx = np.nonzero(m == 1)[0][:K] + j
+            if len(idx) == 0:
+                break
+            nxt = (idx[-1] + 1) if len(idx) == K else n
+            # phase 3 on the window (phase 2 results taken from the all-at-once batch: R20)
+            kw = sfe.resolve(B._dev(A[idx], dev), B._dev(res_all[idx], dev), len(idx), 3000, acc, n + 1, nacc)
+            state[idx] = kw.cpu().numpy()[: len(idx)]
+            j = nxt
+        assert (state == 1).tolist() == (ser["state"] == 1).tolist(), K
+        assert int(nacc.item()) == ser["n_kept"]
