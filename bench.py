@@ -1,0 +1,292 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line: Y-drop GCUPS and kept alignments/s on 1 B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path over one batch: sfe_pack (target, query + reverse
+complement) -> sfe_ydrop_batch (binning, persistent queue, systolic Y-drop DP with traceback,
+CIGAR emission) -> sfe_resolve, on device-resident inputs (`value`), and the same through
+sfe_extend_host with pinned HOST buffers (`e2e`).  Default workload = BASELINE.json configs[1]
+(C2, divergent cross-species regime, 25,000 anchors); --workload c4 is the kernel
+microbenchmark (configs[3]).  The path does not shard (BASELINE.json: one GPU, no collectives):
+--gpus N runs N independent replicas ("replicas only"), value = sum over ranks.
+
+--impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+SCRATCH_GB = {"c1": 2, "c2": 28, "c4": 64, "c3s": 24, "c5s": 24}
+
+
+def make_workload(name):
+    from paper_2606_06811_b200 import workloads as W
+    if name == "c1":
+        return W.config1(), "BASELINE.json configs[0]: tiny high-identity pair, 256 anchors"
+    if name == "c2":
+        return W.config2(), "BASELINE.json configs[1]: divergent cross-species regime, 2 Mbp, 25,000 anchors"
+    if name == "c4":
+        return W.config4(), "BASELINE.json configs[3]: 65,536 independent pairs, log-normal lengths"
+    if name == "c3s":
+        return W.config3(t_len=1_000_000, n_anchors=5_000), "configs[2] scaled 1/10: 1 Mbp, 5,000 anchors (prefix-scale run)"
+    if name == "c5s":
+        return W.config5(t_len=10_000_000, n_anchors=100_000), "configs[4] scaled 1/10: 10 Mbp, 100,000 anchors"
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons, pw = [], [], set(), []
+        for ln in self.f:
+            c = [x.strip() for x in ln.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        os.unlink(self.f.name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        busy = sorted(sm)[len(sm) // 2:]                      # upper half = samples under load
+        return {"sm_mhz": float(np.median(busy)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(w, budget_s):
+    """The oracle as it stands, one thread, on a strided sample of the workload's anchors until
+    ~budget_s seconds of CPU work are done.  Returns (cells, seconds, n_anchors_done)."""
+    from oracle import sfe_oracle as O
+    O.lib()
+    sc = O.scoring()
+    n = len(w.anchors)
+    qrc = w.query_rc
+    stride = max(1, n // 4096)
+    order = [i for s in range(stride) for i in range(s, n, stride)]
+    cells = 0; done = 0
+    t0 = time.perf_counter()
+    for i in order:
+        a = w.anchors[i]; p = w.pairs[int(a[2])]
+        qlim = (int(p[2]), int(p[3])) if a[3] > 0 else (len(w.query) - int(p[3]), len(w.query) - int(p[2]))
+        r, _ = O.extend_anchor(w.target, w.query if a[3] > 0 else qrc, int(a[0]), int(a[1]), sc,
+                               t_lim=(int(p[0]), int(p[1])), q_lim=qlim, want_ops=True)
+        cells += r.cells; done += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    return cells, time.perf_counter() - t0, done
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w, desc = make_workload(args.workload)
+    per_step = max(2.0, min(20.0, 100.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_sample(w, per_step / 4)
+    cells = 0; secs = 0.0; nd = 0
+    for _ in range(args.steps):
+        c, s, d = oracle_sample(w, per_step)
+        cells += c; secs += s; nd += d
+    v = cells / secs / 1e9
+    sample = f"{nd // max(1, args.steps)} of {len(w.anchors)} anchors per step (strided), two-sided extension with CIGAR, 1 thread"
+    print(json.dumps({"impl": "reference", "metric": "ydrop_gcups", "value": v, "unit": "GCUPS", "n_gpus": args.gpus,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(1, args.steps),
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+                      "config": {"workload": f"{args.workload}: {desc}"},
+                      "cpu_baseline": {"value": v, "unit": "GCUPS", "cores": 1, "kind": "oracle", "sample": sample},
+                      "e2e": {"value": v, "unit": "GCUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c4", "c3s", "c5s"])
+    ap.add_argument("--flags", default="cigar", choices=["cigar", "score"])
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--limit-anchors", type=int, default=0, help="profiling aid: keep every k-th anchor so that N remain")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as entry
+    from paper_2606_06811_b200 import binding as B, sassinfo
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    entry.build()
+
+    w, desc = make_workload(args.workload)
+    if args.limit_anchors and args.limit_anchors < len(w.anchors):
+        w.anchors = w.anchors[:: len(w.anchors) // args.limit_anchors][: args.limit_anchors]
+        desc += f" [profiling subset: {len(w.anchors)} anchors]"
+    n = len(w.anchors)
+    flags = B.WANT_CIGAR if args.flags == "cigar" else B.SCORE_ONLY
+    free_b, _ = torch.cuda.mem_get_info(dev)
+    scratch = min(SCRATCH_GB[args.workload] << 30, int(free_b * 0.6))
+    sfe = B.Sfe(local, scratch)
+    sc = B.scoring()
+
+    # device-resident inputs
+    t_ascii = torch.from_numpy(w.target_ascii().copy()).to(dev)
+    q_ascii = torch.from_numpy(w.query_ascii().copy()).to(dev)
+    anchors_np = B.make_anchors(w.anchors); pairs_np = B.make_pairs(w.pairs)
+    anchors = B._dev(anchors_np, dev); pairs = B._dev(pairs_np, dev)
+    acc = torch.zeros((n + 1) * B.BOX_DT.itemsize, dtype=torch.uint8, device=dev)
+    nacc = torch.zeros(1, dtype=torch.int64, device=dev)
+    stats = torch.zeros(B.STATS_DT.itemsize, dtype=torch.uint8, device=dev)
+    cigar_cap = max(1 << 20, 96 * n)
+    state = {}
+
+    def step():
+        nacc.zero_(); stats.zero_()
+        tp = sfe.pack(t_ascii, with_rc=False)
+        qp = sfe.pack(q_ascii, with_rc=True)
+        res, pool, used = sfe.ydrop_batch(tp[:2], len(w.target), qp, len(w.query), pairs, len(w.pairs), anchors, n, sc, flags,
+                                          cigar_cap)
+        keep = sfe.resolve(anchors, res, n, sc.min_score, acc, n + 1, nacc, stats)
+        state.update(res=res, keep=keep)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    barrier()
+    info0 = sfe.last_batch_info()
+    st = stats.cpu().numpy().view(B.STATS_DT)[0]
+    cells_step = int(st["cells_total"]); kept_step = int(st["n_kept"]); covered_step = int(st["n_covered"])
+    cells_cov = int(st["cells_covered"])
+
+    sampler = ClockSampler(local)
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    kernel_us = 0.0; launches = 0
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+        inf = sfe.last_batch_info()
+        kernel_us += inf["ydrop_kernel_us"]
+        launches += inf["launches"] * 3 + 9      # ydrop + join + scan/emit per pass; pack x3, tickets x3, resolve x2, memset
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    tot_cells = torch.tensor([float(cells_step * args.steps)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX); dist.all_reduce(tot_cells, op=dist.ReduceOp.SUM)
+    ms = float(t.item())
+    gcups = float(tot_cells.item()) / (ms * 1e-3) / 1e9
+
+    # e2e: host buffers through the C ABI, H2D/D2H inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        t_host = torch.from_numpy(w.target_ascii().copy()).pin_memory().numpy()
+        q_host = torch.from_numpy(w.query_ascii().copy()).pin_memory().numpy()
+        for _ in range(2):
+            ho = sfe.extend_host(t_host, q_host, pairs_np, anchors_np, sc, flags, cigar_cap)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            ho = sfe.extend_host(t_host, q_host, pairs_np, anchors_np, sc, flags, cigar_cap)
+        torch.cuda.synchronize(dev)
+        dt = time.perf_counter() - t0
+        h2d = len(t_host) + len(q_host) + anchors_np.nbytes + pairs_np.nbytes
+        d2h = n * B.RESULT_DT.itemsize + n + 4 * int(ho["cigar_used"]) + B.STATS_DT.itemsize + 8
+        e2e_cells = int(ho["stats"]["cells_total"]) * args.steps * world
+        e2e = {"value": e2e_cells / dt / 1e9, "unit": "GCUPS", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "ms_per_step": 1e3 * dt / args.steps, "kept_per_s": int(ho["stats"]["n_kept"]) * args.steps / dt}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # roofline of the dominant kernel (integer issue)
+    hl = sassinfo.hot_loop(traceback=bool(flags & B.WANT_CIGAR))
+    r_alu, _ = sfe.probe_int_issue(1, 20000); r_dpx, _ = sfe.probe_int_issue(2, 20000)
+    r_fma, _ = sfe.probe_int_issue(3, 20000); r_mix, _ = sfe.probe_int_issue(0, 20000)
+    f_mhz = clocks.get("sm_mhz") or 1965.0
+    fmax = clocks.get("sm_max_mhz") or 1965.0
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    # probe rates are per max-clock cycle; the limiting resource per cell:
+    r_alu_eff = min(r_alu, r_dpx)
+    cyc_per_cell = max(hl["alu"] / r_alu_eff, hl["fma"] / r_fma, hl["per_cell"] / max(r_mix, r_alu_eff))
+    peak_gcups = n_sm * fmax * 1e6 / cyc_per_cell / 1e9
+    k_gcups = cells_step * args.steps / (kernel_us * 1e-6) / 1e9 if kernel_us > 0 else None
+    roof = {"bound": "alu", "achieved": k_gcups, "peak": peak_gcups, "unit": "GCUPS", "frac": (k_gcups / peak_gcups) if k_gcups else None,
+            "traffic": None, "kernel": "ydrop_kernel<%s>" % ("traceback" if flags else "score-only"),
+            "kernel_share_of_step": kernel_us * 1e-3 / ms,
+            "detail": {"instr_per_cell_sass": hl["per_cell"], "alu_per_cell": hl["alu"], "fma_per_cell": hl["fma"],
+                       "lsu_per_cell": hl["lsu"], "R_alu": r_alu, "R_dpx": r_dpx, "R_imad": r_fma, "R_mixed": r_mix,
+                       "R_unit": "lane-instr/clk/SM at sm_max_mhz", "n_sm": n_sm, "f_mhz_used": fmax,
+                       "f_mhz_sampled": f_mhz, "peak_source": "measured by sfe_probe_int_issue in this run",
+                       "tb_bytes_per_step": info0["tb_bytes"], "tb_gbs": info0["tb_bytes"] * args.steps / (kernel_us * 1e-6) / 1e9 if kernel_us else None,
+                       "lane_efficiency": cells_step / (32.0 * info0["steps"]) if info0["steps"] else None}}
+
+    oc, osec, od = oracle_sample(w, args.cpu_seconds)
+    cpu = {"value": oc / osec / 1e9, "unit": "GCUPS", "cores": 1, "kind": "oracle",
+           "sample": f"{od} of {n} anchors (strided), two-sided extension with CIGAR, {osec:.1f} s"}
+
+    line = {"metric": "ydrop_gcups", "value": gcups, "unit": "GCUPS", "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "l2": "inputs+traceback per step exceed L2 (126 MB)",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU", "scoring": "HOXD70/400/30/ydrop 9400/lag 32/tau 3000"},
+            "kept_alignments_per_s": kept_step * args.steps * world / (ms * 1e-3),
+            "kept": kept_step, "cells_per_step": cells_step,
+            "speculation_waste": {"ext": covered_step / n if n else None, "cells": cells_cov / cells_step if cells_step else None},
+            "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roof, "cpu_baseline": cpu,
+            "batch_info": info0}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -154,7 +154,8 @@ int sfe_extend_host(sfe_ctx *ctx, const char *t_ascii_host, int64_t t_len, const
  * (VIADDMNMX/VIMNMX3), 3 = IMAD only.  sfe_last_batch_info returns counters of the most recent
  * sfe_ydrop_batch on this ctx: [0] kernel launches, [1] halves run, [2] halves re-run after a
  * traceback overflow, [3] traceback bytes written, [4] DP steps (warp wavefronts) executed,
- * [5] halves that took the wide path. */
+ * [5] halves that took the wide path, [6] device time of the Y-drop kernel launches in microseconds
+ * (CUDA events on the ctx stream; synchronises on the last one). */
 int sfe_probe_int_issue(sfe_ctx *ctx, int mix, int iters, double *lane_ops_per_clk_per_sm, double *elapsed_ms);
 int sfe_last_batch_info(sfe_ctx *ctx, int64_t info[8]);
 

@@ -226,7 +226,7 @@ class Sfe:
     def last_batch_info(self):
         a = (C.c_int64 * 8)()
         _check(lib().sfe_last_batch_info(self.h, a), "sfe_last_batch_info")
-        keys = ("launches", "halves", "halves_rerun", "tb_bytes", "steps", "wide", "r6", "r7")
+        keys = ("launches", "halves", "halves_rerun", "tb_bytes", "steps", "wide", "ydrop_kernel_us", "r7")
         return dict(zip(keys, list(a)))
 
 

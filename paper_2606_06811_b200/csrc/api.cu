@@ -49,6 +49,8 @@ struct sfe_ctx {
     // host-API staging
     DevBuf h_tascii, h_qascii, h_t2, h_tm, h_q2, h_qm, h_r2, h_rm, h_pairs, h_anchors, h_results, h_keep, h_cigar, h_acc, h_small;
     long long info[8];
+    cudaEvent_t ev0, ev1; bool ev_pending;
+    double kernel_us;
 };
 
 static char g_err_detail[512] = "";
@@ -58,6 +60,8 @@ void sfe_note_cuda_error(cudaError_t e, const char *file, int line)
     cudaGetLastError();
 }
 extern "C" const char *sfe_last_error_detail(void) { return g_err_detail; }
+
+static void harvest_kernel_time(sfe_ctx *c);
 
 static const char *const k_errs[] = {"ok", "invalid argument", "out of memory", "CUDA error", "value outside supported range"};
 
@@ -88,6 +92,8 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
     c->n_chunks = (int)nch;
     c->pool = nullptr; c->chunk_prev = nullptr; c->counters = nullptr; c->counters_host = nullptr;
     memset(c->info, 0, sizeof c->info);
+    c->ev_pending = false; c->kernel_us = 0.0;
+    if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) { delete c; return SFE_ECUDA; }
     if (cudaMalloc((void **)&c->pool, (size_t)nch * SFE_CHUNK_BYTES) != cudaSuccess ||
         cudaMalloc((void **)&c->chunk_prev, (size_t)nch * sizeof(int32_t)) != cudaSuccess ||
         cudaMalloc((void **)&c->counters, CNT_N * sizeof(unsigned long long)) != cudaSuccess ||
@@ -108,6 +114,7 @@ extern "C" int sfe_destroy(sfe_ctx *c)
     if (c->chunk_prev) cudaFree(c->chunk_prev);
     if (c->counters) cudaFree(c->counters);
     if (c->counters_host) cudaFreeHost(c->counters_host);
+    cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1);
     DevBuf *bufs[] = {&c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
                       &c->h_t2, &c->h_tm, &c->h_q2, &c->h_qm, &c->h_r2, &c->h_rm, &c->h_pairs, &c->h_anchors, &c->h_results,
                       &c->h_keep, &c->h_cigar, &c->h_acc, &c->h_small};
@@ -156,7 +163,35 @@ extern "C" int sfe_probe_int_issue(sfe_ctx *c, int mix, int iters, double *lane_
 extern "C" int sfe_last_batch_info(sfe_ctx *c, int64_t info[8])
 {
     if (!c || !info) return SFE_EINVAL;
+    harvest_kernel_time(c);
+    c->info[6] = (long long)(c->kernel_us + 0.5);
+    if (c->info[4] == 0) {   // score-only batches do not read the counters back inside the call
+        if (cudaMemcpyAsync(c->counters_host, c->counters, CNT_N * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream) == cudaSuccess &&
+            cudaStreamSynchronize(c->stream) == cudaSuccess) { c->info[4] = (long long)c->counters_host[CNT_STEPS]; c->info[5] = (long long)c->counters_host[CNT_WIDE]; }
+        else cudaGetLastError();
+    }
     for (int k = 0; k < 8; k++) info[k] = c->info[k];
+    return SFE_OK;
+}
+
+// add the device time of the last timed ydrop launch to kernel_us (needs the stream to have passed ev1)
+static void harvest_kernel_time(sfe_ctx *c)
+{
+    if (!c->ev_pending) return;
+    float ms = 0.f;
+    if (cudaEventSynchronize(c->ev1) == cudaSuccess && cudaEventElapsedTime(&ms, c->ev0, c->ev1) == cudaSuccess) c->kernel_us += 1e3 * (double)ms;
+    else cudaGetLastError();
+    c->ev_pending = false;
+}
+
+static int timed_ydrop(sfe_ctx *c, const YdParams &p, bool want_tb)
+{
+    harvest_kernel_time(c);
+    SFE_CUDA_CHECK(cudaEventRecord(c->ev0, c->stream));
+    const int rc = sfe_launch_ydrop(p, want_tb, c->n_sm, c->stream);
+    if (rc) return rc;
+    SFE_CUDA_CHECK(cudaEventRecord(c->ev1, c->stream));
+    c->ev_pending = true;
     return SFE_OK;
 }
 
@@ -190,6 +225,7 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
     if (2 * n_anchors > 0x7ffffff0LL) return SFE_ELIMIT;
     SFE_CUDA_CHECK(cudaSetDevice(c->device));
     memset(c->info, 0, sizeof c->info);
+    c->ev_pending = false; c->kernel_us = 0.0;
     if (cigar_pool_used_dev) SFE_CUDA_CHECK(cudaMemsetAsync(cigar_pool_used_dev, 0, sizeof(int64_t), c->stream));
     if (n_anchors == 0) return SFE_OK;
 
@@ -218,7 +254,7 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
     SFE_CUDA_CHECK(cudaMemsetAsync(c->counters, 0, CNT_N * sizeof(unsigned long long), c->stream));
     if ((rc = sfe_launch_tickets(anchors_dev, n_anchors, pairs_dev, n_pairs, q_len, !(flags & SFE_NO_BINNING),
                                  (unsigned int *)c->hist.p, (int32_t *)c->tickets.p, c->stream))) return rc;
-    if ((rc = sfe_launch_ydrop(p, want_tb, c->n_sm, c->stream))) return rc;
+    if ((rc = timed_ydrop(c, p, want_tb))) return rc;
     c->info[0] += 1; c->info[1] += 2 * n_anchors;
     if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, nullptr, n_anchors, c->pool, c->chunk_prev, want_tb,
                               results_dev, c->stream))) return rc;
@@ -249,7 +285,7 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
         const long long n_sel = (long long)c->counters_host[CNT_RERUN];
         if (n_sel <= 0) break;
         p.n_tickets = 2 * n_sel;
-        if ((rc = sfe_launch_ydrop(p, true, c->n_sm, c->stream))) return rc;
+        if ((rc = timed_ydrop(c, p, true))) return rc;
         c->info[0] += 1; c->info[1] += 2 * n_sel; c->info[2] += 2 * n_sel;
         if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, (const long long *)c->sel.p, n_sel, c->pool,
                                   c->chunk_prev, 1, results_dev, c->stream))) return rc;
