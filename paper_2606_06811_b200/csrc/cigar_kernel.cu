@@ -48,15 +48,15 @@ static __device__ int walk_half(const sfe_half &h, const uint32_t *pool, const i
         const int lane = i & 31;
         const int t = j - cs + lane;
         const uint32_t w = cur.rec(hdr + 1 + (t >> 3))[lane];
-        const uint32_t nib = (w >> ((t & 7) * 4)) & 15u;
+        const uint32_t nib = (w >> ((7 - (t & 7)) * 4)) & 15u;   // bit3 !M, bit2 !E, bit1 E ext, bit0 F ext
         int op = -1;
         if (state == 0) {
-            if (!(nib & 1u)) { op = SFE_OP_M; i--; j--; }
-            else state = (nib & 2u) ? 2 : 1;
+            if (!(nib & 8u)) { op = SFE_OP_M; i--; j--; }
+            else state = (nib & 4u) ? 2 : 1;
         } else if (state == 1) {
-            op = SFE_OP_I; i--; if (!(nib & 4u)) state = 0;
+            op = SFE_OP_I; i--; if (!(nib & 2u)) state = 0;
         } else {
-            op = SFE_OP_D; j--; if (!(nib & 8u)) state = 0;
+            op = SFE_OP_D; j--; if (!(nib & 1u)) state = 0;
         }
         if (op >= 0) {
             if (op == cur_op) run++;

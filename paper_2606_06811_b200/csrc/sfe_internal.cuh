@@ -18,7 +18,7 @@
 #define SFE_RING 1024                               // boundary-ring capacity in columns
 #define SFE_EXCH_BYTES 256                          // 32 lanes x 8 B
 #define SFE_ROW_STRIDE (SFE_EXCH_BYTES + SFE_RING)  // bytes: exchange area + RING/8 segments x 8 B
-#define SFE_SELRING 1024                            // selector ring capacity in columns
+#define SFE_SELRING 1024                            // selector ring capacity in columns (>= SFE_MAX_STEPS + 160: the next strip re-reads the window start)
 #define SFE_WARP_SMEM (8 * SFE_ROW_STRIDE + (SFE_SELRING + 8) * 2)
 #define SFE_MAX_STEPS (SFE_RING - 160)              // a strip wider than this takes the wide path
 

@@ -18,6 +18,7 @@
 #include "sfe_internal.cuh"
 
 #define FULL 0xffffffffu
+#define SFE_BLOCK_THREADS 192     // 6 warps x 12.3 KB of shared memory; 3 blocks = 18 warps per SM
 #define ST_PASS_OVERFLOW 0x100u   // internal: traceback arena ran out during this pass
 
 // PRMT with the sign-replicate selector mode (bit 3 of a selector nibble), which __byte_perm masks off
@@ -70,29 +71,69 @@ static __device__ __forceinline__ void fill_bnd_neg(char *wbase, int lo, int hi,
 
 struct TbWriter {
     uint32_t *pool; int32_t *chunk_prev; unsigned long long *counters; int n_chunks;
+    uint32_t *ptr;          // this lane's word of the next record
+    int left;               // records left in the current chunk
     int cur_chunk; int nrec; bool ok;
     __device__ __forceinline__ void put(uint32_t word, int lane)
     {
         if (!ok) return;
-        if ((nrec & (SFE_CHUNK_RECS - 1)) == 0) {
+        if (left == 0) {
             int c = 0;
             if (lane == 0) c = (int)atomicAdd(&counters[CNT_CHUNK], 1ULL);
             c = __shfl_sync(FULL, c, 0);
             if (c >= n_chunks) { ok = false; return; }
             if (lane == 0) chunk_prev[c] = cur_chunk;
             cur_chunk = c;
+            ptr = pool + (size_t)c * SFE_CHUNK_RECS * 32 + lane;
+            left = SFE_CHUNK_RECS;
         }
-        pool[((size_t)cur_chunk * SFE_CHUNK_RECS + (nrec & (SFE_CHUNK_RECS - 1))) * 32 + lane] = word;
-        nrec++;
+        *ptr = word;
+        ptr += 32; left--; nrec++;
     }
 };
 
+// Integer adds forced onto the FMA pipe (IMAD): the ALU pipe is the binding resource of this kernel
+// (profiles/r1_01), the FMA pipe is otherwise idle.
+static __device__ __forceinline__ int fma_add(int a, int b)
+{
+    int r;
+    asm("mad.lo.s32 %0, %1, 1, %2;" : "=r"(r) : "r"(a), "r"(b));
+    return r;
+}
+// (a & ~b) | (c & b) in one LOP3
+static __device__ __forceinline__ int lop3_sel(int a, int b, int c)
+{
+    int r;
+    asm("lop3.b32 %0, %1, %2, %3, 0xB8;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+    return r;
+}
+static __device__ __forceinline__ int fma_mad(int a, int b, int c)   // a * b + c
+{
+    int r;
+    asm("mad.lo.s32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+    return r;
+}
+static __device__ __forceinline__ int fma_sub(int a, int b)      // a - b
+{
+    int r;
+    asm("mad.lo.s32 %0, %1, -1, %2;" : "=r"(r) : "r"(b), "r"(a));
+    return r;
+}
+// acc = (acc << 1) | (sign bit of x): one SHF.L.W
+static __device__ __forceinline__ uint32_t shift_in_sign(uint32_t acc, int x) { return __funnelshift_l((uint32_t)x, acc, 1); }
+
 // One group of 8 wavefront steps.  Everything indexed by k is an immediate after unrolling.
+// Per cell the ALU pipe sees: PRMT, IADD3 (M), 2 x VIADDMNMX (E, F), VIMNMX3 (H), SHF + LOP3 (alive gate),
+// 4 x SHF (traceback bits), SHF + VIMNMX (best); the FMA pipe sees the 8 subtractions / shift-adds.
+// Traceback nibble of step k sits at bits 4(7-k)..4(7-k)+3 of acc:
+//   bit3 = H not from M, bit2 = H not from E, bit1 = E extended, bit0 = F extended (R11).
+// gneg = -(dead-bit pattern): gneg' = 2 gneg + g with g = 0 (alive) / -1 (dead); step k at bit 7-k of -gneg.
+// bm shifts in one bit per step: 1 iff that step raised the lane-local best (strict '>', R7).
 template <bool TB, bool EDGE>
-static __device__ __forceinline__ void run_group8(int &upH, int &upE, int &dg, int &F, int &Hgl, int &best, int &best_t,
-                                                  uint32_t &acc, uint32_t &ga, const uint32_t srow_lo,
-                                                  const uint32_t srow_hi, const int T, const int OX, const int X,
-                                                  const char *rptr, char *wptr, const uint16_t *selp, const int t0,
+static __device__ __forceinline__ void run_group8(int &upH, int &upE, int &dg, int &F, int &Hgl, int &best, uint32_t &bm,
+                                                  uint32_t &acc, int &gneg, const uint32_t srow_lo,
+                                                  const uint32_t srow_hi, const int T, const int OX, const int tox,
+                                                  const int X, const char *rptr, char *wptr, const uint16_t *selp,
                                                   const int col0, const int m)
 {
 #pragma unroll
@@ -104,17 +145,19 @@ static __device__ __forceinline__ void run_group8(int &upH, int &upE, int &dg, i
         const int Fn = __viaddmax_s32(F, -X, Hgl);         // Hgl = H(i,j-1) - OX (ungated: R6 lemma)
         int H = __vimax3_s32(M, E, Fn);
         if (EDGE) { if (col0 + k > m) H = SFE_NEG; }       // beyond the target end
-        const int Hg = H - OX;
-        const bool alive = H >= T;
+        const int d = fma_sub(H, T);                       // alive <=> d >= 0 (R5)
+        const int Hg = fma_add(d, tox);                    // H - OX, as d + (T - OX) so that it stays an IMAD
+        const int gmask = d >> 31;                         // 0 alive, -1 dead
         if (TB) {
-            // R11: bit0 = H not from M, bit1 = H not from E, bit2 = E extended, bit3 = F extended
-            const uint32_t nib = (uint32_t)(H != M) | ((uint32_t)(H != E) << 1) | ((uint32_t)(E != upH) << 2) |
-                                 ((uint32_t)(Fn != Hgl) << 3);
-            acc |= nib << (4 * k);
+            acc = shift_in_sign(acc, fma_sub(M, H));       // M < H  <=> H not from M
+            acc = shift_in_sign(acc, fma_sub(E, H));       // E < H  <=> H not from E
+            acc = shift_in_sign(acc, fma_sub(upH, E));     // upH < E <=> E extended (open wins ties)
+            acc = shift_in_sign(acc, fma_sub(Hgl, Fn));    // Hgl < F <=> F extended
         }
-        if (alive) ga |= 1u << k;
-        if (H > best) { best = H; best_t = t0 + k; }       // R7: strict, lane-local order is row-major
-        const int msgH = alive ? Hg : SFE_NEG;
+        gneg = fma_mad(gneg, 2, gmask);
+        bm = shift_in_sign(bm, fma_sub(best, H));          // best < H <=> new lane-local best
+        best = max(best, H);
+        const int msgH = lop3_sel(Hg, gmask, SFE_NEG);     // one LOP3: dead cells send NEG
         *(int2 *)(wptr + k * SFE_ROW_STRIDE) = make_int2(msgH, E);
         dg = upH; F = Fn; Hgl = Hg;
         __syncwarp();
@@ -158,7 +201,7 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
     const int OX = p.OX, X = p.X;
     TbWriter tb;
     tb.pool = p.pool; tb.chunk_prev = p.chunk_prev; tb.counters = p.counters; tb.n_chunks = p.n_chunks;
-    tb.cur_chunk = -1; tb.nrec = 0; tb.ok = TB;
+    tb.cur_chunk = -1; tb.nrec = 0; tb.ok = TB; tb.ptr = nullptr; tb.left = 0;
 
     int best = 0, best_i = 0, best_j = 0;     // lane-local first maximum
     int cumA = 0, cumB = 0;                    // lane-local best through the previous strip / the one before
@@ -183,12 +226,13 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) ab = max(ab, __shfl_xor_sync(FULL, ab, o));
         const int B = max(pm, ab);
-        const int T = !active ? 0x7fffffff : (p.ydrop_inf ? SFE_T_INF : B - p.Y);
+        const int T = !active ? (1 << 29) : (p.ydrop_inf ? SFE_T_INF : B - p.Y);   // rows beyond the query: never alive (scores < 2^29, R25)
         uint32_t srow_lo;
         if (!active) srow_lo = 0x80808080u;
         else if (r == 0) srow_lo = 0u;
         else srow_lo = p.srow[sfe_base(g.qc, g.qm, g.q0 + (long long)g.d * r)];
         const uint32_t srow_hi = p.srow_hi;
+        const int tox = T - OX;
 
         if (TB) {   // strip header record: word0 = cs, word1 = previous header's record index
             const int hdr = tb.nrec;
@@ -205,36 +249,43 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
             upH = u.x; upE = u.y;
             if (s == 0) dg = -OX;                           // R8: H(0,0) = 0 enters as the diagonal of (0,0)
         }
-        int first = 0x7fffffff, last = -1, best_t = -1;
+        int first_t = 0x7fffffff, last_t = -1, best_t = -1;   // step indices of the first / last alive cell of my row
+        uint32_t bm = 0;
         const int best_before = best;
         int t0 = 0;
         bool bail = false;
+        const bool is0 = lane == 0, is31 = lane == 31;
+        char *const exch_w = wsm + lane * 8;
+        const char *const exch_r = wsm + (lane - 1) * 8;
+        char *const bnd = wsm + SFE_EXCH_BYTES;
+        int gneg = 0;
         for (;; t0 += 8) {
             const int cmax = cs + t0 + 7;                   // lane 0's last column of this group
             if (sel_hi <= cmax) { fill_sel(selring, g, sel_hi, cmax + 129, lane); sel_hi = cmax + 129; }
             if (bnd_valid <= cmax + 1) { fill_bnd_neg(wsm, bnd_valid, bnd_valid + 64, lane); bnd_valid += 64; }
             const int base8 = (cs + t0) >> 3;
-            const char *rptr = (lane == 0) ? wsm + SFE_EXCH_BYTES + ((base8 + 1) & (SFE_RING / 8 - 1)) * 8
-                                           : wsm + (lane - 1) * 8;
-            char *wptr = (lane == 31) ? wsm + SFE_EXCH_BYTES + ((base8 - 3) & (SFE_RING / 8 - 1)) * 8 : wsm + lane * 8;
+            const char *rptr = is0 ? bnd + ((base8 + 1) & (SFE_RING / 8 - 1)) * 8 : exch_r;
+            char *wptr = is31 ? bnd + ((base8 - 3) & (SFE_RING / 8 - 1)) * 8 : exch_w;
             const int col0 = cs + t0 - lane;
             const uint16_t *selp = selring + (col0 & (SFE_SELRING - 1));
-            uint32_t acc = 0, ga = 0;
+            uint32_t acc = 0;
             if (cmax > g.m)
-                run_group8<TB, true>(upH, upE, dg, F, Hgl, best, best_t, acc, ga, srow_lo, srow_hi, T, OX, X, rptr, wptr,
-                                     selp, t0, col0, g.m);
+                run_group8<TB, true>(upH, upE, dg, F, Hgl, best, bm, acc, gneg, srow_lo, srow_hi, T, OX, tox, X, rptr, wptr,
+                                     selp, col0, g.m);
             else
-                run_group8<TB, false>(upH, upE, dg, F, Hgl, best, best_t, acc, ga, srow_lo, srow_hi, T, OX, X, rptr, wptr,
-                                      selp, t0, col0, g.m);
+                run_group8<TB, false>(upH, upE, dg, F, Hgl, best, bm, acc, gneg, srow_lo, srow_hi, T, OX, tox, X, rptr, wptr,
+                                      selp, col0, g.m);
             if (TB) tb.put(acc, lane);
-            if (ga) {
-                if (first == 0x7fffffff) first = col0 + __ffs(ga) - 1;
-                last = col0 + 31 - __clz(ga);
+            const uint32_t al = ~(uint32_t)(-gneg) & 0xffu; // alive bits of this group, step k at bit 7-k
+            if (bm & 0xffu) best_t = t0 + 8 - __ffs(bm & 0xffu);   // the latest strict increase of this group
+            if (al) {
+                first_t = min(first_t, t0 + __clz(al) - 24);
+                last_t = t0 + 8 - __ffs(al);
             }
-            const bool any = __any_sync(FULL, ga != 0);
-            if (!any && cs + t0 + 8 > prevR + 1) { t0 += 8; break; }
+            if (!__any_sync(FULL, al != 0) && cs + t0 + 8 > prevR + 1) { t0 += 8; break; }
             if (t0 + 8 >= SFE_MAX_STEPS) { t0 += 8; bail = true; break; }
         }
+        const int first = last_t < 0 ? 0x7fffffff : cs - lane + first_t, last = last_t < 0 ? -1 : cs - lane + last_t;
         total_steps += t0;
         if (t0 > max_steps) max_steps = t0;
         if (bail) { wide = true; break; }
@@ -274,7 +325,7 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
 
 // Persistent kernel: every warp pulls anchor-half tickets from one atomic counter (a3).
 template <bool TB>
-__global__ void __launch_bounds__(128) ydrop_kernel(const YdParams p)
+__global__ void __launch_bounds__(SFE_BLOCK_THREADS) ydrop_kernel(const YdParams p)
 {
     extern __shared__ __align__(16) char smem[];
     const int lane = sfe_lane();
@@ -291,7 +342,7 @@ __global__ void __launch_bounds__(128) ydrop_kernel(const YdParams p)
 
 int sfe_launch_ydrop(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st)
 {
-    const int warps_per_block = 4;
+    const int warps_per_block = SFE_BLOCK_THREADS / 32;
     const size_t smem = (size_t)warps_per_block * SFE_WARP_SMEM;
     static bool attr_done = false;
     if (!attr_done) {
@@ -300,14 +351,14 @@ int sfe_launch_ydrop(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st)
         attr_done = true;
     }
     int bps = 0;
-    if (want_tb) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<true>, 128, smem);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<false>, 128, smem);
+    if (want_tb) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<true>, SFE_BLOCK_THREADS, smem);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<false>, SFE_BLOCK_THREADS, smem);
     if (bps < 1) return SFE_ECUDA;
     long long blocks = (long long)n_sm * bps;
     const long long need = (p.n_tickets + warps_per_block - 1) / warps_per_block;
     if (blocks > need) blocks = need;
     if (blocks < 1) blocks = 1;
-    if (want_tb) ydrop_kernel<true><<<(unsigned)blocks, 128, smem, st>>>(p);
-    else ydrop_kernel<false><<<(unsigned)blocks, 128, smem, st>>>(p);
+    if (want_tb) ydrop_kernel<true><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
+    else ydrop_kernel<false><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
     SFE_LAUNCH_CHECK();
 }
