@@ -48,9 +48,10 @@ enum {
 /* per-anchor status bits (sfe_result.status) */
 #define SFE_ST_TB_OVERFLOW 1u         /* traceback arena exhausted even when run alone: no CIGAR */
 #define SFE_ST_CIGAR_OVERFLOW 2u      /* cigar pool too small: ops not written (n_ops is valid)   */
-#define SFE_ST_WIDE 4u                /* a half took the wide-band (global-memory ring) path     */
+#define SFE_ST_WIDE 4u                /* informational: a half took the wide-band (global ring) path */
 #define SFE_ST_SCORE_LIMIT 8u         /* R25: |score| would exceed 2^29                           */
-#define SFE_ST_BAD_ANCHOR 16u         /* anchor outside its pair's limits: nothing computed      */
+#define SFE_ST_BAD_ANCHOR 16u
+#define SFE_ST_BAND_LIMIT 32u          /* live band wider than 65,376 columns: half not computed    */         /* anchor outside its pair's limits: nothing computed      */
 
 /* CIGAR op word: (length << 4) | code ; M = aligned pair, I = query base vs gap, D = target base
  * vs gap (R12). */

@@ -19,7 +19,7 @@ OK, EINVAL, ENOMEM, ECUDA, ELIMIT = 0, -1, -2, -3, -4
 YDROP_INF = 0x7FFFFFFF
 PRUNE_LAG = 32
 WANT_CIGAR, SCORE_ONLY, NO_BINNING = 1, 0, 2
-ST_TB_OVERFLOW, ST_CIGAR_OVERFLOW, ST_WIDE, ST_SCORE_LIMIT, ST_BAD_ANCHOR = 1, 2, 4, 8, 16
+ST_TB_OVERFLOW, ST_CIGAR_OVERFLOW, ST_WIDE, ST_SCORE_LIMIT, ST_BAD_ANCHOR, ST_BAND_LIMIT = 1, 2, 4, 8, 16, 32
 OP_M, OP_I, OP_D = 0, 1, 2
 
 EXPORTS = ("sfe_create", "sfe_destroy", "sfe_strerror", "sfe_last_error_detail", "sfe_pack", "sfe_ydrop_batch", "sfe_resolve",

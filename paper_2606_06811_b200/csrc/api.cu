@@ -45,7 +45,7 @@ struct sfe_ctx {
     uint32_t *pool; int32_t *chunk_prev; int n_chunks;
     unsigned long long *counters;     // device, CNT_N
     unsigned long long *counters_host;  // pinned
-    DevBuf halves, tickets, sel, hist, blkmin, act, misc;
+    DevBuf halves, tickets, sel, hist, blkmin, act, misc, wide_tickets, wide_ring;
     // host-API staging
     DevBuf h_tascii, h_qascii, h_t2, h_tm, h_q2, h_qm, h_r2, h_rm, h_pairs, h_anchors, h_results, h_keep, h_cigar, h_acc, h_small;
     long long info[8];
@@ -115,7 +115,7 @@ extern "C" int sfe_destroy(sfe_ctx *c)
     if (c->counters) cudaFree(c->counters);
     if (c->counters_host) cudaFreeHost(c->counters_host);
     cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1);
-    DevBuf *bufs[] = {&c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
+    DevBuf *bufs[] = {&c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
                       &c->h_t2, &c->h_tm, &c->h_q2, &c->h_qm, &c->h_r2, &c->h_rm, &c->h_pairs, &c->h_anchors, &c->h_results,
                       &c->h_keep, &c->h_cigar, &c->h_acc, &c->h_small};
     for (DevBuf *b : bufs) b->release();
@@ -232,6 +232,8 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
     if ((rc = c->halves.ensure((size_t)(2 * n_anchors) * sizeof(sfe_half)))) return rc;
     if ((rc = c->tickets.ensure((size_t)(2 * n_anchors) * sizeof(int32_t)))) return rc;
     if ((rc = c->hist.ensure(64 * sizeof(unsigned int)))) return rc;
+    if ((rc = c->wide_tickets.ensure((size_t)(2 * n_anchors) * sizeof(int32_t)))) return rc;
+    if ((rc = c->wide_ring.ensure((size_t)SFE_WIDE_WARPS * RingGeom<SFE_WIDE_RING_LOG2>::WARP_BYTES))) return rc;
     if (want_tb && (rc = c->sel.ensure((size_t)n_anchors * sizeof(long long)))) return rc;
 
     YdParams p;
@@ -241,6 +243,7 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
     p.pairs = pairs_dev; p.anchors = anchors_dev; p.tickets = (const int32_t *)c->tickets.p; p.n_tickets = 2 * n_anchors;
     p.counters = c->counters; p.halves = (sfe_half *)c->halves.p; p.pool = c->pool; p.chunk_prev = c->chunk_prev;
     p.n_chunks = want_tb ? c->n_chunks : 0; p.n_pairs = n_pairs;
+    p.wide_ring = (char *)c->wide_ring.p; p.wide_tickets = (int32_t *)c->wide_tickets.p;
     p.OX = sc->gap_open + sc->gap_extend; p.X = sc->gap_extend;
     p.ydrop_inf = sc->ydrop == SFE_YDROP_INF; p.Y = p.ydrop_inf ? 0 : sc->ydrop;
     for (int a = 0; a < 4; a++) {

@@ -87,7 +87,7 @@ __global__ void join_count_kernel(const sfe_anchor *anchors, const sfe_half *hal
     r.cells = f.cells + b.cells;
     r.cigar_off = -1; r.n_ops = 0; r.n_ops_back = 0;
     int nf = 0;
-    if (want_cigar && !(st & (ST_PASS_OVERFLOW | SFE_ST_BAD_ANCHOR | SFE_ST_WIDE))) {
+    if (want_cigar && !(st & (ST_PASS_OVERFLOW | SFE_ST_BAD_ANCHOR | SFE_ST_BAND_LIMIT))) {
         const int nb = walk_half<false>(b, pool, chunk_prev, nullptr, 0);
         nf = walk_half<false>(f, pool, chunk_prev, nullptr, 0);
         r.n_ops_back = nb; r.n_ops = nb + nf;

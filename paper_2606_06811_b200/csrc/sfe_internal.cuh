@@ -7,6 +7,7 @@
 
 #define SFE_NEG (-(1 << 30))            // "minus infinity" of the DP (R6)
 #define SFE_T_INF (-(1 << 29))          // threshold used for SFE_YDROP_INF (R27): every real cell is above it
+#define SFE_ST_WIDE_PENDING 0x200u    // internal: the strip outgrew the shared-memory window; re-run by the wide kernel
 #define SFE_OOB_SCORE 0xE0000000u       // substitution "score" of a column beyond the target end (-2^29)
 
 // ---- shared-memory geometry of one warp -------------------------
@@ -15,12 +16,21 @@
 // exchange area; the last lane's messages go to the boundary ring that lane 0 of the NEXT strip
 // reads.  Everything is laid out in 8 "rows", one per step of an unrolled group of 8 steps, so
 // that every access in the unrolled loop is base + immediate.
-#define SFE_RING 1024                               // boundary-ring capacity in columns
+// The ring capacity is a template parameter: 2^10 columns in shared memory for the normal kernel,
+// 2^16 columns in global memory (L2) for the wide-band kernel that re-runs the rare halves whose
+// strip exceeds the shared-memory window.
 #define SFE_EXCH_BYTES 256                          // 32 lanes x 8 B
-#define SFE_ROW_STRIDE (SFE_EXCH_BYTES + SFE_RING)  // bytes: exchange area + RING/8 segments x 8 B
-#define SFE_SELRING 1024                            // selector ring capacity in columns (>= SFE_MAX_STEPS + 160: the next strip re-reads the window start)
-#define SFE_WARP_SMEM (8 * SFE_ROW_STRIDE + (SFE_SELRING + 8) * 2)
-#define SFE_MAX_STEPS (SFE_RING - 160)              // a strip wider than this takes the wide path
+#define SFE_RING_LOG2 10
+#define SFE_WIDE_RING_LOG2 16
+template <int RL2> struct RingGeom {
+    static constexpr int RING = 1 << RL2;                        // boundary-ring capacity in columns
+    static constexpr int ROW_STRIDE = SFE_EXCH_BYTES + RING;     // bytes: exchange area + RING/8 segments x 8 B
+    static constexpr int SELRING = RING;                         // selector ring (>= MAX_STEPS + 160: the next strip re-reads the window start)
+    static constexpr int WARP_BYTES = 8 * ROW_STRIDE + (SELRING + 8) * 2;
+    static constexpr int MAX_STEPS = RING - 160;                 // a strip wider than this bails out
+};
+#define SFE_WARP_SMEM (RingGeom<SFE_RING_LOG2>::WARP_BYTES)
+#define SFE_WIDE_WARPS 148                          // warps of the wide-band kernel (one per block)
 
 // ---- traceback arena --------------------------------------------------------------------------
 // Record = 32 lanes x one 32-bit word (8 cells x 4 bits) = 128 B, written coalesced by one warp
@@ -42,7 +52,7 @@ struct sfe_half {                 // result of one one-sided extension (a7)
     int32_t max_steps;            // widest strip
 };
 
-enum { CNT_TICKET = 0, CNT_CHUNK, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_N = 8 };
+enum { CNT_TICKET = 0, CNT_CHUNK, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_N = 16 };
 
 struct YdParams {
     const uint8_t *t_codes, *t_nmask;
@@ -61,8 +71,8 @@ struct YdParams {
     int32_t OX, X, Y, ydrop_inf;
     uint32_t srow[5];             // packed int8 scores of a query base A,C,G,T,N against A,C,G,T
     uint32_t srow_hi;             // bytes: n_score, 0x00, 0xE0 (OOB), 0x00
-    int32_t *wide_ring;           // global-memory boundary rings for the wide path (per warp), or NULL
-    int32_t wide_cols;
+    char *wide_ring;              // global-memory rings of the wide-band kernel: SFE_WIDE_WARPS x RingGeom<16>::WARP_BYTES
+    int32_t *wide_tickets;        // halves that bailed out of the normal kernel in this pass
 };
 
 static __device__ __forceinline__ int sfe_lane() { return threadIdx.x & 31; }

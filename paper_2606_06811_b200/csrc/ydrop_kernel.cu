@@ -29,10 +29,11 @@ static __device__ __forceinline__ int prmt_sx(uint32_t lo, uint32_t hi, uint32_t
     return r;
 }
 
+template <int RL2>
 static __device__ __forceinline__ int bnd_off(int c)
 {
     const int u = c + 7;
-    return (u & 7) * SFE_ROW_STRIDE + SFE_EXCH_BYTES + ((u >> 3) & (SFE_RING / 8 - 1)) * 8;
+    return (u & 7) * RingGeom<RL2>::ROW_STRIDE + SFE_EXCH_BYTES + ((u >> 3) & (RingGeom<RL2>::RING / 8 - 1)) * 8;
 }
 
 struct HalfGeom {
@@ -51,21 +52,23 @@ static __device__ __forceinline__ uint32_t col_selector(const HalfGeom &g, int c
 }
 
 // fill selector-ring entries for columns [lo, hi)
+template <int RL2>
 static __device__ __forceinline__ void fill_sel(uint16_t *selring, const HalfGeom &g, int lo, int hi, int lane)
 {
     for (int c = lo + lane; c < hi; c += 32) {
         const uint16_t v = (uint16_t)col_selector(g, c);
-        const int idx = c & (SFE_SELRING - 1);
+        const int idx = c & (RingGeom<RL2>::SELRING - 1);
         selring[idx] = v;
-        if (idx < 8) selring[idx + SFE_SELRING] = v;
+        if (idx < 8) selring[idx + RingGeom<RL2>::SELRING] = v;
     }
     __syncwarp();
 }
 
 // fill boundary-ring entries for columns [lo, hi) with "dead"
+template <int RL2>
 static __device__ __forceinline__ void fill_bnd_neg(char *wbase, int lo, int hi, int lane)
 {
-    for (int c = lo + lane; c < hi; c += 32) *(int2 *)(wbase + bnd_off(c)) = make_int2(SFE_NEG, SFE_NEG);
+    for (int c = lo + lane; c < hi; c += 32) *(int2 *)(wbase + bnd_off<RL2>(c)) = make_int2(SFE_NEG, SFE_NEG);
     __syncwarp();
 }
 
@@ -129,7 +132,7 @@ static __device__ __forceinline__ uint32_t shift_in_sign(uint32_t acc, int x) { 
 //   bit3 = H not from M, bit2 = H not from E, bit1 = E extended, bit0 = F extended (R11).
 // gneg = -(dead-bit pattern): gneg' = 2 gneg + g with g = 0 (alive) / -1 (dead); step k at bit 7-k of -gneg.
 // bm shifts in one bit per step: 1 iff that step raised the lane-local best (strict '>', R7).
-template <bool TB, bool EDGE>
+template <bool TB, bool EDGE, int RL2, bool GLOBAL>
 static __device__ __forceinline__ void run_group8(int &upH, int &upE, int &dg, int &F, int &Hgl, int &best, uint32_t &bm,
                                                   uint32_t &acc, int &gneg, const uint32_t srow_lo,
                                                   const uint32_t srow_hi, const int T, const int OX, const int tox,
@@ -138,7 +141,7 @@ static __device__ __forceinline__ void run_group8(int &upH, int &upE, int &dg, i
 {
 #pragma unroll
     for (int k = 0; k < 8; k++) {
-        const uint32_t sel = selp[k];
+        const uint32_t sel = GLOBAL ? __ldcg(selp + k) : selp[k];
         const int s = prmt_sx(srow_lo, srow_hi, sel);
         const int M = dg + s + OX;                         // dg = H(i-1,j-1) - OX, or NEG if dead
         const int E = __viaddmax_s32(upE, -X, upH);        // upH = H(i-1,j) - OX, or NEG if dead
@@ -158,18 +161,20 @@ static __device__ __forceinline__ void run_group8(int &upH, int &upE, int &dg, i
         bm = shift_in_sign(bm, fma_sub(best, H));          // best < H <=> new lane-local best
         best = max(best, H);
         const int msgH = lop3_sel(Hg, gmask, SFE_NEG);     // one LOP3: dead cells send NEG
-        *(int2 *)(wptr + k * SFE_ROW_STRIDE) = make_int2(msgH, E);
+        *(int2 *)(wptr + k * RingGeom<RL2>::ROW_STRIDE) = make_int2(msgH, E);
         dg = upH; F = Fn; Hgl = Hg;
         __syncwarp();
-        const int2 u = *(const int2 *)(rptr + k * SFE_ROW_STRIDE);
+        const int2 u = GLOBAL ? __ldcg((const int2 *)(rptr + k * RingGeom<RL2>::ROW_STRIDE))
+                              : *(const int2 *)(rptr + k * RingGeom<RL2>::ROW_STRIDE);
         upH = u.x; upE = u.y;
     }
 }
 
-template <bool TB>
+template <bool TB, int RL2, bool GLOBAL>
 static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, const int lane)
 {
-    uint16_t *selring = (uint16_t *)(wsm + 8 * SFE_ROW_STRIDE);
+    typedef RingGeom<RL2> G;
+    uint16_t *selring = (uint16_t *)(wsm + 8 * G::ROW_STRIDE);
     sfe_half out;
     out.score = 0; out.end_i = 0; out.end_j = 0; out.status = 0; out.cells = 0;
     out.last_hdr = -1; out.last_chunk = -1; out.n_strips = 0; out.n_rec = 0; out.steps = 0; out.max_steps = 0;
@@ -242,10 +247,10 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
         n_strips++;
 
         if (sel_hi < cs - 32) sel_hi = cs - 32;
-        if (bnd_valid <= cs) { fill_bnd_neg(wsm, bnd_valid, cs + 64, lane); bnd_valid = cs + 64; }
+        if (bnd_valid <= cs) { fill_bnd_neg<RL2>(wsm, bnd_valid, cs + 64, lane); bnd_valid = cs + 64; }
         int upH = SFE_NEG, upE = SFE_NEG, dg = SFE_NEG, F = SFE_NEG, Hgl = SFE_NEG;
         if (lane == 0) {
-            const int2 u = *(const int2 *)(wsm + bnd_off(cs));
+            const int2 u = GLOBAL ? __ldcg((const int2 *)(wsm + bnd_off<RL2>(cs))) : *(const int2 *)(wsm + bnd_off<RL2>(cs));
             upH = u.x; upE = u.y;
             if (s == 0) dg = -OX;                           // R8: H(0,0) = 0 enters as the diagonal of (0,0)
         }
@@ -261,19 +266,19 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
         int gneg = 0;
         for (;; t0 += 8) {
             const int cmax = cs + t0 + 7;                   // lane 0's last column of this group
-            if (sel_hi <= cmax) { fill_sel(selring, g, sel_hi, cmax + 129, lane); sel_hi = cmax + 129; }
-            if (bnd_valid <= cmax + 1) { fill_bnd_neg(wsm, bnd_valid, bnd_valid + 64, lane); bnd_valid += 64; }
+            if (sel_hi <= cmax) { fill_sel<RL2>(selring, g, sel_hi, cmax + 129, lane); sel_hi = cmax + 129; }
+            if (bnd_valid <= cmax + 1) { fill_bnd_neg<RL2>(wsm, bnd_valid, bnd_valid + 64, lane); bnd_valid += 64; }
             const int base8 = (cs + t0) >> 3;
-            const char *rptr = is0 ? bnd + ((base8 + 1) & (SFE_RING / 8 - 1)) * 8 : exch_r;
-            char *wptr = is31 ? bnd + ((base8 - 3) & (SFE_RING / 8 - 1)) * 8 : exch_w;
+            const char *rptr = is0 ? bnd + ((base8 + 1) & (G::RING / 8 - 1)) * 8 : exch_r;
+            char *wptr = is31 ? bnd + ((base8 - 3) & (G::RING / 8 - 1)) * 8 : exch_w;
             const int col0 = cs + t0 - lane;
-            const uint16_t *selp = selring + (col0 & (SFE_SELRING - 1));
+            const uint16_t *selp = selring + (col0 & (G::SELRING - 1));
             uint32_t acc = 0;
             if (cmax > g.m)
-                run_group8<TB, true>(upH, upE, dg, F, Hgl, best, bm, acc, gneg, srow_lo, srow_hi, T, OX, tox, X, rptr, wptr,
+                run_group8<TB, true, RL2, GLOBAL>(upH, upE, dg, F, Hgl, best, bm, acc, gneg, srow_lo, srow_hi, T, OX, tox, X, rptr, wptr,
                                      selp, col0, g.m);
             else
-                run_group8<TB, false>(upH, upE, dg, F, Hgl, best, bm, acc, gneg, srow_lo, srow_hi, T, OX, tox, X, rptr, wptr,
+                run_group8<TB, false, RL2, GLOBAL>(upH, upE, dg, F, Hgl, best, bm, acc, gneg, srow_lo, srow_hi, T, OX, tox, X, rptr, wptr,
                                       selp, col0, g.m);
             if (TB) tb.put(acc, lane);
             const uint32_t al = ~(uint32_t)(-gneg) & 0xffu; // alive bits of this group, step k at bit 7-k
@@ -283,7 +288,7 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
                 last_t = t0 + 8 - __ffs(al);
             }
             if (!__any_sync(FULL, al != 0) && cs + t0 + 8 > prevR + 1) { t0 += 8; break; }
-            if (t0 + 8 >= SFE_MAX_STEPS) { t0 += 8; bail = true; break; }
+            if (t0 + 8 >= G::MAX_STEPS) { t0 += 8; bail = true; break; }
         }
         const int first = last_t < 0 ? 0x7fffffff : cs - lane + first_t, last = last_t < 0 ? -1 : cs - lane + last_t;
         total_steps += t0;
@@ -311,7 +316,9 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
     for (int o = 16; o > 0; o >>= 1) cells += __shfl_xor_sync(FULL, cells, o);
 
     out.score = bs; out.end_i = bi; out.end_j = bj; out.cells = cells;
-    out.status = (wide ? SFE_ST_WIDE : 0u) | ((TB && !tb.ok) ? ST_PASS_OVERFLOW : 0u);
+    // normal kernel: a bail-out is re-run by the wide kernel; wide kernel: a bail-out is final (band limit)
+    out.status = (wide ? (GLOBAL ? (SFE_ST_WIDE | SFE_ST_BAND_LIMIT) : SFE_ST_WIDE_PENDING) : (GLOBAL ? SFE_ST_WIDE : 0u)) |
+                 ((TB && !tb.ok) ? ST_PASS_OVERFLOW : 0u);
     out.last_hdr = last_hdr; out.last_chunk = tb.cur_chunk; out.n_strips = n_strips; out.n_rec = tb.nrec;
     out.steps = total_steps; out.max_steps = max_steps;
     if (lane == 0) {
@@ -319,7 +326,7 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
         atomicAdd(&p.counters[CNT_STEPS], (unsigned long long)total_steps);
         if (TB) atomicAdd(&p.counters[CNT_TBBYTES], (unsigned long long)tb.nrec * 128ULL);
         if (TB && !tb.ok) atomicAdd(&p.counters[CNT_OVERFLOW], 1ULL);
-        if (wide) atomicAdd(&p.counters[CNT_WIDE], 1ULL);
+        if (wide && !GLOBAL) atomicAdd(&p.counters[CNT_WIDE], 1ULL);
     }
 }
 
@@ -335,7 +342,34 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS) ydrop_kernel(const YdParams
         if (lane == 0) tk = atomicAdd(&p.counters[CNT_TICKET], 1ULL);
         tk = __shfl_sync(FULL, tk, 0);
         if ((long long)tk >= p.n_tickets) break;
-        extend_half<TB>(p, p.tickets[tk], wsm, lane);
+        extend_half<TB, SFE_RING_LOG2, false>(p, p.tickets[tk], wsm, lane);
+        __syncwarp();
+    }
+}
+
+// Halves whose strip outgrew the shared-memory window (status SFE_ST_WIDE_PENDING) are collected ...
+__global__ void select_wide_kernel(const YdParams p)
+{
+    const long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (x >= p.n_tickets) return;
+    const int hid = p.tickets[x];
+    if (p.halves[hid].status & SFE_ST_WIDE_PENDING) p.wide_tickets[atomicAdd(&p.counters[CNT_WIDE_N], 1ULL)] = hid;
+}
+
+// ... and re-run, bit-exactly the same algorithm, with 2^16-column rings in global memory (one warp per
+// block, always launched: the ticket count is read on the device, so no host synchronisation).
+template <bool TB>
+__global__ void __launch_bounds__(32) ydrop_wide_kernel(const YdParams p)
+{
+    const int lane = sfe_lane();
+    char *wsm = p.wide_ring + (size_t)blockIdx.x * RingGeom<SFE_WIDE_RING_LOG2>::WARP_BYTES;
+    const long long n = (long long)*((volatile unsigned long long *)&p.counters[CNT_WIDE_N]);
+    for (;;) {
+        unsigned long long tk = 0;
+        if (lane == 0) tk = atomicAdd(&p.counters[CNT_WIDE_TICKET], 1ULL);
+        tk = __shfl_sync(FULL, tk, 0);
+        if ((long long)tk >= n) break;
+        extend_half<TB, SFE_WIDE_RING_LOG2, true>(p, p.wide_tickets[tk], wsm, lane);
         __syncwarp();
     }
 }
@@ -360,5 +394,9 @@ int sfe_launch_ydrop(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st)
     if (blocks < 1) blocks = 1;
     if (want_tb) ydrop_kernel<true><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
     else ydrop_kernel<false><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
+    const int bs = 256;
+    select_wide_kernel<<<(unsigned)((p.n_tickets + bs - 1) / bs), bs, 0, st>>>(p);
+    if (want_tb) ydrop_wide_kernel<true><<<SFE_WIDE_WARPS, 32, 0, st>>>(p);
+    else ydrop_wide_kernel<false><<<SFE_WIDE_WARPS, 32, 0, st>>>(p);
     SFE_LAUNCH_CHECK();
 }

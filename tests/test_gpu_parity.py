@@ -158,3 +158,30 @@ def test_windowed_resolve_equals_serial(sfe, oracle):
             j = nxt
         assert (state == 1).tolist() == (ser["state"] == 1).tolist(), K
         assert int(nacc.item()) == ser["n_kept"]
+
+
+def test_wide_band_path(sfe, oracle):
+    """Bands wider than the 1024-column shared-memory window are re-run by the global-memory-ring
+    kernel and stay bit-exact: huge ydrop, and ydrop = infinity on 1.6 kbp."""
+    T = W.randseq(41, 2600); mu = W.mutate(T, 0.05, 0.01, W.Stream(42)); Q = mu.seq
+    k = np.searchsorted(mu.t_idx, [1300, 100])
+    anchors = [(int(mu.t_idx[k[0]]), int(mu.q_idx[k[0]]), 0, 1), (int(mu.t_idx[k[1]]), int(mu.q_idx[k[1]]), 0, 1)]
+    w = _wl(T, Q, anchors)
+    out = H.gpu_run(sfe, w, ydrop=40000)
+    assert out["info"]["wide"] >= 2
+    for i in range(2):
+        H.assert_anchor_equal(out, w, i, ydrop=40000)
+        assert int(out["results"][i]["status"]) & B.ST_WIDE
+    w = _wl(T[:1600], Q[:1600], [(0, 0, 0, 1), (800, int(mu.q_idx[np.searchsorted(mu.t_idx, 800)]), 0, 1)])
+    w.anchors[1, 0] = int(mu.t_idx[np.searchsorted(mu.t_idx, 800)])
+    out = H.gpu_run(sfe, w, ydrop=B.YDROP_INF)
+    assert out["info"]["wide"] >= 1
+    for i in range(2):
+        H.assert_anchor_equal(out, w, i, ydrop=B.YDROP_INF)
+    # A17 (SURVEY Appendix A): 300-bp core + random tails, band up to ~700 columns: normal kernel, no wide path
+    core = W.randseq(7, 300)
+    w = _wl(np.concatenate([core, W.randseq(8, 1500)]), np.concatenate([core, W.randseq(9, 1500)]), [(0, 0, 0, 1), (150, 150, 0, 1)])
+    out = H.gpu_run(sfe, w)
+    assert out["info"]["wide"] == 0
+    H.assert_anchor_equal(out, w, 0); H.assert_anchor_equal(out, w, 1)
+    assert int(out["results"][0]["cells"]) == 598524 + 1 and int(out["results"][0]["score"]) == 28831
