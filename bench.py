@@ -254,15 +254,17 @@ def main():
     f_mhz = clocks.get("sm_mhz") or 1965.0
     fmax = clocks.get("sm_max_mhz") or 1965.0
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
-    # probe rates are per max-clock cycle; the limiting resource per cell:
-    r_alu_eff = min(r_alu, r_dpx)
-    cyc_per_cell = max(hl["alu"] / r_alu_eff, hl["fma"] / r_fma, hl["per_cell"] / max(r_mix, r_alu_eff))
+    # probe rates are per max-clock cycle.  ALU and FMA are separate 16-lane pipes (2 cycles per warp
+    # instruction per SM sub-partition); DPX (VIADDMNMX/VIMNMX3) issues to the ALU pipe at the plain ALU rate.
+    # Cycles per cell per SM = the slowest of the ALU pipe, the FMA pipe (IMAD) and instruction issue as a whole.
+    r_alu_pipe = min(r_alu, r_dpx)
+    cyc_per_cell = max(hl["alu"] / r_alu_pipe, hl["fma"] / r_fma, hl["per_cell"] / max(r_mix, r_alu, r_dpx))
     peak_gcups = n_sm * fmax * 1e6 / cyc_per_cell / 1e9
     k_gcups = cells_step * args.steps / (kernel_us * 1e-6) / 1e9 if kernel_us > 0 else None
     roof = {"bound": "alu", "achieved": k_gcups, "peak": peak_gcups, "unit": "GCUPS", "frac": (k_gcups / peak_gcups) if k_gcups else None,
             "traffic": None, "kernel": "ydrop_kernel<%s>" % ("traceback" if flags else "score-only"),
             "kernel_share_of_step": kernel_us * 1e-3 / ms,
-            "detail": {"instr_per_cell_sass": hl["per_cell"], "alu_per_cell": hl["alu"], "fma_per_cell": hl["fma"],
+            "detail": {"instr_per_cell_sass": hl["per_cell"], "alu_per_cell": hl["alu"], "dpx_per_cell": hl["dpx"], "fma_per_cell": hl["fma"],
                        "lsu_per_cell": hl["lsu"], "R_alu": r_alu, "R_dpx": r_dpx, "R_imad": r_fma, "R_mixed": r_mix,
                        "R_unit": "lane-instr/clk/SM at sm_max_mhz", "n_sm": n_sm, "f_mhz_used": fmax,
                        "f_mhz_sampled": f_mhz, "peak_source": "measured by sfe_probe_int_issue in this run",

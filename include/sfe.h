@@ -50,8 +50,9 @@ enum {
 #define SFE_ST_CIGAR_OVERFLOW 2u      /* cigar pool too small: ops not written (n_ops is valid)   */
 #define SFE_ST_WIDE 4u                /* informational: a half took the wide-band (global ring) path */
 #define SFE_ST_SCORE_LIMIT 8u         /* R25: |score| would exceed 2^29                           */
-#define SFE_ST_BAD_ANCHOR 16u
-#define SFE_ST_BAND_LIMIT 32u          /* live band wider than 65,376 columns: half not computed    */         /* anchor outside its pair's limits: nothing computed      */
+#define SFE_ST_BAD_ANCHOR 16u         /* anchor outside its pair's limits: nothing computed          */
+#define SFE_ST_BAND_LIMIT 32u         /* live band wider than 65,344 columns: half not computed      */
+#define SFE_ST_INTERNAL 64u           /* traceback walk did not reach the origin (a library bug)     */
 
 /* CIGAR op word: (length << 4) | code ; M = aligned pair, I = query base vs gap, D = target base
  * vs gap (R12). */
@@ -151,7 +152,7 @@ int sfe_extend_host(sfe_ctx *ctx, const char *t_ascii_host, int64_t t_len, const
 /* Measurement helpers.  sfe_probe_int_issue runs a register-only microbenchmark
  * of the Y-drop kernel's own integer opcode mix on every SM and reports sustained
  * lane-instructions per clock per SM (the R of the integer-issue roofline).  mix: 0 = the
- * kernel's mix (ALU + DPX + IMAD), 1 = ALU-pipe only (IADD3/LOP3), 2 = DPX only
+ * kernel's mix (ALU + DPX + IMAD), 1 = ALU-pipe only (SHF/LOP3), 2 = DPX only
  * (VIADDMNMX/VIMNMX3), 3 = IMAD only.  sfe_last_batch_info returns counters of the most recent
  * sfe_ydrop_batch on this ctx: [0] kernel launches, [1] halves run, [2] halves re-run after a
  * traceback overflow, [3] traceback bytes written, [4] DP steps (warp wavefronts) executed,

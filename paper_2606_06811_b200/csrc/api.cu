@@ -5,15 +5,13 @@
 #include <string.h>
 #include "sfe_internal.cuh"
 
-#define ST_PASS_OVERFLOW 0x100u
 
 // launchers defined next to their kernels
 int sfe_launch_ydrop(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st);
 int sfe_launch_join(const sfe_anchor *anchors, const sfe_half *halves, long long n, const long long *sel, long long n_sel,
-                    const uint32_t *pool, const int32_t *chunk_prev, int want_cigar, sfe_result *results, cudaStream_t st);
-int sfe_launch_scan_emit(const sfe_half *halves, long long n, const long long *sel, long long n_sel, const uint32_t *pool,
-                         const int32_t *chunk_prev, sfe_result *results, uint32_t *cigar_pool, long long cap,
-                         long long *pool_used, cudaStream_t st);
+                    int want_cigar, sfe_result *results, cudaStream_t st);
+int sfe_launch_scan_emit(const sfe_half *halves, long long n, const long long *sel, long long n_sel, const uint32_t *stage,
+                         sfe_result *results, uint32_t *cigar_pool, long long cap, long long *pool_used, cudaStream_t st);
 int sfe_launch_pack(const char *ascii, long long len, uint8_t *codes2, uint8_t *nmask, uint8_t *rc_codes2,
                     uint8_t *rc_nmask, cudaStream_t st);
 int sfe_launch_resolve(const sfe_anchor *anchors, const sfe_result *results, long long n, int min_score, sfe_box *accepted,
@@ -45,7 +43,7 @@ struct sfe_ctx {
     uint32_t *pool; int32_t *chunk_prev; int n_chunks;
     unsigned long long *counters;     // device, CNT_N
     unsigned long long *counters_host;  // pinned
-    DevBuf halves, tickets, sel, hist, blkmin, act, misc, wide_tickets, wide_ring;
+    DevBuf halves, tickets, sel, hist, blkmin, act, misc, wide_tickets, wide_ring, ops_stage;
     // host-API staging
     DevBuf h_tascii, h_qascii, h_t2, h_tm, h_q2, h_qm, h_r2, h_rm, h_pairs, h_anchors, h_results, h_keep, h_cigar, h_acc, h_small;
     long long info[8];
@@ -115,7 +113,7 @@ extern "C" int sfe_destroy(sfe_ctx *c)
     if (c->counters) cudaFree(c->counters);
     if (c->counters_host) cudaFreeHost(c->counters_host);
     cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1);
-    DevBuf *bufs[] = {&c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
+    DevBuf *bufs[] = {&c->ops_stage, &c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
                       &c->h_t2, &c->h_tm, &c->h_q2, &c->h_qm, &c->h_r2, &c->h_rm, &c->h_pairs, &c->h_anchors, &c->h_results,
                       &c->h_keep, &c->h_cigar, &c->h_acc, &c->h_small};
     for (DevBuf *b : bufs) b->release();
@@ -235,6 +233,12 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
     if ((rc = c->wide_tickets.ensure((size_t)(2 * n_anchors) * sizeof(int32_t)))) return rc;
     if ((rc = c->wide_ring.ensure((size_t)SFE_WIDE_WARPS * RingGeom<SFE_WIDE_RING_LOG2>::WARP_BYTES))) return rc;
     if (want_tb && (rc = c->sel.ensure((size_t)n_anchors * sizeof(long long)))) return rc;
+    // ops arena: every staged op ends up in the caller's pool, plus two header words per segment
+    // (one segment per SFE_WALK_OPS ops, at least one per half)
+    const unsigned long long ops_cap = want_tb ? (unsigned long long)cigar_pool_cap + (unsigned long long)cigar_pool_cap / (SFE_WALK_OPS / 2) +
+                                                     4ULL * (unsigned long long)n_anchors + 64ULL : 0ULL;
+    if (ops_cap > 0xfffffff0ULL) return SFE_ELIMIT;               // segment offsets are 32-bit
+    if (want_tb && (rc = c->ops_stage.ensure((size_t)ops_cap * sizeof(uint32_t)))) return rc;
 
     YdParams p;
     memset(&p, 0, sizeof p);
@@ -244,6 +248,7 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
     p.counters = c->counters; p.halves = (sfe_half *)c->halves.p; p.pool = c->pool; p.chunk_prev = c->chunk_prev;
     p.n_chunks = want_tb ? c->n_chunks : 0; p.n_pairs = n_pairs;
     p.wide_ring = (char *)c->wide_ring.p; p.wide_tickets = (int32_t *)c->wide_tickets.p;
+    p.ops_stage = (uint32_t *)c->ops_stage.p; p.ops_cap = ops_cap;
     p.OX = sc->gap_open + sc->gap_extend; p.X = sc->gap_extend;
     p.ydrop_inf = sc->ydrop == SFE_YDROP_INF; p.Y = p.ydrop_inf ? 0 : sc->ydrop;
     for (int a = 0; a < 4; a++) {
@@ -259,11 +264,10 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
                                  (unsigned int *)c->hist.p, (int32_t *)c->tickets.p, c->stream))) return rc;
     if ((rc = timed_ydrop(c, p, want_tb))) return rc;
     c->info[0] += 1; c->info[1] += 2 * n_anchors;
-    if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, nullptr, n_anchors, c->pool, c->chunk_prev, want_tb,
-                              results_dev, c->stream))) return rc;
+    if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, nullptr, n_anchors, want_tb, results_dev, c->stream))) return rc;
     if (!want_tb) return SFE_OK;
-    if ((rc = sfe_launch_scan_emit(p.halves, n_anchors, nullptr, n_anchors, c->pool, c->chunk_prev, results_dev,
-                                   cigar_pool_dev, cigar_pool_cap, (long long *)cigar_pool_used_dev, c->stream))) return rc;
+    if ((rc = sfe_launch_scan_emit(p.halves, n_anchors, nullptr, n_anchors, p.ops_stage, results_dev, cigar_pool_dev,
+                                   cigar_pool_cap, (long long *)cigar_pool_used_dev, c->stream))) return rc;
 
     // traceback-arena overflow: re-run the anchors that did not fit, with the arena emptied
     long long prev_overflow = -1;
@@ -290,11 +294,9 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
         p.n_tickets = 2 * n_sel;
         if ((rc = timed_ydrop(c, p, true))) return rc;
         c->info[0] += 1; c->info[1] += 2 * n_sel; c->info[2] += 2 * n_sel;
-        if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, (const long long *)c->sel.p, n_sel, c->pool,
-                                  c->chunk_prev, 1, results_dev, c->stream))) return rc;
-        if ((rc = sfe_launch_scan_emit(p.halves, n_anchors, (const long long *)c->sel.p, n_sel, c->pool, c->chunk_prev,
-                                       results_dev, cigar_pool_dev, cigar_pool_cap, (long long *)cigar_pool_used_dev,
-                                       c->stream))) return rc;
+        if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, (const long long *)c->sel.p, n_sel, 1, results_dev, c->stream))) return rc;
+        if ((rc = sfe_launch_scan_emit(p.halves, n_anchors, (const long long *)c->sel.p, n_sel, p.ops_stage, results_dev,
+                                       cigar_pool_dev, cigar_pool_cap, (long long *)cigar_pool_used_dev, c->stream))) return rc;
     }
     return SFE_OK;
 }

@@ -1,78 +1,17 @@
-// cigar_kernel.cu -- a8: join the two halves of every anchor and emit run-length CIGARs by walking
-// the 4-bit traceback pointers that ydrop_kernel spilled to the HBM arena (R11, R12).
+// cigar_kernel.cu -- a8, second part: join the two halves of every anchor and place the run-length
+// CIGARs (R11, R12) at deterministic, anchor-ordered offsets of the caller's pool.
 //
-// Pass 1 (join_count): one thread per anchor joins the halves into sfe_result (score, box, cells,
-// status) and, if a CIGAR is wanted, walks both halves once to count their runs.
-// An exclusive scan over n_ops gives deterministic pool offsets in anchor order.
-// Pass 2 (emit): the same walk again, writing ops.  The backward half's walk order (far end ->
-// anchor) is already the output order; the forward half is written from the end of its slot.
+// The traceback walk itself happens inside ydrop_kernel (walk_traceback): the warp that computed a
+// half walks its 4-bit pointers right away and stages the ops, in walk order (end cell -> origin),
+// as a backward-linked list of segments in the ops arena.  What is left here is cheap and parallel:
+//   join_kernel   one thread per anchor: score, box, cells, status, n_ops = n_ops(back) + n_ops(fwd);
+//   scan_offsets  exclusive scan of n_ops in anchor order -> cigar_off;
+//   emit_kernel   one warp per anchor copies the staged ops: the backward half's walk order (far end
+//                 -> anchor) is already the output order, the forward half is reversed.
 #include "sfe_internal.cuh"
 
-#define ST_PASS_OVERFLOW 0x100u
-
-struct TbCursor {          // random access to a half's records, cheap for monotonically decreasing indices
-    const uint32_t *pool; const int32_t *chunk_prev;
-    int chunk, ord;        // current chunk id and its ordinal in the half's list
-    int last_chunk, last_ord;
-    __device__ __forceinline__ const uint32_t *rec(int ridx)
-    {
-        const int o = ridx / SFE_CHUNK_RECS;
-        if (o > ord) { chunk = last_chunk; ord = last_ord; }   // rare: header / record straddle a chunk edge
-        while (ord > o) { chunk = chunk_prev[chunk]; ord--; }
-        return pool + ((size_t)chunk * SFE_CHUNK_RECS + (ridx - o * SFE_CHUNK_RECS)) * 32;
-    }
-};
-
-// Walk one half from its end cell to the origin.  EMIT == false: returns the number of runs.
-// EMIT == true: writes runs; step = +1 writes dst[0], dst[1], ... in walk order, step = -1 writes
-// dst[0], dst[-1], ...
-template <bool EMIT>
-static __device__ int walk_half(const sfe_half &h, const uint32_t *pool, const int32_t *chunk_prev, uint32_t *dst, int step)
-{
-    if (h.end_i == 0 && h.end_j == 0) return 0;
-    TbCursor cur; cur.pool = pool; cur.chunk_prev = chunk_prev; cur.chunk = h.last_chunk;
-    cur.ord = (h.n_rec - 1) / SFE_CHUNK_RECS;
-    cur.last_chunk = cur.chunk; cur.last_ord = cur.ord;
-    // locate the header of the strip holding the end row
-    int strip = h.n_strips - 1, hdr = h.last_hdr;
-    int i = h.end_i, j = h.end_j;
-    const uint32_t *hr = cur.rec(hdr);
-    while (strip > (i >> 5)) { hdr = (int)hr[1]; strip--; hr = cur.rec(hdr); }
-    int cs = (int)hr[0], prev_hdr = (int)hr[1];
-    int state = 0, cur_op = -1, run = 0, nruns = 0;
-    while (!(i == 0 && j == 0 && state == 0)) {
-        if ((i >> 5) < strip) {                     // crossed into the strip above
-            hdr = prev_hdr; strip--;
-            hr = cur.rec(hdr); cs = (int)hr[0]; prev_hdr = (int)hr[1];
-        }
-        const int lane = i & 31;
-        const int t = j - cs + lane;
-        const uint32_t w = cur.rec(hdr + 1 + (t >> 3))[lane];
-        const uint32_t nib = (w >> ((7 - (t & 7)) * 4)) & 15u;   // bit3 !M, bit2 !E, bit1 E ext, bit0 F ext
-        int op = -1;
-        if (state == 0) {
-            if (!(nib & 8u)) { op = SFE_OP_M; i--; j--; }
-            else state = (nib & 4u) ? 2 : 1;
-        } else if (state == 1) {
-            op = SFE_OP_I; i--; if (!(nib & 2u)) state = 0;
-        } else {
-            op = SFE_OP_D; j--; if (!(nib & 1u)) state = 0;
-        }
-        if (op >= 0) {
-            if (op == cur_op) run++;
-            else {
-                if (cur_op >= 0) { if (EMIT) { *dst = ((uint32_t)run << 4) | (uint32_t)cur_op; dst += step; } nruns++; }
-                cur_op = op; run = 1;
-            }
-        }
-    }
-    if (cur_op >= 0) { if (EMIT) { *dst = ((uint32_t)run << 4) | (uint32_t)cur_op; } nruns++; }
-    return nruns;
-}
-
-__global__ void join_count_kernel(const sfe_anchor *anchors, const sfe_half *halves, long long n, const long long *sel,
-                                  long long n_sel, const uint32_t *pool, const int32_t *chunk_prev, int want_cigar,
-                                  sfe_result *results, int32_t *nops_fwd)
+__global__ void join_kernel(const sfe_anchor *anchors, const sfe_half *halves, long long n, const long long *sel,
+                            long long n_sel, int want_cigar, sfe_result *results)
 {
     const long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (x >= n_sel) return;
@@ -81,24 +20,22 @@ __global__ void join_count_kernel(const sfe_anchor *anchors, const sfe_half *hal
     const sfe_anchor an = anchors[a];
     sfe_result r;
     r.score_fwd = f.score; r.score_bwd = b.score; r.score = f.score + b.score;
-    uint32_t st = (f.status | b.status);
+    const uint32_t st = (f.status | b.status);
     r.tstart = an.tpos - b.end_j; r.tend = an.tpos + f.end_j;
     r.qstart = an.qpos - b.end_i; r.qend = an.qpos + f.end_i;
     r.cells = f.cells + b.cells;
     r.cigar_off = -1; r.n_ops = 0; r.n_ops_back = 0;
-    int nf = 0;
-    if (want_cigar && !(st & (ST_PASS_OVERFLOW | SFE_ST_BAD_ANCHOR | SFE_ST_BAND_LIMIT))) {
-        const int nb = walk_half<false>(b, pool, chunk_prev, nullptr, 0);
-        nf = walk_half<false>(f, pool, chunk_prev, nullptr, 0);
-        r.n_ops_back = nb; r.n_ops = nb + nf;
+    if (want_cigar && !(st & (SFE_ST_PASS_OVERFLOW | SFE_ST_BAD_ANCHOR | SFE_ST_BAND_LIMIT | SFE_ST_INTERNAL))) {
+        r.n_ops_back = b.n_ops; r.n_ops = b.n_ops + f.n_ops;
     }
-    r.status = (st & 0xffu) | ((st & ST_PASS_OVERFLOW) ? SFE_ST_TB_OVERFLOW : 0u);
+    r.status = (st & 0xffu) | ((st & SFE_ST_PASS_OVERFLOW) ? SFE_ST_TB_OVERFLOW : 0u) |
+               ((st & SFE_ST_OPS_OVERFLOW) ? SFE_ST_CIGAR_OVERFLOW : 0u);
     results[a] = r;
-    if (nops_fwd) nops_fwd[a] = nf;
 }
 
 // exclusive scan of results[].n_ops into results[].cigar_off (single block, running carry).
-// Anchors flagged SFE_ST_TB_OVERFLOW keep cigar_off = -1 and contribute nothing in this pass.
+// Anchors flagged SFE_ST_TB_OVERFLOW / SFE_ST_CIGAR_OVERFLOW keep cigar_off = -1 and contribute
+// nothing in this pass; anchors that already have an offset (earlier pass) are skipped.
 __global__ void scan_offsets_kernel(sfe_result *results, long long n, long long *pool_used, long long cap)
 {
     __shared__ long long warp_sums[32];
@@ -133,38 +70,55 @@ __global__ void scan_offsets_kernel(sfe_result *results, long long n, long long 
     if (threadIdx.x == 0) *pool_used = carry;
 }
 
-__global__ void emit_kernel(const sfe_half *halves, long long n, const long long *sel, long long n_sel, const uint32_t *pool,
-                            const int32_t *chunk_prev, const sfe_result *results, uint32_t *cigar_pool)
+// Copy one half's staged ops.  The segments form a backward-linked list; the last one holds the walk
+// indices [n - count, n).  dir = +1: walk index x goes to dst[x]; dir = -1: to dst[n - 1 - x].
+static __device__ void copy_half_ops(const sfe_half &h, const uint32_t *stage, uint32_t *dst, int dir, int lane)
 {
-    const long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    int hi = h.n_ops;
+    uint32_t seg = h.ops_seg;
+    while (seg != SFE_NO_SEG && hi > 0) {
+        const uint32_t prev = stage[seg];
+        const int cnt = (int)stage[seg + 1];
+        const int lo = hi - cnt;
+        for (int x = lane; x < cnt; x += 32) {
+            const int w = lo + x;
+            dst[dir > 0 ? w : h.n_ops - 1 - w] = stage[seg + 2 + x];
+        }
+        hi = lo; seg = prev;
+    }
+}
+
+__global__ void emit_kernel(const sfe_half *halves, long long n, const long long *sel, long long n_sel,
+                            const uint32_t *stage, const sfe_result *results, uint32_t *cigar_pool)
+{
+    const long long x = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
     if (x >= n_sel) return;
     const long long a = sel ? sel[x] : x;
     const sfe_result r = results[a];
     if (r.n_ops <= 0 || r.cigar_off < 0 || (r.status & (SFE_ST_CIGAR_OVERFLOW | SFE_ST_TB_OVERFLOW))) return;
     uint32_t *dst = cigar_pool + r.cigar_off;
-    walk_half<true>(halves[2 * a + 1], pool, chunk_prev, dst, +1);
-    walk_half<true>(halves[2 * a], pool, chunk_prev, dst + r.n_ops - 1, -1);
+    copy_half_ops(halves[2 * a + 1], stage, dst, +1, lane);
+    copy_half_ops(halves[2 * a], stage, dst + r.n_ops_back, -1, lane);
 }
 
 int sfe_launch_join(const sfe_anchor *anchors, const sfe_half *halves, long long n, const long long *sel, long long n_sel,
-                    const uint32_t *pool, const int32_t *chunk_prev, int want_cigar, sfe_result *results, cudaStream_t st)
+                    int want_cigar, sfe_result *results, cudaStream_t st)
 {
     if (n_sel <= 0) return SFE_OK;
     const int bs = 128;
-    join_count_kernel<<<(unsigned)((n_sel + bs - 1) / bs), bs, 0, st>>>(anchors, halves, n, sel, n_sel, pool, chunk_prev,
-                                                                     want_cigar, results, nullptr);
+    join_kernel<<<(unsigned)((n_sel + bs - 1) / bs), bs, 0, st>>>(anchors, halves, n, sel, n_sel, want_cigar, results);
     SFE_LAUNCH_CHECK();
 }
 
-int sfe_launch_scan_emit(const sfe_half *halves, long long n, const long long *sel, long long n_sel, const uint32_t *pool,
-                         const int32_t *chunk_prev, sfe_result *results, uint32_t *cigar_pool, long long cap,
-                         long long *pool_used, cudaStream_t st)
+int sfe_launch_scan_emit(const sfe_half *halves, long long n, const long long *sel, long long n_sel, const uint32_t *stage,
+                         sfe_result *results, uint32_t *cigar_pool, long long cap, long long *pool_used, cudaStream_t st)
 {
     if (n <= 0) return SFE_OK;
     scan_offsets_kernel<<<1, 1024, 0, st>>>(results, n, pool_used, cap);
     if (n_sel > 0) {
-        const int bs = 128;
-        emit_kernel<<<(unsigned)((n_sel + bs - 1) / bs), bs, 0, st>>>(halves, n, sel, n_sel, pool, chunk_prev, results, cigar_pool);
+        const int bs = 256;                                   // 8 anchors per block, one warp each
+        emit_kernel<<<(unsigned)((n_sel * 32 + bs - 1) / bs), bs, 0, st>>>(halves, n, sel, n_sel, stage, results, cigar_pool);
     }
     SFE_LAUNCH_CHECK();
 }

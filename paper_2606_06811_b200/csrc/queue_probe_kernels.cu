@@ -2,7 +2,6 @@
 // overflow re-run selection, and the integer-issue microbenchmark used for the roofline (8(d)).
 #include "sfe_internal.cuh"
 
-#define ST_PASS_OVERFLOW 0x100u
 
 // ---- a3: bins -----------------------------------------------------------------------------------
 // Length proxy of a half = min(rows available, columns available) to the pair's limit
@@ -79,7 +78,7 @@ __global__ void select_overflow_kernel(const sfe_half *halves, long long n_ancho
 {
     const long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (a >= n_anchors) return;
-    if ((halves[2 * a].status | halves[2 * a + 1].status) & ST_PASS_OVERFLOW) {
+    if ((halves[2 * a].status | halves[2 * a + 1].status) & SFE_ST_PASS_OVERFLOW) {
         const unsigned long long k = atomicAdd(n_sel, 1ULL);
         sel[k] = a; tickets[2 * k] = (int32_t)(2 * a); tickets[2 * k + 1] = (int32_t)(2 * a + 1);
     }
@@ -107,8 +106,8 @@ __global__ void __launch_bounds__(256) probe_kernel(int iters, int seed, int *si
     for (int it = 0; it < iters; it++) {
 #pragma unroll
         for (int c = 0; c < PROBE_CHAINS; c++) {
-            if (MIX == 1) {            // ALU pipe: IADD3 + LOP3
-                asm volatile("add.s32 %0, %0, %1;" : "+r"(a[c]) : "r"(b[c]));
+            if (MIX == 1) {            // ALU pipe only: SHF + LOP3 (an add.s32 would become IMAD.IADD on the FMA pipe)
+                asm volatile("shf.l.wrap.b32 %0, %0, %1, 3;" : "+r"(a[c]) : "r"(b[c]));
                 asm volatile("xor.b32 %0, %0, %1;" : "+r"(b[c]) : "r"(a[c]));
             } else if (MIX == 2) {     // DPX: VIADDMNMX + VIMNMX3
                 a[c] = __viaddmax_s32(a[c], k1, b[c]);

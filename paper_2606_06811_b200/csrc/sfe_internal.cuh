@@ -8,6 +8,8 @@
 #define SFE_NEG (-(1 << 30))            // "minus infinity" of the DP (R6)
 #define SFE_T_INF (-(1 << 29))          // threshold used for SFE_YDROP_INF (R27): every real cell is above it
 #define SFE_ST_WIDE_PENDING 0x200u    // internal: the strip outgrew the shared-memory window; re-run by the wide kernel
+#define SFE_ST_PASS_OVERFLOW 0x100u   // internal: the traceback arena ran out during this pass; the anchor is re-run
+#define SFE_ST_OPS_OVERFLOW 0x400u    // internal: the ops arena ran out; reported as SFE_ST_CIGAR_OVERFLOW
 #define SFE_OOB_SCORE 0xE0000000u       // substitution "score" of a column beyond the target end (-2^29)
 
 // ---- shared-memory geometry of one warp -------------------------
@@ -25,34 +27,47 @@
 template <int RL2> struct RingGeom {
     static constexpr int RING = 1 << RL2;                        // boundary-ring capacity in columns
     static constexpr int ROW_STRIDE = SFE_EXCH_BYTES + RING;     // bytes: exchange area + RING/8 segments x 8 B
-    static constexpr int SELRING = RING;                         // selector ring (>= MAX_STEPS + 160: the next strip re-reads the window start)
-    static constexpr int WARP_BYTES = 8 * ROW_STRIDE + (SELRING + 8) * 2;
-    static constexpr int MAX_STEPS = RING - 160;                 // a strip wider than this bails out
+    static constexpr int SELRING = RING;                         // selector ring (>= MAX_STEPS + 192: the next strip re-reads the window start)
+    static constexpr int WARP_BYTES = 8 * ROW_STRIDE + (SELRING + 16) * 2;
+    static constexpr int MAX_STEPS = RING - 192;                 // a strip wider than this bails out (multiple of 16)
 };
 #define SFE_WARP_SMEM (RingGeom<SFE_RING_LOG2>::WARP_BYTES)
 #define SFE_WIDE_WARPS 148                          // warps of the wide-band kernel (one per block)
 
 // ---- traceback arena --------------------------------------------------------------------------
-// Record = 32 lanes x one 32-bit word (8 cells x 4 bits) = 128 B, written coalesced by one warp
-// per group of 8 steps.  Records live in 64 KiB chunks handed out by an atomic counter; a half's
-// chunks form a backward-linked list (chunk_prev).
-#define SFE_CHUNK_RECS 512
-#define SFE_CHUNK_BYTES (SFE_CHUNK_RECS * 128)
+// Record = 32 lanes x two 32-bit words (16 cells x 4 bits) = 256 B, written coalesced (one 8-byte
+// store per lane) by one warp per group of 16 steps; lane l owns words 2l (steps 0-7) and 2l+1
+// (steps 8-15).  Records live in 64 KiB chunks handed out by an atomic counter; a half's chunks
+// form a backward-linked list (chunk_prev).
+#define SFE_REC_WORDS 64
+#define SFE_REC_BYTES (SFE_REC_WORDS * 4)
+#define SFE_CHUNK_RECS 256
+#define SFE_CHUNK_BYTES (SFE_CHUNK_RECS * SFE_REC_BYTES)
+
+// ---- CIGAR staging ------------------------------------------------------------------------------
+// The warp that computed a half walks its traceback right away (ydrop_kernel.cu, walk_traceback) and
+// stages the run-length ops, in walk order (end cell -> origin), as segments in the ops arena:
+//   word 0 = offset of the previous segment of the same half (SFE_NO_SEG if none), word 1 = number
+//   of ops, then the ops.  emit_kernel copies them to their final, anchor-ordered place (a8).
+#define SFE_NO_SEG 0xffffffffu
+#define SFE_WALK_WIN_RECS 8                         // traceback records held in shared memory while walking
+#define SFE_WALK_OPS 512                            // ops staged in shared memory between flushes
+#define SFE_WALK_SMEM (SFE_WALK_WIN_RECS * SFE_REC_BYTES + SFE_WALK_OPS * 4)
 
 struct sfe_half {                 // result of one one-sided extension (a7)
     int32_t score;
     int32_t end_i, end_j;         // argbest, rows / columns relative to the anchor
     uint32_t status;
     unsigned long long cells;     // R28
-    int32_t last_hdr;             // record index of the last strip's header record, -1 if none
-    int32_t last_chunk;           // chunk id holding the last record, -1 if none
+    uint32_t ops_seg;             // offset of the last staged segment in the ops arena, SFE_NO_SEG if none
+    int32_t n_ops;                // run-length ops of this half (valid even if they could not be staged)
     int32_t n_strips;
-    int32_t n_rec;                // records written
+    int32_t n_rec;                // traceback records written
     int32_t steps;                // warp wavefronts executed
     int32_t max_steps;            // widest strip
 };
 
-enum { CNT_TICKET = 0, CNT_CHUNK, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_N = 16 };
+enum { CNT_TICKET = 0, CNT_CHUNK, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_OPS, CNT_N = 16 };
 
 struct YdParams {
     const uint8_t *t_codes, *t_nmask;
@@ -73,6 +88,8 @@ struct YdParams {
     uint32_t srow_hi;             // bytes: n_score, 0x00, 0xE0 (OOB), 0x00
     char *wide_ring;              // global-memory rings of the wide-band kernel: SFE_WIDE_WARPS x RingGeom<16>::WARP_BYTES
     int32_t *wide_tickets;        // halves that bailed out of the normal kernel in this pass
+    uint32_t *ops_stage;          // ops arena (segments, see above); counters[CNT_OPS] = words used
+    unsigned long long ops_cap;   // capacity of the ops arena in words
 };
 
 static __device__ __forceinline__ int sfe_lane() { return threadIdx.x & 31; }

@@ -18,8 +18,11 @@
 #include "sfe_internal.cuh"
 
 #define FULL 0xffffffffu
+#ifndef SFE_BLOCK_THREADS
 #define SFE_BLOCK_THREADS 192     // 6 warps x 12.3 KB of shared memory; 3 blocks = 18 warps per SM
-#define ST_PASS_OVERFLOW 0x100u   // internal: traceback arena ran out during this pass
+#endif
+// Ordering of a lane's message store and the next lane's load of it inside one wavefront step.
+#define SFE_STEP_FENCE() __syncwarp()
 
 // PRMT with the sign-replicate selector mode (bit 3 of a selector nibble), which __byte_perm masks off
 static __device__ __forceinline__ int prmt_sx(uint32_t lo, uint32_t hi, uint32_t sel)
@@ -29,10 +32,14 @@ static __device__ __forceinline__ int prmt_sx(uint32_t lo, uint32_t hi, uint32_t
     return r;
 }
 
+// Boundary-ring address of column c: row (c-1) mod 8, segment ((c-1) div 8) mod RING/8.  Strips start
+// at a multiple of 16 and groups hold 16 steps, so lane 0 (reading column cs+t0+k+1) and lane 31
+// (writing column cs+t0+k-31) both touch row k&7 and segment base + (k>>3) with an EVEN base: no
+// ring wrap inside a group, every access of the unrolled loop is base + immediate.
 template <int RL2>
 static __device__ __forceinline__ int bnd_off(int c)
 {
-    const int u = c + 7;
+    const int u = c - 1;
     return (u & 7) * RingGeom<RL2>::ROW_STRIDE + SFE_EXCH_BYTES + ((u >> 3) & (RingGeom<RL2>::RING / 8 - 1)) * 8;
 }
 
@@ -59,7 +66,7 @@ static __device__ __forceinline__ void fill_sel(uint16_t *selring, const HalfGeo
         const uint16_t v = (uint16_t)col_selector(g, c);
         const int idx = c & (RingGeom<RL2>::SELRING - 1);
         selring[idx] = v;
-        if (idx < 8) selring[idx + RingGeom<RL2>::SELRING] = v;
+        if (idx < 16) selring[idx + RingGeom<RL2>::SELRING] = v;
     }
     __syncwarp();
 }
@@ -74,10 +81,10 @@ static __device__ __forceinline__ void fill_bnd_neg(char *wbase, int lo, int hi,
 
 struct TbWriter {
     uint32_t *pool; int32_t *chunk_prev; unsigned long long *counters; int n_chunks;
-    uint32_t *ptr;          // this lane's word of the next record
+    uint32_t *ptr;          // this lane's word pair of the next record
     int left;               // records left in the current chunk
     int cur_chunk; int nrec; bool ok;
-    __device__ __forceinline__ void put(uint32_t word, int lane)
+    __device__ __forceinline__ void put(uint32_t w0, uint32_t w1, int lane)
     {
         if (!ok) return;
         if (left == 0) {
@@ -87,35 +94,15 @@ struct TbWriter {
             if (c >= n_chunks) { ok = false; return; }
             if (lane == 0) chunk_prev[c] = cur_chunk;
             cur_chunk = c;
-            ptr = pool + (size_t)c * SFE_CHUNK_RECS * 32 + lane;
+            ptr = pool + (size_t)c * SFE_CHUNK_RECS * SFE_REC_WORDS + 2 * lane;
             left = SFE_CHUNK_RECS;
         }
-        *ptr = word;
-        ptr += 32; left--; nrec++;
+        *(uint2 *)ptr = make_uint2(w0, w1);
+        ptr += SFE_REC_WORDS; left--; nrec++;
     }
 };
 
-// Integer adds forced onto the FMA pipe (IMAD): the ALU pipe is the binding resource of this kernel
-// (profiles/r1_01), the FMA pipe is otherwise idle.
-static __device__ __forceinline__ int fma_add(int a, int b)
-{
-    int r;
-    asm("mad.lo.s32 %0, %1, 1, %2;" : "=r"(r) : "r"(a), "r"(b));
-    return r;
-}
-// (a & ~b) | (c & b) in one LOP3
-static __device__ __forceinline__ int lop3_sel(int a, int b, int c)
-{
-    int r;
-    asm("lop3.b32 %0, %1, %2, %3, 0xB8;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
-    return r;
-}
-static __device__ __forceinline__ int fma_mad(int a, int b, int c)   // a * b + c
-{
-    int r;
-    asm("mad.lo.s32 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
-    return r;
-}
+// Integer subtraction on the FMA pipe (IMAD), which the ALU-heavy hot loop leaves mostly idle.
 static __device__ __forceinline__ int fma_sub(int a, int b)      // a - b
 {
     int r;
@@ -125,22 +112,29 @@ static __device__ __forceinline__ int fma_sub(int a, int b)      // a - b
 // acc = (acc << 1) | (sign bit of x): one SHF.L.W
 static __device__ __forceinline__ uint32_t shift_in_sign(uint32_t acc, int x) { return __funnelshift_l((uint32_t)x, acc, 1); }
 
-// One group of 8 wavefront steps.  Everything indexed by k is an immediate after unrolling.
-// Per cell the ALU pipe sees: PRMT, IADD3 (M), 2 x VIADDMNMX (E, F), VIMNMX3 (H), SHF + LOP3 (alive gate),
-// 4 x SHF (traceback bits), SHF + VIMNMX (best); the FMA pipe sees the 8 subtractions / shift-adds.
-// Traceback nibble of step k sits at bits 4(7-k)..4(7-k)+3 of acc:
+// One group of 16 wavefront steps.  Everything indexed by k is an immediate after unrolling.
+// Per cell: LDS.U16 + PRMT (score), IADD3 (M), 2 x VIADDMNMX (E, F), VIMNMX3 (H), compare + select
+// (alive gate, R5/R6), 4 x (subtract + funnel shift) for the traceback nibble, VIMNMX (best), and
+// the message STS.64 / LDS.64.  The kernel is issue-bound (profiles/r1_02), so what counts is the
+// number of instructions, not the pipe they run on; the subtractions stay on the FMA pipe (IMAD).
+// Traceback nibble of step k sits at bits 4(7-(k&7)).. of acc0 (k < 8) / acc1 (k >= 8):
 //   bit3 = H not from M, bit2 = H not from E, bit1 = E extended, bit0 = F extended (R11).
-// gneg = -(dead-bit pattern): gneg' = 2 gneg + g with g = 0 (alive) / -1 (dead); step k at bit 7-k of -gneg.
-// bm shifts in one bit per step: 1 iff that step raised the lane-local best (strict '>', R7).
+// dead: bit 15-k set iff the cell of step k is dead.
+// The position of a new lane-local best (strict '>', R7) is found after the group, only by the
+// lanes whose best rose: the first k with H_k == best is the last strict increase.
 template <bool TB, bool EDGE, int RL2, bool GLOBAL>
-static __device__ __forceinline__ void run_group8(int &upH, int &upE, int &dg, int &F, int &Hgl, int &best, uint32_t &bm,
-                                                  uint32_t &acc, int &gneg, const uint32_t srow_lo,
-                                                  const uint32_t srow_hi, const int T, const int OX, const int tox,
-                                                  const int X, const char *rptr, char *wptr, const uint16_t *selp,
-                                                  const int col0, const int m)
+static __device__ __forceinline__ void run_group16(int &upH, int &upE, int &dg, int &F, int &Hgl, int &best, int &best_t,
+                                                   uint32_t &acc0, uint32_t &acc1, uint32_t &dead, const uint32_t srow_lo,
+                                                   const uint32_t srow_hi, const int T, const int OX, const int X,
+                                                   const char *rptr, char *wptr, const uint16_t *selp, const int col0,
+                                                   const int m, const int t0)
 {
+    typedef RingGeom<RL2> G;
+    const int best_in = best;
+    int Hk[16];
 #pragma unroll
-    for (int k = 0; k < 8; k++) {
+    for (int k = 0; k < 16; k++) {
+        const int off = (k & 7) * G::ROW_STRIDE + (k >> 3) * 8;
         const uint32_t sel = GLOBAL ? __ldcg(selp + k) : selp[k];
         const int s = prmt_sx(srow_lo, srow_hi, sel);
         const int M = dg + s + OX;                         // dg = H(i-1,j-1) - OX, or NEG if dead
@@ -148,36 +142,179 @@ static __device__ __forceinline__ void run_group8(int &upH, int &upE, int &dg, i
         const int Fn = __viaddmax_s32(F, -X, Hgl);         // Hgl = H(i,j-1) - OX (ungated: R6 lemma)
         int H = __vimax3_s32(M, E, Fn);
         if (EDGE) { if (col0 + k > m) H = SFE_NEG; }       // beyond the target end
-        const int d = fma_sub(H, T);                       // alive <=> d >= 0 (R5)
-        const int Hg = fma_add(d, tox);                    // H - OX, as d + (T - OX) so that it stays an IMAD
-        const int gmask = d >> 31;                         // 0 alive, -1 dead
+        Hk[k] = H;
+        const bool isdead = H < T;                         // R5: alive <=> H >= T
+        const int Hg = H - OX;
         if (TB) {
+            uint32_t &acc = k < 8 ? acc0 : acc1;
             acc = shift_in_sign(acc, fma_sub(M, H));       // M < H  <=> H not from M
             acc = shift_in_sign(acc, fma_sub(E, H));       // E < H  <=> H not from E
             acc = shift_in_sign(acc, fma_sub(upH, E));     // upH < E <=> E extended (open wins ties)
             acc = shift_in_sign(acc, fma_sub(Hgl, Fn));    // Hgl < F <=> F extended
         }
-        gneg = fma_mad(gneg, 2, gmask);
-        bm = shift_in_sign(bm, fma_sub(best, H));          // best < H <=> new lane-local best
+        if (isdead) dead |= 0x8000u >> k;
+#ifdef SFE_OPT_BEST3
+        if (k & 1) best = __vimax3_s32(best, Hk[k - 1], H);
+#else
         best = max(best, H);
-        const int msgH = lop3_sel(Hg, gmask, SFE_NEG);     // one LOP3: dead cells send NEG
-        *(int2 *)(wptr + k * RingGeom<RL2>::ROW_STRIDE) = make_int2(msgH, E);
+#endif
+        const int msgH = isdead ? SFE_NEG : Hg;            // dead cells send NEG on the diagonal / open edge
+        *(int2 *)(wptr + off) = make_int2(msgH, E);
         dg = upH; F = Fn; Hgl = Hg;
-        __syncwarp();
-        const int2 u = GLOBAL ? __ldcg((const int2 *)(rptr + k * RingGeom<RL2>::ROW_STRIDE))
-                              : *(const int2 *)(rptr + k * RingGeom<RL2>::ROW_STRIDE);
+        SFE_STEP_FENCE();
+        const int2 u = GLOBAL ? __ldcg((const int2 *)(rptr + off)) : *(const int2 *)(rptr + off);
         upH = u.x; upE = u.y;
+    }
+    if (best > best_in) {
+        int kk = 15;
+#pragma unroll
+        for (int k = 14; k >= 0; k--) kk = Hk[k] == best ? k : kk;
+        best_t = t0 + kk;
     }
 }
 
+// ---- a8, first part: warp-cooperative traceback walk ---------------------------------------------
+// Runs in the warp that has just finished the half, while its records are the most recently
+// written lines of the arena.  Control flow is uniform: every lane holds the same (i, j, state).
+// A window of SFE_WALK_WIN_RECS records of the current strip is copied to shared memory (each lane
+// loads its own 8 bytes of every record: coalesced); then up to 32 consecutive path cells are
+// examined at once -- lane k looks at the k-th cell in the current direction (diagonal for state
+// H, up for E, left for F, R11) -- and a ballot finds where the run stops.
+struct TbReader {                       // random access to this half's records; all lanes hold the same cursor
+    const uint32_t *pool; const int32_t *chunk_prev;
+    int chunk, ord, last_chunk, last_ord, nrec;
+    bool bad;                           // an index outside the half's records was asked for (never expected)
+    __device__ __forceinline__ const uint32_t *rec(int ridx)
+    {
+        if (ridx < 0 || ridx >= nrec) { bad = true; ridx = 0; }
+        const int o = ridx / SFE_CHUNK_RECS;
+        if (o > ord) { chunk = last_chunk; ord = last_ord; }   // rare: the indices are visited in decreasing order
+        while (ord > o) { chunk = __ldcg(chunk_prev + chunk); ord--; }
+        return pool + ((size_t)chunk * SFE_CHUNK_RECS + (ridx - o * SFE_CHUNK_RECS)) * SFE_REC_WORDS;
+    }
+};
+
+struct OpsWriter {                      // run-length encoder + staging of the ops in walk order
+    uint32_t *buf;                      // SFE_WALK_OPS words of shared memory
+    uint32_t *stage; unsigned long long *used; unsigned long long cap;
+    int nbuf, nops, cur_op, run; uint32_t prev_seg; bool ok;
+    __device__ __forceinline__ void flush(int lane)
+    {
+        if (nbuf == 0) return;
+        __syncwarp();
+        if (ok) {
+            unsigned long long base = 0;
+            if (lane == 0) base = atomicAdd(used, (unsigned long long)(nbuf + 2));
+            base = __shfl_sync(FULL, base, 0);
+            if (base + (unsigned long long)(nbuf + 2) > cap) ok = false;
+            else {
+                if (lane == 0) { stage[base] = prev_seg; stage[base + 1] = (uint32_t)nbuf; }
+                for (int x = lane; x < nbuf; x += 32) stage[base + 2 + x] = buf[x];
+                prev_seg = (uint32_t)base;
+            }
+        }
+        nbuf = 0;
+        __syncwarp();
+    }
+    __device__ __forceinline__ void push(int lane)
+    {
+        if (lane == 0) buf[nbuf] = ((uint32_t)run << 4) | (uint32_t)cur_op;
+        nbuf++; nops++;
+        if (nbuf == SFE_WALK_OPS) flush(lane);
+    }
+    __device__ __forceinline__ void emit(int op, int cnt, int lane)
+    {
+        if (cnt <= 0) return;
+        if (op == cur_op) { run += cnt; return; }
+        if (cur_op >= 0) push(lane);
+        cur_op = op; run = cnt;
+    }
+};
+
+// Returns false if the walk did not reach the origin (internal error guard).
+static __device__ bool walk_traceback(const YdParams &p, TbReader &rd, const int end_i, const int end_j, int hdr, int strip,
+                                      char *wk, const int lane, uint32_t &ops_seg, int &n_ops, bool &ops_ok)
+{
+    uint32_t *win = (uint32_t *)wk;
+    OpsWriter ow;
+    ow.buf = (uint32_t *)(wk + SFE_WALK_WIN_RECS * SFE_REC_BYTES);
+    ow.stage = p.ops_stage; ow.used = &p.counters[CNT_OPS]; ow.cap = p.ops_cap;
+    ow.nbuf = 0; ow.nops = 0; ow.cur_op = -1; ow.run = 0; ow.prev_seg = SFE_NO_SEG; ow.ok = true;
+    ops_seg = SFE_NO_SEG; n_ops = 0; ops_ok = true;
+    if (end_i == 0 && end_j == 0) return true;
+    __syncwarp();                                        // the records of this half, written lane by lane, are visible
+    int i = end_i, j = end_j, state = 0;
+    const uint32_t *hr = rd.rec(hdr);
+    int cs = (int)__ldcg(hr), prev_hdr = (int)__ldcg(hr + 1);
+    while (strip > (i >> 5)) { hdr = prev_hdr; strip--; hr = rd.rec(hdr); cs = (int)__ldcg(hr); prev_hdr = (int)__ldcg(hr + 1); }
+    int win_lo = 0, win_hi = -1;                         // record groups of this strip held in win[]
+    long long guard = 3LL * ((long long)end_i + end_j) + 4LL * (strip + 1) + 64;
+    while (!(i == 0 && j == 0 && state == 0)) {
+        if (--guard < 0 || rd.bad) return false;
+        if ((i >> 5) < strip) {                          // crossed into the strip above
+            hdr = prev_hdr; strip--;
+            hr = rd.rec(hdr); cs = (int)__ldcg(hr); prev_hdr = (int)__ldcg(hr + 1);
+            win_hi = -1;
+        }
+        const int L = i & 31;
+        const int t = j - cs + L;                        // step of cell (i, j) in its strip
+        const int g = t >> 4;
+        if (g > win_hi || g < win_lo) {                  // (re)load the window: groups g-7 .. g
+            __syncwarp();
+            win_hi = g; win_lo = max(0, g - (SFE_WALK_WIN_RECS - 1));
+            for (int x = win_hi; x >= win_lo; x--) {
+                const uint2 v = __ldcg((const uint2 *)(rd.rec(hdr + 1 + x) + 2 * lane));
+                *(uint2 *)(win + (x - win_lo) * SFE_REC_WORDS + 2 * lane) = v;
+            }
+            __syncwarp();
+        }
+        // lane k examines the k-th cell from (i, j) in the direction of the current state
+        const int di = state == 2 ? 0 : 1, dj = state == 1 ? 0 : 1;
+        const int Lk = L - lane * di;
+        const int tk = t - lane * (di + dj);
+        const bool valid = Lk >= 0 && tk >= 0 && (tk >> 4) >= win_lo;
+        uint32_t nib = 0;
+        if (valid) nib = (win[((tk >> 4) - win_lo) * SFE_REC_WORDS + 2 * Lk + ((tk >> 3) & 1)] >> ((7 - (tk & 7)) * 4)) & 15u;
+        // nib: bit3 = H not from M, bit2 = H not from E, bit1 = E extended, bit0 = F extended
+        const bool cont = state == 0 ? !(nib & 8u) : (state == 1 ? (nib & 2u) != 0 : (nib & 1u) != 0);
+        const bool origin = i == lane * di && j == lane * dj;   // the walk ends at (0,0), whose own nibble says "from M"
+        const uint32_t stop = __ballot_sync(FULL, !(valid && cont) || origin);
+        const uint32_t vmask = __ballot_sync(FULL, valid);
+        const int pstop = stop ? __ffs(stop) - 1 : 32;   // cells 0 .. pstop-1 continue the run
+        const bool stop_valid = pstop < 32 && ((vmask >> pstop) & 1u);
+        if (state == 0) {
+            ow.emit(SFE_OP_M, pstop, lane);
+            i -= pstop; j -= pstop;
+            if (stop_valid && !(i == 0 && j == 0)) {     // cell pstop is not from M: switch to its gap state, same cell
+                const uint32_t nb = __shfl_sync(FULL, nib, pstop);
+                state = (nb & 4u) ? 2 : 1;
+            }
+        } else if (state == 1) {                         // E: every visited cell emits I; the cell that opened returns to H
+            const int cnt = stop_valid ? pstop + 1 : pstop;
+            ow.emit(SFE_OP_I, cnt, lane);
+            i -= cnt;
+            if (stop_valid) state = 0;
+        } else {                                         // F likewise with D
+            const int cnt = stop_valid ? pstop + 1 : pstop;
+            ow.emit(SFE_OP_D, cnt, lane);
+            j -= cnt;
+            if (stop_valid) state = 0;
+        }
+    }
+    if (ow.cur_op >= 0) ow.push(lane);
+    ow.flush(lane);
+    ops_seg = ow.prev_seg; n_ops = ow.nops; ops_ok = ow.ok;
+    return true;
+}
+
 template <bool TB, int RL2, bool GLOBAL>
-static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, const int lane)
+static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, char *wk, const int lane)
 {
     typedef RingGeom<RL2> G;
     uint16_t *selring = (uint16_t *)(wsm + 8 * G::ROW_STRIDE);
     sfe_half out;
     out.score = 0; out.end_i = 0; out.end_j = 0; out.status = 0; out.cells = 0;
-    out.last_hdr = -1; out.last_chunk = -1; out.n_strips = 0; out.n_rec = 0; out.steps = 0; out.max_steps = 0;
+    out.ops_seg = SFE_NO_SEG; out.n_ops = 0; out.n_strips = 0; out.n_rec = 0; out.steps = 0; out.max_steps = 0;
 
     const long long a = hid >> 1;
     const int dir = hid & 1;
@@ -237,60 +374,70 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
         else if (r == 0) srow_lo = 0u;
         else srow_lo = p.srow[sfe_base(g.qc, g.qm, g.q0 + (long long)g.d * r)];
         const uint32_t srow_hi = p.srow_hi;
-        const int tox = T - OX;
 
-        if (TB) {   // strip header record: word0 = cs, word1 = previous header's record index
+        if (TB) {   // strip header record: lane 0's word pair = (cs, previous header's record index)
             const int hdr = tb.nrec;
-            tb.put(lane == 0 ? (uint32_t)cs : (lane == 1 ? (uint32_t)last_hdr : (uint32_t)s), lane);
+            tb.put(lane == 0 ? (uint32_t)cs : (uint32_t)s, lane == 0 ? (uint32_t)last_hdr : 0u, lane);
             last_hdr = hdr;
         }
         n_strips++;
 
         if (sel_hi < cs - 32) sel_hi = cs - 32;
         if (bnd_valid <= cs) { fill_bnd_neg<RL2>(wsm, bnd_valid, cs + 64, lane); bnd_valid = cs + 64; }
+        int refill_at = min(sel_hi, bnd_valid - 1);         // first cmax that needs a ring refill
         int upH = SFE_NEG, upE = SFE_NEG, dg = SFE_NEG, F = SFE_NEG, Hgl = SFE_NEG;
         if (lane == 0) {
             const int2 u = GLOBAL ? __ldcg((const int2 *)(wsm + bnd_off<RL2>(cs))) : *(const int2 *)(wsm + bnd_off<RL2>(cs));
             upH = u.x; upE = u.y;
             if (s == 0) dg = -OX;                           // R8: H(0,0) = 0 enters as the diagonal of (0,0)
         }
-        int first_t = 0x7fffffff, last_t = -1, best_t = -1;   // step indices of the first / last alive cell of my row
-        uint32_t bm = 0;
+        // alive bits (step k of the group at bit 15-k) of the first / last group of my row that had an alive cell
+        uint32_t first_al = 0, last_al = 0;
+        int first_g = 0, last_g = 0, best_t = -1;
         const int best_before = best;
         int t0 = 0;
         bool bail = false;
+        // Message pointers.  Lanes 1..31 read the exchange slot of the lane above and lanes 0..30 write
+        // their own (fixed addresses); lane 0 reads and lane 31 writes the boundary ring, whose byte
+        // offset advances by 16 (two segments) per group.
         const bool is0 = lane == 0, is31 = lane == 31;
-        char *const exch_w = wsm + lane * 8;
-        const char *const exch_r = wsm + (lane - 1) * 8;
         char *const bnd = wsm + SFE_EXCH_BYTES;
-        int gneg = 0;
-        for (;; t0 += 8) {
-            const int cmax = cs + t0 + 7;                   // lane 0's last column of this group
-            if (sel_hi <= cmax) { fill_sel<RL2>(selring, g, sel_hi, cmax + 129, lane); sel_hi = cmax + 129; }
-            if (bnd_valid <= cmax + 1) { fill_bnd_neg<RL2>(wsm, bnd_valid, bnd_valid + 64, lane); bnd_valid += 64; }
-            const int base8 = (cs + t0) >> 3;
-            const char *rptr = is0 ? bnd + ((base8 + 1) & (G::RING / 8 - 1)) * 8 : exch_r;
-            char *wptr = is31 ? bnd + ((base8 - 3) & (G::RING / 8 - 1)) * 8 : exch_w;
+        const char *const rbase = is0 ? bnd : wsm + (lane - 1) * 8;
+        char *const wbase = is31 ? bnd : wsm + lane * 8;
+        const int rstride = is0 ? 16 : 0, wstride = is31 ? 16 : 0;
+        int roff = is0 ? (cs & (G::RING - 1)) : 0;           // column cs+t0+k+1 -> segment (cs+t0)/8 + (k>>3)
+        int woff = is31 ? ((cs - 32) & (G::RING - 1)) : 0;   // column cs+t0+k-31 -> segment (cs+t0-32)/8 + (k>>3)
+        for (;; t0 += 16) {
+            const int cmax = cs + t0 + 15;                  // lane 0's last column of this group
+            if (cmax >= refill_at) {
+                if (sel_hi <= cmax) { fill_sel<RL2>(selring, g, sel_hi, cmax + 129, lane); sel_hi = cmax + 129; }
+                if (bnd_valid <= cmax + 1) { fill_bnd_neg<RL2>(wsm, bnd_valid, bnd_valid + 64, lane); bnd_valid += 64; }
+                refill_at = min(sel_hi, bnd_valid - 1);
+            }
+            const char *rptr = rbase + roff;
+            char *wptr = wbase + woff;
+            roff = (roff + rstride) & (G::RING - 1);
+            woff = (woff + wstride) & (G::RING - 1);
             const int col0 = cs + t0 - lane;
             const uint16_t *selp = selring + (col0 & (G::SELRING - 1));
-            uint32_t acc = 0;
+            uint32_t acc0 = 0, acc1 = 0, dead = 0;
             if (cmax > g.m)
-                run_group8<TB, true, RL2, GLOBAL>(upH, upE, dg, F, Hgl, best, bm, acc, gneg, srow_lo, srow_hi, T, OX, tox, X, rptr, wptr,
-                                     selp, col0, g.m);
+                run_group16<TB, true, RL2, GLOBAL>(upH, upE, dg, F, Hgl, best, best_t, acc0, acc1, dead, srow_lo, srow_hi, T, OX, X,
+                                                   rptr, wptr, selp, col0, g.m, t0);
             else
-                run_group8<TB, false, RL2, GLOBAL>(upH, upE, dg, F, Hgl, best, bm, acc, gneg, srow_lo, srow_hi, T, OX, tox, X, rptr, wptr,
-                                      selp, col0, g.m);
-            if (TB) tb.put(acc, lane);
-            const uint32_t al = ~(uint32_t)(-gneg) & 0xffu; // alive bits of this group, step k at bit 7-k
-            if (bm & 0xffu) best_t = t0 + 8 - __ffs(bm & 0xffu);   // the latest strict increase of this group
+                run_group16<TB, false, RL2, GLOBAL>(upH, upE, dg, F, Hgl, best, best_t, acc0, acc1, dead, srow_lo, srow_hi, T, OX, X,
+                                                    rptr, wptr, selp, col0, g.m, t0);
+            if (TB) tb.put(acc0, acc1, lane);
+            const uint32_t al = ~dead & 0xffffu;
             if (al) {
-                first_t = min(first_t, t0 + __clz(al) - 24);
-                last_t = t0 + 8 - __ffs(al);
+                if (!first_al) { first_al = al; first_g = t0; }
+                last_al = al; last_g = t0;
             }
-            if (!__any_sync(FULL, al != 0) && cs + t0 + 8 > prevR + 1) { t0 += 8; break; }
-            if (t0 + 8 >= G::MAX_STEPS) { t0 += 8; bail = true; break; }
+            if (!__any_sync(FULL, al != 0) && cs + t0 + 16 > prevR + 1) { t0 += 16; break; }
+            if (t0 + 16 >= G::MAX_STEPS) { t0 += 16; bail = true; break; }
         }
-        const int first = last_t < 0 ? 0x7fffffff : cs - lane + first_t, last = last_t < 0 ? -1 : cs - lane + last_t;
+        const int first = first_al ? cs - lane + first_g + __clz(first_al) - 16 : 0x7fffffff;
+        const int last = last_al ? cs - lane + last_g + 16 - __ffs(last_al) : -1;
         total_steps += t0;
         if (t0 > max_steps) max_steps = t0;
         if (bail) { wide = true; break; }
@@ -301,7 +448,7 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
         if (R31 < 0) break;                                 // last row of the strip has no alive cell
         bnd_valid = cs + t0 - 31;                           // lane 31 wrote columns cs-31 .. cs+t0-32
         prevR = R31;
-        cs = L31 & ~7;
+        cs = L31 & ~15;
     }
 
     // warp reduction of the lane-local first maxima: key (score desc, i asc, j asc) (R7)
@@ -314,17 +461,29 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) cells += __shfl_xor_sync(FULL, cells, o);
+    // every lane holds the same winner; the broadcast makes that visible to the compiler's uniformity
+    // analysis, so that the walk below (and the next half after it) compiles as warp-uniform code
+    bs = __shfl_sync(FULL, bs, 0); bi = __shfl_sync(FULL, bi, 0); bj = __shfl_sync(FULL, bj, 0);
 
     out.score = bs; out.end_i = bi; out.end_j = bj; out.cells = cells;
     // normal kernel: a bail-out is re-run by the wide kernel; wide kernel: a bail-out is final (band limit)
     out.status = (wide ? (GLOBAL ? (SFE_ST_WIDE | SFE_ST_BAND_LIMIT) : SFE_ST_WIDE_PENDING) : (GLOBAL ? SFE_ST_WIDE : 0u)) |
-                 ((TB && !tb.ok) ? ST_PASS_OVERFLOW : 0u);
-    out.last_hdr = last_hdr; out.last_chunk = tb.cur_chunk; out.n_strips = n_strips; out.n_rec = tb.nrec;
+                 ((TB && !tb.ok) ? SFE_ST_PASS_OVERFLOW : 0u);
+    out.n_strips = n_strips; out.n_rec = tb.nrec;
+    if (TB && tb.ok && !wide) {                             // a8: walk the pointers now, stage the run-length ops
+        TbReader rd;
+        rd.pool = p.pool; rd.chunk_prev = p.chunk_prev; rd.chunk = tb.cur_chunk; rd.ord = (tb.nrec - 1) / SFE_CHUNK_RECS;
+        rd.last_chunk = rd.chunk; rd.last_ord = rd.ord; rd.nrec = tb.nrec; rd.bad = false;
+        bool ops_ok = true;
+        if (!walk_traceback(p, rd, bi, bj, last_hdr, n_strips - 1, wk, lane, out.ops_seg, out.n_ops, ops_ok))
+            out.status |= SFE_ST_INTERNAL;
+        if (!ops_ok) out.status |= SFE_ST_OPS_OVERFLOW;
+    }
     out.steps = total_steps; out.max_steps = max_steps;
     if (lane == 0) {
         p.halves[hid] = out;
         atomicAdd(&p.counters[CNT_STEPS], (unsigned long long)total_steps);
-        if (TB) atomicAdd(&p.counters[CNT_TBBYTES], (unsigned long long)tb.nrec * 128ULL);
+        if (TB) atomicAdd(&p.counters[CNT_TBBYTES], (unsigned long long)tb.nrec * (unsigned long long)SFE_REC_BYTES);
         if (TB && !tb.ok) atomicAdd(&p.counters[CNT_OVERFLOW], 1ULL);
         if (wide && !GLOBAL) atomicAdd(&p.counters[CNT_WIDE], 1ULL);
     }
@@ -342,7 +501,7 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS) ydrop_kernel(const YdParams
         if (lane == 0) tk = atomicAdd(&p.counters[CNT_TICKET], 1ULL);
         tk = __shfl_sync(FULL, tk, 0);
         if ((long long)tk >= p.n_tickets) break;
-        extend_half<TB, SFE_RING_LOG2, false>(p, p.tickets[tk], wsm, lane);
+        extend_half<TB, SFE_RING_LOG2, false>(p, p.tickets[tk], wsm, wsm, lane);
         __syncwarp();
     }
 }
@@ -361,6 +520,7 @@ __global__ void select_wide_kernel(const YdParams p)
 template <bool TB>
 __global__ void __launch_bounds__(32) ydrop_wide_kernel(const YdParams p)
 {
+    __shared__ __align__(16) char wk[SFE_WALK_SMEM];         // traceback-walk window + ops staging (the rings are in global memory)
     const int lane = sfe_lane();
     char *wsm = p.wide_ring + (size_t)blockIdx.x * RingGeom<SFE_WIDE_RING_LOG2>::WARP_BYTES;
     const long long n = (long long)*((volatile unsigned long long *)&p.counters[CNT_WIDE_N]);
@@ -369,7 +529,7 @@ __global__ void __launch_bounds__(32) ydrop_wide_kernel(const YdParams p)
         if (lane == 0) tk = atomicAdd(&p.counters[CNT_WIDE_TICKET], 1ULL);
         tk = __shfl_sync(FULL, tk, 0);
         if ((long long)tk >= n) break;
-        extend_half<TB, SFE_WIDE_RING_LOG2, true>(p, p.wide_tickets[tk], wsm, lane);
+        extend_half<TB, SFE_WIDE_RING_LOG2, true>(p, p.wide_tickets[tk], wsm, wk, lane);
         __syncwarp();
     }
 }
