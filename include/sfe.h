@@ -159,6 +159,18 @@ int sfe_extend_host(sfe_ctx *ctx, const char *t_ascii_host, int64_t t_len, const
  * [5] halves that took the wide path, [6] device time of the Y-drop kernel launches in microseconds
  * (CUDA events on the ctx stream; synchronises on the last one). */
 int sfe_probe_int_issue(sfe_ctx *ctx, int mix, int iters, double *lane_ops_per_clk_per_sm, double *elapsed_ms);
+
+/* Per-half profile of the most recent sfe_ydrop_batch on this ctx (Fig. 5: the
+ * spread of per-anchor extension runtimes is what defeats static load balancing).  Entry 2a is the
+ * forward half of anchor a, 2a+1 the backward half.  cycles = SM clock cycles from ticket to
+ * result (DP + traceback walk), steps = warp wavefronts, smid / wslot = where it ran.  Copies
+ * min(n, 2 * n_anchors) entries to profile_host; synchronises the stream. */
+typedef struct {
+    int64_t cells, cycles;
+    int32_t steps, n_strips, max_steps, n_ops;
+    uint32_t smid, wslot, status, reserved;
+} sfe_half_profile;
+int sfe_last_half_profile(sfe_ctx *ctx, int64_t n, sfe_half_profile *profile_host);
 int sfe_last_batch_info(sfe_ctx *ctx, int64_t info[8]);
 
 #ifdef __cplusplus

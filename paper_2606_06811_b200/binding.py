@@ -23,7 +23,7 @@ ST_TB_OVERFLOW, ST_CIGAR_OVERFLOW, ST_WIDE, ST_SCORE_LIMIT, ST_BAD_ANCHOR, ST_BA
 OP_M, OP_I, OP_D = 0, 1, 2
 
 EXPORTS = ("sfe_create", "sfe_destroy", "sfe_strerror", "sfe_last_error_detail", "sfe_pack", "sfe_ydrop_batch", "sfe_resolve",
-           "sfe_extend_host", "sfe_probe_int_issue", "sfe_last_batch_info")
+           "sfe_extend_host", "sfe_probe_int_issue", "sfe_last_batch_info", "sfe_last_half_profile")
 
 
 class Scoring(C.Structure):
@@ -46,6 +46,8 @@ BOX_DT = np.dtype([("tstart", "<i8"), ("tend", "<i8"), ("qstart", "<i8"), ("qend
                    ("strand", "<i4"), ("reserved", "<i4")])
 STATS_DT = np.dtype([("n_anchors", "<i8"), ("n_kept", "<i8"), ("n_covered", "<i8"), ("n_below", "<i8"),
                      ("cells_total", "<u8"), ("cells_covered", "<u8")])
+HALF_PROFILE_DT = np.dtype([("cells", "<i8"), ("cycles", "<i8"), ("steps", "<i4"), ("n_strips", "<i4"), ("max_steps", "<i4"),
+                            ("n_ops", "<i4"), ("smid", "<u4"), ("wslot", "<u4"), ("status", "<u4"), ("reserved", "<u4")])
 assert ANCHOR_DT.itemsize == 24 and PAIR_DT.itemsize == 32 and RESULT_DT.itemsize == 72 and BOX_DT.itemsize == 40
 
 HOXD70 = ((91, -114, -31, -123), (-114, 100, -125, -31), (-31, -125, 100, -114), (-123, -31, -114, 91))
@@ -77,6 +79,7 @@ def lib():
         _lib.sfe_resolve.argtypes = [vp, vp, vp, i64, i32, vp, i64, vp, vp, vp]
         _lib.sfe_extend_host.argtypes = [vp, vp, i64, vp, i64, vp, i32, vp, i64, C.POINTER(Scoring), u32,
                                          vp, vp, vp, i64, C.POINTER(i64), C.POINTER(Stats)]
+        _lib.sfe_last_half_profile.argtypes = [vp, i64, vp]
         _lib.sfe_probe_int_issue.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib.sfe_last_batch_info.argtypes = [vp, C.POINTER(i64)]
     return _lib
@@ -223,10 +226,16 @@ class Sfe:
         _check(lib().sfe_probe_int_issue(self.h, mix, iters, C.byref(r), C.byref(ms)), "sfe_probe_int_issue")
         return r.value, ms.value
 
+    def last_half_profile(self, n_halves: int) -> np.ndarray:
+        """Per-half (cells, cycles, steps, SM, warp slot, ...) of the most recent ydrop_batch (entry 2a / 2a+1 = fwd / bwd of anchor a)."""
+        out = np.zeros(max(n_halves, 1), dtype=HALF_PROFILE_DT)
+        _check(lib().sfe_last_half_profile(self.h, n_halves, C.c_void_p(out.ctypes.data)), "sfe_last_half_profile")
+        return out[:n_halves]
+
     def last_batch_info(self):
         a = (C.c_int64 * 8)()
         _check(lib().sfe_last_batch_info(self.h, a), "sfe_last_batch_info")
-        keys = ("launches", "halves", "halves_rerun", "tb_bytes", "steps", "wide", "ydrop_kernel_us", "r7")
+        keys = ("launches", "halves", "halves_rerun", "tb_bytes", "steps", "wide", "ydrop_kernel_us", "n_profile")
         return dict(zip(keys, list(a)))
 
 

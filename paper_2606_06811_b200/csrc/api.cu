@@ -2,6 +2,7 @@
 // Every step of the path runs in the kernels of this directory; there is no CPU fallback.
 #include <new>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 #include "sfe_internal.cuh"
 
@@ -20,8 +21,9 @@ int sfe_launch_resolve(const sfe_anchor *anchors, const sfe_result *results, lon
 int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe_pair *pairs, int n_pairs, long long q_len,
                        bool binned, unsigned int *hist, int32_t *tickets, cudaStream_t st);
 int sfe_launch_select_overflow(const sfe_half *halves, long long n_anchors, long long *sel, int32_t *tickets,
-                               unsigned long long *n_sel, cudaStream_t st);
+                               unsigned long long *counters, int n_chunks, cudaStream_t st);
 int sfe_launch_probe(int mix, int iters, int blocks, int *sink, cudaStream_t st);
+int sfe_launch_ring_init(int32_t *ring, SfeFreeRing *st, int n_chunks, cudaStream_t stream);
 
 struct DevBuf {                       // grow-only device scratch
     void *p = nullptr; size_t cap = 0;
@@ -40,7 +42,7 @@ struct DevBuf {                       // grow-only device scratch
 
 struct sfe_ctx {
     int device; cudaStream_t stream; int n_sm; int clock_khz;
-    uint32_t *pool; int32_t *chunk_prev; int n_chunks;
+    uint32_t *pool; int32_t *chunk_prev; int32_t *free_ring; SfeFreeRing *ring_state; int n_chunks;
     unsigned long long *counters;     // device, CNT_N
     unsigned long long *counters_host;  // pinned
     DevBuf halves, tickets, sel, hist, blkmin, act, misc, wide_tickets, wide_ring, ops_stage;
@@ -88,18 +90,21 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
     if (nch < 4) nch = 4;
     if (nch > 0x7ffffff0LL / SFE_CHUNK_RECS) nch = 0x7ffffff0LL / SFE_CHUNK_RECS;   // record indices are int32
     c->n_chunks = (int)nch;
-    c->pool = nullptr; c->chunk_prev = nullptr; c->counters = nullptr; c->counters_host = nullptr;
+    c->pool = nullptr; c->chunk_prev = nullptr; c->free_ring = nullptr; c->ring_state = nullptr; c->counters = nullptr; c->counters_host = nullptr;
     memset(c->info, 0, sizeof c->info);
     c->ev_pending = false; c->kernel_us = 0.0;
     if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) { delete c; return SFE_ECUDA; }
     if (cudaMalloc((void **)&c->pool, (size_t)nch * SFE_CHUNK_BYTES) != cudaSuccess ||
         cudaMalloc((void **)&c->chunk_prev, (size_t)nch * sizeof(int32_t)) != cudaSuccess ||
+        cudaMalloc((void **)&c->free_ring, (size_t)nch * sizeof(int32_t)) != cudaSuccess ||
+        cudaMalloc((void **)&c->ring_state, sizeof(SfeFreeRing)) != cudaSuccess ||
         cudaMalloc((void **)&c->counters, CNT_N * sizeof(unsigned long long)) != cudaSuccess ||
         cudaMallocHost((void **)&c->counters_host, CNT_N * sizeof(unsigned long long)) != cudaSuccess) {
         cudaGetLastError();
         sfe_destroy(c);
         return SFE_ENOMEM;
     }
+    if (sfe_launch_ring_init(c->free_ring, c->ring_state, c->n_chunks, c->stream) != SFE_OK) { sfe_destroy(c); return SFE_ECUDA; }
     *out = c;
     return SFE_OK;
 }
@@ -110,6 +115,8 @@ extern "C" int sfe_destroy(sfe_ctx *c)
     cudaSetDevice(c->device);
     if (c->pool) cudaFree(c->pool);
     if (c->chunk_prev) cudaFree(c->chunk_prev);
+    if (c->free_ring) cudaFree(c->free_ring);
+    if (c->ring_state) cudaFree(c->ring_state);
     if (c->counters) cudaFree(c->counters);
     if (c->counters_host) cudaFreeHost(c->counters_host);
     cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1);
@@ -169,6 +176,25 @@ extern "C" int sfe_last_batch_info(sfe_ctx *c, int64_t info[8])
         else cudaGetLastError();
     }
     for (int k = 0; k < 8; k++) info[k] = c->info[k];
+    return SFE_OK;
+}
+
+extern "C" int sfe_last_half_profile(sfe_ctx *c, int64_t n, sfe_half_profile *out)
+{
+    if (!c || n < 0 || (n > 0 && !out)) return SFE_EINVAL;
+    if (n > c->info[7]) n = c->info[7];
+    if (n == 0) return SFE_OK;
+    SFE_CUDA_CHECK(cudaSetDevice(c->device));
+    sfe_half *h = (sfe_half *)malloc((size_t)n * sizeof(sfe_half));
+    if (!h) return SFE_ENOMEM;
+    if (cudaMemcpyAsync(h, c->halves.p, (size_t)n * sizeof(sfe_half), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess) { cudaGetLastError(); free(h); return SFE_ECUDA; }
+    for (int64_t k = 0; k < n; k++) {
+        out[k].cells = (int64_t)h[k].cells; out[k].cycles = h[k].cycles; out[k].steps = h[k].steps;
+        out[k].n_strips = h[k].n_strips; out[k].max_steps = h[k].max_steps; out[k].n_ops = h[k].n_ops;
+        out[k].smid = h[k].smid; out[k].wslot = h[k].wslot; out[k].status = h[k].status; out[k].reserved = 0;
+    }
+    free(h);
     return SFE_OK;
 }
 
@@ -244,9 +270,9 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
     memset(&p, 0, sizeof p);
     p.t_codes = t_codes2; p.t_nmask = t_nmask; p.q_codes = q_codes2; p.q_nmask = q_nmask;
     p.qrc_codes = qrc_codes2; p.qrc_nmask = qrc_nmask; p.t_len = t_len; p.q_len = q_len;
-    p.pairs = pairs_dev; p.anchors = anchors_dev; p.tickets = (const int32_t *)c->tickets.p; p.n_tickets = 2 * n_anchors;
-    p.counters = c->counters; p.halves = (sfe_half *)c->halves.p; p.pool = c->pool; p.chunk_prev = c->chunk_prev;
-    p.n_chunks = want_tb ? c->n_chunks : 0; p.n_pairs = n_pairs;
+    p.pairs = pairs_dev; p.anchors = anchors_dev; p.tickets = (const int32_t *)c->tickets.p; p.n_tickets = 2 * n_anchors; p.seg_tickets = (flags & SFE_NO_BINNING) ? 0 : 4LL * c->n_sm;
+    p.counters = c->counters; p.halves = (sfe_half *)c->halves.p; p.pool = c->pool; p.chunk_prev = c->chunk_prev; p.free_ring = c->free_ring; p.ring_state = c->ring_state;
+    p.n_chunks = want_tb ? c->n_chunks : 0; p.n_pairs = n_pairs; p.max_warps = 0x7fffffff;
     p.wide_ring = (char *)c->wide_ring.p; p.wide_tickets = (int32_t *)c->wide_tickets.p;
     p.ops_stage = (uint32_t *)c->ops_stage.p; p.ops_cap = ops_cap;
     p.OX = sc->gap_open + sc->gap_extend; p.X = sc->gap_extend;
@@ -263,13 +289,14 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
     if ((rc = sfe_launch_tickets(anchors_dev, n_anchors, pairs_dev, n_pairs, q_len, !(flags & SFE_NO_BINNING),
                                  (unsigned int *)c->hist.p, (int32_t *)c->tickets.p, c->stream))) return rc;
     if ((rc = timed_ydrop(c, p, want_tb))) return rc;
-    c->info[0] += 1; c->info[1] += 2 * n_anchors;
+    c->info[0] += 1; c->info[1] += 2 * n_anchors; c->info[7] = 2 * n_anchors;
     if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, nullptr, n_anchors, want_tb, results_dev, c->stream))) return rc;
     if (!want_tb) return SFE_OK;
     if ((rc = sfe_launch_scan_emit(p.halves, n_anchors, nullptr, n_anchors, p.ops_stage, results_dev, cigar_pool_dev,
                                    cigar_pool_cap, (long long *)cigar_pool_used_dev, c->stream))) return rc;
 
-    // traceback-arena overflow: re-run the anchors that did not fit, with the arena emptied
+    // traceback-arena overflow: a half that found no free chunk finished score-only; every half returns its chunks
+    // when it ends, so the arena is free again here: re-run the anchors that did not fit, among themselves
     long long prev_overflow = -1;
     for (;;) {
         SFE_CUDA_CHECK(cudaMemcpyAsync(c->counters_host, c->counters, CNT_N * sizeof(unsigned long long),
@@ -285,13 +312,17 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
         prev_overflow = n_over;
         SFE_CUDA_CHECK(cudaMemsetAsync(c->counters, 0, CNT_N * sizeof(unsigned long long), c->stream));
         if ((rc = sfe_launch_select_overflow(p.halves, n_anchors, (long long *)c->sel.p, (int32_t *)c->tickets.p,
-                                             &c->counters[CNT_RERUN], c->stream))) return rc;
+                                             c->counters, c->n_chunks, c->stream))) return rc;
         SFE_CUDA_CHECK(cudaMemcpyAsync(c->counters_host, c->counters, CNT_N * sizeof(unsigned long long),
                                        cudaMemcpyDeviceToHost, c->stream));
         SFE_CUDA_CHECK(cudaStreamSynchronize(c->stream));
         const long long n_sel = (long long)c->counters_host[CNT_RERUN];
         if (n_sel <= 0) break;
         p.n_tickets = 2 * n_sel;
+        // admission: every admitted warp can get the chunks of the neediest half, so each pass completes halves
+        const long long need = (long long)c->counters_host[CNT_MAXNEED] > 0 ? (long long)c->counters_host[CNT_MAXNEED] : 1;
+        const long long admit = c->n_chunks / need;
+        p.max_warps = (int)(admit < 1 ? 1 : (admit > 0x7fffffffLL ? 0x7fffffffLL : admit));
         if ((rc = timed_ydrop(c, p, true))) return rc;
         c->info[0] += 1; c->info[1] += 2 * n_sel; c->info[2] += 2 * n_sel;
         if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, (const long long *)c->sel.p, n_sel, 1, results_dev, c->stream))) return rc;

@@ -71,24 +71,52 @@ int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe
     SFE_LAUNCH_CHECK();
 }
 
+// ---- free-chunk ring of the traceback arena (sfe_internal.cuh: SfeFreeRing) ------------------------
+__global__ void ring_init_kernel(int32_t *ring, SfeFreeRing *st, int n_chunks)
+{
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i < n_chunks) ring[i] = (int32_t)i;
+    if (i == 0) { st->head = 0ULL; st->tail = (unsigned long long)n_chunks; st->avail = n_chunks; }
+}
+
+int sfe_launch_ring_init(int32_t *ring, SfeFreeRing *st, int n_chunks, cudaStream_t stream)
+{
+    const int bs = 256;
+    ring_init_kernel<<<(unsigned)((n_chunks + bs - 1) / bs), bs, 0, stream>>>(ring, st, n_chunks);
+    SFE_LAUNCH_CHECK();
+}
+
 // ---- overflow re-run selection --------------------------------------------------------------------
 // Anchors with a half whose traceback did not fit in this pass: append to sel[], and make tickets.
+// A half that overflowed went on score-only to its end, so the chunks it needs are known exactly:
+// one record per strip header and per 16 steps.  Halves that need more than the whole arena are
+// not selected (their anchor keeps SFE_ST_TB_OVERFLOW); the largest need goes to counters[CNT_MAXNEED].
+static __device__ __forceinline__ long long half_need_chunks(const sfe_half &h)
+{
+    const long long recs = (long long)h.n_strips + (long long)h.steps / 16 + 2;
+    return (recs + SFE_CHUNK_RECS - 1) / SFE_CHUNK_RECS;
+}
+
 __global__ void select_overflow_kernel(const sfe_half *halves, long long n_anchors, long long *sel, int32_t *tickets,
-                                       unsigned long long *n_sel)
+                                       unsigned long long *counters, int n_chunks)
 {
     const long long a = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (a >= n_anchors) return;
     if ((halves[2 * a].status | halves[2 * a + 1].status) & SFE_ST_PASS_OVERFLOW) {
-        const unsigned long long k = atomicAdd(n_sel, 1ULL);
+        const long long n0 = half_need_chunks(halves[2 * a]), n1 = half_need_chunks(halves[2 * a + 1]);
+        const long long need = n0 > n1 ? n0 : n1;
+        if (need > n_chunks) return;
+        atomicMax(&counters[CNT_MAXNEED], (unsigned long long)need);
+        const unsigned long long k = atomicAdd(&counters[CNT_RERUN], 1ULL);
         sel[k] = a; tickets[2 * k] = (int32_t)(2 * a); tickets[2 * k + 1] = (int32_t)(2 * a + 1);
     }
 }
 
 int sfe_launch_select_overflow(const sfe_half *halves, long long n_anchors, long long *sel, int32_t *tickets,
-                               unsigned long long *n_sel, cudaStream_t st)
+                               unsigned long long *counters, int n_chunks, cudaStream_t st)
 {
     const int bs = 256;
-    select_overflow_kernel<<<(unsigned)((n_anchors + bs - 1) / bs), bs, 0, st>>>(halves, n_anchors, sel, tickets, n_sel);
+    select_overflow_kernel<<<(unsigned)((n_anchors + bs - 1) / bs), bs, 0, st>>>(halves, n_anchors, sel, tickets, counters, n_chunks);
     SFE_LAUNCH_CHECK();
 }
 

@@ -39,6 +39,9 @@ template <int RL2> struct RingGeom {
 // store per lane) by one warp per group of 16 steps; lane l owns words 2l (steps 0-7) and 2l+1
 // (steps 8-15).  Records live in 64 KiB chunks handed out by an atomic counter; a half's chunks
 // form a backward-linked list (chunk_prev).
+// Chunks are recycled: a lock-free ring of free chunk ids (SfeFreeRing) hands them out and takes them
+// back as soon as the warp that filled them has walked its traceback, so the arena only has to hold
+// what the resident warps need at the same time.
 #define SFE_REC_WORDS 64
 #define SFE_REC_BYTES (SFE_REC_WORDS * 4)
 #define SFE_CHUNK_RECS 256
@@ -65,9 +68,17 @@ struct sfe_half {                 // result of one one-sided extension (a7)
     int32_t n_rec;                // traceback records written
     int32_t steps;                // warp wavefronts executed
     int32_t max_steps;            // widest strip
+    long long cycles;             // SM clock cycles from ticket to result (DP + traceback walk)
+    uint32_t smid, wslot;         // SM and hardware warp slot that ran it
 };
 
-enum { CNT_TICKET = 0, CNT_CHUNK, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_OPS, CNT_N = 16 };
+enum { CNT_TICKET = 0, CNT_UNUSED1, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_OPS, CNT_MAXNEED, CNT_CLASS0, CNT_CLASS1, CNT_CLASS2, CNT_CLASS3, CNT_N = 16 };
+
+struct SfeFreeRing {              // persistent across launches: every half returns its chunks before it ends
+    unsigned long long head;      // pops issued
+    unsigned long long tail;      // pushes issued
+    long long avail;              // chunks that may still be popped (decremented before head moves)
+};
 
 struct YdParams {
     const uint8_t *t_codes, *t_nmask;
@@ -77,11 +88,15 @@ struct YdParams {
     const sfe_anchor *anchors;
     const int32_t *tickets;       // half ids (2*anchor + dir), in issue order
     long long n_tickets;
+    long long seg_tickets;        // tickets reserved per warp-slot class (0 = no reservation), see ydrop_kernel
     unsigned long long *counters; // CNT_*
     sfe_half *halves;             // [2 * n_anchors]
     uint32_t *pool;               // traceback arena
     int32_t *chunk_prev;
+    int32_t *free_ring;           // n_chunks slots: a chunk id, or -1 while the slot is empty
+    SfeFreeRing *ring_state;
     int32_t n_chunks;
+    int32_t max_warps;            // warps of the normal kernel allowed to work in this pass
     int32_t n_pairs;
     int32_t OX, X, Y, ydrop_inf;
     uint32_t srow[5];             // packed int8 scores of a query base A,C,G,T,N against A,C,G,T

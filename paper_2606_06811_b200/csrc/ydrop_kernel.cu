@@ -18,6 +18,9 @@
 #include "sfe_internal.cuh"
 
 #define FULL 0xffffffffu
+#ifndef SFE_MIN_BLOCKS
+#define SFE_MIN_BLOCKS 3
+#endif
 #ifndef SFE_BLOCK_THREADS
 #define SFE_BLOCK_THREADS 192     // 6 warps x 12.3 KB of shared memory; 3 blocks = 18 warps per SM
 #endif
@@ -58,15 +61,37 @@ static __device__ __forceinline__ uint32_t col_selector(const HalfGeom &g, int c
     return b == 4 ? 0xCCC4u : 0x8880u + 0x1111u * (uint32_t)b;
 }
 
-// fill selector-ring entries for columns [lo, hi)
+// fill selector-ring entries for columns [lo, hi).  Common case (every column has a target base): each
+// lane takes one byte of the 2-bit plane = 4 bases, plus their 4 mask bits -- two loads per 4 columns.
 template <int RL2>
 static __device__ __forceinline__ void fill_sel(uint16_t *selring, const HalfGeom &g, int lo, int hi, int lane)
 {
-    for (int c = lo + lane; c < hi; c += 32) {
-        const uint16_t v = (uint16_t)col_selector(g, c);
-        const int idx = c & (RingGeom<RL2>::SELRING - 1);
-        selring[idx] = v;
-        if (idx < 16) selring[idx + RingGeom<RL2>::SELRING] = v;
+    typedef RingGeom<RL2> G;
+    if (lo <= 0 || hi - 1 > g.m) {                          // strip start / right edge of the DP matrix: per column
+        for (int c = lo + lane; c < hi; c += 32) {
+            const uint16_t v = (uint16_t)col_selector(g, c);
+            const int idx = c & (G::SELRING - 1);
+            selring[idx] = v;
+            if (idx < 16) selring[idx + G::SELRING] = v;
+        }
+    } else {
+        const long long ka = g.t0 + (long long)g.d * lo, kb = g.t0 + (long long)g.d * (hi - 1);
+        const long long kmin = ka < kb ? ka : kb, kmax = ka < kb ? kb : ka;
+        for (long long B = (kmin >> 2) + lane; B <= (kmax >> 2); B += 32) {
+            const uint32_t cb = g.tc[B];
+            const uint32_t mb = (uint32_t)g.tm[B >> 1] >> ((B & 1) * 4);
+#pragma unroll
+            for (int e = 0; e < 4; e++) {
+                const int c = g.d * (int)(4 * B + e - g.t0);
+                if (c >= lo && c < hi) {
+                    const uint32_t code = (cb >> (2 * e)) & 3u;
+                    const uint16_t v = (uint16_t)(((mb >> e) & 1u) ? 0xCCC4u : 0x8880u + 0x1111u * code);
+                    const int idx = c & (G::SELRING - 1);
+                    selring[idx] = v;
+                    if (idx < 16) selring[idx + G::SELRING] = v;
+                }
+            }
+        }
     }
     __syncwarp();
 }
@@ -79,8 +104,45 @@ static __device__ __forceinline__ void fill_bnd_neg(char *wbase, int lo, int hi,
     __syncwarp();
 }
 
+// Free-chunk ring (sfe_internal.cuh).  Called by the whole warp; lane 0 does the memory operations and
+// every loop runs on a broadcast value, so control flow stays warp-uniform (a loop inside a
+// lane-divergent region makes ptxas clone the whole DP loop with real WARPSYNCs).  Both spins wait
+// for one bounded action of another resident warp (the matching push / pop has already reserved the
+// slot), never for work.
+static __device__ __forceinline__ int chunk_pop(int32_t *ring, SfeFreeRing *st, int n_chunks, int lane)
+{
+    long long a = 0; unsigned long long h = 0;
+    if (lane == 0) {
+        a = (long long)atomicAdd((unsigned long long *)&st->avail, ~0ULL);            // avail--
+        if (a <= 0) atomicAdd((unsigned long long *)&st->avail, 1ULL);                // nothing left: undo
+        else h = atomicAdd(&st->head, 1ULL);
+    }
+    a = __shfl_sync(FULL, a, 0);
+    if (a <= 0) return -1;
+    volatile int32_t *slot = ring + (h % (unsigned long long)n_chunks);
+    int id = -1;
+    do {
+        if (lane == 0) id = *slot;
+        id = __shfl_sync(FULL, id, 0);
+    } while (id < 0);
+    if (lane == 0) *slot = -1;
+    return id;
+}
+static __device__ __forceinline__ void chunk_push(int32_t *ring, SfeFreeRing *st, int n_chunks, int id, int lane)
+{
+    unsigned long long t = 0;
+    if (lane == 0) t = atomicAdd(&st->tail, 1ULL);
+    int32_t *slot = ring + (t % (unsigned long long)n_chunks);
+    int old = -1;
+    do {                                                   // the pop that owns this slot may not have emptied it yet
+        if (lane == 0) old = atomicCAS(slot, -1, id);
+        old = __shfl_sync(FULL, old, 0);
+    } while (old != -1);
+    if (lane == 0) atomicAdd((unsigned long long *)&st->avail, 1ULL);
+}
+
 struct TbWriter {
-    uint32_t *pool; int32_t *chunk_prev; unsigned long long *counters; int n_chunks;
+    uint32_t *pool; int32_t *chunk_prev; int32_t *ring; SfeFreeRing *ring_state; int n_chunks;
     uint32_t *ptr;          // this lane's word pair of the next record
     int left;               // records left in the current chunk
     int cur_chunk; int nrec; bool ok;
@@ -88,10 +150,8 @@ struct TbWriter {
     {
         if (!ok) return;
         if (left == 0) {
-            int c = 0;
-            if (lane == 0) c = (int)atomicAdd(&counters[CNT_CHUNK], 1ULL);
-            c = __shfl_sync(FULL, c, 0);
-            if (c >= n_chunks) { ok = false; return; }
+            const int c = chunk_pop(ring, ring_state, n_chunks, lane);
+            if (c < 0) { ok = false; return; }
             if (lane == 0) chunk_prev[c] = cur_chunk;
             cur_chunk = c;
             ptr = pool + (size_t)c * SFE_CHUNK_RECS * SFE_REC_WORDS + 2 * lane;
@@ -99,6 +159,23 @@ struct TbWriter {
         }
         *(uint2 *)ptr = make_uint2(w0, w1);
         ptr += SFE_REC_WORDS; left--; nrec++;
+    }
+    // give every chunk of this half back (after the walk, or when the half is abandoned)
+    __device__ __forceinline__ void release(int lane)
+    {
+        // One fence per half: this warp's record stores must have landed before a chunk changes owner.
+        // (A gpu-scope fence also invalidates the SM's L1, so it is not done per chunk.)
+#ifndef SFE_DBG_NOFENCE
+        __threadfence();
+#endif
+        __syncwarp();
+        int c = cur_chunk;
+        while (c >= 0) {
+            const int prev = __ldcg(chunk_prev + c);        // same address in every lane
+            chunk_push(ring, ring_state, n_chunks, c, lane);
+            c = prev;
+        }
+        cur_chunk = -1;
     }
 };
 
@@ -315,6 +392,8 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
     sfe_half out;
     out.score = 0; out.end_i = 0; out.end_j = 0; out.status = 0; out.cells = 0;
     out.ops_seg = SFE_NO_SEG; out.n_ops = 0; out.n_strips = 0; out.n_rec = 0; out.steps = 0; out.max_steps = 0;
+    out.cycles = 0; out.smid = 0; out.wslot = 0;
+    const long long clk0 = clock64();
 
     const long long a = hid >> 1;
     const int dir = hid & 1;
@@ -342,7 +421,7 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
 
     const int OX = p.OX, X = p.X;
     TbWriter tb;
-    tb.pool = p.pool; tb.chunk_prev = p.chunk_prev; tb.counters = p.counters; tb.n_chunks = p.n_chunks;
+    tb.pool = p.pool; tb.chunk_prev = p.chunk_prev; tb.ring = p.free_ring; tb.ring_state = p.ring_state; tb.n_chunks = p.n_chunks;
     tb.cur_chunk = -1; tb.nrec = 0; tb.ok = TB; tb.ptr = nullptr; tb.left = 0;
 
     int best = 0, best_i = 0, best_j = 0;     // lane-local first maximum
@@ -479,7 +558,14 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
             out.status |= SFE_ST_INTERNAL;
         if (!ops_ok) out.status |= SFE_ST_OPS_OVERFLOW;
     }
+    if (TB) tb.release(lane);
     out.steps = total_steps; out.max_steps = max_steps;
+    {   // per-half profile (Fig. 5: per-anchor runtime spread): SM cycles spent, where it ran
+        unsigned smid, wslot;
+        asm("mov.u32 %0, %%smid;" : "=r"(smid));
+        asm("mov.u32 %0, %%warpid;" : "=r"(wslot));
+        out.cycles = clock64() - clk0; out.smid = smid; out.wslot = wslot;
+    }
     if (lane == 0) {
         p.halves[hid] = out;
         atomicAdd(&p.counters[CNT_STEPS], (unsigned long long)total_steps);
@@ -491,18 +577,39 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
 
 // Persistent kernel: every warp pulls anchor-half tickets from one atomic counter (a3).
 template <bool TB>
-__global__ void __launch_bounds__(SFE_BLOCK_THREADS) ydrop_kernel(const YdParams p)
+__global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kernel(const YdParams p)
 {
     extern __shared__ __align__(16) char smem[];
     const int lane = sfe_lane();
     char *wsm = smem + (threadIdx.x >> 5) * SFE_WARP_SMEM;
-    for (;;) {
-        unsigned long long tk = 0;
-        if (lane == 0) tk = atomicAdd(&p.counters[CNT_TICKET], 1ULL);
-        tk = __shfl_sync(FULL, tk, 0);
-        if ((long long)tk >= p.n_tickets) break;
-        extend_half<TB, SFE_RING_LOG2, false>(p, p.tickets[tk], wsm, wsm, lane);
-        __syncwarp();
+    // re-run passes after a traceback-arena overflow admit only as many warps as the arena can serve
+    if ((int)(blockIdx.x * (SFE_BLOCK_THREADS / 32) + (threadIdx.x >> 5)) >= p.max_warps) return;
+    // Ticket queue (a3): tickets are sorted longest bin first and every warp takes the next one (LPT order).
+    // One extension is a serial chain of wavefront steps (R4 allows only 32 rows in flight), so the longest
+    // halves decide when the kernel ends -- and the SM's schedulers strongly favour the lowest hardware warp
+    // slots (measured with sfe_last_half_profile: 140 cycles per step in slots 0-3, 310 in slots 16-19, 18 warps
+    // resident).  The longest tickets are therefore reserved: segment k (n_sm x 4 tickets) is served first by
+    // the warps of slot class k = slot / 4, k = 0..3; then everybody drains the main queue and, at the end,
+    // whatever is left in any segment.
+    unsigned wslot;
+    asm("mov.u32 %0, %%warpid;" : "=r"(wslot));
+    const long long seg = p.seg_tickets;
+    const int my_class = (int)(wslot >> 2);
+    for (int phase = 0; phase < 6; phase++) {
+        // phase 0: my class's segment; phase 1: main queue; phases 2..5: leftovers of segments 0..3
+        const int k = phase == 0 ? my_class : phase - 2;
+        if (phase != 1 && (k > 3 || seg == 0)) continue;
+        const long long lo = phase == 1 ? 4 * seg : k * seg;
+        const long long hi = phase == 1 ? p.n_tickets : (lo + seg < p.n_tickets ? lo + seg : p.n_tickets);
+        unsigned long long *cnt = &p.counters[phase == 1 ? CNT_TICKET : CNT_CLASS0 + k];
+        for (;;) {
+            unsigned long long tk = 0;
+            if (lane == 0) tk = atomicAdd(cnt, 1ULL);
+            tk = __shfl_sync(FULL, tk, 0);
+            if (lo + (long long)tk >= hi) break;
+            extend_half<TB, SFE_RING_LOG2, false>(p, p.tickets[lo + tk], wsm, wsm, lane);
+            __syncwarp();
+        }
     }
 }
 

@@ -185,3 +185,23 @@ def test_wide_band_path(sfe, oracle):
     assert out["info"]["wide"] == 0
     H.assert_anchor_equal(out, w, 0); H.assert_anchor_equal(out, w, 1)
     assert int(out["results"][0]["cells"]) == 598524 + 1 and int(out["results"][0]["score"]) == 28831
+
+
+def test_tiny_arena_recycles_and_reruns(oracle):
+    """A 6 MiB traceback arena (96 chunks) for a batch that writes ~8x more: chunks are recycled as soon as a
+    half has been walked, halves that find no free chunk finish score-only and are re-run; results stay bit-exact."""
+    import __graft_entry__ as entry
+    entry.build()
+    s = B.Sfe(0, 6 << 20)
+    try:
+        w = W.config1(n_segments=12, seg_len=1500, slot=2600, per_seg=4)
+        out = H.gpu_run(s, w)
+        assert out["info"]["tb_bytes"] > 6 * (6 << 20)
+        for i in range(len(w.anchors)):
+            H.assert_anchor_equal(out, w, i)
+        H.assert_resolve_equal(out, w)
+        # a second batch on the same context: the free ring is intact after the first one
+        out2 = H.gpu_run(s, w)
+        assert (out2["results"] == out["results"]).all() and (out2["cigar"][: out2["cigar_used"]] == out["cigar"][: out["cigar_used"]]).all()
+    finally:
+        s.close()
