@@ -53,6 +53,7 @@ enum {
 #define SFE_ST_BAD_ANCHOR 16u         /* anchor outside its pair's limits: nothing computed          */
 #define SFE_ST_BAND_LIMIT 32u         /* live band wider than 65,344 columns: half not computed      */
 #define SFE_ST_INTERNAL 64u           /* traceback walk did not reach the origin (a library bug)     */
+#define SFE_ST_SKIPPED 128u           /* sfe_speculate: covered before its window, never extended    */
 
 /* CIGAR op word: (length << 4) | code ; M = aligned pair, I = query base vs gap, D = target base
  * vs gap (R12). */
@@ -92,10 +93,14 @@ typedef struct {
 
 typedef struct { int64_t tstart, tend, qstart, qend; int32_t strand; int32_t reserved; } sfe_box;
 
-/* counters accumulated by sfe_resolve (R29) */
+/* counters accumulated by sfe_resolve / sfe_speculate (R29); never reset by the library.
+ * waste (shadow work): by count  1 - (n_kept + n_below) / n_extended,
+ *                                    by cells  cells_covered / cells_total. */
 typedef struct sfe_stats {
     int64_t n_anchors, n_kept, n_covered, n_below;
-    uint64_t cells_total, cells_covered;  /* cells of all anchors / of covered ones (shadow work) */
+    uint64_t cells_total, cells_covered;  /* cells of all extended anchors / of covered ones (shadow work) */
+    int64_t n_extended;                   /* anchors that went through sfe_ydrop_batch                     */
+    int64_t n_windows;                    /* resolve calls / speculative windows                           */
 } sfe_stats;
 
 /* Create a context on `device` that enqueues on `cuda_stream` (a cudaStream_t, may be NULL for
@@ -139,6 +144,26 @@ int sfe_ydrop_batch(sfe_ctx *ctx, const uint8_t *t_codes2_dev, const uint8_t *t_
 int sfe_resolve(sfe_ctx *ctx, const sfe_anchor *anchors_dev, const sfe_result *results_dev, int64_t n,
                 int32_t min_score, sfe_box *accepted_dev, int64_t accepted_cap, int64_t *n_accepted_dev,
                 uint8_t *keep_dev, sfe_stats *stats_dev);
+
+/* Algorithm 3 end to end on device buffers.  Repeats until every anchor is decided:
+ *   phase 1  scan forward from the cursor: anchors covered by an accepted box are final (keep 0, result
+ *            zeroed with SFE_ST_SKIPPED, never extended); the next window_k uncovered anchors form the window;
+ *   phase 2  sfe_ydrop_batch on the window (flags as there);
+ *   phase 3  the resolve rule in window order; kept boxes are appended to accepted_dev.
+ * Anchors must be in anchor order (the order Algorithm 1 would visit them).  The kept set equals
+ * Algorithm 1's for every window_k >= 1 (R20, P7); window_k trades waste for parallelism.
+ * results_dev / keep_dev have n_anchors entries in anchor order; CIGARs of all extended anchors go to the
+ * pool (offsets grow window by window).  accepted_dev / n_accepted_dev as in sfe_resolve (boxes carried in
+ * are honoured).  Synchronises the stream once per window (it reads the window size). */
+int sfe_speculate(sfe_ctx *ctx, const uint8_t *t_codes2_dev, const uint8_t *t_nmask_dev, int64_t t_len,
+                  const uint8_t *q_codes2_dev, const uint8_t *q_nmask_dev,
+                  const uint8_t *qrc_codes2_dev, const uint8_t *qrc_nmask_dev, int64_t q_len,
+                  const sfe_pair *pairs_dev, int32_t n_pairs,
+                  const sfe_anchor *anchors_dev, int64_t n_anchors,
+                  const sfe_scoring *scoring_host, uint32_t flags, int64_t window_k,
+                  sfe_result *results_dev, uint8_t *keep_dev,
+                  uint32_t *cigar_pool_dev, int64_t cigar_pool_cap, int64_t *cigar_pool_used_dev,
+                  sfe_box *accepted_dev, int64_t accepted_cap, int64_t *n_accepted_dev, sfe_stats *stats_dev);
 
 /* End-to-end convenience with HOST buffers (bench.py's e2e leg): copies the ASCII sequences and
  * anchors to the device, packs, extends (flags as above), resolves in one window, copies

@@ -19,11 +19,11 @@ OK, EINVAL, ENOMEM, ECUDA, ELIMIT = 0, -1, -2, -3, -4
 YDROP_INF = 0x7FFFFFFF
 PRUNE_LAG = 32
 WANT_CIGAR, SCORE_ONLY, NO_BINNING = 1, 0, 2
-ST_TB_OVERFLOW, ST_CIGAR_OVERFLOW, ST_WIDE, ST_SCORE_LIMIT, ST_BAD_ANCHOR, ST_BAND_LIMIT = 1, 2, 4, 8, 16, 32
+ST_TB_OVERFLOW, ST_CIGAR_OVERFLOW, ST_WIDE, ST_SCORE_LIMIT, ST_BAD_ANCHOR, ST_BAND_LIMIT, ST_INTERNAL, ST_SKIPPED = 1, 2, 4, 8, 16, 32, 64, 128
 OP_M, OP_I, OP_D = 0, 1, 2
 
 EXPORTS = ("sfe_create", "sfe_destroy", "sfe_strerror", "sfe_last_error_detail", "sfe_pack", "sfe_ydrop_batch", "sfe_resolve",
-           "sfe_extend_host", "sfe_probe_int_issue", "sfe_last_batch_info", "sfe_last_half_profile")
+           "sfe_speculate", "sfe_extend_host", "sfe_probe_int_issue", "sfe_last_batch_info", "sfe_last_half_profile")
 
 
 class Scoring(C.Structure):
@@ -33,7 +33,7 @@ class Scoring(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [("n_anchors", C.c_int64), ("n_kept", C.c_int64), ("n_covered", C.c_int64), ("n_below", C.c_int64),
-                ("cells_total", C.c_uint64), ("cells_covered", C.c_uint64)]
+                ("cells_total", C.c_uint64), ("cells_covered", C.c_uint64), ("n_extended", C.c_int64), ("n_windows", C.c_int64)]
 
 
 # numpy mirrors of the POD structs (layout = the C structs of sfe.h)
@@ -45,7 +45,7 @@ RESULT_DT = np.dtype([("score", "<i4"), ("score_fwd", "<i4"), ("score_bwd", "<i4
 BOX_DT = np.dtype([("tstart", "<i8"), ("tend", "<i8"), ("qstart", "<i8"), ("qend", "<i8"),
                    ("strand", "<i4"), ("reserved", "<i4")])
 STATS_DT = np.dtype([("n_anchors", "<i8"), ("n_kept", "<i8"), ("n_covered", "<i8"), ("n_below", "<i8"),
-                     ("cells_total", "<u8"), ("cells_covered", "<u8")])
+                     ("cells_total", "<u8"), ("cells_covered", "<u8"), ("n_extended", "<i8"), ("n_windows", "<i8")])
 HALF_PROFILE_DT = np.dtype([("cells", "<i8"), ("cycles", "<i8"), ("steps", "<i4"), ("n_strips", "<i4"), ("max_steps", "<i4"),
                             ("n_ops", "<i4"), ("smid", "<u4"), ("wslot", "<u4"), ("status", "<u4"), ("reserved", "<u4")])
 assert ANCHOR_DT.itemsize == 24 and PAIR_DT.itemsize == 32 and RESULT_DT.itemsize == 72 and BOX_DT.itemsize == 40
@@ -76,6 +76,8 @@ def lib():
         _lib.sfe_pack.argtypes = [vp, vp, i64, vp, vp, vp, vp]
         _lib.sfe_ydrop_batch.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp, i64, vp, i32, vp, i64,
                                          C.POINTER(Scoring), u32, vp, vp, i64, vp]
+        _lib.sfe_speculate.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp, i64, vp, i32, vp, i64, C.POINTER(Scoring), u32, i64,
+                                       vp, vp, vp, i64, vp, vp, i64, vp, vp]
         _lib.sfe_resolve.argtypes = [vp, vp, vp, i64, i32, vp, i64, vp, vp, vp]
         _lib.sfe_extend_host.argtypes = [vp, vp, i64, vp, i64, vp, i32, vp, i64, C.POINTER(Scoring), u32,
                                          vp, vp, vp, i64, C.POINTER(i64), C.POINTER(Stats)]
@@ -190,6 +192,34 @@ class Sfe:
                                      C.byref(sc), flags, _ptr(res), _ptr(pool), cigar_cap if want else 0,
                                      _ptr(used) if want else C.c_void_p(0)), "sfe_ydrop_batch")
         return res, pool, used
+
+    # ---- sfe_speculate ------------------------------------------------------------------------------
+    def speculate(self, t_pack, t_len, q_pack, q_len, pairs_dev, n_pairs, anchors_dev, n_anchors, sc: Scoring, window_k: int,
+                  flags: int = WANT_CIGAR, cigar_cap: int = 0, accepted_dev=None, n_accepted_dev=None, stats_dev=None):
+        """Algorithm 3 on device buffers.  Returns dict(results, keep, pool, used, accepted, n_accepted, stats) of CUDA tensors."""
+        torch = _torch()
+        n = max(n_anchors, 1)
+        res = torch.zeros(n * RESULT_DT.itemsize, dtype=torch.uint8, device=self.device)
+        keep = torch.zeros(n, dtype=torch.uint8, device=self.device)
+        want = bool(flags & WANT_CIGAR)
+        if want and cigar_cap <= 0:
+            cigar_cap = max(1024, 64 * n_anchors)
+        pool = torch.zeros(max(cigar_cap, 1), dtype=torch.int32, device=self.device) if want else None
+        used = torch.zeros(1, dtype=torch.int64, device=self.device)
+        if accepted_dev is None:
+            accepted_dev = torch.zeros((n + 1) * BOX_DT.itemsize, dtype=torch.uint8, device=self.device)
+            n_accepted_dev = torch.zeros(1, dtype=torch.int64, device=self.device)
+        if stats_dev is None:
+            stats_dev = torch.zeros(STATS_DT.itemsize, dtype=torch.uint8, device=self.device)
+        cap = accepted_dev.numel() // BOX_DT.itemsize
+        rc2 = q_pack[2] if len(q_pack) > 2 else None
+        rcm = q_pack[3] if len(q_pack) > 3 else None
+        _check(lib().sfe_speculate(self.h, _ptr(t_pack[0]), _ptr(t_pack[1]), t_len, _ptr(q_pack[0]), _ptr(q_pack[1]), _ptr(rc2),
+                                   _ptr(rcm), q_len, _ptr(pairs_dev), n_pairs, _ptr(anchors_dev), n_anchors, C.byref(sc), flags,
+                                   window_k, _ptr(res), _ptr(keep), _ptr(pool), cigar_cap if want else 0,
+                                   _ptr(used) if want else C.c_void_p(0), _ptr(accepted_dev), cap, _ptr(n_accepted_dev),
+                                   _ptr(stats_dev)), "sfe_speculate")
+        return dict(results=res, keep=keep, pool=pool, used=used, accepted=accepted_dev, n_accepted=n_accepted_dev, stats=stats_dev)
 
     # ---- sfe_resolve --------------------------------------------------------------------------------
     def resolve(self, anchors_dev, results_dev, n, min_score, accepted_dev, accepted_cap, n_accepted_dev, stats_dev=None):

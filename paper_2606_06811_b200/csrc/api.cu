@@ -23,6 +23,15 @@ int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe
 int sfe_launch_select_overflow(const sfe_half *halves, long long n_anchors, long long *sel, int32_t *tickets,
                                unsigned long long *counters, int n_chunks, cudaStream_t st);
 int sfe_launch_probe(int mix, int iters, int blocks, int *sink, cudaStream_t st);
+int sfe_launch_spec_prepare(const sfe_anchor *anchors, long long n, long long *blkmin, void *state, const sfe_box *accepted,
+                            const long long *n_accepted, sfe_box *act, cudaStream_t st);
+int sfe_launch_spec_scan(void *state, const sfe_anchor *anchors, long long n, const long long *blkmin, long long K, sfe_box *act,
+                         long long *win_idx, sfe_anchor *win_anchors, uint8_t *keep, sfe_result *results, sfe_stats *stats,
+                         cudaStream_t st);
+int sfe_launch_spec_commit(void *state, const sfe_anchor *win_anchors, const sfe_result *wres, const long long *win_idx,
+                           const long long *blkmin, int min_score, sfe_box *accepted, long long accepted_cap, sfe_box *act,
+                           sfe_box *local, uint8_t *keep, sfe_result *results, sfe_stats *stats, cudaStream_t st);
+int sfe_launch_spec_finish(const void *state, long long *n_accepted_io, cudaStream_t st);
 int sfe_launch_ring_init(int32_t *ring, SfeFreeRing *st, int n_chunks, cudaStream_t stream);
 
 struct DevBuf {                       // grow-only device scratch
@@ -46,6 +55,8 @@ struct sfe_ctx {
     unsigned long long *counters;     // device, CNT_N
     unsigned long long *counters_host;  // pinned
     DevBuf halves, tickets, sel, hist, blkmin, act, misc, wide_tickets, wide_ring, ops_stage;
+    DevBuf sp_state, sp_idx, sp_anchors, sp_results, sp_local, sp_blkmin, sp_act;   // sfe_speculate
+    long long *state_host;            // pinned, 8 words
     // host-API staging
     DevBuf h_tascii, h_qascii, h_t2, h_tm, h_q2, h_qm, h_r2, h_rm, h_pairs, h_anchors, h_results, h_keep, h_cigar, h_acc, h_small;
     long long info[8];
@@ -90,7 +101,7 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
     if (nch < 4) nch = 4;
     if (nch > 0x7ffffff0LL / SFE_CHUNK_RECS) nch = 0x7ffffff0LL / SFE_CHUNK_RECS;   // record indices are int32
     c->n_chunks = (int)nch;
-    c->pool = nullptr; c->chunk_prev = nullptr; c->free_ring = nullptr; c->ring_state = nullptr; c->counters = nullptr; c->counters_host = nullptr;
+    c->pool = nullptr; c->chunk_prev = nullptr; c->free_ring = nullptr; c->ring_state = nullptr; c->counters = nullptr; c->counters_host = nullptr; c->state_host = nullptr;
     memset(c->info, 0, sizeof c->info);
     c->ev_pending = false; c->kernel_us = 0.0;
     if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) { delete c; return SFE_ECUDA; }
@@ -99,7 +110,8 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
         cudaMalloc((void **)&c->free_ring, (size_t)nch * sizeof(int32_t)) != cudaSuccess ||
         cudaMalloc((void **)&c->ring_state, sizeof(SfeFreeRing)) != cudaSuccess ||
         cudaMalloc((void **)&c->counters, CNT_N * sizeof(unsigned long long)) != cudaSuccess ||
-        cudaMallocHost((void **)&c->counters_host, CNT_N * sizeof(unsigned long long)) != cudaSuccess) {
+        cudaMallocHost((void **)&c->counters_host, CNT_N * sizeof(unsigned long long)) != cudaSuccess ||
+        cudaMallocHost((void **)&c->state_host, 8 * sizeof(long long)) != cudaSuccess) {
         cudaGetLastError();
         sfe_destroy(c);
         return SFE_ENOMEM;
@@ -119,8 +131,9 @@ extern "C" int sfe_destroy(sfe_ctx *c)
     if (c->ring_state) cudaFree(c->ring_state);
     if (c->counters) cudaFree(c->counters);
     if (c->counters_host) cudaFreeHost(c->counters_host);
+    if (c->state_host) cudaFreeHost(c->state_host);
     cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1);
-    DevBuf *bufs[] = {&c->ops_stage, &c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
+    DevBuf *bufs[] = {&c->sp_state, &c->sp_idx, &c->sp_anchors, &c->sp_results, &c->sp_local, &c->sp_blkmin, &c->sp_act, &c->ops_stage, &c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
                       &c->h_t2, &c->h_tm, &c->h_q2, &c->h_qm, &c->h_r2, &c->h_rm, &c->h_pairs, &c->h_anchors, &c->h_results,
                       &c->h_keep, &c->h_cigar, &c->h_acc, &c->h_small};
     for (DevBuf *b : bufs) b->release();
@@ -232,12 +245,14 @@ static int check_scoring(const sfe_scoring *s)
     return SFE_OK;
 }
 
-extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *t_nmask, int64_t t_len,
-                               const uint8_t *q_codes2, const uint8_t *q_nmask, const uint8_t *qrc_codes2,
-                               const uint8_t *qrc_nmask, int64_t q_len, const sfe_pair *pairs_dev, int32_t n_pairs,
-                               const sfe_anchor *anchors_dev, int64_t n_anchors, const sfe_scoring *sc, uint32_t flags,
-                               sfe_result *results_dev, uint32_t *cigar_pool_dev, int64_t cigar_pool_cap,
-                               int64_t *cigar_pool_used_dev)
+// first_of_series: reset the pool cursor and the batch info; later batches of a series (sfe_speculate's
+// windows) append their ops to the same pool and accumulate the info counters.
+static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *t_nmask, int64_t t_len,
+                            const uint8_t *q_codes2, const uint8_t *q_nmask, const uint8_t *qrc_codes2,
+                            const uint8_t *qrc_nmask, int64_t q_len, const sfe_pair *pairs_dev, int32_t n_pairs,
+                            const sfe_anchor *anchors_dev, int64_t n_anchors, const sfe_scoring *sc, uint32_t flags,
+                            sfe_result *results_dev, uint32_t *cigar_pool_dev, int64_t cigar_pool_cap,
+                            int64_t *cigar_pool_used_dev, bool first_of_series)
 {
     if (!c || n_anchors < 0 || t_len < 0 || q_len < 0 || n_pairs < 0) return SFE_EINVAL;
     int rc = check_scoring(sc);
@@ -248,9 +263,11 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
     if (want_tb && (!cigar_pool_dev || cigar_pool_cap < 0 || !cigar_pool_used_dev)) return SFE_EINVAL;
     if (2 * n_anchors > 0x7ffffff0LL) return SFE_ELIMIT;
     SFE_CUDA_CHECK(cudaSetDevice(c->device));
-    memset(c->info, 0, sizeof c->info);
-    c->ev_pending = false; c->kernel_us = 0.0;
-    if (cigar_pool_used_dev) SFE_CUDA_CHECK(cudaMemsetAsync(cigar_pool_used_dev, 0, sizeof(int64_t), c->stream));
+    if (first_of_series) {
+        memset(c->info, 0, sizeof c->info);
+        c->ev_pending = false; c->kernel_us = 0.0;
+        if (cigar_pool_used_dev) SFE_CUDA_CHECK(cudaMemsetAsync(cigar_pool_used_dev, 0, sizeof(int64_t), c->stream));
+    }
     if (n_anchors == 0) return SFE_OK;
 
     if ((rc = c->halves.ensure((size_t)(2 * n_anchors) * sizeof(sfe_half)))) return rc;
@@ -330,6 +347,62 @@ extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_
                                        cigar_pool_dev, cigar_pool_cap, (long long *)cigar_pool_used_dev, c->stream))) return rc;
     }
     return SFE_OK;
+}
+
+extern "C" int sfe_ydrop_batch(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *t_nmask, int64_t t_len,
+                               const uint8_t *q_codes2, const uint8_t *q_nmask, const uint8_t *qrc_codes2,
+                               const uint8_t *qrc_nmask, int64_t q_len, const sfe_pair *pairs_dev, int32_t n_pairs,
+                               const sfe_anchor *anchors_dev, int64_t n_anchors, const sfe_scoring *sc, uint32_t flags,
+                               sfe_result *results_dev, uint32_t *cigar_pool_dev, int64_t cigar_pool_cap,
+                               int64_t *cigar_pool_used_dev)
+{
+    return ydrop_batch_impl(c, t_codes2, t_nmask, t_len, q_codes2, q_nmask, qrc_codes2, qrc_nmask, q_len, pairs_dev, n_pairs,
+                            anchors_dev, n_anchors, sc, flags, results_dev, cigar_pool_dev, cigar_pool_cap, cigar_pool_used_dev, true);
+}
+
+extern "C" int sfe_speculate(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *t_nmask, int64_t t_len,
+                             const uint8_t *q_codes2, const uint8_t *q_nmask, const uint8_t *qrc_codes2,
+                             const uint8_t *qrc_nmask, int64_t q_len, const sfe_pair *pairs_dev, int32_t n_pairs,
+                             const sfe_anchor *anchors_dev, int64_t n_anchors, const sfe_scoring *sc, uint32_t flags,
+                             int64_t window_k, sfe_result *results_dev, uint8_t *keep_dev, uint32_t *cigar_pool_dev,
+                             int64_t cigar_pool_cap, int64_t *cigar_pool_used_dev, sfe_box *accepted_dev,
+                             int64_t accepted_cap, int64_t *n_accepted_dev, sfe_stats *stats_dev)
+{
+    if (!c || n_anchors < 0 || window_k < 1 || accepted_cap < 0) return SFE_EINVAL;
+    int rc = check_scoring(sc);
+    if (rc) return rc;
+    if (n_anchors > 0 && (!anchors_dev || !results_dev || !keep_dev || !accepted_dev || !n_accepted_dev)) return SFE_EINVAL;
+    SFE_CUDA_CHECK(cudaSetDevice(c->device));
+    memset(c->info, 0, sizeof c->info);
+    c->ev_pending = false; c->kernel_us = 0.0;
+    if (cigar_pool_used_dev) SFE_CUDA_CHECK(cudaMemsetAsync(cigar_pool_used_dev, 0, sizeof(int64_t), c->stream));
+    if (n_anchors == 0) return SFE_OK;
+    const long long K = window_k < n_anchors ? window_k : n_anchors;
+    if ((rc = c->sp_state.ensure(64)) || (rc = c->sp_idx.ensure((size_t)K * sizeof(long long))) ||
+        (rc = c->sp_anchors.ensure((size_t)K * sizeof(sfe_anchor))) || (rc = c->sp_results.ensure((size_t)K * sizeof(sfe_result))) ||
+        (rc = c->sp_local.ensure((size_t)(K + 1) * sizeof(sfe_box))) ||
+        (rc = c->sp_blkmin.ensure((size_t)((n_anchors + 31) / 32 + 32) * sizeof(long long))) ||
+        (rc = c->sp_act.ensure((size_t)(n_anchors + accepted_cap + 1) * sizeof(sfe_box)))) return rc;
+    long long *blkmin = (long long *)c->sp_blkmin.p;
+    sfe_box *act = (sfe_box *)c->sp_act.p;
+    if ((rc = sfe_launch_spec_prepare(anchors_dev, n_anchors, blkmin, c->sp_state.p, accepted_dev, (const long long *)n_accepted_dev,
+                                      act, c->stream))) return rc;
+    for (long long win = 0;; win++) {
+        if ((rc = sfe_launch_spec_scan(c->sp_state.p, anchors_dev, n_anchors, blkmin, K, act, (long long *)c->sp_idx.p,
+                                       (sfe_anchor *)c->sp_anchors.p, keep_dev, results_dev, stats_dev, c->stream))) return rc;
+        SFE_CUDA_CHECK(cudaMemcpyAsync(c->state_host, c->sp_state.p, 5 * sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
+        SFE_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+        const long long wn = c->state_host[1];
+        if (wn <= 0) break;
+        if ((rc = ydrop_batch_impl(c, t_codes2, t_nmask, t_len, q_codes2, q_nmask, qrc_codes2, qrc_nmask, q_len, pairs_dev, n_pairs,
+                                   (const sfe_anchor *)c->sp_anchors.p, wn, sc, flags, (sfe_result *)c->sp_results.p,
+                                   cigar_pool_dev, cigar_pool_cap, cigar_pool_used_dev, false))) return rc;
+        harvest_kernel_time(c);
+        if ((rc = sfe_launch_spec_commit(c->sp_state.p, (const sfe_anchor *)c->sp_anchors.p, (const sfe_result *)c->sp_results.p,
+                                         (const long long *)c->sp_idx.p, blkmin, sc->min_score, accepted_dev, accepted_cap, act,
+                                         (sfe_box *)c->sp_local.p, keep_dev, results_dev, stats_dev, c->stream))) return rc;
+    }
+    return sfe_launch_spec_finish(c->sp_state.p, (long long *)n_accepted_dev, c->stream);
 }
 
 extern "C" int sfe_resolve(sfe_ctx *c, const sfe_anchor *anchors_dev, const sfe_result *results_dev, int64_t n,

@@ -123,6 +123,7 @@ __global__ void resolve_kernel(const sfe_anchor *anchors, const sfe_result *resu
         if (stats && commit) {
             stats->n_anchors += n; stats->n_kept += c_kept; stats->n_covered += c_cov; stats->n_below += c_below;
             stats->cells_total += cells_tot; stats->cells_covered += cells_cov;
+            stats->n_extended += n; stats->n_windows += 1;
         }
     }
 }
@@ -135,5 +136,217 @@ int sfe_launch_resolve(const sfe_anchor *anchors, const sfe_result *results, lon
     const int bs = 256;
     block_min_kernel<<<(unsigned)((n + bs - 1) / bs), bs, 0, st>>>(anchors, n, blkmin);
     resolve_kernel<<<1, 32, 0, st>>>(anchors, results, n, min_score, accepted, accepted_cap, n_accepted_io, keep, stats, blkmin, act);
+    SFE_LAUNCH_CHECK();
+}
+
+// =====================================================================================================
+// Algorithm 3 as a device-side loop: sfe_speculate's three phases per window.
+//   spec_scan    phase 1: from the cursor, test anchors against the ACTIVE accepted boxes;
+//                covered anchors are final (the accepted set only grows): keep = 0, result = "skipped";
+//                the first K uncovered anchors become the window (their indices and a compact copy).
+//   (phase 2 = sfe_ydrop_batch on the compact window)
+//   spec_commit  phase 3: in window order, the resolve rule against the boxes kept
+//                earlier IN THIS WINDOW (older boxes were already tested by the scan); results and keep
+//                flags are scattered back to anchor order; kept boxes join `accepted` and the active list.
+// The active list persists across windows in device memory; a box leaves it when its tend is below the
+// suffix minimum of tpos over all anchors not yet scanned (exact for any anchor order).
+// =====================================================================================================
+struct SpecState { long long cursor, win_n, nact, nacc, overflow; };
+
+__global__ void suffix_min_kernel(long long *blkmin, long long nblk)
+{
+    const int lane = threadIdx.x & 31;
+    long long carry = 0x7fffffffffffffffLL;
+    for (long long hi = nblk; hi > 0; hi -= 32) {
+        const long long b = hi - 1 - lane;
+        long long v = (b >= 0) ? blkmin[b] : 0x7fffffffffffffffLL;
+        for (int o = 1; o < 32; o <<= 1) { const long long y = __shfl_up_sync(FULL, v, o); if (lane >= o && y < v) v = y; }
+        v = v < carry ? v : carry;
+        if (b >= 0) blkmin[b] = v;
+        carry = __shfl_sync(FULL, v, 31);
+    }
+}
+
+__global__ void spec_init_kernel(SpecState *st, const sfe_box *accepted, const long long *n_accepted, sfe_box *act)
+{
+    const int lane = threadIdx.x & 31;
+    const long long nacc = *n_accepted;
+    for (long long k = lane; k < nacc; k += 32) act[k] = accepted[k];
+    if (lane == 0) { st->cursor = 0; st->win_n = 0; st->nact = nacc; st->nacc = nacc; st->overflow = 0; }
+}
+
+// stable in-place compaction of the live boxes (tend >= tmin); returns the new count (whole warp)
+static __device__ long long retire_boxes(sfe_box *act, long long nact, long long tmin, int lane)
+{
+    long long w = 0;
+    for (long long base = 0; base < nact; base += 32) {
+        const long long k = base + lane;
+        sfe_box b; bool live = false;
+        if (k < nact) { b = act[k]; live = b.tend >= tmin; }
+        const unsigned m = __ballot_sync(FULL, live);
+        __syncwarp();
+        if (live) act[w + __popc(m & ((1u << lane) - 1))] = b;
+        w += __popc(m);
+        __syncwarp();
+    }
+    return w;
+}
+
+// single warp
+__global__ void spec_scan_kernel(SpecState *st, const sfe_anchor *anchors, long long n, const long long *blkmin, long long K,
+                                 sfe_box *act, long long *win_idx, sfe_anchor *win_anchors, uint8_t *keep,
+                                 sfe_result *results, sfe_stats *stats)
+{
+    const int lane = threadIdx.x & 31;
+    long long j = st->cursor, nact = st->nact, wn = 0, c_cov = 0;
+    while (j < n && wn < K) {
+        const long long blk = j >> 5;
+        nact = retire_boxes(act, nact, blkmin[blk], lane);
+        const long long i = (blk << 5) + lane;
+        const bool valid = i >= j && i < n;
+        long long tp = 0, qp = 0; int strand = 0;
+        sfe_anchor an;
+        if (valid) { an = anchors[i]; tp = an.tpos; qp = an.qpos; strand = an.strand >= 0 ? 1 : -1; }
+        bool cov = false;
+        for (long long k = 0; k < nact; k++) { const sfe_box b = act[k]; cov = cov || box_has(b, tp, qp, strand); }
+        cov = cov && valid;
+        const unsigned um = __ballot_sync(FULL, valid && !cov);
+        const int rank = __popc(um & ((1u << lane) - 1));
+        // take uncovered anchors in order until the window is full; the cursor stops after the last one taken
+        const long long room = K - wn;
+        const int n_unc = __popc(um);
+        long long next_j = ((blk + 1) << 5) < n ? ((blk + 1) << 5) : n;
+        if (n_unc > room) {
+            // the (room+1)-th uncovered lane and everything after it stay for the next window
+            unsigned m = um; int stop_lane = 0;
+            for (long long r = 0; r <= room; r++) { stop_lane = __ffs(m) - 1; m &= m - 1; }
+            next_j = (blk << 5) + stop_lane;
+        }
+        const bool in_range = valid && i < next_j;
+        if (in_range && !cov) { win_idx[wn + rank] = i; win_anchors[wn + rank] = an; }
+        if (in_range && cov) {
+            keep[i] = 0;
+            sfe_result r; r.score = r.score_fwd = r.score_bwd = 0; r.status = SFE_ST_SKIPPED;
+            r.tstart = r.tend = tp; r.qstart = r.qend = qp; r.cigar_off = -1; r.n_ops = r.n_ops_back = 0; r.cells = 0;
+            results[i] = r;
+        }
+        c_cov += __popc(__ballot_sync(FULL, in_range && cov));
+        wn += n_unc > room ? room : n_unc;
+        j = next_j;
+    }
+    if (lane == 0) {
+        st->cursor = j; st->win_n = wn; st->nact = nact;
+        if (stats) { stats->n_anchors += c_cov; stats->n_covered += c_cov; }
+    }
+}
+
+// single warp; wres = results of the compact window (phase 2)
+__global__ void spec_commit_kernel(SpecState *st, const sfe_anchor *win_anchors, const sfe_result *wres, const long long *win_idx,
+                                   const long long *blkmin, int min_score, sfe_box *accepted, long long accepted_cap,
+                                   sfe_box *act, sfe_box *local, uint8_t *keep, sfe_result *results, sfe_stats *stats)
+{
+    const int lane = threadIdx.x & 31;
+    const long long wn = st->win_n;
+    long long nacc = st->nacc, nloc = 0;
+    long long c_kept = 0, c_cov = 0, c_below = 0;
+    unsigned long long cells_tot = 0, cells_cov = 0;
+    bool overflow = false;
+    for (long long base = 0; base < wn; base += 32) {
+        nloc = retire_boxes(local, nloc, blkmin[win_idx[base] >> 5], lane);
+        const long long w = base + lane;
+        const bool valid = w < wn;
+        long long tp = 0, qp = 0, gi = 0; int strand = 0, score = 0; unsigned long long cells = 0;
+        sfe_box mine; mine.tstart = mine.tend = mine.qstart = mine.qend = 0; mine.strand = 0; mine.reserved = 0;
+        sfe_result r;
+        if (valid) {
+            gi = win_idx[w]; r = wres[w];
+            tp = win_anchors[w].tpos; qp = win_anchors[w].qpos; strand = win_anchors[w].strand >= 0 ? 1 : -1;
+            score = r.score; cells = r.cells;
+            mine.tstart = r.tstart; mine.tend = r.tend; mine.qstart = r.qstart; mine.qend = r.qend; mine.strand = strand;
+        }
+        bool cov = false;
+        for (long long k = 0; k < nloc; k++) { const sfe_box b = local[k]; cov = cov || box_has(b, tp, qp, strand); }
+        cov = cov && valid;
+        bool cand = valid && !cov && score >= min_score;
+        bool kept = false;
+        unsigned mask = __ballot_sync(FULL, cand);
+        while (mask) {
+            const int leader = __ffs(mask) - 1;
+            if (lane == leader) { kept = true; cand = false; }
+            sfe_box lb;
+            lb.tstart = __shfl_sync(FULL, mine.tstart, leader); lb.tend = __shfl_sync(FULL, mine.tend, leader);
+            lb.qstart = __shfl_sync(FULL, mine.qstart, leader); lb.qend = __shfl_sync(FULL, mine.qend, leader);
+            lb.strand = __shfl_sync(FULL, mine.strand, leader); lb.reserved = 0;
+            if (valid && lane > leader && !cov && box_has(lb, tp, qp, strand)) { cov = true; cand = false; }
+            if (lane == leader) {
+                local[nloc] = lb;
+                if (nacc < accepted_cap) accepted[nacc] = lb;
+            }
+            if (nacc >= accepted_cap) overflow = true;
+            nloc++; nacc++;
+            __syncwarp();
+            mask = __ballot_sync(FULL, cand);
+        }
+        if (valid) {
+            keep[gi] = cov ? 0 : (kept ? 1 : 2);
+            results[gi] = r;
+            c_kept += kept; c_cov += cov; c_below += (!cov && !kept);
+            cells_tot += cells; if (cov) cells_cov += cells;
+        }
+    }
+    // the boxes of this window that can still cover a later anchor join the persistent active list
+    long long nact = st->nact;
+    for (long long k = lane; k < nloc; k += 32) act[nact + k] = local[k];
+    nact += nloc;
+    for (int o = 16; o > 0; o >>= 1) {
+        c_kept += __shfl_xor_sync(FULL, c_kept, o); c_cov += __shfl_xor_sync(FULL, c_cov, o);
+        c_below += __shfl_xor_sync(FULL, c_below, o);
+        cells_tot += __shfl_xor_sync(FULL, cells_tot, o); cells_cov += __shfl_xor_sync(FULL, cells_cov, o);
+    }
+    if (lane == 0) {
+        st->nact = nact; st->nacc = nacc; if (overflow) st->overflow = 1;
+        if (stats) {
+            stats->n_anchors += wn; stats->n_kept += c_kept; stats->n_covered += c_cov; stats->n_below += c_below;
+            stats->cells_total += cells_tot; stats->cells_covered += cells_cov;
+            stats->n_extended += wn; stats->n_windows += 1;
+        }
+    }
+}
+
+__global__ void spec_finish_kernel(const SpecState *st, long long *n_accepted_io)
+{
+    if (threadIdx.x == 0) *n_accepted_io = st->overflow ? -st->nacc : st->nacc;
+}
+
+int sfe_launch_spec_prepare(const sfe_anchor *anchors, long long n, long long *blkmin, void *state, const sfe_box *accepted,
+                            const long long *n_accepted, sfe_box *act, cudaStream_t st)
+{
+    const int bs = 256;
+    block_min_kernel<<<(unsigned)((n + bs - 1) / bs), bs, 0, st>>>(anchors, n, blkmin);
+    suffix_min_kernel<<<1, 32, 0, st>>>(blkmin, (n + 31) >> 5);
+    spec_init_kernel<<<1, 32, 0, st>>>((SpecState *)state, accepted, n_accepted, act);
+    SFE_LAUNCH_CHECK();
+}
+
+int sfe_launch_spec_scan(void *state, const sfe_anchor *anchors, long long n, const long long *blkmin, long long K, sfe_box *act,
+                         long long *win_idx, sfe_anchor *win_anchors, uint8_t *keep, sfe_result *results, sfe_stats *stats,
+                         cudaStream_t st)
+{
+    spec_scan_kernel<<<1, 32, 0, st>>>((SpecState *)state, anchors, n, blkmin, K, act, win_idx, win_anchors, keep, results, stats);
+    SFE_LAUNCH_CHECK();
+}
+
+int sfe_launch_spec_commit(void *state, const sfe_anchor *win_anchors, const sfe_result *wres, const long long *win_idx,
+                           const long long *blkmin, int min_score, sfe_box *accepted, long long accepted_cap, sfe_box *act,
+                           sfe_box *local, uint8_t *keep, sfe_result *results, sfe_stats *stats, cudaStream_t st)
+{
+    spec_commit_kernel<<<1, 32, 0, st>>>((SpecState *)state, win_anchors, wres, win_idx, blkmin, min_score, accepted, accepted_cap,
+                                         act, local, keep, results, stats);
+    SFE_LAUNCH_CHECK();
+}
+
+int sfe_launch_spec_finish(const void *state, long long *n_accepted_io, cudaStream_t st)
+{
+    spec_finish_kernel<<<1, 32, 0, st>>>((const SpecState *)state, n_accepted_io);
     SFE_LAUNCH_CHECK();
 }

@@ -37,7 +37,7 @@ def test_struct_layouts_match_header():
     assert C.sizeof(B.Scoring) == 22 * 4
     assert B.ANCHOR_DT.itemsize == 24 and B.PAIR_DT.itemsize == 32
     assert B.RESULT_DT.itemsize == 72 and B.RESULT_DT.fields["cells"][1] == 64
-    assert B.BOX_DT.itemsize == 40 and B.STATS_DT.itemsize == C.sizeof(B.Stats) == 48
+    assert B.BOX_DT.itemsize == 40 and B.STATS_DT.itemsize == C.sizeof(B.Stats) == 64 and B.HALF_PROFILE_DT.itemsize == 48
 
 
 def test_strerror_and_null_args(built):

@@ -205,3 +205,58 @@ def test_tiny_arena_recycles_and_reruns(oracle):
         assert (out2["results"] == out["results"]).all() and (out2["cigar"][: out2["cigar_used"]] == out["cigar"][: out["cigar_used"]]).all()
     finally:
         s.close()
+
+
+def _speculate(sfe, w, K, flags=B.WANT_CIGAR, **sc_kw):
+    import torch
+    dev = sfe.device
+    sc = B.scoring(**sc_kw)
+    tp = sfe.pack(torch.from_numpy(w.target_ascii().copy()).to(dev), with_rc=False)
+    qp = sfe.pack(torch.from_numpy(w.query_ascii().copy()).to(dev), with_rc=True)
+    n = len(w.anchors)
+    o = sfe.speculate(tp[:2], len(w.target), qp, len(w.query), B._dev(B.make_pairs(w.pairs), dev), len(w.pairs),
+                      B._dev(B.make_anchors(w.anchors), dev), n, sc, K, flags)
+    torch.cuda.synchronize()
+    out = dict(results=B.results_to_numpy(o["results"], n), keep=o["keep"].cpu().numpy()[:n],
+               stats=o["stats"].cpu().numpy().view(B.STATS_DT)[0], n_accepted=int(o["n_accepted"].item()))
+    if flags & B.WANT_CIGAR:
+        out["cigar"] = o["pool"].cpu().numpy().view(np.uint32); out["cigar_used"] = int(o["used"].item())
+    return out
+
+
+@pytest.mark.parametrize("K", [1, 3, 32, 50, 10_000])
+def test_speculate_equals_serial_loop(sfe, oracle, K):
+    """sfe_speculate (Alg. 3: scan / extend / commit per window, all on the device) keeps exactly what Alg. 1
+    keeps for every window size (P7); every anchor it extended is bit-exact against the oracle; anchors covered
+    before their window are never extended; the waste counters add up."""
+    w = W.config2(t_len=60_000, n_segments=30, per_seg=8, n_decoys=40, min_len=150, max_len=700)
+    n = len(w.anchors)
+    ser = oracle.serial_loop(w.target, w.query, w.query_rc, w.pairs, w.anchors, oracle.scoring(), want_results=False)
+    out = _speculate(sfe, w, K)
+    assert out["keep"].tolist() == ser["state"].tolist(), K
+    st = out["stats"]
+    skipped = (out["results"]["status"] & B.ST_SKIPPED) != 0
+    assert int(st["n_anchors"]) == n and int(st["n_kept"]) == ser["n_kept"] == out["n_accepted"]
+    assert int(st["n_extended"]) == int((~skipped).sum()) and int(st["n_kept"] + st["n_covered"] + st["n_below"]) == n
+    assert (out["keep"][skipped] == 0).all()
+    # serial semantics extend exactly the anchors that are not covered; speculation extends a superset
+    serial_ext = ser["state"] != 0
+    assert (~skipped)[serial_ext].all()
+    if K == 1:
+        assert int(st["n_extended"]) == int(serial_ext.sum())          # K = 1 is Algorithm 1: no shadow work
+    else:
+        assert int(st["n_extended"]) >= int(serial_ext.sum())
+    assert int(st["cells_total"]) == int(out["results"]["cells"][~skipped].sum())
+    for i in np.nonzero(~skipped)[0][:: max(1, int((~skipped).sum()) // 40)]:
+        H.assert_anchor_equal(out, w, int(i))
+
+
+def test_speculate_config1_windows(sfe, oracle):
+    """configs[0] through the windowed path: 64 kept for every K; K = 256 computes all 256 (75 % shadow work),
+    K = 1 only the 64 that the serial loop extends."""
+    w = W.config1()
+    for K, n_ext in ((256, 256), (1, 64)):
+        out = _speculate(sfe, w, K, flags=B.SCORE_ONLY)
+        assert int((out["keep"] == 1).sum()) == 64 and int(out["stats"]["n_extended"]) == n_ext, K
+    full = H.gpu_run(sfe, w, flags=B.SCORE_ONLY)
+    assert out["keep"].tolist() == full["keep"].tolist()
