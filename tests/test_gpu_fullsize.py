@@ -1,0 +1,183 @@
+"""-m gpu parity tests at BASELINE.json's full sizes, in the launch configuration bench.py times.
+
+The oracle cannot run 10^10..10^12 cells, so at full size the CUDA path is checked
+  (a) on sampled outputs the oracle computes one by one: a seeded sample of anchors plus the largest
+      extensions (score, halves, box, cell count, CIGAR: bit-exact);
+  (b) by properties that hold at any size and need neither side's code: every emitted CIGAR, rescored
+      against the sequences with the R12 rule, reproduces the reported score and consumes exactly
+      the box; the keep flags satisfy the in-order containment rule (R17/R18) given the reported
+      boxes; the counters add up.
+C1 is covered in full by test_gpu_parity.py.  C5 runs at 1/10 scale (10 Mbp, 100,000 anchors: SURVEY 8(d)
+allows the prefix-scale run; the full 1 M anchors take minutes per pass)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2606_06811_b200 import binding as B, workloads as W  # noqa: E402
+
+import gpu_harness as H  # noqa: E402
+
+TAU = 3000
+SUB = np.array(B.HOXD70, np.int64)
+
+
+@pytest.fixture(scope="module")
+def sfe_big():
+    import __graft_entry__ as entry
+    entry.build()
+    s = B.Sfe(0, 24 << 30)
+    yield s
+    s.close()
+
+
+def check_cigar(w, i, g, cigar):
+    """The ops of anchor i rescore to its score and consume exactly its box; the first n_ops_back ops end at the anchor."""
+    a = w.anchors[i]
+    Q = w.query if a[3] > 0 else w.query_rc
+    T = w.target
+    n = int(g["n_ops"])
+    if n == 0:                                         # both halves empty (R8): score 0, box = the anchor point
+        assert int(g["score"]) == 0 and int(g["tstart"]) == int(g["tend"]) == int(a[0]) and int(g["qstart"]) == int(g["qend"]) == int(a[1])
+        return
+    assert int(g["cigar_off"]) >= 0, (i, int(g["status"]))
+    words = cigar[int(g["cigar_off"]): int(g["cigar_off"]) + n].astype(np.int64)
+    ln = words >> 4; op = words & 15
+    assert ((op >= 0) & (op <= 2)).all() and (ln > 0).all()
+    dq = np.where(op != 2, ln, 0); dt = np.where(op != 1, ln, 0)
+    q0 = int(g["qstart"]) + np.concatenate([[0], np.cumsum(dq)[:-1]]) if n else np.zeros(0, np.int64)
+    t0 = int(g["tstart"]) + np.concatenate([[0], np.cumsum(dt)[:-1]]) if n else np.zeros(0, np.int64)
+    assert int(g["qstart"]) + int(dq.sum()) == int(g["qend"]) and int(g["tstart"]) + int(dt.sum()) == int(g["tend"]), i
+    nb = int(g["n_ops_back"])
+    assert int(g["qstart"]) + int(dq[:nb].sum()) == int(a[1]) and int(g["tstart"]) + int(dt[:nb].sum()) == int(a[0]), i
+    score = -int((400 + 30 * ln[op != 0]).sum())
+    m = op == 0
+    if m.any():
+        # expand the M runs into base index arrays
+        lens = ln[m]; tot = int(lens.sum())
+        starts = np.repeat(np.cumsum(lens) - lens, lens)
+        off = np.arange(tot) - starts
+        qi = np.repeat(q0[m], lens) + off; ti = np.repeat(t0[m], lens) + off
+        qa = Q[qi].astype(np.int64); ta = T[ti].astype(np.int64)
+        isn = (qa > 3) | (ta > 3)
+        s = np.where(isn, -100, SUB[np.minimum(qa, 3), np.minimum(ta, 3)])
+        score += int(s.sum())
+    assert score == int(g["score"]), (i, score, int(g["score"]))
+    # within a half no two adjacent runs share an op (R12); the junction may repeat one
+    same = np.nonzero(op[1:] == op[:-1])[0] + 1
+    assert all(int(k) == nb for k in same), (i, same[:4], nb)
+
+
+def check_resolve_rule(w, res, keep, skipped=None):
+    """keep flags vs the rule, from the reported boxes only: kept <=> score >= tau and not inside an earlier kept box
+    of the same strand; covered <=> inside one; below <=> neither.  O(n log n + candidates) via the tpos order."""
+    A = w.anchors
+    n = len(A)
+    tpos = A[:, 0]; qpos = A[:, 1]; strand = np.where(A[:, 3] >= 0, 1, -1)
+    order = np.argsort(tpos, kind="stable"); ts = tpos[order]
+    covered = np.zeros(n, bool)
+    for j in np.nonzero(keep == 1)[0]:
+        lo = np.searchsorted(ts, res["tstart"][j], "left"); hi = np.searchsorted(ts, res["tend"][j], "right")
+        c = order[lo:hi]
+        c = c[(c > j) & (strand[c] == strand[j]) & (qpos[c] >= res["qstart"][j]) & (qpos[c] <= res["qend"][j])]
+        covered[c] = True
+    assert ((keep == 0) == covered).all(), np.nonzero((keep == 0) != covered)[0][:8]
+    ext = ~covered if skipped is None else ~skipped
+    assert ((keep == 1) == (~covered & (res["score"] >= TAU) & ext)).all()
+    assert ((keep == 2) == (~covered & (res["score"] < TAU))).all()
+    if skipped is not None:
+        assert covered[skipped].all()            # never-extended anchors are covered ones
+
+
+def sample_indices(res, n, k, seed, mask=None):
+    rng = np.random.default_rng(seed)
+    pool = np.arange(n) if mask is None else np.nonzero(mask)[0]
+    pick = set(rng.choice(pool, min(k, len(pool)), replace=False).tolist())
+    cells = res["cells"].astype(np.int64).copy()
+    if mask is not None:
+        cells[~mask] = -1
+    pick.update(np.argsort(-cells)[:6].tolist())     # the largest extensions
+    pick.update(np.argsort(cells + (cells < 0) * (1 << 62))[:3].tolist())   # and the smallest
+    return sorted(pick)
+
+
+def test_config2_full(sfe_big, oracle):
+    """configs[1], all 25,000 anchors in one speculative batch + resolve, as bench.py's default run."""
+    w = W.config2()
+    n = len(w.anchors)
+    out = H.gpu_run(sfe_big, w)
+    res = out["results"]
+    assert not (res["status"] & ~np.uint32(B.ST_WIDE)).any()
+    for i in sample_indices(res, n, 40, 2):
+        H.assert_anchor_equal(out, w, i)
+    check_resolve_rule(w, res, out["keep"])
+    st = out["stats"]
+    assert int(st["n_anchors"]) == n and int(st["n_kept"]) == int((out["keep"] == 1).sum()) == out["n_accepted"]
+    assert int(st["cells_total"]) == int(res["cells"].sum())
+    assert int(st["cells_covered"]) == int(res["cells"][out["keep"] == 0].sum())
+    for i in np.nonzero(out["keep"] == 1)[0]:
+        check_cigar(w, int(i), res[i], out["cigar"])
+    for i in np.nonzero(out["keep"] != 1)[0][::50]:
+        check_cigar(w, int(i), res[i], out["cigar"])
+
+
+def test_config4_full(sfe_big, oracle):
+    """configs[3], 65,536 independent pairs (forward + backward for every anchor, no subsumption)."""
+    w = W.config4()
+    n = len(w.anchors)
+    out = H.gpu_run(sfe_big, w)
+    res = out["results"]
+    assert not (res["status"] & ~np.uint32(B.ST_WIDE)).any()
+    assert int(out["info"]["halves_rerun"]) == 0           # 24 GiB of recycled arena is enough for ~27 GB of pointers
+    for i in sample_indices(res, n, 40, 4):
+        H.assert_anchor_equal(out, w, i)
+    assert int((out["keep"] == 0).sum()) == 0 and ((out["keep"] == 1) == (res["score"] >= TAU)).all()
+    check_resolve_rule(w, res, out["keep"])
+    for i in range(0, n, 97):
+        check_cigar(w, i, res[i], out["cigar"])
+
+
+def _speculate_full(sfe, w, K, cigar_cap):
+    import torch
+    dev = sfe.device
+    tp = sfe.pack(torch.from_numpy(w.target_ascii().copy()).to(dev), with_rc=False)
+    qp = sfe.pack(torch.from_numpy(w.query_ascii().copy()).to(dev), with_rc=True)
+    n = len(w.anchors)
+    o = sfe.speculate(tp[:2], len(w.target), qp, len(w.query), B._dev(B.make_pairs(w.pairs), dev), len(w.pairs),
+                      B._dev(B.make_anchors(w.anchors), dev), n, B.scoring(), K, B.WANT_CIGAR, cigar_cap)
+    torch.cuda.synchronize()
+    return dict(results=B.results_to_numpy(o["results"], n), keep=o["keep"].cpu().numpy()[:n],
+                stats=o["stats"].cpu().numpy().view(B.STATS_DT)[0], n_accepted=int(o["n_accepted"].item()),
+                cigar=o["pool"].cpu().numpy().view(np.uint32), cigar_used=int(o["used"].item()))
+
+
+def _check_speculated(w, out, seed, n_sample):
+    res = out["results"]; keep = out["keep"]; n = len(w.anchors)
+    skipped = (res["status"] & B.ST_SKIPPED) != 0
+    bad = res["status"] & np.uint32(B.ST_TB_OVERFLOW | B.ST_CIGAR_OVERFLOW | B.ST_INTERNAL | B.ST_BAND_LIMIT | B.ST_BAD_ANCHOR)
+    assert not bad[keep == 1].any() and not (bad & np.uint32(B.ST_INTERNAL | B.ST_BAND_LIMIT | B.ST_BAD_ANCHOR)).any()
+    check_resolve_rule(w, res, keep, skipped)
+    st = out["stats"]
+    assert int(st["n_anchors"]) == n and int(st["n_extended"]) == int((~skipped).sum())
+    assert int(st["n_kept"]) == int((keep == 1).sum()) == out["n_accepted"]
+    assert int(st["cells_total"]) == int(res["cells"][~skipped].sum())
+    for i in np.nonzero(keep == 1)[0]:
+        check_cigar(w, int(i), res[i], out["cigar"])
+    ok = ~skipped & (bad == 0)
+    for i in sample_indices(res, n, n_sample, seed, ok):
+        H.assert_anchor_equal(out, w, i)
+
+
+def test_config3_full_windowed(sfe_big, oracle):
+    """configs[2] (10 Mbp, 50,000 dense anchors, extensions of 10^4..10^5 rows) through sfe_speculate."""
+    w = W.config3()
+    out = _speculate_full(sfe_big, w, 1024, 1 << 26)
+    _check_speculated(w, out, 3, 24)
+    assert int((out["keep"] == 0).sum()) > 0.9 * len(w.anchors)        # "most are subsumed under serial order"
+
+
+def test_config5_scaled_windowed(sfe_big, oracle):
+    """configs[4] at 1/10 scale (10 Mbp with N runs and segmental duplications, 100,000 anchors), K = 64."""
+    w = W.config5(t_len=10_000_000, n_anchors=100_000)
+    out = _speculate_full(sfe_big, w, 64, 1 << 26)
+    _check_speculated(w, out, 5, 24)
