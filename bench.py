@@ -24,7 +24,8 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-SCRATCH_GB = {"c1": 2, "c2": 28, "c4": 64, "c3s": 24, "c5s": 24}
+SCRATCH_GB = {"c1": 2, "c2": 16, "c4": 24, "c3": 32, "c3s": 24, "c5s": 32, "c5": 48}   # traceback arena (chunks are recycled)
+DEFAULT_WINDOW = {"c3": 1024, "c3s": 1024, "c5s": 64, "c5": 64}   # Algorithm 3's K for the dense-anchor workloads; others: one batch
 
 
 def make_workload(name):
@@ -35,6 +36,10 @@ def make_workload(name):
         return W.config2(), "BASELINE.json configs[1]: divergent cross-species regime, 2 Mbp, 25,000 anchors"
     if name == "c4":
         return W.config4(), "BASELINE.json configs[3]: 65,536 independent pairs, log-normal lengths"
+    if name == "c3":
+        return W.config3(), "BASELINE.json configs[2]: high-identity primate-like regime, 10 Mbp, 50,000 dense anchors"
+    if name == "c5":
+        return W.config5(), "BASELINE.json configs[4]: chromosome-scale pair, 100 Mbp, 1,000,000 anchors"
     if name == "c3s":
         return W.config3(t_len=1_000_000, n_anchors=5_000), "configs[2] scaled 1/10: 1 Mbp, 5,000 anchors (prefix-scale run)"
     if name == "c5s":
@@ -135,7 +140,9 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c4", "c3s", "c5s"])
+    ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c4", "c3", "c3s", "c5s", "c5"])
+    ap.add_argument("--window", type=int, default=-1, help="Algorithm 3's K (sfe_speculate); 0 = one batch over all anchors; -1 = workload default")
+    ap.add_argument("--sweep-k", default="", help="comma-separated K values: one extra timed pass each (PAPER.md:163, Fig. 3)")
     ap.add_argument("--flags", default="cigar", choices=["cigar", "score"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-e2e", action="store_true")
@@ -176,17 +183,30 @@ def main():
     acc = torch.zeros((n + 1) * B.BOX_DT.itemsize, dtype=torch.uint8, device=dev)
     nacc = torch.zeros(1, dtype=torch.int64, device=dev)
     stats = torch.zeros(B.STATS_DT.itemsize, dtype=torch.uint8, device=dev)
-    cigar_cap = max(1 << 20, 96 * n)
+    cigar_cap = max(1 << 26 if DEFAULT_WINDOW.get(args.workload, 0) or args.window > 0 else 1 << 20, 96 * n)
     state = {}
 
-    def step():
+    window = DEFAULT_WINDOW.get(args.workload, 0) if args.window < 0 else args.window
+
+    def step(K=None):
+        K = window if K is None else K
         nacc.zero_(); stats.zero_()
         tp = sfe.pack(t_ascii, with_rc=False)
         qp = sfe.pack(q_ascii, with_rc=True)
-        res, pool, used = sfe.ydrop_batch(tp[:2], len(w.target), qp, len(w.query), pairs, len(w.pairs), anchors, n, sc, flags,
-                                          cigar_cap)
-        keep = sfe.resolve(anchors, res, n, sc.min_score, acc, n + 1, nacc, stats)
-        state.update(res=res, keep=keep)
+        if K > 0:
+            o = sfe.speculate(tp[:2], len(w.target), qp, len(w.query), pairs, len(w.pairs), anchors, n, sc, K, flags, cigar_cap,
+                              accepted_dev=acc, n_accepted_dev=nacc, stats_dev=stats)
+            state.update(res=o["results"], keep=o["keep"])
+        else:
+            res, pool, used = sfe.ydrop_batch(tp[:2], len(w.target), qp, len(w.query), pairs, len(w.pairs), anchors, n, sc, flags,
+                                              cigar_cap)
+            keep = sfe.resolve(anchors, res, n, sc.min_score, acc, n + 1, nacc, stats)
+            state.update(res=res, keep=keep)
+
+    def launches_of(info, n_windows, K):
+        # pack x3; per Y-drop pass: tickets x3, ydrop, select_wide, ydrop_wide, join, scan, emit (+ select_overflow on re-runs);
+        # one batch: block_min + resolve; windows: prepare x3, scan + commit per window, finish
+        return 3 + 9 * info["launches"] + (info["launches"] - max(1, n_windows)) + ((3 + 2 * n_windows + 1) if K > 0 else 2)
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -200,7 +220,7 @@ def main():
     info0 = sfe.last_batch_info()
     st = stats.cpu().numpy().view(B.STATS_DT)[0]
     cells_step = int(st["cells_total"]); kept_step = int(st["n_kept"]); covered_step = int(st["n_covered"])
-    cells_cov = int(st["cells_covered"])
+    cells_cov = int(st["cells_covered"]); ext_step = int(st["n_extended"]); below_step = int(st["n_below"]); windows_step = int(st["n_windows"])
 
     sampler = ClockSampler(local)
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
@@ -211,7 +231,7 @@ def main():
         step()
         inf = sfe.last_batch_info()
         kernel_us += inf["ydrop_kernel_us"]
-        launches += inf["launches"] * 3 + 9      # ydrop + join + scan/emit per pass; pack x3, tickets x3, resolve x2, memset
+        launches += launches_of(inf, windows_step, window)
     e1.record()
     barrier()
     ms = e0.elapsed_time(e1)
@@ -229,11 +249,11 @@ def main():
         t_host = torch.from_numpy(w.target_ascii().copy()).pin_memory().numpy()
         q_host = torch.from_numpy(w.query_ascii().copy()).pin_memory().numpy()
         for _ in range(2):
-            ho = sfe.extend_host(t_host, q_host, pairs_np, anchors_np, sc, flags, cigar_cap)
+            ho = sfe.extend_host(t_host, q_host, pairs_np, anchors_np, sc, flags, cigar_cap, window)
         barrier()
         t0 = time.perf_counter()
         for _ in range(args.steps):
-            ho = sfe.extend_host(t_host, q_host, pairs_np, anchors_np, sc, flags, cigar_cap)
+            ho = sfe.extend_host(t_host, q_host, pairs_np, anchors_np, sc, flags, cigar_cap, window)
         torch.cuda.synchronize(dev)
         dt = time.perf_counter() - t0
         h2d = len(t_host) + len(q_host) + anchors_np.nbytes + pairs_np.nbytes
@@ -241,6 +261,19 @@ def main():
         e2e_cells = int(ho["stats"]["cells_total"]) * args.steps * world
         e2e = {"value": e2e_cells / dt / 1e9, "unit": "GCUPS", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": 1e3 * dt / args.steps, "kept_per_s": int(ho["stats"]["n_kept"]) * args.steps / dt}
+
+    # f4: batch-size sweep (Fig. 3): one timed pass per K, same inputs
+    sweep = []
+    for K in [int(x) for x in args.sweep_k.split(",") if x.strip()]:
+        step(K); torch.cuda.synchronize(dev)
+        k0 = torch.cuda.Event(enable_timing=True); k1 = torch.cuda.Event(enable_timing=True)
+        k0.record(); step(K); k1.record(); torch.cuda.synchronize(dev)
+        s2 = stats.cpu().numpy().view(B.STATS_DT)[0]; kms = k0.elapsed_time(k1)
+        sweep.append({"k": K, "ms": kms, "gcups": float(s2["cells_total"]) / (kms * 1e-3) / 1e9, "windows": int(s2["n_windows"]),
+                      "extended": int(s2["n_extended"]), "kept": int(s2["n_kept"]),
+                      "waste_ext": 1.0 - (int(s2["n_kept"]) + int(s2["n_below"])) / max(1, int(s2["n_extended"])),
+                      "waste_cells": float(s2["cells_covered"]) / max(1.0, float(s2["cells_total"])),
+                      "kept_per_s": int(s2["n_kept"]) / (kms * 1e-3)})
 
     if rank != 0:
         if world > 1:
@@ -278,13 +311,16 @@ def main():
     line = {"metric": "ydrop_gcups", "value": gcups, "unit": "GCUPS", "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "l2": "inputs+traceback per step exceed L2 (126 MB)",
+            "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "window_k": window,
+                       "l2": "inputs+traceback per step exceed L2 (126 MB)",
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "scoring": "HOXD70/400/30/ydrop 9400/lag 32/tau 3000"},
             "kept_alignments_per_s": kept_step * args.steps * world / (ms * 1e-3),
             "kept": kept_step, "cells_per_step": cells_step,
-            "speculation_waste": {"ext": covered_step / n if n else None, "cells": cells_cov / cells_step if cells_step else None},
+            "extended": ext_step, "windows": windows_step,
+            "speculation_waste": {"ext": 1.0 - (kept_step + below_step) / ext_step if ext_step else None,
+                                  "cells": cells_cov / cells_step if cells_step else None},
             "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roof, "cpu_baseline": cpu,
-            "batch_info": info0}
+            "batch_info": info0, "k_sweep": sweep or None}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -174,6 +174,13 @@ int sfe_extend_host(sfe_ctx *ctx, const char *t_ascii_host, int64_t t_len, const
                     sfe_result *results_host, uint8_t *keep_host,
                     uint32_t *cigar_host, int64_t cigar_cap, int64_t *cigar_used_host, sfe_stats *stats_host);
 
+/* The same with Algorithm 3's windows (sfe_speculate, window_k >= 1) between the copies. */
+int sfe_speculate_host(sfe_ctx *ctx, const char *t_ascii_host, int64_t t_len, const char *q_ascii_host, int64_t q_len,
+                       const sfe_pair *pairs_host, int32_t n_pairs, const sfe_anchor *anchors_host, int64_t n_anchors,
+                       const sfe_scoring *scoring_host, uint32_t flags, int64_t window_k,
+                       sfe_result *results_host, uint8_t *keep_host,
+                       uint32_t *cigar_host, int64_t cigar_cap, int64_t *cigar_used_host, sfe_stats *stats_host);
+
 /* Measurement helpers.  sfe_probe_int_issue runs a register-only microbenchmark
  * of the Y-drop kernel's own integer opcode mix on every SM and reports sustained
  * lane-instructions per clock per SM (the R of the integer-issue roofline).  mix: 0 = the

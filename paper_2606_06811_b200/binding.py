@@ -23,7 +23,7 @@ ST_TB_OVERFLOW, ST_CIGAR_OVERFLOW, ST_WIDE, ST_SCORE_LIMIT, ST_BAD_ANCHOR, ST_BA
 OP_M, OP_I, OP_D = 0, 1, 2
 
 EXPORTS = ("sfe_create", "sfe_destroy", "sfe_strerror", "sfe_last_error_detail", "sfe_pack", "sfe_ydrop_batch", "sfe_resolve",
-           "sfe_speculate", "sfe_extend_host", "sfe_probe_int_issue", "sfe_last_batch_info", "sfe_last_half_profile")
+           "sfe_speculate", "sfe_extend_host", "sfe_speculate_host", "sfe_probe_int_issue", "sfe_last_batch_info", "sfe_last_half_profile")
 
 
 class Scoring(C.Structure):
@@ -82,6 +82,8 @@ def lib():
         _lib.sfe_extend_host.argtypes = [vp, vp, i64, vp, i64, vp, i32, vp, i64, C.POINTER(Scoring), u32,
                                          vp, vp, vp, i64, C.POINTER(i64), C.POINTER(Stats)]
         _lib.sfe_last_half_profile.argtypes = [vp, i64, vp]
+        _lib.sfe_speculate_host.argtypes = [vp, vp, i64, vp, i64, vp, i32, vp, i64, C.POINTER(Scoring), u32, i64,
+                                            vp, vp, vp, i64, C.POINTER(i64), C.POINTER(Stats)]
         _lib.sfe_probe_int_issue.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib.sfe_last_batch_info.argtypes = [vp, C.POINTER(i64)]
     return _lib
@@ -231,8 +233,9 @@ class Sfe:
 
     # ---- sfe_extend_host ------------------------------------------------------------------------------
     def extend_host(self, t_ascii: np.ndarray, q_ascii: np.ndarray, pairs: np.ndarray, anchors: np.ndarray, sc: Scoring,
-                    flags: int = WANT_CIGAR, cigar_cap: int = 0):
-        """Host buffers in, host buffers out (numpy).  Returns dict(results, keep, cigar, cigar_used, stats)."""
+                    flags: int = WANT_CIGAR, cigar_cap: int = 0, window_k: int = 0):
+        """Host buffers in, host buffers out (numpy).  window_k >= 1 selects sfe_speculate_host (Algorithm 3's windows).
+        Returns dict(results, keep, cigar, cigar_used, stats)."""
         n = len(anchors)
         t_ascii = np.ascontiguousarray(t_ascii, dtype=np.uint8); q_ascii = np.ascontiguousarray(q_ascii, dtype=np.uint8)
         pairs = np.ascontiguousarray(pairs); anchors = np.ascontiguousarray(anchors)
@@ -244,9 +247,12 @@ class Sfe:
         cig = np.zeros(max(cigar_cap, 1), dtype=np.uint32)
         used = C.c_int64(0); st = Stats()
         vp = lambda a: C.c_void_p(a.ctypes.data)
-        _check(lib().sfe_extend_host(self.h, vp(t_ascii), len(t_ascii), vp(q_ascii), len(q_ascii), vp(pairs), len(pairs),
-                                     vp(anchors), n, C.byref(sc), flags, vp(res), vp(keep), vp(cig) if want else C.c_void_p(0),
-                                     cigar_cap if want else 0, C.byref(used), C.byref(st)), "sfe_extend_host")
+        tail = (vp(res), vp(keep), vp(cig) if want else C.c_void_p(0), cigar_cap if want else 0, C.byref(used), C.byref(st))
+        head = (self.h, vp(t_ascii), len(t_ascii), vp(q_ascii), len(q_ascii), vp(pairs), len(pairs), vp(anchors), n, C.byref(sc), flags)
+        if window_k >= 1:
+            _check(lib().sfe_speculate_host(*head, window_k, *tail), "sfe_speculate_host")
+        else:
+            _check(lib().sfe_extend_host(*head, *tail), "sfe_extend_host")
         return dict(results=res, keep=keep, cigar=cig, cigar_used=used.value,
                     stats={k: getattr(st, k) for k, _ in Stats._fields_})
 

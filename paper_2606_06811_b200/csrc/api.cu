@@ -420,10 +420,11 @@ extern "C" int sfe_resolve(sfe_ctx *c, const sfe_anchor *anchors_dev, const sfe_
                               keep_dev, stats_dev, (long long *)c->blkmin.p, (sfe_box *)c->act.p, c->stream);
 }
 
-extern "C" int sfe_extend_host(sfe_ctx *c, const char *t_ascii, int64_t t_len, const char *q_ascii, int64_t q_len,
-                               const sfe_pair *pairs, int32_t n_pairs, const sfe_anchor *anchors, int64_t n_anchors,
-                               const sfe_scoring *sc, uint32_t flags, sfe_result *results_host, uint8_t *keep_host,
-                               uint32_t *cigar_host, int64_t cigar_cap, int64_t *cigar_used_host, sfe_stats *stats_host)
+// window_k <= 0: one speculative batch over all anchors + one resolve; window_k >= 1: sfe_speculate
+static int extend_host_impl(sfe_ctx *c, const char *t_ascii, int64_t t_len, const char *q_ascii, int64_t q_len,
+                            const sfe_pair *pairs, int32_t n_pairs, const sfe_anchor *anchors, int64_t n_anchors,
+                            const sfe_scoring *sc, uint32_t flags, int64_t window_k, sfe_result *results_host, uint8_t *keep_host,
+                            uint32_t *cigar_host, int64_t cigar_cap, int64_t *cigar_used_host, sfe_stats *stats_host)
 {
     if (!c || !t_ascii || !q_ascii || !pairs || !anchors || !sc || !results_host || !keep_host) return SFE_EINVAL;
     if (t_len <= 0 || q_len <= 0 || n_pairs <= 0 || n_anchors <= 0) return SFE_EINVAL;
@@ -452,12 +453,20 @@ extern "C" int sfe_extend_host(sfe_ctx *c, const char *t_ascii, int64_t t_len, c
     if ((rc = sfe_pack(c, (const char *)c->h_tascii.p, t_len, (uint8_t *)c->h_t2.p, (uint8_t *)c->h_tm.p, nullptr, nullptr))) return rc;
     if ((rc = sfe_pack(c, (const char *)c->h_qascii.p, q_len, (uint8_t *)c->h_q2.p, (uint8_t *)c->h_qm.p, (uint8_t *)c->h_r2.p,
                        (uint8_t *)c->h_rm.p))) return rc;
-    if ((rc = sfe_ydrop_batch(c, (uint8_t *)c->h_t2.p, (uint8_t *)c->h_tm.p, t_len, (uint8_t *)c->h_q2.p, (uint8_t *)c->h_qm.p,
-                              (uint8_t *)c->h_r2.p, (uint8_t *)c->h_rm.p, q_len, (sfe_pair *)c->h_pairs.p, n_pairs,
-                              (sfe_anchor *)c->h_anchors.p, n_anchors, sc, flags, (sfe_result *)c->h_results.p,
-                              (uint32_t *)c->h_cigar.p, cigar_cap, (int64_t *)d_used))) return rc;
-    if ((rc = sfe_resolve(c, (sfe_anchor *)c->h_anchors.p, (sfe_result *)c->h_results.p, n_anchors, sc->min_score,
-                          (sfe_box *)c->h_acc.p, n_anchors, (int64_t *)(d_used + 1), (uint8_t *)c->h_keep.p, d_stats))) return rc;
+    if (window_k >= 1) {
+        if ((rc = sfe_speculate(c, (uint8_t *)c->h_t2.p, (uint8_t *)c->h_tm.p, t_len, (uint8_t *)c->h_q2.p, (uint8_t *)c->h_qm.p,
+                                (uint8_t *)c->h_r2.p, (uint8_t *)c->h_rm.p, q_len, (sfe_pair *)c->h_pairs.p, n_pairs,
+                                (sfe_anchor *)c->h_anchors.p, n_anchors, sc, flags, window_k, (sfe_result *)c->h_results.p,
+                                (uint8_t *)c->h_keep.p, (uint32_t *)c->h_cigar.p, cigar_cap, (int64_t *)d_used, (sfe_box *)c->h_acc.p,
+                                n_anchors, (int64_t *)(d_used + 1), d_stats))) return rc;
+    } else {
+        if ((rc = sfe_ydrop_batch(c, (uint8_t *)c->h_t2.p, (uint8_t *)c->h_tm.p, t_len, (uint8_t *)c->h_q2.p, (uint8_t *)c->h_qm.p,
+                                  (uint8_t *)c->h_r2.p, (uint8_t *)c->h_rm.p, q_len, (sfe_pair *)c->h_pairs.p, n_pairs,
+                                  (sfe_anchor *)c->h_anchors.p, n_anchors, sc, flags, (sfe_result *)c->h_results.p,
+                                  (uint32_t *)c->h_cigar.p, cigar_cap, (int64_t *)d_used))) return rc;
+        if ((rc = sfe_resolve(c, (sfe_anchor *)c->h_anchors.p, (sfe_result *)c->h_results.p, n_anchors, sc->min_score,
+                              (sfe_box *)c->h_acc.p, n_anchors, (int64_t *)(d_used + 1), (uint8_t *)c->h_keep.p, d_stats))) return rc;
+    }
     SFE_CUDA_CHECK(cudaMemcpyAsync(results_host, c->h_results.p, (size_t)n_anchors * sizeof(sfe_result), cudaMemcpyDeviceToHost, st));
     SFE_CUDA_CHECK(cudaMemcpyAsync(keep_host, c->h_keep.p, (size_t)n_anchors, cudaMemcpyDeviceToHost, st));
     long long used = 0;
@@ -471,4 +480,24 @@ extern "C" int sfe_extend_host(sfe_ctx *c, const char *t_ascii, int64_t t_len, c
     if (stats_host) SFE_CUDA_CHECK(cudaMemcpyAsync(stats_host, d_stats, sizeof(sfe_stats), cudaMemcpyDeviceToHost, st));
     SFE_CUDA_CHECK(cudaStreamSynchronize(st));
     return SFE_OK;
+}
+
+extern "C" int sfe_extend_host(sfe_ctx *c, const char *t_ascii, int64_t t_len, const char *q_ascii, int64_t q_len,
+                               const sfe_pair *pairs, int32_t n_pairs, const sfe_anchor *anchors, int64_t n_anchors,
+                               const sfe_scoring *sc, uint32_t flags, sfe_result *results_host, uint8_t *keep_host,
+                               uint32_t *cigar_host, int64_t cigar_cap, int64_t *cigar_used_host, sfe_stats *stats_host)
+{
+    return extend_host_impl(c, t_ascii, t_len, q_ascii, q_len, pairs, n_pairs, anchors, n_anchors, sc, flags, 0, results_host,
+                            keep_host, cigar_host, cigar_cap, cigar_used_host, stats_host);
+}
+
+extern "C" int sfe_speculate_host(sfe_ctx *c, const char *t_ascii, int64_t t_len, const char *q_ascii, int64_t q_len,
+                                  const sfe_pair *pairs, int32_t n_pairs, const sfe_anchor *anchors, int64_t n_anchors,
+                                  const sfe_scoring *sc, uint32_t flags, int64_t window_k, sfe_result *results_host,
+                                  uint8_t *keep_host, uint32_t *cigar_host, int64_t cigar_cap, int64_t *cigar_used_host,
+                                  sfe_stats *stats_host)
+{
+    if (window_k < 1) return SFE_EINVAL;
+    return extend_host_impl(c, t_ascii, t_len, q_ascii, q_len, pairs, n_pairs, anchors, n_anchors, sc, flags, window_k,
+                            results_host, keep_host, cigar_host, cigar_cap, cigar_used_host, stats_host);
 }

@@ -14,6 +14,7 @@
 #include "sfe_internal.cuh"
 
 #define FULL 0xffffffffu
+#define RES_ACT_S 64                  // active boxes mirrored in shared memory by resolve_kernel
 
 __global__ void block_min_kernel(const sfe_anchor *anchors, long long n, long long *blkmin)
 {
@@ -26,6 +27,37 @@ __global__ void block_min_kernel(const sfe_anchor *anchors, long long n, long lo
 static __device__ __forceinline__ bool box_has(const sfe_box &b, long long t, long long q, int strand)
 {
     return b.strand == strand && b.tstart <= t && t <= b.tend && b.qstart <= q && q <= b.qend;
+}
+
+// Decide one block of 32 anchors in anchor order (whole warp).  live = valid and not covered by an older box;
+// cand = live and score >= tau.  kept(l) = cand(l) and no kept lower lane's box contains l's point.
+// Only a candidate whose box reaches the smallest tpos among the later live lanes can cover anybody in the
+// block ("reaching").  The reaching candidates are visited in lane order: one that is already covered is not
+// kept and covers nobody; otherwise it is kept and every later live lane tests itself against its box in
+// parallel.  Rounds <= kept reaching candidates (none for disjoint boxes such as C4's); the non-reaching
+// candidates are kept iff nothing covered them.  Returns the kept mask; cov is updated for every live lane
+// (candidate or below tau: R17 is tested before R16).
+static __device__ unsigned decide_block(bool live, bool cand, bool &cov, const sfe_box &mine, long long tp, long long qp, int strand,
+                                        int lane)
+{
+    __shared__ sfe_box sb[32];
+    __syncwarp();
+    sb[lane] = mine;
+    long long suf = live ? tp : 0x7fffffffffffffffLL;             // inclusive suffix minimum of tpos over live lanes
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const long long y = __shfl_down_sync(FULL, suf, o); if (lane + o < 32 && y < suf) suf = y; }
+    long long after = __shfl_down_sync(FULL, suf, 1);
+    if (lane == 31) after = 0x7fffffffffffffffLL;
+    const unsigned reach = __ballot_sync(FULL, cand && mine.tend >= after);
+    unsigned covm = 0;
+    for (unsigned m = reach; m; m &= m - 1) {
+        const int l = __ffs(m) - 1;
+        if ((covm >> l) & 1u) continue;
+        const sfe_box b = sb[l];
+        covm |= __ballot_sync(FULL, live && lane > l && box_has(b, tp, qp, strand));
+    }
+    if ((covm >> lane) & 1u) cov = true;
+    return __ballot_sync(FULL, cand && !((covm >> lane) & 1u));
 }
 
 // single warp
@@ -50,63 +82,76 @@ __global__ void resolve_kernel(const sfe_anchor *anchors, const sfe_result *resu
     long long nacc = *n_accepted_io;
     long long nact = 0;
     const bool commit = results != nullptr;
-    // active list starts as every box carried in
-    for (long long k = lane; k < nacc; k += 32) act[k] = accepted[k];
+    // The warp is latency-bound, so: the next block's anchors / results are loaded one iteration ahead, the first
+    // RES_ACT_S active boxes are mirrored in shared memory (retire pass and cover scan read the mirror).
+    __shared__ sfe_box act_s[RES_ACT_S];
+    for (long long k = lane; k < nacc; k += 32) { const sfe_box b = accepted[k]; act[k] = b; if (k < RES_ACT_S) act_s[k] = b; }
     nact = nacc;
     __syncwarp();
     long long c_kept = 0, c_cov = 0, c_below = 0;
     unsigned long long cells_tot = 0, cells_cov = 0;
     bool overflow = false;
+    struct Item { long long tp, qp, tmin; int strand, score; unsigned long long cells; sfe_box box; bool valid; };
+    auto load_item = [&](long long blk) {
+        Item it;
+        const long long i = (blk << 5) + lane;
+        it.valid = i < n; it.tp = 0; it.qp = 0; it.strand = 0; it.score = 0; it.cells = 0;
+        it.box.tstart = it.box.tend = it.box.qstart = it.box.qend = 0; it.box.strand = 0; it.box.reserved = 0;
+        it.tmin = blkmin[blk];
+        if (it.valid) {
+            const sfe_anchor an = anchors[i];
+            it.tp = an.tpos; it.qp = an.qpos; it.strand = an.strand >= 0 ? 1 : -1;
+            if (commit) {
+                const sfe_result r = results[i];
+                it.score = r.score; it.cells = r.cells;
+                it.box.tstart = r.tstart; it.box.tend = r.tend; it.box.qstart = r.qstart; it.box.qend = r.qend; it.box.strand = it.strand;
+            }
+        }
+        return it;
+    };
+    Item nxt = load_item(0);
     for (long long blk = 0; blk < nblk; blk++) {
-        // retire boxes that end before every remaining anchor (stable in-place compaction)
-        {
-            const long long tmin = blkmin[blk];
+        const Item cur = nxt;
+        if (blk + 1 < nblk) nxt = load_item(blk + 1);
+        if (nact > 0) {                                   // retire boxes that end before every remaining anchor (stable compaction)
             long long w = 0;
+            const bool from_s = nact <= RES_ACT_S;
             for (long long base = 0; base < nact; base += 32) {
                 const long long k = base + lane;
                 sfe_box b; bool live = false;
-                if (k < nact) { b = act[k]; live = b.tend >= tmin; }
+                if (k < nact) { b = from_s ? act_s[k] : act[k]; live = b.tend >= cur.tmin; }
                 const unsigned m = __ballot_sync(FULL, live);
-                if (live) act[w + __popc(m & ((1u << lane) - 1))] = b;
+                __syncwarp();
+                if (live) { const long long d = w + __popc(m & ((1u << lane) - 1)); act[d] = b; if (d < RES_ACT_S) act_s[d] = b; }
                 w += __popc(m);
                 __syncwarp();
             }
             nact = w;
         }
         const long long i = (blk << 5) + lane;
-        const bool valid = i < n;
-        long long tp = 0, qp = 0; int strand = 0, score = 0; unsigned long long cells = 0;
-        sfe_box mine; mine.tstart = mine.tend = mine.qstart = mine.qend = 0; mine.strand = 0; mine.reserved = 0;
-        if (valid) {
-            tp = anchors[i].tpos; qp = anchors[i].qpos; strand = anchors[i].strand >= 0 ? 1 : -1;
-            if (commit) {
-                score = results[i].score; cells = results[i].cells;
-                mine.tstart = results[i].tstart; mine.tend = results[i].tend;
-                mine.qstart = results[i].qstart; mine.qend = results[i].qend; mine.strand = strand;
-            }
-        }
+        const bool valid = cur.valid;
+        const long long tp = cur.tp, qp = cur.qp; const int strand = cur.strand, score = cur.score;
+        const unsigned long long cells = cur.cells;
+        const sfe_box mine = cur.box;
         bool cov = false;
-        for (long long k = 0; k < nact; k++) { const sfe_box b = act[k]; cov = cov || box_has(b, tp, qp, strand); }
+        const long long ns = nact < RES_ACT_S ? nact : RES_ACT_S;
+        for (long long k = 0; k < ns; k++) { const sfe_box b = act_s[k]; cov = cov || box_has(b, tp, qp, strand); }
+        for (long long k = ns; k < nact; k++) { const sfe_box b = act[k]; cov = cov || box_has(b, tp, qp, strand); }
         cov = cov && valid;
-        bool cand = valid && !cov && commit && score >= min_score;
-        bool kept = false;
-        unsigned mask = __ballot_sync(FULL, cand);
-        while (mask) {
-            const int leader = __ffs(mask) - 1;
-            if (lane == leader) { kept = true; cand = false; }
-            sfe_box lb;
-            lb.tstart = __shfl_sync(FULL, mine.tstart, leader); lb.tend = __shfl_sync(FULL, mine.tend, leader);
-            lb.qstart = __shfl_sync(FULL, mine.qstart, leader); lb.qend = __shfl_sync(FULL, mine.qend, leader);
-            lb.strand = __shfl_sync(FULL, mine.strand, leader); lb.reserved = 0;
-            if (valid && lane > leader && !cov && box_has(lb, tp, qp, strand)) { cov = true; cand = false; }
-            if (lane == leader) {
-                if (nacc < accepted_cap) { accepted[nacc] = lb; act[nact] = lb; }
-            }
-            if (nacc < accepted_cap) { nact++; } else overflow = true;
-            nacc++;
-            __syncwarp();
-            mask = __ballot_sync(FULL, cand);
+        const bool live = valid && !cov, cand = live && commit && score >= min_score;
+        const unsigned kmask = decide_block(live, cand, cov, mine, tp, qp, strand, lane);
+        const bool kept = (kmask >> lane) & 1u;
+        if (kept) {                                               // append the kept boxes in lane order
+            const long long r = __popc(kmask & ((1u << lane) - 1));
+            if (nacc + r < accepted_cap) { accepted[nacc + r] = mine; act[nact + r] = mine; if (nact + r < RES_ACT_S) act_s[nact + r] = mine; }
         }
+        {
+            const long long nk = __popc(kmask);
+            const long long fit = nacc + nk <= accepted_cap ? nk : (accepted_cap > nacc ? accepted_cap - nacc : 0);
+            if (fit < nk) overflow = true;
+            nact += fit; nacc += nk;
+        }
+        __syncwarp();
         if (valid) {
             keep[i] = commit ? (cov ? 0 : (kept ? 1 : 2)) : (cov ? 0 : 1);
             c_kept += kept; c_cov += cov; c_below += (!cov && !kept);
@@ -267,26 +312,20 @@ __global__ void spec_commit_kernel(SpecState *st, const sfe_anchor *win_anchors,
         bool cov = false;
         for (long long k = 0; k < nloc; k++) { const sfe_box b = local[k]; cov = cov || box_has(b, tp, qp, strand); }
         cov = cov && valid;
-        bool cand = valid && !cov && score >= min_score;
-        bool kept = false;
-        unsigned mask = __ballot_sync(FULL, cand);
-        while (mask) {
-            const int leader = __ffs(mask) - 1;
-            if (lane == leader) { kept = true; cand = false; }
-            sfe_box lb;
-            lb.tstart = __shfl_sync(FULL, mine.tstart, leader); lb.tend = __shfl_sync(FULL, mine.tend, leader);
-            lb.qstart = __shfl_sync(FULL, mine.qstart, leader); lb.qend = __shfl_sync(FULL, mine.qend, leader);
-            lb.strand = __shfl_sync(FULL, mine.strand, leader); lb.reserved = 0;
-            if (valid && lane > leader && !cov && box_has(lb, tp, qp, strand)) { cov = true; cand = false; }
-            if (lane == leader) {
-                local[nloc] = lb;
-                if (nacc < accepted_cap) accepted[nacc] = lb;
-            }
-            if (nacc >= accepted_cap) overflow = true;
-            nloc++; nacc++;
-            __syncwarp();
-            mask = __ballot_sync(FULL, cand);
+        const bool live = valid && !cov, cand = live && score >= min_score;
+        const unsigned kmask = decide_block(live, cand, cov, mine, tp, qp, strand, lane);
+        const bool kept = (kmask >> lane) & 1u;
+        if (kept) {
+            const long long r = __popc(kmask & ((1u << lane) - 1));
+            local[nloc + r] = mine;
+            if (nacc + r < accepted_cap) accepted[nacc + r] = mine;
         }
+        {
+            const long long nk = __popc(kmask);
+            if (nacc + nk > accepted_cap) overflow = true;
+            nloc += nk; nacc += nk;
+        }
+        __syncwarp();
         if (valid) {
             keep[gi] = cov ? 0 : (kept ? 1 : 2);
             results[gi] = r;

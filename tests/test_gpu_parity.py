@@ -260,3 +260,33 @@ def test_speculate_config1_windows(sfe, oracle):
         assert int((out["keep"] == 1).sum()) == 64 and int(out["stats"]["n_extended"]) == n_ext, K
     full = H.gpu_run(sfe, w, flags=B.SCORE_ONLY)
     assert out["keep"].tolist() == full["keep"].tolist()
+
+
+@pytest.mark.parametrize("seed,n,spread", [(1, 1000, 40), (2, 5000, 400), (3, 257, 5), (4, 4096, 3000)])
+def test_resolve_random_boxes(sfe, oracle, seed, n, spread):
+    """sfe_resolve alone on synthetic (score, box) records: dense chains of mutually covering boxes, below-tau
+    anchors inside kept boxes (covered, not 'below': R17 is tested before R16), both strands, unsorted ties."""
+    import torch
+    rng = np.random.default_rng(seed)
+    tpos = np.sort(rng.integers(0, n * spread // 8 + 50, n)); qpos = tpos + rng.integers(-30, 30, n)
+    strand = np.where(rng.random(n) < 0.3, -1, 1)
+    anchors = np.stack([tpos, qpos, np.zeros(n, np.int64), strand], 1).astype(np.int64)
+    score = rng.integers(2000, 4500, n)
+    lo_t = rng.integers(0, spread, n); hi_t = rng.integers(0, spread, n); lo_q = rng.integers(0, spread, n); hi_q = rng.integers(0, spread, n)
+    boxes = np.stack([tpos - lo_t, tpos + hi_t, qpos - lo_q, qpos + hi_q], 1)
+    state, acc = oracle.resolve(anchors, score, boxes, 3000)
+    res = np.zeros(n, B.RESULT_DT)
+    res["score"] = score; res["tstart"] = boxes[:, 0]; res["tend"] = boxes[:, 1]; res["qstart"] = boxes[:, 2]; res["qend"] = boxes[:, 3]
+    res["cells"] = 7
+    dev = sfe.device
+    accd = torch.zeros((n + 1) * B.BOX_DT.itemsize, dtype=torch.uint8, device=dev)
+    nacc = torch.zeros(1, dtype=torch.int64, device=dev)
+    stats = torch.zeros(B.STATS_DT.itemsize, dtype=torch.uint8, device=dev)
+    keep = sfe.resolve(B._dev(B.make_anchors(anchors), dev), B._dev(res, dev), n, 3000, accd, n + 1, nacc, stats).cpu().numpy()[:n]
+    assert keep.tolist() == state.tolist()
+    assert int(nacc.item()) == len(acc)
+    got = accd.cpu().numpy()[: len(acc) * B.BOX_DT.itemsize].view(B.BOX_DT)
+    assert [(int(b["tstart"]), int(b["tend"]), int(b["qstart"]), int(b["qend"]), int(b["strand"])) for b in got] == [tuple(int(x) for x in b) for b in acc]
+    st = stats.cpu().numpy().view(B.STATS_DT)[0]
+    assert (int(st["n_kept"]), int(st["n_covered"]), int(st["n_below"])) == (int((state == 1).sum()), int((state == 0).sum()), int((state == 2).sum()))
+    assert int(st["cells_covered"]) == 7 * int((state == 0).sum())
