@@ -142,6 +142,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c4", "c3", "c3s", "c5s", "c5"])
     ap.add_argument("--window", type=int, default=-1, help="Algorithm 3's K (sfe_speculate); 0 = one batch over all anchors; -1 = workload default")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "block", "systolic"],
+                    help="block: the cooperative-warps kernel (one CTA per half) for every half; auto / systolic: one warp per half")
     ap.add_argument("--sweep-k", default="", help="comma-separated K values: one extra timed pass each (PAPER.md:163, Fig. 3)")
     ap.add_argument("--flags", default="cigar", choices=["cigar", "score"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -170,6 +172,7 @@ def main():
         desc += f" [profiling subset: {len(w.anchors)} anchors]"
     n = len(w.anchors)
     flags = B.WANT_CIGAR if args.flags == "cigar" else B.SCORE_ONLY
+    flags |= {"auto": 0, "block": B.BLOCK_KERNEL, "systolic": B.NO_BLOCK_KERNEL}[args.kernel]
     free_b, _ = torch.cuda.mem_get_info(dev)
     scratch = min(SCRATCH_GB[args.workload] << 30, int(free_b * 0.6))
     sfe = B.Sfe(local, scratch)
@@ -295,7 +298,7 @@ def main():
     peak_gcups = n_sm * fmax * 1e6 / cyc_per_cell / 1e9
     k_gcups = cells_step * args.steps / (kernel_us * 1e-6) / 1e9 if kernel_us > 0 else None
     roof = {"bound": "alu", "achieved": k_gcups, "peak": peak_gcups, "unit": "GCUPS", "frac": (k_gcups / peak_gcups) if k_gcups else None,
-            "traffic": None, "kernel": "ydrop_kernel<%s>" % ("traceback" if flags else "score-only"),
+            "traffic": None, "kernel": "ydrop_kernel<%s>" % ("traceback" if flags & B.WANT_CIGAR else "score-only"),
             "kernel_share_of_step": kernel_us * 1e-3 / ms,
             "detail": {"instr_per_cell_sass": hl["per_cell"], "alu_per_cell": hl["alu"], "dpx_per_cell": hl["dpx"], "fma_per_cell": hl["fma"],
                        "lsu_per_cell": hl["lsu"], "R_alu": r_alu, "R_dpx": r_dpx, "R_imad": r_fma, "R_mixed": r_mix,
@@ -311,7 +314,7 @@ def main():
     line = {"metric": "ydrop_gcups", "value": gcups, "unit": "GCUPS", "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "window_k": window,
+            "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "window_k": window, "kernel": args.kernel,
                        "l2": "inputs+traceback per step exceed L2 (126 MB)",
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "scoring": "HOXD70/400/30/ydrop 9400/lag 32/tau 3000"},
             "kept_alignments_per_s": kept_step * args.steps * world / (ms * 1e-3),

@@ -44,6 +44,9 @@ enum {
 #define SFE_WANT_CIGAR 1u             /* spill traceback pointers to HBM and emit CIGARs         */
 #define SFE_SCORE_ONLY 0u             /* scores, boxes and cell counts only                      */
 #define SFE_NO_BINNING 2u             /* tickets in anchor order (default: longest-first bins)   */
+#define SFE_BLOCK_KERNEL 4u           /* every half on the cooperative-warps kernel (one CTA per half, rows in order,
+                                         block-wide prefix maximum for F; same results)  */
+#define SFE_NO_BLOCK_KERNEL 8u        /* overrides SFE_BLOCK_KERNEL                               */
 
 /* per-anchor status bits (sfe_result.status) */
 #define SFE_ST_TB_OVERFLOW 1u         /* traceback arena exhausted even when run alone: no CIGAR */
@@ -189,7 +192,7 @@ int sfe_speculate_host(sfe_ctx *ctx, const char *t_ascii_host, int64_t t_len, co
  * sfe_ydrop_batch on this ctx: [0] kernel launches, [1] halves run, [2] halves re-run after a
  * traceback overflow, [3] traceback bytes written, [4] DP steps (warp wavefronts) executed,
  * [5] halves that took the wide path, [6] device time of the Y-drop kernel launches in microseconds
- * (CUDA events on the ctx stream; synchronises on the last one). */
+ * (CUDA events on the ctx stream; synchronises on the last one), [7] halves computed by the block kernel. */
 int sfe_probe_int_issue(sfe_ctx *ctx, int mix, int iters, double *lane_ops_per_clk_per_sm, double *elapsed_ms);
 
 /* Per-half profile of the most recent sfe_ydrop_batch on this ctx (Fig. 5: the

@@ -8,7 +8,7 @@
 
 
 // launchers defined next to their kernels
-int sfe_launch_ydrop(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st);
+int sfe_launch_ydrop(const YdParams &p, bool want_tb, bool use_block, int n_sm, cudaStream_t st);
 int sfe_launch_join(const sfe_anchor *anchors, const sfe_half *halves, long long n, const long long *sel, long long n_sel,
                     int want_cigar, sfe_result *results, cudaStream_t st);
 int sfe_launch_scan_emit(const sfe_half *halves, long long n, const long long *sel, long long n_sel, const uint32_t *stage,
@@ -59,7 +59,7 @@ struct sfe_ctx {
     long long *state_host;            // pinned, 8 words
     // host-API staging
     DevBuf h_tascii, h_qascii, h_t2, h_tm, h_q2, h_qm, h_r2, h_rm, h_pairs, h_anchors, h_results, h_keep, h_cigar, h_acc, h_small;
-    long long info[8];
+    long long info[8]; long long n_profile;
     cudaEvent_t ev0, ev1; bool ev_pending;
     double kernel_us;
 };
@@ -103,7 +103,7 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
     c->n_chunks = (int)nch;
     c->pool = nullptr; c->chunk_prev = nullptr; c->free_ring = nullptr; c->ring_state = nullptr; c->counters = nullptr; c->counters_host = nullptr; c->state_host = nullptr;
     memset(c->info, 0, sizeof c->info);
-    c->ev_pending = false; c->kernel_us = 0.0;
+    c->ev_pending = false; c->kernel_us = 0.0; c->n_profile = 0;
     if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) { delete c; return SFE_ECUDA; }
     if (cudaMalloc((void **)&c->pool, (size_t)nch * SFE_CHUNK_BYTES) != cudaSuccess ||
         cudaMalloc((void **)&c->chunk_prev, (size_t)nch * sizeof(int32_t)) != cudaSuccess ||
@@ -185,7 +185,7 @@ extern "C" int sfe_last_batch_info(sfe_ctx *c, int64_t info[8])
     c->info[6] = (long long)(c->kernel_us + 0.5);
     if (c->info[4] == 0) {   // score-only batches do not read the counters back inside the call
         if (cudaMemcpyAsync(c->counters_host, c->counters, CNT_N * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream) == cudaSuccess &&
-            cudaStreamSynchronize(c->stream) == cudaSuccess) { c->info[4] = (long long)c->counters_host[CNT_STEPS]; c->info[5] = (long long)c->counters_host[CNT_WIDE]; }
+            cudaStreamSynchronize(c->stream) == cudaSuccess) { c->info[4] = (long long)c->counters_host[CNT_STEPS]; c->info[5] = (long long)c->counters_host[CNT_WIDE]; c->info[7] = (long long)c->counters_host[CNT_BLOCK_HALVES]; }
         else cudaGetLastError();
     }
     for (int k = 0; k < 8; k++) info[k] = c->info[k];
@@ -195,7 +195,7 @@ extern "C" int sfe_last_batch_info(sfe_ctx *c, int64_t info[8])
 extern "C" int sfe_last_half_profile(sfe_ctx *c, int64_t n, sfe_half_profile *out)
 {
     if (!c || n < 0 || (n > 0 && !out)) return SFE_EINVAL;
-    if (n > c->info[7]) n = c->info[7];
+    if (n > c->n_profile) n = c->n_profile;
     if (n == 0) return SFE_OK;
     SFE_CUDA_CHECK(cudaSetDevice(c->device));
     sfe_half *h = (sfe_half *)malloc((size_t)n * sizeof(sfe_half));
@@ -221,11 +221,18 @@ static void harvest_kernel_time(sfe_ctx *c)
     c->ev_pending = false;
 }
 
-static int timed_ydrop(sfe_ctx *c, const YdParams &p, bool want_tb)
+// The row-synchronous block kernel (cooperative warps per half, f2) takes the pass only when asked to: it is
+// bit-exact but, at one thread per window column, still slower per extension than the systolic chain.
+static bool pick_block_kernel(const sfe_ctx *, long long, uint32_t flags)
+{
+    return (flags & SFE_BLOCK_KERNEL) != 0 && (flags & SFE_NO_BLOCK_KERNEL) == 0;
+}
+
+static int timed_ydrop(sfe_ctx *c, const YdParams &p, bool want_tb, uint32_t flags)
 {
     harvest_kernel_time(c);
     SFE_CUDA_CHECK(cudaEventRecord(c->ev0, c->stream));
-    const int rc = sfe_launch_ydrop(p, want_tb, c->n_sm, c->stream);
+    const int rc = sfe_launch_ydrop(p, want_tb, pick_block_kernel(c, p.n_tickets, flags), c->n_sm, c->stream);
     if (rc) return rc;
     SFE_CUDA_CHECK(cudaEventRecord(c->ev1, c->stream));
     c->ev_pending = true;
@@ -305,8 +312,8 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
     SFE_CUDA_CHECK(cudaMemsetAsync(c->counters, 0, CNT_N * sizeof(unsigned long long), c->stream));
     if ((rc = sfe_launch_tickets(anchors_dev, n_anchors, pairs_dev, n_pairs, q_len, !(flags & SFE_NO_BINNING),
                                  (unsigned int *)c->hist.p, (int32_t *)c->tickets.p, c->stream))) return rc;
-    if ((rc = timed_ydrop(c, p, want_tb))) return rc;
-    c->info[0] += 1; c->info[1] += 2 * n_anchors; c->info[7] = 2 * n_anchors;
+    if ((rc = timed_ydrop(c, p, want_tb, flags))) return rc;
+    c->info[0] += 1; c->info[1] += 2 * n_anchors; c->n_profile = 2 * n_anchors;
     if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, nullptr, n_anchors, want_tb, results_dev, c->stream))) return rc;
     if (!want_tb) return SFE_OK;
     if ((rc = sfe_launch_scan_emit(p.halves, n_anchors, nullptr, n_anchors, p.ops_stage, results_dev, cigar_pool_dev,
@@ -322,6 +329,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
         c->info[3] += (long long)c->counters_host[CNT_TBBYTES];
         c->info[4] += (long long)c->counters_host[CNT_STEPS];
         c->info[5] += (long long)c->counters_host[CNT_WIDE];
+        c->info[7] += (long long)c->counters_host[CNT_BLOCK_HALVES];
         const long long n_over = (long long)c->counters_host[CNT_OVERFLOW];
         if (n_over == 0) break;
         // no progress possible: the anchors that overflowed were already running alone
@@ -340,7 +348,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
         const long long need = (long long)c->counters_host[CNT_MAXNEED] > 0 ? (long long)c->counters_host[CNT_MAXNEED] : 1;
         const long long admit = c->n_chunks / need;
         p.max_warps = (int)(admit < 1 ? 1 : (admit > 0x7fffffffLL ? 0x7fffffffLL : admit));
-        if ((rc = timed_ydrop(c, p, true))) return rc;
+        if ((rc = timed_ydrop(c, p, true, flags))) return rc;
         c->info[0] += 1; c->info[1] += 2 * n_sel; c->info[2] += 2 * n_sel;
         if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, (const long long *)c->sel.p, n_sel, 1, results_dev, c->stream))) return rc;
         if ((rc = sfe_launch_scan_emit(p.halves, n_anchors, (const long long *)c->sel.p, n_sel, p.ops_stage, results_dev,

@@ -10,6 +10,7 @@
 #define SFE_ST_WIDE_PENDING 0x200u    // internal: the strip outgrew the shared-memory window; re-run by the wide kernel
 #define SFE_ST_PASS_OVERFLOW 0x100u   // internal: the traceback arena ran out during this pass; the anchor is re-run
 #define SFE_ST_OPS_OVERFLOW 0x400u    // internal: the ops arena ran out; reported as SFE_ST_CIGAR_OVERFLOW
+#define SFE_ST_BLOCK 0x800u           // internal: computed by the row-synchronous block kernel
 #define SFE_OOB_SCORE 0xE0000000u       // substitution "score" of a column beyond the target end (-2^29)
 
 // ---- shared-memory geometry of one warp -------------------------
@@ -72,7 +73,7 @@ struct sfe_half {                 // result of one one-sided extension (a7)
     uint32_t smid, wslot;         // SM and hardware warp slot that ran it
 };
 
-enum { CNT_TICKET = 0, CNT_UNUSED1, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_OPS, CNT_MAXNEED, CNT_CLASS0, CNT_CLASS1, CNT_CLASS2, CNT_CLASS3, CNT_N = 16 };
+enum { CNT_TICKET = 0, CNT_UNUSED1, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_OPS, CNT_MAXNEED, CNT_CLASS0, CNT_CLASS1, CNT_CLASS2, CNT_CLASS3, CNT_BLOCK_HALVES, CNT_N = 16 };
 
 struct SfeFreeRing {              // persistent across launches: every half returns its chunks before it ends
     unsigned long long head;      // pops issued

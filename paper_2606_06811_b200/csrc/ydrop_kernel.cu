@@ -16,8 +16,8 @@
 //     which is exactly what is final when row r starts in this schedule.
 // Dead cells are gated only on the diagonal/open edge (R6 lemma).
 #include "sfe_internal.cuh"
+#include "ydrop_common.cuh"
 
-#define FULL 0xffffffffu
 #ifndef SFE_MIN_BLOCKS
 #define SFE_MIN_BLOCKS 3
 #endif
@@ -26,14 +26,6 @@
 #endif
 // Ordering of a lane's message store and the next lane's load of it inside one wavefront step.
 #define SFE_STEP_FENCE() __syncwarp()
-
-// PRMT with the sign-replicate selector mode (bit 3 of a selector nibble), which __byte_perm masks off
-static __device__ __forceinline__ int prmt_sx(uint32_t lo, uint32_t hi, uint32_t sel)
-{
-    int r;
-    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(lo), "r"(hi), "r"(sel));
-    return r;
-}
 
 // Boundary-ring address of column c: row (c-1) mod 8, segment ((c-1) div 8) mod RING/8.  Strips start
 // at a multiple of 16 and groups hold 16 steps, so lane 0 (reading column cs+t0+k+1) and lane 31
@@ -44,21 +36,6 @@ static __device__ __forceinline__ int bnd_off(int c)
 {
     const int u = c - 1;
     return (u & 7) * RingGeom<RL2>::ROW_STRIDE + SFE_EXCH_BYTES + ((u >> 3) & (RingGeom<RL2>::RING / 8 - 1)) * 8;
-}
-
-struct HalfGeom {
-    const uint8_t *qc, *qm, *tc, *tm;
-    long long q0, t0;     // base index of row i / column j is q0 + d*i, t0 + d*j (i, j >= 1)
-    int d;
-    int n, m;
-};
-
-static __device__ __forceinline__ uint32_t col_selector(const HalfGeom &g, int c)
-{
-    if (c <= 0) return 0x8880u;
-    if (c > g.m) return 0x6555u;                         // -> SFE_OOB_SCORE
-    const int b = sfe_base(g.tc, g.tm, g.t0 + (long long)g.d * c);
-    return b == 4 ? 0xCCC4u : 0x8880u + 0x1111u * (uint32_t)b;
 }
 
 // fill selector-ring entries for columns [lo, hi).  Common case (every column has a target base): each
@@ -102,43 +79,6 @@ static __device__ __forceinline__ void fill_bnd_neg(char *wbase, int lo, int hi,
 {
     for (int c = lo + lane; c < hi; c += 32) *(int2 *)(wbase + bnd_off<RL2>(c)) = make_int2(SFE_NEG, SFE_NEG);
     __syncwarp();
-}
-
-// Free-chunk ring (sfe_internal.cuh).  Called by the whole warp; lane 0 does the memory operations and
-// every loop runs on a broadcast value, so control flow stays warp-uniform (a loop inside a
-// lane-divergent region makes ptxas clone the whole DP loop with real WARPSYNCs).  Both spins wait
-// for one bounded action of another resident warp (the matching push / pop has already reserved the
-// slot), never for work.
-static __device__ __forceinline__ int chunk_pop(int32_t *ring, SfeFreeRing *st, int n_chunks, int lane)
-{
-    long long a = 0; unsigned long long h = 0;
-    if (lane == 0) {
-        a = (long long)atomicAdd((unsigned long long *)&st->avail, ~0ULL);            // avail--
-        if (a <= 0) atomicAdd((unsigned long long *)&st->avail, 1ULL);                // nothing left: undo
-        else h = atomicAdd(&st->head, 1ULL);
-    }
-    a = __shfl_sync(FULL, a, 0);
-    if (a <= 0) return -1;
-    volatile int32_t *slot = ring + (h % (unsigned long long)n_chunks);
-    int id = -1;
-    do {
-        if (lane == 0) id = *slot;
-        id = __shfl_sync(FULL, id, 0);
-    } while (id < 0);
-    if (lane == 0) *slot = -1;
-    return id;
-}
-static __device__ __forceinline__ void chunk_push(int32_t *ring, SfeFreeRing *st, int n_chunks, int id, int lane)
-{
-    unsigned long long t = 0;
-    if (lane == 0) t = atomicAdd(&st->tail, 1ULL);
-    int32_t *slot = ring + (t % (unsigned long long)n_chunks);
-    int old = -1;
-    do {                                                   // the pop that owns this slot may not have emptied it yet
-        if (lane == 0) old = atomicCAS(slot, -1, id);
-        old = __shfl_sync(FULL, old, 0);
-    } while (old != -1);
-    if (lane == 0) atomicAdd((unsigned long long *)&st->avail, 1ULL);
 }
 
 struct TbWriter {
@@ -271,43 +211,6 @@ struct TbReader {                       // random access to this half's records;
     }
 };
 
-struct OpsWriter {                      // run-length encoder + staging of the ops in walk order
-    uint32_t *buf;                      // SFE_WALK_OPS words of shared memory
-    uint32_t *stage; unsigned long long *used; unsigned long long cap;
-    int nbuf, nops, cur_op, run; uint32_t prev_seg; bool ok;
-    __device__ __forceinline__ void flush(int lane)
-    {
-        if (nbuf == 0) return;
-        __syncwarp();
-        if (ok) {
-            unsigned long long base = 0;
-            if (lane == 0) base = atomicAdd(used, (unsigned long long)(nbuf + 2));
-            base = __shfl_sync(FULL, base, 0);
-            if (base + (unsigned long long)(nbuf + 2) > cap) ok = false;
-            else {
-                if (lane == 0) { stage[base] = prev_seg; stage[base + 1] = (uint32_t)nbuf; }
-                for (int x = lane; x < nbuf; x += 32) stage[base + 2 + x] = buf[x];
-                prev_seg = (uint32_t)base;
-            }
-        }
-        nbuf = 0;
-        __syncwarp();
-    }
-    __device__ __forceinline__ void push(int lane)
-    {
-        if (lane == 0) buf[nbuf] = ((uint32_t)run << 4) | (uint32_t)cur_op;
-        nbuf++; nops++;
-        if (nbuf == SFE_WALK_OPS) flush(lane);
-    }
-    __device__ __forceinline__ void emit(int op, int cnt, int lane)
-    {
-        if (cnt <= 0) return;
-        if (op == cur_op) { run += cnt; return; }
-        if (cur_op >= 0) push(lane);
-        cur_op = op; run = cnt;
-    }
-};
-
 // Returns false if the walk did not reach the origin (internal error guard).
 static __device__ bool walk_traceback(const YdParams &p, TbReader &rd, const int end_i, const int end_j, int hdr, int strip,
                                       char *wk, const int lane, uint32_t &ops_seg, int &n_ops, bool &ops_ok)
@@ -395,29 +298,12 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
     out.cycles = 0; out.smid = 0; out.wslot = 0;
     const long long clk0 = clock64();
 
-    const long long a = hid >> 1;
-    const int dir = hid & 1;
-    const sfe_anchor an = p.anchors[a];
     HalfGeom g;
-    bool bad = an.pair < 0 || an.pair >= p.n_pairs;
-    sfe_pair pr = {0, 0, 0, 0};
-    if (!bad) pr = p.pairs[an.pair];
-    long long qb, qe;
-    if (an.strand >= 0) { g.qc = p.q_codes; g.qm = p.q_nmask; qb = pr.q_begin; qe = pr.q_end; }
-    else { g.qc = p.qrc_codes; g.qm = p.qrc_nmask; qb = p.q_len - pr.q_end; qe = p.q_len - pr.q_begin; }
-    g.tc = p.t_codes; g.tm = p.t_nmask;
-    bad = bad || an.tpos < pr.t_begin || an.tpos > pr.t_end || an.qpos < qb || an.qpos > qe || g.qc == nullptr ||
-          pr.t_begin < 0 || pr.t_end > p.t_len || qb < 0 || qe > p.q_len;
-    if (bad) {
+    if (!half_setup(p, hid, g)) {
         out.status = SFE_ST_BAD_ANCHOR;
         if (lane == 0) p.halves[hid] = out;
         return;
     }
-    long long nn, mm;
-    if (dir == 0) { nn = qe - an.qpos; mm = pr.t_end - an.tpos; g.q0 = an.qpos - 1; g.t0 = an.tpos - 1; g.d = 1; }
-    else { nn = an.qpos - qb; mm = an.tpos - pr.t_begin; g.q0 = an.qpos; g.t0 = an.tpos; g.d = -1; }
-    const long long LIM = 0x7ffffff0LL - 4096;
-    g.n = (int)(nn < LIM ? nn : LIM); g.m = (int)(mm < LIM ? mm : LIM);
 
     const int OX = p.OX, X = p.X;
     TbWriter tb;
@@ -641,26 +527,35 @@ __global__ void __launch_bounds__(32) ydrop_wide_kernel(const YdParams p)
     }
 }
 
-int sfe_launch_ydrop(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st)
+int sfe_launch_ydrop_block(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st);
+
+// use_block: the whole pass goes to the row-synchronous block kernel (ydrop_block_kernel.cu) instead of the
+// warp-systolic one; either way halves whose band outgrew the window are re-run by the wide kernel.
+int sfe_launch_ydrop(const YdParams &p, bool want_tb, bool use_block, int n_sm, cudaStream_t st)
 {
-    const int warps_per_block = SFE_BLOCK_THREADS / 32;
-    const size_t smem = (size_t)warps_per_block * SFE_WARP_SMEM;
-    static bool attr_done = false;
-    if (!attr_done) {
-        if (cudaFuncSetAttribute(ydrop_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SFE_ECUDA;
-        if (cudaFuncSetAttribute(ydrop_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SFE_ECUDA;
-        attr_done = true;
+    if (use_block) {
+        const int rc = sfe_launch_ydrop_block(p, want_tb, n_sm, st);
+        if (rc) return rc;
+    } else {
+        const int warps_per_block = SFE_BLOCK_THREADS / 32;
+        const size_t smem = (size_t)warps_per_block * SFE_WARP_SMEM;
+        static bool attr_done = false;
+        if (!attr_done) {
+            if (cudaFuncSetAttribute(ydrop_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SFE_ECUDA;
+            if (cudaFuncSetAttribute(ydrop_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SFE_ECUDA;
+            attr_done = true;
+        }
+        int bps = 0;
+        if (want_tb) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<true>, SFE_BLOCK_THREADS, smem);
+        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<false>, SFE_BLOCK_THREADS, smem);
+        if (bps < 1) return SFE_ECUDA;
+        long long blocks = (long long)n_sm * bps;
+        const long long need = (p.n_tickets + warps_per_block - 1) / warps_per_block;
+        if (blocks > need) blocks = need;
+        if (blocks < 1) blocks = 1;
+        if (want_tb) ydrop_kernel<true><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
+        else ydrop_kernel<false><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
     }
-    int bps = 0;
-    if (want_tb) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<true>, SFE_BLOCK_THREADS, smem);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<false>, SFE_BLOCK_THREADS, smem);
-    if (bps < 1) return SFE_ECUDA;
-    long long blocks = (long long)n_sm * bps;
-    const long long need = (p.n_tickets + warps_per_block - 1) / warps_per_block;
-    if (blocks > need) blocks = need;
-    if (blocks < 1) blocks = 1;
-    if (want_tb) ydrop_kernel<true><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
-    else ydrop_kernel<false><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
     const int bs = 256;
     select_wide_kernel<<<(unsigned)((p.n_tickets + bs - 1) / bs), bs, 0, st>>>(p);
     if (want_tb) ydrop_wide_kernel<true><<<SFE_WIDE_WARPS, 32, 0, st>>>(p);
