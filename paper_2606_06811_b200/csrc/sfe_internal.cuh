@@ -29,7 +29,7 @@ template <int RL2> struct RingGeom {
     static constexpr int RING = 1 << RL2;                        // boundary-ring capacity in columns
     static constexpr int ROW_STRIDE = SFE_EXCH_BYTES + RING;     // bytes: exchange area + RING/8 segments x 8 B
     static constexpr int SELRING = RING;                         // selector ring (>= MAX_STEPS + 192: the next strip re-reads the window start)
-    static constexpr int WARP_BYTES = 8 * ROW_STRIDE + (SELRING + 16) * 2;
+    static constexpr int WARP_BYTES = 8 * ROW_STRIDE + (SELRING + 32) * 2;
     static constexpr int MAX_STEPS = RING - 192;                 // a strip wider than this bails out (multiple of 16)
 };
 #define SFE_WARP_SMEM (RingGeom<SFE_RING_LOG2>::WARP_BYTES)

@@ -27,8 +27,10 @@
 // them, and then advances up to 32 path cells per ballot exactly as walk_traceback does.
 #include "ydrop_common.cuh"
 
-#define BK_THREADS 1024
-#define BK_WIN 1024                      // columns of the live window = threads
+#define BK_THREADS 256
+#define BK_WARPS 8
+#define BK_CPT 4                         // columns per thread
+#define BK_WIN 1024                      // columns of the live window = BK_THREADS * BK_CPT
 #define BK_WALK_WORDS 4096               // log words staged in shared memory by the walk
 #define BK_DIR 64                        // rows indexed per staged window
 #define BK_CHUNK_WORDS (SFE_CHUNK_BYTES / 4)
@@ -91,7 +93,7 @@ static __device__ bool block_walk(const YdParams &p, BkShared &sh, const int end
                 while (k < BK_DIR && e - 2 >= lo) {
                     const int nw = (int)sh.walk[e - 1 - lo], c0 = (int)sh.walk[e - 2 - lo];
                     const int start = e - 2 - nw;
-                    if (nw < 4 || nw > 128 || start < lo) break;
+                    if (nw < 16 || nw > 128 || start < lo) break;
                     sh.dir_base[k] = start; sh.dir_c0[k] = c0; sh.dir_nw[k] = nw;
                     e = start; k++;
                 }
@@ -110,9 +112,7 @@ static __device__ bool block_walk(const YdParams &p, BkShared &sh, const int end
             const int pos = jx - sh.dir_c0[k];
             valid = pos >= 0 && pos < 8 * sh.dir_nw[k];
             if (valid) {
-                const uint32_t *w = sh.walk + (sh.dir_base[k] - base0) + 4 * (pos >> 5);
-                const int b = pos & 31;
-                nib = ((w[0] >> b) & 1u) | (((w[1] >> b) & 1u) << 1) | (((w[2] >> b) & 1u) << 2) | (((w[3] >> b) & 1u) << 3);
+                nib = (sh.walk[(sh.dir_base[k] - base0) + (pos >> 3)] >> (4 * (pos & 7))) & 15u;
             }
         }
         // nib: bit3 = H not from M, bit2 = H not from E, bit1 = E extended, bit0 = F extended (R11)
@@ -173,12 +173,15 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
 
     if (tid < 64) sh.cum[tid] = 0;
     if (tid == 0) { sh.best = 0; sh.best_i = 0; sh.best_j = 0; sh.best_chunk = -1; sh.best_wpos = 0; }
-    if (tid < 32) sh.edge[tid] = SFE_NEG;
+    if (tid < BK_WARPS) sh.edge[tid] = SFE_NEG;
     __syncthreads();
 
-    int ws = 0, ws_prev = 0;                              // window start of this / the previous row (multiples of 32)
-    int mycol = -1, Hu = SFE_NEG, Eu = SFE_NEG;           // previous-row state of my column: gated H - OX, E
-    uint32_t sel = 0x8880u;
+    int ws = 0, ws_prev = 0;                              // window start of this / the previous row (multiples of 128)
+    int myc0 = -1;                                        // first of my BK_CPT columns
+    int Hu[BK_CPT], Eu[BK_CPT];                           // previous-row state of my columns: gated H - OX, E
+    uint32_t sel[BK_CPT];
+#pragma unroll
+    for (int k = 0; k < BK_CPT; k++) { Hu[k] = SFE_NEG; Eu[k] = SFE_NEG; sel[k] = 0x8880u; }
     unsigned long long cells = 0;
     int rows_done = 0, max_width = 0;
     bool wide = false;
@@ -188,69 +191,90 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
         const uint32_t srow_lo = srow_nxt;
         if (i < g.n) srow_nxt = p.srow[sfe_base(g.qc, g.qm, g.q0 + (long long)g.d * (i + 1))];   // prefetched for the next row
         const int T = p.ydrop_inf ? SFE_T_INF : (i >= 32 ? sh.cum[(i - 32) & 63] : 0) - p.Y;    // R4
-        // ---- my column in this row's window ----
-        const int c = ws + ((tid - ws) & (BK_WIN - 1));
-        if (c != mycol) { mycol = c; Hu = SFE_NEG; Eu = SFE_NEG; sel = col_selector(g, c); }
-        const int pcol = c - ws;                          // position in the window
-        const int rank = (warp - (ws >> 5)) & 31;         // my warp's position in the window
-        // ---- diagonal: the left neighbour's previous-row value ----
-        int Hd = __shfl_up_sync(FULL, Hu, 1);
-        if (lane == 0) Hd = (c - 1 - ws_prev < BK_WIN) ? sh.edge[(warp - 1) & 31] : SFE_NEG;
-        if (pcol == 0) Hd = SFE_NEG;
-        if (i == 0 && c == 0) Hd = -OX;                   // the origin
-        const int s = prmt_sx(srow_lo, srow_hi, sel);
-        const int M = Hd + s + OX;
-        const int E = __viaddmax_s32(Eu, -X, Hu);
-        int Ht = max(M, E);
-        if (c > g.m) Ht = SFE_NEG;
-        // ---- F: block-wide exclusive prefix maximum of a_p = H~ - O + X p ----
-        const int a = Ht - OX + X * (pcol + 1);
-        const int incl = warp_scan_max(a, lane);
+        // ---- my columns in this row's window ----
+        const int q = ((tid * BK_CPT) - ws) & (BK_WIN - 1);       // window position of my first column
+        const int c0 = ws + q;
+        if (c0 != myc0) {
+            myc0 = c0;
+#pragma unroll
+            for (int k = 0; k < BK_CPT; k++) { Hu[k] = SFE_NEG; Eu[k] = SFE_NEG; sel[k] = col_selector(g, c0 + k); }
+        }
+        const int rank = (warp - (ws >> 7)) & (BK_WARPS - 1);     // my warp's position in the window
+        // ---- diagonal of my first column: the left neighbour's previous-row value ----
+        int Hd0 = __shfl_up_sync(FULL, Hu[BK_CPT - 1], 1);
+        if (lane == 0) Hd0 = (c0 - 1 - ws_prev < BK_WIN) ? sh.edge[(warp - 1) & (BK_WARPS - 1)] : SFE_NEG;
+        if (q == 0) Hd0 = SFE_NEG;
+        if (i == 0 && c0 == 0) Hd0 = -OX;                 // the origin
+        int M[BK_CPT], E[BK_CPT], Ht[BK_CPT], pa[BK_CPT];
+#pragma unroll
+        for (int k = 0; k < BK_CPT; k++) {
+            const int Hd = k == 0 ? Hd0 : Hu[k - 1];
+            const int s = prmt_sx(srow_lo, srow_hi, sel[k]);
+            M[k] = Hd + s + OX;
+            E[k] = __viaddmax_s32(Eu[k], -X, Hu[k]);
+            Ht[k] = max(M[k], E[k]);
+            if (c0 + k > g.m) Ht[k] = SFE_NEG;
+            const int a = Ht[k] - OX + X * (q + k + 1);   // a_p = H~ - O + X p
+            pa[k] = k == 0 ? a : max(pa[k - 1], a);
+        }
+        // ---- F: block-wide exclusive prefix maximum ----
+        const int incl = warp_scan_max(pa[BK_CPT - 1], lane);
         int excl = __shfl_up_sync(FULL, incl, 1);
         if (lane == 0) excl = BK_NINF;
-        const int Ht_left_w = __shfl_up_sync(FULL, Ht, 1);
-        if (lane == 31) { sh.tot[rank] = incl; sh.tex[rank] = excl; sh.tht[rank] = Ht; }
+        const int my_tex = max(excl, pa[BK_CPT - 2]);     // what my last column sees from inside the warp
+        int lHt = __shfl_up_sync(FULL, Ht[BK_CPT - 1], 1);
+        const int lpre_in = __shfl_up_sync(FULL, my_tex, 1);
+        if (lane == 31) { sh.tot[rank] = incl; sh.tex[rank] = my_tex; sh.tht[rank] = Ht[BK_CPT - 1]; }
         __syncthreads();                                                                      // B1
-        const int t_l = sh.tot[lane];
+        const int t_l = lane < BK_WARPS ? sh.tot[lane] : BK_NINF;
         const int carry_prev = __reduce_max_sync(FULL, lane < rank - 1 ? t_l : BK_NINF);      // ranks < rank - 1
         const int carry = rank > 0 ? max(carry_prev, sh.tot[rank - 1]) : BK_NINF;             // ranks < rank
-        const int pre = max(excl, carry);
-        const int F = pcol == 0 ? SFE_NEG : pre - X * pcol;
-        int H = max(Ht, F);
-        if (c > g.m) H = SFE_NEG;
-        const bool alive = H >= T;                        // R5
-        uint32_t plane = 0;
-        if (TB) {
-            // left neighbour's H~ and F, for "F extended" (R11: open wins ties)
-            int Ht_left = Ht_left_w, pre_left = __shfl_up_sync(FULL, pre, 1);
-            if (lane == 0 && rank > 0) { Ht_left = sh.tht[rank - 1]; pre_left = max(sh.tex[rank - 1], carry_prev); }
-            const int F_left = pcol <= 1 ? SFE_NEG : pre_left - X * (pcol - 1);
-            const int Hgl = pcol == 0 ? SFE_NEG : max(Ht_left, F_left) - OX;
-            const uint32_t b3 = __ballot_sync(FULL, M < H), b2 = __ballot_sync(FULL, E < H);
-            const uint32_t b1 = __ballot_sync(FULL, Hu < E), b0 = __ballot_sync(FULL, Hgl < F);
-            // lanes 0..3 keep the four plane words until the row's extent is known
-            plane = lane == 0 ? b0 : lane == 1 ? b1 : lane == 2 ? b2 : b3;
+        const int pre0 = max(excl, carry);
+        // final H of the column left of my first one (for "F extended", R11)
+        int lpre = max(lpre_in, carry);
+        if (lane == 0 && rank > 0) { lHt = sh.tht[rank - 1]; lpre = max(sh.tex[rank - 1], carry_prev); }
+        int Hprev = q == 0 ? SFE_NEG : max(lHt, q == 1 ? SFE_NEG : lpre - X * (q - 1));
+        uint32_t nibs = 0;
+        int hmax = SFE_NEG, hcol = 0x7fffffff, cl = 0x7fffffff, cr = -1;
+#pragma unroll
+        for (int k = 0; k < BK_CPT; k++) {
+            const int pk = q + k;
+            const int pre = k == 0 ? pre0 : max(pre0, pa[k - 1]);
+            const int F = pk == 0 ? SFE_NEG : pre - X * pk;
+            int H = max(Ht[k], F);
+            if (c0 + k > g.m) H = SFE_NEG;
+            const bool alive = H >= T;                    // R5
+            if (TB) {
+                const int Hgl = pk == 0 ? SFE_NEG : Hprev - OX;
+                const uint32_t nib = ((M[k] < H) ? 8u : 0u) | ((E[k] < H) ? 4u : 0u) | ((Hu[k] < E[k]) ? 2u : 0u) | ((Hgl < F) ? 1u : 0u);
+                nibs |= nib << (4 * k);
+            }
+            Hprev = H;
+            Hu[k] = alive ? H - OX : SFE_NEG;
+            Eu[k] = E[k];
+            if (alive) {
+                if (H > hmax) { hmax = H; hcol = c0 + k; }
+                cl = min(cl, c0 + k); cr = c0 + k;
+            }
         }
-        // ---- new state, row statistics ----
-        Hu = alive ? H - OX : SFE_NEG;
-        Eu = E;
-        const int hm = __reduce_max_sync(FULL, alive ? H : SFE_NEG);
-        const int hc = __reduce_min_sync(FULL, (alive && H == hm) ? c : 0x7fffffff);
-        const int cl = __reduce_min_sync(FULL, alive ? c : 0x7fffffff);
-        const int cr = __reduce_max_sync(FULL, alive ? c : -1);
-        if (lane == 31) sh.edge[warp] = Hu;
-        if (lane == 0) { sh.wmax[warp] = hm; sh.wcol[warp] = hc; sh.wL[warp] = cl; sh.wR[warp] = cr; }
+        // ---- row statistics ----
+        const int hm = __reduce_max_sync(FULL, hmax);
+        const int hc = __reduce_min_sync(FULL, hmax == hm ? hcol : 0x7fffffff);
+        const int wl = __reduce_min_sync(FULL, cl);
+        const int wr = __reduce_max_sync(FULL, cr);
+        if (lane == 31) sh.edge[warp] = Hu[BK_CPT - 1];
+        if (lane == 0) { sh.wmax[warp] = hm; sh.wcol[warp] = hc; sh.wL[warp] = wl; sh.wR[warp] = wr; }
         __syncthreads();                                                                      // B2
-        const int L = __reduce_min_sync(FULL, sh.wL[lane]);
-        const int R = __reduce_max_sync(FULL, sh.wR[lane]);
+        const int L = __reduce_min_sync(FULL, lane < BK_WARPS ? sh.wL[lane] : 0x7fffffff);
+        const int R = __reduce_max_sync(FULL, lane < BK_WARPS ? sh.wR[lane] : -1);
         if (R < 0) break;                                 // first row without an alive cell: all later rows are dead
         rows_done = i + 1;
         cells += (unsigned long long)(R - L + 1);
         max_width = max(max_width, R - L + 1);
-        // ---- row record: the warps between the first and the last alive column store their plane words ----
+        // ---- row record: the warps between the first and the last alive column store 16 bits per thread ----
         if (TB && tb_ok) {
-            const int r_lo = (L - ws) >> 5, r_hi = (R - ws) >> 5;
-            const int nw = 4 * (r_hi - r_lo + 1);
+            const int r_lo = (L - ws) >> 7, r_hi = (R - ws) >> 7;
+            const int nw = 16 * (r_hi - r_lo + 1);
             if (wpos + nw + 2 > BK_CHUNK_WORDS) {         // next chunk (uniform decision)
                 if (warp == 0) {
                     if (cur_chunk >= 0 && lane == 0) p.pool[(size_t)cur_chunk * BK_CHUNK_WORDS] = (uint32_t)wpos;
@@ -265,16 +289,16 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
             }
             if (tb_ok) {
                 uint32_t *rec = p.pool + (size_t)cur_chunk * BK_CHUNK_WORDS + wpos;
-                if (rank >= r_lo && rank <= r_hi && lane < 4) rec[4 * (rank - r_lo) + lane] = plane;
-                if (tid == 0) { rec[nw] = (uint32_t)(ws + 32 * r_lo); rec[nw + 1] = (uint32_t)nw; }
+                if (rank >= r_lo && rank <= r_hi) ((uint16_t *)rec)[32 * (rank - r_lo) + lane] = (uint16_t)nibs;
+                if (tid == 0) { rec[nw] = (uint32_t)(ws + 128 * r_lo); rec[nw + 1] = (uint32_t)nw; }
                 wpos += nw + 2; n_words += nw + 2;
             }
         }
         // ---- warp 0: cumulative best (for T of row i + 32) and the first maximum (R7) ----
         if (warp == 0) {
-            const int wm = sh.wmax[lane];
+            const int wm = lane < BK_WARPS ? sh.wmax[lane] : SFE_NEG;
             const int gm = __reduce_max_sync(FULL, wm);
-            const int gc = __reduce_min_sync(FULL, wm == gm ? sh.wcol[lane] : 0x7fffffff);
+            const int gc = __reduce_min_sync(FULL, (lane < BK_WARPS && wm == gm) ? sh.wcol[lane] : 0x7fffffff);
             if (lane == 0) {
                 const int prev = i > 0 ? sh.cum[(i - 1) & 63] : 0;
                 sh.cum[i & 63] = max(prev, gm);
@@ -282,9 +306,9 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
             }
         }
         // ---- next row's window ----
-        if (R - (L & ~31) >= BK_WIN - 1) { wide = true; break; }   // an alive cell in the last column the next window could hold
+        if (R - (L & ~127) >= BK_WIN - 1) { wide = true; break; }  // an alive cell in the last column the next window could hold
         ws_prev = ws;
-        ws = L & ~31;
+        ws = L & ~127;
     }
     __syncthreads();
     if (TB && cur_chunk >= 0 && tid == 0) p.pool[(size_t)cur_chunk * BK_CHUNK_WORDS] = (uint32_t)wpos;
@@ -323,7 +347,7 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
 
 // Persistent CTAs: each pulls the next half from the ticket list (longest bin first).
 template <bool TB>
-__global__ void __launch_bounds__(BK_THREADS, 1) ydrop_block_kernel(const YdParams p)
+__global__ void __launch_bounds__(BK_THREADS, 2) ydrop_block_kernel(const YdParams p)
 {
     __shared__ BkShared sh;
     __shared__ unsigned long long tk_s;
@@ -340,7 +364,7 @@ __global__ void __launch_bounds__(BK_THREADS, 1) ydrop_block_kernel(const YdPara
 
 int sfe_launch_ydrop_block(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st)
 {
-    long long blocks = p.n_tickets < n_sm ? p.n_tickets : n_sm;
+    long long blocks = p.n_tickets < 2LL * n_sm ? p.n_tickets : 2LL * n_sm;      // two CTAs of 8 warps per SM
     if (blocks < 1) blocks = 1;
     if (want_tb) ydrop_block_kernel<true><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
     else ydrop_block_kernel<false><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);

@@ -18,6 +18,9 @@
 #include "sfe_internal.cuh"
 #include "ydrop_common.cuh"
 
+#ifndef SFE_LONG_SKEW
+#define SFE_LONG_SKEW 2           // lane skew used for the reserved (longest) tickets; 1 = same as the others
+#endif
 #ifndef SFE_MIN_BLOCKS
 #define SFE_MIN_BLOCKS 3
 #endif
@@ -31,10 +34,10 @@
 // at a multiple of 16 and groups hold 16 steps, so lane 0 (reading column cs+t0+k+1) and lane 31
 // (writing column cs+t0+k-31) both touch row k&7 and segment base + (k>>3) with an EVEN base: no
 // ring wrap inside a group, every access of the unrolled loop is base + immediate.
-template <int RL2>
+template <int RL2, int SK>
 static __device__ __forceinline__ int bnd_off(int c)
 {
-    const int u = c - 1;
+    const int u = c - SK;
     return (u & 7) * RingGeom<RL2>::ROW_STRIDE + SFE_EXCH_BYTES + ((u >> 3) & (RingGeom<RL2>::RING / 8 - 1)) * 8;
 }
 
@@ -49,7 +52,7 @@ static __device__ __forceinline__ void fill_sel(uint16_t *selring, const HalfGeo
             const uint16_t v = (uint16_t)col_selector(g, c);
             const int idx = c & (G::SELRING - 1);
             selring[idx] = v;
-            if (idx < 16) selring[idx + G::SELRING] = v;
+            if (idx < 32) selring[idx + G::SELRING] = v;
         }
     } else {
         const long long ka = g.t0 + (long long)g.d * lo, kb = g.t0 + (long long)g.d * (hi - 1);
@@ -65,7 +68,7 @@ static __device__ __forceinline__ void fill_sel(uint16_t *selring, const HalfGeo
                     const uint16_t v = (uint16_t)(((mb >> e) & 1u) ? 0xCCC4u : 0x8880u + 0x1111u * code);
                     const int idx = c & (G::SELRING - 1);
                     selring[idx] = v;
-                    if (idx < 16) selring[idx + G::SELRING] = v;
+                    if (idx < 32) selring[idx + G::SELRING] = v;
                 }
             }
         }
@@ -74,10 +77,10 @@ static __device__ __forceinline__ void fill_sel(uint16_t *selring, const HalfGeo
 }
 
 // fill boundary-ring entries for columns [lo, hi) with "dead"
-template <int RL2>
+template <int RL2, int SK>
 static __device__ __forceinline__ void fill_bnd_neg(char *wbase, int lo, int hi, int lane)
 {
-    for (int c = lo + lane; c < hi; c += 32) *(int2 *)(wbase + bnd_off<RL2>(c)) = make_int2(SFE_NEG, SFE_NEG);
+    for (int c = lo + lane; c < hi; c += 32) *(int2 *)(wbase + bnd_off<RL2, SK>(c)) = make_int2(SFE_NEG, SFE_NEG);
     __syncwarp();
 }
 
@@ -139,8 +142,11 @@ static __device__ __forceinline__ uint32_t shift_in_sign(uint32_t acc, int x) { 
 // dead: bit 15-k set iff the cell of step k is dead.
 // The position of a new lane-local best (strict '>', R7) is found after the group, only by the
 // lanes whose best rose: the first k with H_k == best is the last strict increase.
-template <bool TB, bool EDGE, int RL2, bool GLOBAL>
-static __device__ __forceinline__ void run_group16(int &upH, int &upE, int &dg, int &F, int &Hgl, int &best, int &best_t,
+// SK = lane skew in columns.  SK = 1: lane l is one column behind lane l-1 (fewest idle steps per strip).
+// SK = 2: two columns behind, so the message loaded in step k is consumed in step k+2 and its LDS latency
+// leaves the per-step dependency chain: a shorter step for the halves whose serial chain bounds the run.
+template <bool TB, bool EDGE, int RL2, bool GLOBAL, int SK>
+static __device__ __forceinline__ void run_group16(int &upH, int &upE, int2 &pend, uint32_t &sel_nx, int &dg, int &F, int &Hgl, int &best, int &best_t,
                                                    uint32_t &acc0, uint32_t &acc1, uint32_t &dead, const uint32_t srow_lo,
                                                    const uint32_t srow_hi, const int T, const int OX, const int X,
                                                    const char *rptr, char *wptr, const uint16_t *selp, const int col0,
@@ -152,7 +158,8 @@ static __device__ __forceinline__ void run_group16(int &upH, int &upE, int &dg, 
 #pragma unroll
     for (int k = 0; k < 16; k++) {
         const int off = (k & 7) * G::ROW_STRIDE + (k >> 3) * 8;
-        const uint32_t sel = GLOBAL ? __ldcg(selp + k) : selp[k];
+        const uint32_t sel = sel_nx;                       // loaded a whole step ahead: off the critical path
+        sel_nx = GLOBAL ? __ldcg(selp + k + 1) : selp[k + 1];
         const int s = prmt_sx(srow_lo, srow_hi, sel);
         const int M = dg + s + OX;                         // dg = H(i-1,j-1) - OX, or NEG if dead
         const int E = __viaddmax_s32(upE, -X, upH);        // upH = H(i-1,j) - OX, or NEG if dead
@@ -180,7 +187,8 @@ static __device__ __forceinline__ void run_group16(int &upH, int &upE, int &dg, 
         dg = upH; F = Fn; Hgl = Hg;
         SFE_STEP_FENCE();
         const int2 u = GLOBAL ? __ldcg((const int2 *)(rptr + off)) : *(const int2 *)(rptr + off);
-        upH = u.x; upE = u.y;
+        if (SK == 1) { upH = u.x; upE = u.y; }             // the lane above is one column ahead: used in the next step
+        else { upH = pend.x; upE = pend.y; pend = u; }     // two columns ahead: used the step after next
     }
     if (best > best_in) {
         int kk = 15;
@@ -212,6 +220,7 @@ struct TbReader {                       // random access to this half's records;
 };
 
 // Returns false if the walk did not reach the origin (internal error guard).
+template <int SK>
 static __device__ bool walk_traceback(const YdParams &p, TbReader &rd, const int end_i, const int end_j, int hdr, int strip,
                                       char *wk, const int lane, uint32_t &ops_seg, int &n_ops, bool &ops_ok)
 {
@@ -237,7 +246,7 @@ static __device__ bool walk_traceback(const YdParams &p, TbReader &rd, const int
             win_hi = -1;
         }
         const int L = i & 31;
-        const int t = j - cs + L;                        // step of cell (i, j) in its strip
+        const int t = j - cs + SK * L;                   // step of cell (i, j) in its strip
         const int g = t >> 4;
         if (g > win_hi || g < win_lo) {                  // (re)load the window: groups g-7 .. g
             __syncwarp();
@@ -251,7 +260,7 @@ static __device__ bool walk_traceback(const YdParams &p, TbReader &rd, const int
         // lane k examines the k-th cell from (i, j) in the direction of the current state
         const int di = state == 2 ? 0 : 1, dj = state == 1 ? 0 : 1;
         const int Lk = L - lane * di;
-        const int tk = t - lane * (di + dj);
+        const int tk = t - lane * (SK * di + dj);
         const bool valid = Lk >= 0 && tk >= 0 && (tk >> 4) >= win_lo;
         uint32_t nib = 0;
         if (valid) nib = (win[((tk >> 4) - win_lo) * SFE_REC_WORDS + 2 * Lk + ((tk >> 3) & 1)] >> ((7 - (tk & 7)) * 4)) & 15u;
@@ -287,8 +296,10 @@ static __device__ bool walk_traceback(const YdParams &p, TbReader &rd, const int
     return true;
 }
 
-template <bool TB, int RL2, bool GLOBAL>
-static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, char *wk, const int lane)
+template <bool TB, int RL2, bool GLOBAL, int SK>
+// Returns false only when SK == 2 and a strip outgrew the shared-memory window (skew 2 needs 31 more steps per strip):
+// nothing has been published then, and the caller runs the half again with SK == 1.
+static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, char *wk, const int lane)
 {
     typedef RingGeom<RL2> G;
     uint16_t *selring = (uint16_t *)(wsm + 8 * G::ROW_STRIDE);
@@ -302,7 +313,7 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
     if (!half_setup(p, hid, g)) {
         out.status = SFE_ST_BAD_ANCHOR;
         if (lane == 0) p.halves[hid] = out;
-        return;
+        return true;
     }
 
     const int OX = p.OX, X = p.X;
@@ -315,7 +326,7 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
     unsigned long long cells = 0;
     int cs = 0, prevR = -1;
     int bnd_valid = 0;                         // boundary ring holds row (r0-1) for columns < bnd_valid
-    int sel_hi = -32;                          // selector ring is filled for columns < sel_hi
+    int sel_hi = -32 * SK;                     // selector ring is filled for columns < sel_hi (lane 31 starts at column -31 SK)
     int total_steps = 0, max_steps = 0, last_hdr = -1, n_strips = 0;
     bool wide = false;
 
@@ -347,13 +358,15 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
         }
         n_strips++;
 
-        if (sel_hi < cs - 32) sel_hi = cs - 32;
-        if (bnd_valid <= cs) { fill_bnd_neg<RL2>(wsm, bnd_valid, cs + 64, lane); bnd_valid = cs + 64; }
-        int refill_at = min(sel_hi, bnd_valid - 1);         // first cmax that needs a ring refill
+        if (sel_hi < cs - 32 * SK) sel_hi = cs - 32 * SK;
+        if (bnd_valid <= cs + SK - 1) { fill_bnd_neg<RL2, SK>(wsm, bnd_valid, cs + 64, lane); bnd_valid = cs + 64; }
+        int refill_at = min(sel_hi - 1, bnd_valid - SK);     // first cmax that needs a ring refill (the selector of column cmax+1 is prefetched)
         int upH = SFE_NEG, upE = SFE_NEG, dg = SFE_NEG, F = SFE_NEG, Hgl = SFE_NEG;
+        int2 pend = make_int2(SFE_NEG, SFE_NEG);
         if (lane == 0) {
-            const int2 u = GLOBAL ? __ldcg((const int2 *)(wsm + bnd_off<RL2>(cs))) : *(const int2 *)(wsm + bnd_off<RL2>(cs));
+            const int2 u = GLOBAL ? __ldcg((const int2 *)(wsm + bnd_off<RL2, SK>(cs))) : *(const int2 *)(wsm + bnd_off<RL2, SK>(cs));
             upH = u.x; upE = u.y;
+            if (SK == 2) pend = GLOBAL ? __ldcg((const int2 *)(wsm + bnd_off<RL2, SK>(cs + 1))) : *(const int2 *)(wsm + bnd_off<RL2, SK>(cs + 1));
             if (s == 0) dg = -OX;                           // R8: H(0,0) = 0 enters as the diagonal of (0,0)
         }
         // alive bits (step k of the group at bit 15-k) of the first / last group of my row that had an alive cell
@@ -367,30 +380,31 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
         // offset advances by 16 (two segments) per group.
         const bool is0 = lane == 0, is31 = lane == 31;
         char *const bnd = wsm + SFE_EXCH_BYTES;
-        const char *const rbase = is0 ? bnd : wsm + (lane - 1) * 8;
+        const char *const rbase = is0 ? bnd : wsm + (lane - 1) * 8;           // (exchange slots do not depend on the skew)
         char *const wbase = is31 ? bnd : wsm + lane * 8;
         const int rstride = is0 ? 16 : 0, wstride = is31 ? 16 : 0;
         int roff = is0 ? (cs & (G::RING - 1)) : 0;           // column cs+t0+k+1 -> segment (cs+t0)/8 + (k>>3)
-        int woff = is31 ? ((cs - 32) & (G::RING - 1)) : 0;   // column cs+t0+k-31 -> segment (cs+t0-32)/8 + (k>>3)
+        int woff = is31 ? ((cs - 32 * SK) & (G::RING - 1)) : 0;   // column cs+t0+k-31 SK -> segment (cs+t0-32 SK)/8 + (k>>3)
         for (;; t0 += 16) {
             const int cmax = cs + t0 + 15;                  // lane 0's last column of this group
             if (cmax >= refill_at) {
-                if (sel_hi <= cmax) { fill_sel<RL2>(selring, g, sel_hi, cmax + 129, lane); sel_hi = cmax + 129; }
-                if (bnd_valid <= cmax + 1) { fill_bnd_neg<RL2>(wsm, bnd_valid, bnd_valid + 64, lane); bnd_valid += 64; }
-                refill_at = min(sel_hi, bnd_valid - 1);
+                if (sel_hi <= cmax + 1) { fill_sel<RL2>(selring, g, sel_hi, cmax + 129, lane); sel_hi = cmax + 129; }
+                if (bnd_valid <= cmax + SK) { fill_bnd_neg<RL2, SK>(wsm, bnd_valid, bnd_valid + 64, lane); bnd_valid += 64; }
+                refill_at = min(sel_hi - 1, bnd_valid - SK);
             }
             const char *rptr = rbase + roff;
             char *wptr = wbase + woff;
             roff = (roff + rstride) & (G::RING - 1);
             woff = (woff + wstride) & (G::RING - 1);
-            const int col0 = cs + t0 - lane;
+            const int col0 = cs + t0 - SK * lane;
             const uint16_t *selp = selring + (col0 & (G::SELRING - 1));
+            uint32_t sel_nx = GLOBAL ? __ldcg(selp) : selp[0];
             uint32_t acc0 = 0, acc1 = 0, dead = 0;
             if (cmax > g.m)
-                run_group16<TB, true, RL2, GLOBAL>(upH, upE, dg, F, Hgl, best, best_t, acc0, acc1, dead, srow_lo, srow_hi, T, OX, X,
+                run_group16<TB, true, RL2, GLOBAL, SK>(upH, upE, pend, sel_nx, dg, F, Hgl, best, best_t, acc0, acc1, dead, srow_lo, srow_hi, T, OX, X,
                                                    rptr, wptr, selp, col0, g.m, t0);
             else
-                run_group16<TB, false, RL2, GLOBAL>(upH, upE, dg, F, Hgl, best, best_t, acc0, acc1, dead, srow_lo, srow_hi, T, OX, X,
+                run_group16<TB, false, RL2, GLOBAL, SK>(upH, upE, pend, sel_nx, dg, F, Hgl, best, best_t, acc0, acc1, dead, srow_lo, srow_hi, T, OX, X,
                                                     rptr, wptr, selp, col0, g.m, t0);
             if (TB) tb.put(acc0, acc1, lane);
             const uint32_t al = ~dead & 0xffffu;
@@ -399,19 +413,19 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
                 last_al = al; last_g = t0;
             }
             if (!__any_sync(FULL, al != 0) && cs + t0 + 16 > prevR + 1) { t0 += 16; break; }
-            if (t0 + 16 >= G::MAX_STEPS) { t0 += 16; bail = true; break; }
+            if (t0 + 16 >= G::MAX_STEPS - 16 * (SK - 1)) { t0 += 16; bail = true; break; }
         }
-        const int first = first_al ? cs - lane + first_g + __clz(first_al) - 16 : 0x7fffffff;
-        const int last = last_al ? cs - lane + last_g + 16 - __ffs(last_al) : -1;
+        const int first = first_al ? cs - SK * lane + first_g + __clz(first_al) - 16 : 0x7fffffff;
+        const int last = last_al ? cs - SK * lane + last_g + 16 - __ffs(last_al) : -1;
         total_steps += t0;
         if (t0 > max_steps) max_steps = t0;
         if (bail) { wide = true; break; }
         if (last >= 0) cells += (unsigned long long)(last - first + 1);
-        if (best > best_before) { best_i = r; best_j = cs + best_t - lane; }
+        if (best > best_before) { best_i = r; best_j = cs + best_t - SK * lane; }
         cumB = cumA; cumA = best;
         const int L31 = __shfl_sync(FULL, first, 31), R31 = __shfl_sync(FULL, last, 31);
         if (R31 < 0) break;                                 // last row of the strip has no alive cell
-        bnd_valid = cs + t0 - 31;                           // lane 31 wrote columns cs-31 .. cs+t0-32
+        bnd_valid = cs + t0 - 31 * SK;                      // lane 31 wrote columns cs-31 SK .. cs+t0-31 SK-1
         prevR = R31;
         cs = L31 & ~15;
     }
@@ -426,6 +440,10 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) cells += __shfl_xor_sync(FULL, cells, o);
+    if (SK == 2 && wide) {                                  // too wide for the skew-2 schedule: give the chunks back, try again with skew 1
+        if (TB) tb.release(lane);
+        return false;
+    }
     // every lane holds the same winner; the broadcast makes that visible to the compiler's uniformity
     // analysis, so that the walk below (and the next half after it) compiles as warp-uniform code
     bs = __shfl_sync(FULL, bs, 0); bi = __shfl_sync(FULL, bi, 0); bj = __shfl_sync(FULL, bj, 0);
@@ -440,7 +458,7 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
         rd.pool = p.pool; rd.chunk_prev = p.chunk_prev; rd.chunk = tb.cur_chunk; rd.ord = (tb.nrec - 1) / SFE_CHUNK_RECS;
         rd.last_chunk = rd.chunk; rd.last_ord = rd.ord; rd.nrec = tb.nrec; rd.bad = false;
         bool ops_ok = true;
-        if (!walk_traceback(p, rd, bi, bj, last_hdr, n_strips - 1, wk, lane, out.ops_seg, out.n_ops, ops_ok))
+        if (!walk_traceback<SK>(p, rd, bi, bj, last_hdr, n_strips - 1, wk, lane, out.ops_seg, out.n_ops, ops_ok))
             out.status |= SFE_ST_INTERNAL;
         if (!ops_ok) out.status |= SFE_ST_OPS_OVERFLOW;
     }
@@ -459,6 +477,7 @@ static __device__ void extend_half(const YdParams &p, const int hid, char *wsm, 
         if (TB && !tb.ok) atomicAdd(&p.counters[CNT_OVERFLOW], 1ULL);
         if (wide && !GLOBAL) atomicAdd(&p.counters[CNT_WIDE], 1ULL);
     }
+    return true;
 }
 
 // Persistent kernel: every warp pulls anchor-half tickets from one atomic counter (a3).
@@ -493,7 +512,10 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kerne
             if (lane == 0) tk = atomicAdd(cnt, 1ULL);
             tk = __shfl_sync(FULL, tk, 0);
             if (lo + (long long)tk >= hi) break;
-            extend_half<TB, SFE_RING_LOG2, false>(p, p.tickets[lo + tk], wsm, wsm, lane);
+            // the reserved (longest) tickets run with a lane skew of 2: a shorter dependent step, a few more idle steps
+            bool done = false;
+            if (phase == 0 && SFE_LONG_SKEW == 2) done = extend_half<TB, SFE_RING_LOG2, false, SFE_LONG_SKEW>(p, p.tickets[lo + tk], wsm, wsm, lane);
+            if (!done) extend_half<TB, SFE_RING_LOG2, false, 1>(p, p.tickets[lo + tk], wsm, wsm, lane);
             __syncwarp();
         }
     }
@@ -522,7 +544,7 @@ __global__ void __launch_bounds__(32) ydrop_wide_kernel(const YdParams p)
         if (lane == 0) tk = atomicAdd(&p.counters[CNT_WIDE_TICKET], 1ULL);
         tk = __shfl_sync(FULL, tk, 0);
         if ((long long)tk >= n) break;
-        extend_half<TB, SFE_WIDE_RING_LOG2, true>(p, p.wide_tickets[tk], wsm, wk, lane);
+        extend_half<TB, SFE_WIDE_RING_LOG2, true, 1>(p, p.wide_tickets[tk], wsm, wk, lane);
         __syncwarp();
     }
 }
