@@ -38,7 +38,9 @@ enum {
 };
 
 #define SFE_YDROP_INF 0x7fffffff      /* R27: no pruning                                        */
-#define SFE_PRUNE_LAG 32              /* R4: the row lag the systolic kernel implements exactly  */
+#define SFE_PRUNE_LAG 32              /* R4: the row lag the systolic kernel implements exactly; prune_lag = 0
+                                         (best so far in row-major order, the serial reading) is accepted
+                                         together with SFE_BLOCK_KERNEL                            */
 
 /* flags of sfe_ydrop_batch */
 #define SFE_WANT_CIGAR 1u             /* spill traceback pointers to HBM and emit CIGARs         */
@@ -69,7 +71,7 @@ typedef struct sfe_ctx sfe_ctx;       /* opaque: stream, scratch arenas, queue c
 /* Scoring (R1, R2, R5, R13, R16).  Supported range: every sub[][] entry and n_score in
  * [-128, 127] (the kernel keeps a query row's scores as packed int8), gap_open >= 0,
  * gap_extend >= 1, gap_open + gap_extend <= 65535, 0 <= ydrop < 2^28 or SFE_YDROP_INF,
- * prune_lag == SFE_PRUNE_LAG; anything else is SFE_ELIMIT / SFE_EINVAL. */
+ * prune_lag == SFE_PRUNE_LAG, or 0 with SFE_BLOCK_KERNEL; anything else is SFE_ELIMIT / SFE_EINVAL. */
 typedef struct {
     int32_t sub[4][4];                /* [query base][target base], A,C,G,T                      */
     int32_t n_score;                  /* any pair involving N                                    */

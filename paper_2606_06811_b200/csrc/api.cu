@@ -239,10 +239,11 @@ static int timed_ydrop(sfe_ctx *c, const YdParams &p, bool want_tb, uint32_t fla
     return SFE_OK;
 }
 
-static int check_scoring(const sfe_scoring *s)
+// prune_lag: 32 (every kernel) or 0 (exact serial-order pruning: the row-synchronous block kernel only)
+static int check_scoring(const sfe_scoring *s, uint32_t flags)
 {
     if (!s) return SFE_EINVAL;
-    if (s->prune_lag != SFE_PRUNE_LAG) return SFE_EINVAL;
+    if (s->prune_lag != SFE_PRUNE_LAG && !(s->prune_lag == 0 && (flags & SFE_BLOCK_KERNEL) && !(flags & SFE_NO_BLOCK_KERNEL))) return SFE_EINVAL;
     for (int a = 0; a < 4; a++)
         for (int b = 0; b < 4; b++)
             if (s->sub[a][b] < -128 || s->sub[a][b] > 127) return SFE_ELIMIT;
@@ -262,7 +263,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
                             int64_t *cigar_pool_used_dev, bool first_of_series)
 {
     if (!c || n_anchors < 0 || t_len < 0 || q_len < 0 || n_pairs < 0) return SFE_EINVAL;
-    int rc = check_scoring(sc);
+    int rc = check_scoring(sc, flags);
     if (rc) return rc;
     const bool want_tb = (flags & SFE_WANT_CIGAR) != 0;
     if (n_anchors > 0 && (!t_codes2 || !t_nmask || !q_codes2 || !q_nmask || !pairs_dev || !anchors_dev || !results_dev)) return SFE_EINVAL;
@@ -300,6 +301,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
     p.wide_ring = (char *)c->wide_ring.p; p.wide_tickets = (int32_t *)c->wide_tickets.p;
     p.ops_stage = (uint32_t *)c->ops_stage.p; p.ops_cap = ops_cap;
     p.OX = sc->gap_open + sc->gap_extend; p.X = sc->gap_extend;
+    p.lag0 = sc->prune_lag == 0;
     p.ydrop_inf = sc->ydrop == SFE_YDROP_INF; p.Y = p.ydrop_inf ? 0 : sc->ydrop;
     for (int a = 0; a < 4; a++) {
         uint32_t w = 0;
@@ -377,7 +379,7 @@ extern "C" int sfe_speculate(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t 
                              int64_t accepted_cap, int64_t *n_accepted_dev, sfe_stats *stats_dev)
 {
     if (!c || n_anchors < 0 || window_k < 1 || accepted_cap < 0) return SFE_EINVAL;
-    int rc = check_scoring(sc);
+    int rc = check_scoring(sc, flags);
     if (rc) return rc;
     if (n_anchors > 0 && (!anchors_dev || !results_dev || !keep_dev || !accepted_dev || !n_accepted_dev)) return SFE_EINVAL;
     SFE_CUDA_CHECK(cudaSetDevice(c->device));

@@ -100,6 +100,7 @@ struct YdParams {
     int32_t max_warps;            // warps of the normal kernel allowed to work in this pass
     int32_t n_pairs;
     int32_t OX, X, Y, ydrop_inf;
+    int32_t lag0;                 // prune_lag == 0 (R4, serial-order pruning): block kernel only
     uint32_t srow[5];             // packed int8 scores of a query base A,C,G,T,N against A,C,G,T
     uint32_t srow_hi;             // bytes: n_score, 0x00, 0xE0 (OOB), 0x00
     char *wide_ring;              // global-memory rings of the wide-band kernel: SFE_WIDE_WARPS x RingGeom<16>::WARP_BYTES

@@ -38,6 +38,7 @@
 #define BK_NINF (-(1 << 30) - (1 << 29)) // identity of the prefix maximum
 
 struct BkShared {
+    int tot2[32];                        // by window rank: warp maximum of H (Lambda = 0: running best inside the row)
     int tot[32], tex[32], tht[32];       // by window rank: warp total of a (inclusive), lane 31's exclusive prefix, lane 31's H~
     int edge[32];                        // by warp id: gated H - OX of lane 31 after the row (next row's diagonal)
     int wmax[32], wcol[32], wL[32], wR[32];
@@ -148,7 +149,7 @@ static __device__ bool block_walk(const YdParams &p, BkShared &sh, const int end
     return true;
 }
 
-template <bool TB>
+template <bool TB, bool LAG0>
 static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh)
 {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -190,7 +191,7 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
     for (int i = 0; i <= g.n; i++) {
         const uint32_t srow_lo = srow_nxt;
         if (i < g.n) srow_nxt = p.srow[sfe_base(g.qc, g.qm, g.q0 + (long long)g.d * (i + 1))];   // prefetched for the next row
-        const int T = p.ydrop_inf ? SFE_T_INF : (i >= 32 ? sh.cum[(i - 32) & 63] : 0) - p.Y;    // R4
+        const int T = p.ydrop_inf ? SFE_T_INF : (i >= 32 ? sh.cum[(i - 32) & 63] : 0) - p.Y;    // R4, Lambda = 32
         // ---- my columns in this row's window ----
         const int q = ((tid * BK_CPT) - ws) & (BK_WIN - 1);       // window position of my first column
         const int c0 = ws + q;
@@ -236,6 +237,7 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
         int Hprev = q == 0 ? SFE_NEG : max(lHt, q == 1 ? SFE_NEG : lpre - X * (q - 1));
         uint32_t nibs = 0;
         int hmax = SFE_NEG, hcol = 0x7fffffff, cl = 0x7fffffff, cr = -1;
+        int Hc[BK_CPT], ph[BK_CPT];
 #pragma unroll
         for (int k = 0; k < BK_CPT; k++) {
             const int pk = q + k;
@@ -243,13 +245,38 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
             const int F = pk == 0 ? SFE_NEG : pre - X * pk;
             int H = max(Ht[k], F);
             if (c0 + k > g.m) H = SFE_NEG;
-            const bool alive = H >= T;                    // R5
             if (TB) {
                 const int Hgl = pk == 0 ? SFE_NEG : Hprev - OX;
                 const uint32_t nib = ((M[k] < H) ? 8u : 0u) | ((E[k] < H) ? 4u : 0u) | ((Hu[k] < E[k]) ? 2u : 0u) | ((Hgl < F) ? 1u : 0u);
                 nibs |= nib << (4 * k);
             }
             Hprev = H;
+            Hc[k] = H;
+            ph[k] = k == 0 ? H : max(ph[k - 1], H);
+        }
+        // Lambda = 0 (R4, the serial reading): the threshold of (i, j) uses the best over alive cells that precede it in
+        // row-major order = max(best of rows < i, prefix maximum of H over the columns left of j): a cell that raises the
+        // best is alive by construction and a dead one lies below it, so the maximum may run over every computed H.
+        int pb0 = BK_NINF, Bprev = 0;
+        if (LAG0) {
+            const int incl2 = warp_scan_max(ph[BK_CPT - 1], lane);
+            int excl2 = __shfl_up_sync(FULL, incl2, 1);
+            if (lane == 0) excl2 = BK_NINF;
+            if (lane == 31) sh.tot2[rank] = incl2;
+            __syncthreads();                                                                  // B1b
+            const int t2 = lane < BK_WARPS ? sh.tot2[lane] : BK_NINF;
+            const int carry2 = __reduce_max_sync(FULL, lane < rank ? t2 : BK_NINF);
+            pb0 = max(excl2, carry2);
+            Bprev = i > 0 ? sh.cum[(i - 1) & 63] : 0;
+        }
+#pragma unroll
+        for (int k = 0; k < BK_CPT; k++) {
+            const int H = Hc[k];
+            bool alive;
+            if (LAG0) {
+                const int pb = k == 0 ? pb0 : max(pb0, ph[k - 1]);
+                alive = p.ydrop_inf ? H >= SFE_T_INF : H >= max(Bprev, pb) - p.Y;
+            } else alive = H >= T;                        // R5
             Hu[k] = alive ? H - OX : SFE_NEG;
             Eu[k] = E[k];
             if (alive) {
@@ -314,7 +341,7 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
     if (TB && cur_chunk >= 0 && tid == 0) p.pool[(size_t)cur_chunk * BK_CHUNK_WORDS] = (uint32_t)wpos;
 
     out.score = sh.best; out.end_i = sh.best_i; out.end_j = sh.best_j; out.cells = cells;
-    out.status = (wide ? SFE_ST_WIDE_PENDING : 0u) | ((TB && !tb_ok) ? SFE_ST_PASS_OVERFLOW : 0u) | SFE_ST_BLOCK;
+    out.status = (wide ? (LAG0 ? SFE_ST_BAND_LIMIT : SFE_ST_WIDE_PENDING) : 0u) | ((TB && !tb_ok) ? SFE_ST_PASS_OVERFLOW : 0u) | SFE_ST_BLOCK;
     out.n_strips = rows_done; out.n_rec = (int)(n_words >> 6); out.steps = rows_done; out.max_steps = max_width;
     // ---- a8: warp 0 walks the row log and stages the ops; then the chunks go back to the ring ----
     if (warp == 0) {
@@ -339,14 +366,14 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
             atomicAdd(&p.counters[CNT_STEPS], (unsigned long long)rows_done);
             if (TB) atomicAdd(&p.counters[CNT_TBBYTES], (unsigned long long)n_words * 4ULL);
             if (TB && !tb_ok) atomicAdd(&p.counters[CNT_OVERFLOW], 1ULL);
-            if (wide) atomicAdd(&p.counters[CNT_WIDE], 1ULL);
+            if (wide && !LAG0) atomicAdd(&p.counters[CNT_WIDE], 1ULL);
             atomicAdd(&p.counters[CNT_BLOCK_HALVES], 1ULL);
         }
     }
 }
 
 // Persistent CTAs: each pulls the next half from the ticket list (longest bin first).
-template <bool TB>
+template <bool TB, bool LAG0>
 __global__ void __launch_bounds__(BK_THREADS, 2) ydrop_block_kernel(const YdParams p)
 {
     __shared__ BkShared sh;
@@ -357,7 +384,7 @@ __global__ void __launch_bounds__(BK_THREADS, 2) ydrop_block_kernel(const YdPara
         const long long tk = (long long)tk_s;
         __syncthreads();
         if (tk >= p.n_tickets) break;
-        block_half<TB>(p, p.tickets[tk], sh);
+        block_half<TB, LAG0>(p, p.tickets[tk], sh);
         __syncthreads();
     }
 }
@@ -366,7 +393,12 @@ int sfe_launch_ydrop_block(const YdParams &p, bool want_tb, int n_sm, cudaStream
 {
     long long blocks = p.n_tickets < 2LL * n_sm ? p.n_tickets : 2LL * n_sm;      // two CTAs of 8 warps per SM
     if (blocks < 1) blocks = 1;
-    if (want_tb) ydrop_block_kernel<true><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
-    else ydrop_block_kernel<false><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
+    if (p.lag0) {
+        if (want_tb) ydrop_block_kernel<true, true><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
+        else ydrop_block_kernel<false, true><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
+    } else {
+        if (want_tb) ydrop_block_kernel<true, false><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
+        else ydrop_block_kernel<false, false><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
+    }
     SFE_LAUNCH_CHECK();
 }

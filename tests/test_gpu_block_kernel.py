@@ -107,3 +107,55 @@ def test_block_config1_full_equals_systolic(sfe, oracle):
     s = H.gpu_run(sfe, w, flags=B.SCORE_ONLY | B.BLOCK_KERNEL)
     for f in ("score", "tstart", "tend", "qstart", "qend", "cells"):
         assert (s["results"][f] == a["results"][f]).all()
+
+
+# ---- f1: exact serial-order pruning (R4 with Lambda = 0) on the GPU ---------------------------------------------------
+LAG0 = dict(prune_lag=0)
+
+
+def test_lag0_order_matters_examples(sfe, oracle):
+    """A10 / A11 and A4 / A5 give different alignments under different 'best so far' orders; the
+    block kernel at prune_lag = 0 reproduces the serial (row-major) reading: A10 -> 191 (2,2) 2M, A4 -> 100 (1,1) 1M."""
+    c = oracle.codes
+    w = _wl(c("AGTACTAAAGA"), c("AGCTAAAGA"), [(0, 0, 0, 1)])
+    out = H.gpu_run(sfe, w, flags=BLK, ydrop=455, **LAG0)
+    g = out["results"][0]
+    assert (int(g["score"]), int(g["tend"]), int(g["qend"]), int(g["cells"])) == (191, 2, 2, 19 + 1)   # + the empty backward half's origin cell
+    assert B.ops_list(out["cigar"], int(g["cigar_off"]), int(g["n_ops"])) == [(2, 0)]
+    H.assert_anchor_equal(out, w, 0, ydrop=455, **LAG0)
+    w = _wl(c("CGCC"), c("CCCC"), [(0, 0, 0, 1)])
+    out = H.gpu_run(sfe, w, flags=BLK, ydrop=120, **LAG0)
+    assert int(out["results"][0]["score"]) == 100 and int(out["results"][0]["tend"]) == 1
+    H.assert_anchor_equal(out, w, 0, ydrop=120, **LAG0)
+    # and prune_lag = 0 is refused without the block kernel
+    with pytest.raises(B.SfeError):
+        H.gpu_run(sfe, w, flags=B.WANT_CIGAR, ydrop=120, **LAG0)
+
+
+@pytest.mark.parametrize("ydrop", [120, 455, 1500, 9400])
+def test_lag0_small_ydrops(sfe, oracle, ydrop):
+    rng = np.random.default_rng(ydrop + 7)
+    T = rng.integers(0, 4, 900).astype(np.uint8)
+    mu = W.mutate(T, 0.08, 0.02, W.Stream(ydrop + 7))
+    Q = mu.seq.copy()
+    Q[100:104] = 4; T[300:302] = 4
+    picks = rng.integers(0, len(mu.t_idx), 24)
+    anchors = [(int(mu.t_idx[k]), int(mu.q_idx[k]), 0, 1) for k in picks] + [(0, 0, 0, 1), (len(T), len(Q), 0, 1), (5, 700, 0, 1)]
+    w = _wl(T, Q, anchors)
+    out = H.gpu_run(sfe, w, flags=BLK, ydrop=ydrop, **LAG0)
+    for i in range(len(anchors)):
+        H.assert_anchor_equal(out, w, i, ydrop=ydrop, **LAG0)
+
+
+def test_lag0_config2_small_and_fidelity(sfe, oracle):
+    """Divergent regime, both strands, at Lambda = 0: bit-exact vs the oracle at Lambda = 0, kept set == Algorithm 1 at
+    Lambda = 0; and the R4 fidelity report: how often Lambda = 32 (the systolic kernel) differs from Lambda = 0."""
+    w = W.config2(t_len=80_000, n_segments=40, per_seg=4, n_decoys=40, min_len=100, max_len=700)
+    out0 = H.gpu_run(sfe, w, flags=BLK, **LAG0)
+    for i in range(len(w.anchors)):
+        H.assert_anchor_equal(out0, w, i, **LAG0)
+    H.assert_resolve_equal(out0, w, **LAG0)
+    out32 = H.gpu_run(sfe, w)
+    same = sum(int(out0["results"][f][i]) == int(out32["results"][f][i]) for i in range(len(w.anchors)) for f in ("score", "tstart", "tend", "qstart", "qend"))
+    assert same >= 0.95 * 5 * len(w.anchors)                      # the two readings rarely differ (SURVEY 8(c) "Why Lambda")
+    assert int(out0["results"]["cells"].sum()) <= int(out32["results"]["cells"].sum())   # Lambda = 0 prunes earlier here
