@@ -134,6 +134,21 @@ def run_reference(args):
                       "e2e": {"value": v, "unit": "GCUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
+def aggregate_replicas(ms, cells, world, device):
+    """Replicas only: every rank runs the same single-GPU job; the job time is the MAX over ranks of the
+    device-timed region, the work is the SUM of the cells the ranks computed.  No data-path collective exists; these two
+    reductions of one float64 each are the whole multi-GPU path (tested with gloo, world size 2, in tests/test_replicas.py)."""
+    if world <= 1:
+        return float(ms), float(cells)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    c = torch.tensor([float(cells)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(c.item())
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -144,6 +159,8 @@ def main():
     ap.add_argument("--window", type=int, default=-1, help="Algorithm 3's K (sfe_speculate); 0 = one batch over all anchors; -1 = workload default")
     ap.add_argument("--kernel", default="auto", choices=["auto", "block", "systolic"],
                     help="block: the cooperative-warps kernel (one CTA per half) for every half; auto / systolic: one warp per half")
+    ap.add_argument("--fidelity", action="store_true",
+                    help="R4 fidelity report: one extra pass at prune_lag = 0 (serial-order pruning, block kernel) compared with the timed Lambda = 32 results")
     ap.add_argument("--sweep-k", default="", help="comma-separated K values: one extra timed pass each (PAPER.md:163, Fig. 3)")
     ap.add_argument("--flags", default="cigar", choices=["cigar", "score"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -239,12 +256,8 @@ def main():
     barrier()
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop()
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    tot_cells = torch.tensor([float(cells_step * args.steps)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX); dist.all_reduce(tot_cells, op=dist.ReduceOp.SUM)
-    ms = float(t.item())
-    gcups = float(tot_cells.item()) / (ms * 1e-3) / 1e9
+    ms, tot_cells = aggregate_replicas(ms, cells_step * args.steps, world, dev)
+    gcups = tot_cells / (ms * 1e-3) / 1e9
 
     # e2e: host buffers through the C ABI, H2D/D2H inside the timed region
     e2e = None
@@ -277,6 +290,28 @@ def main():
                       "waste_ext": 1.0 - (int(s2["n_kept"]) + int(s2["n_below"])) / max(1, int(s2["n_extended"])),
                       "waste_cells": float(s2["cells_covered"]) / max(1.0, float(s2["cells_total"])),
                       "kept_per_s": int(s2["n_kept"]) / (kms * 1e-3)})
+
+    # R4 fidelity: how often does the row-lagged threshold (Lambda = 32) change a result of Lambda = 0?
+    fidelity = None
+    if args.fidelity and window == 0:
+        step(); torch.cuda.synchronize(dev)
+        r32 = B.results_to_numpy(state["res"], n); k32 = state["keep"].cpu().numpy()[:n]
+        sc0 = B.scoring(prune_lag=0)
+        f0 = torch.cuda.Event(enable_timing=True); f1 = torch.cuda.Event(enable_timing=True)
+        tp = sfe.pack(t_ascii, with_rc=False); qp = sfe.pack(q_ascii, with_rc=True)
+        nacc.zero_(); stats.zero_()
+        f0.record()
+        res0, pool0, used0 = sfe.ydrop_batch(tp[:2], len(w.target), qp, len(w.query), pairs, len(w.pairs), anchors, n, sc0,
+                                             B.WANT_CIGAR | B.BLOCK_KERNEL, cigar_cap)
+        keep0 = sfe.resolve(anchors, res0, n, sc0.min_score, acc, n + 1, nacc, stats)
+        f1.record(); torch.cuda.synchronize(dev)
+        r0 = B.results_to_numpy(res0, n); k0 = keep0.cpu().numpy()[:n]
+        box = lambda r: np.stack([r["tstart"], r["tend"], r["qstart"], r["qend"]], 1)
+        fidelity = {"anchors": n, "ms_lag0_block_kernel": f0.elapsed_time(f1),
+                    "score_differs": int((r0["score"] != r32["score"]).sum()), "box_differs": int((box(r0) != box(r32)).any(1).sum()),
+                    "n_ops_differs": int((r0["n_ops"] != r32["n_ops"]).sum()), "keep_differs": int((k0 != k32).sum()),
+                    "kept_lag0": int((k0 == 1).sum()), "kept_lag32": int((k32 == 1).sum()),
+                    "cells_lag32_over_lag0": float(r32["cells"].sum()) / max(1.0, float(r0["cells"].sum()))}
 
     if rank != 0:
         if world > 1:
@@ -323,7 +358,7 @@ def main():
             "speculation_waste": {"ext": 1.0 - (kept_step + below_step) / ext_step if ext_step else None,
                                   "cells": cells_cov / cells_step if cells_step else None},
             "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roof, "cpu_baseline": cpu,
-            "batch_info": info0, "k_sweep": sweep or None}
+            "batch_info": info0, "k_sweep": sweep or None, "lag0_fidelity": fidelity}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
