@@ -134,7 +134,7 @@ static __device__ __forceinline__ uint32_t shift_in_sign(uint32_t acc, int x) { 
 
 // One group of 16 wavefront steps.  Everything indexed by k is an immediate after unrolling.
 // Per cell: LDS.U16 + PRMT (score), IADD3 (M), 2 x VIADDMNMX (E, F), VIMNMX3 (H), compare + select
-// (alive gate, R5/R6), 4 x (subtract + funnel shift) for the traceback nibble, VIMNMX (best), and
+// (alive gate, R5/R6), 4 x (subtract + funnel shift) for the traceback nibble, half a VIMNMX3 (best), and
 // the message STS.64 / LDS.64.  The kernel is issue-bound (profiles/r1_02), so what counts is the
 // number of instructions, not the pipe they run on; the subtractions stay on the FMA pipe (IMAD).
 // Traceback nibble of step k sits at bits 4(7-(k&7)).. of acc0 (k < 8) / acc1 (k >= 8):
@@ -177,11 +177,7 @@ static __device__ __forceinline__ void run_group16(int &upH, int &upE, int2 &pen
             acc = shift_in_sign(acc, fma_sub(Hgl, Fn));    // Hgl < F <=> F extended
         }
         if (isdead) dead |= 0x8000u >> k;
-#ifdef SFE_OPT_BEST3
-        if (k & 1) best = __vimax3_s32(best, Hk[k - 1], H);
-#else
-        best = max(best, H);
-#endif
+        if (k & 1) best = __vimax3_s32(best, Hk[k - 1], H); // one VIMNMX3 per two cells
         const int msgH = isdead ? SFE_NEG : Hg;            // dead cells send NEG on the diagonal / open edge
         *(int2 *)(wptr + off) = make_int2(msgH, E);
         dg = upH; F = Fn; Hgl = Hg;
