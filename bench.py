@@ -25,7 +25,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 SCRATCH_GB = {"c1": 2, "c2": 16, "c4": 24, "c3": 32, "c3s": 24, "c5s": 32, "c5": 48}   # traceback arena (chunks are recycled)
-DEFAULT_WINDOW = {"c3": 1024, "c3s": 1024, "c5s": 64, "c5": 64}   # Algorithm 3's K for the dense-anchor workloads; others: one batch
+DEFAULT_WINDOW = {"c3": 256, "c3s": 256, "c5s": 64, "c5": 64}   # Algorithm 3's K for the dense-anchor workloads; others: one batch
 
 
 def make_workload(name):
@@ -159,6 +159,9 @@ def main():
     ap.add_argument("--window", type=int, default=-1, help="Algorithm 3's K (sfe_speculate); 0 = one batch over all anchors; -1 = workload default")
     ap.add_argument("--kernel", default="auto", choices=["auto", "block", "systolic"],
                     help="block: the cooperative-warps kernel (one CTA per half) for every half; auto / systolic: one warp per half")
+    ap.add_argument("--cigar-for", default="auto", choices=["auto", "all", "kept"],
+                    help="windowed workloads: CIGARs for every extended anchor, or (SFE_CIGAR_KEPT_ONLY) score-only windows + one "
+                         "traceback batch over the kept anchors; auto = kept for windowed workloads")
     ap.add_argument("--fidelity", action="store_true",
                     help="R4 fidelity report: one extra pass at prune_lag = 0 (serial-order pruning, block kernel) compared with the timed Lambda = 32 results")
     ap.add_argument("--sweep-k", default="", help="comma-separated K values: one extra timed pass each (PAPER.md:163, Fig. 3)")
@@ -207,6 +210,9 @@ def main():
     state = {}
 
     window = DEFAULT_WINDOW.get(args.workload, 0) if args.window < 0 else args.window
+    kept_only = window > 0 and args.flags == "cigar" and args.cigar_for in ("auto", "kept")
+    if kept_only:
+        flags |= B.CIGAR_KEPT_ONLY
 
     def step(K=None):
         K = window if K is None else K
@@ -349,7 +355,7 @@ def main():
     line = {"metric": "ydrop_gcups", "value": gcups, "unit": "GCUPS", "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "window_k": window, "kernel": args.kernel,
+            "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "window_k": window, "kernel": args.kernel, "cigar_for": "kept" if kept_only else ("all" if args.flags == "cigar" else "none"),
                        "l2": "inputs+traceback per step exceed L2 (126 MB)",
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "scoring": "HOXD70/400/30/ydrop 9400/lag 32/tau 3000"},
             "kept_alignments_per_s": kept_step * args.steps * world / (ms * 1e-3),

@@ -49,6 +49,9 @@ enum {
 #define SFE_BLOCK_KERNEL 4u           /* every half on the cooperative-warps kernel (one CTA per half, rows in order,
                                          block-wide prefix maximum for F; same results)  */
 #define SFE_NO_BLOCK_KERNEL 8u        /* overrides SFE_BLOCK_KERNEL                               */
+#define SFE_CIGAR_KEPT_ONLY 16u       /* sfe_speculate with SFE_WANT_CIGAR: windows run score-only (the commit rule needs
+                                         score and box only); CIGARs are produced for the KEPT anchors in one
+                                         traceback batch at the end; other anchors get n_ops = 0, cigar_off = -1 */
 
 /* per-anchor status bits (sfe_result.status) */
 #define SFE_ST_TB_OVERFLOW 1u         /* traceback arena exhausted even when run alone: no CIGAR */

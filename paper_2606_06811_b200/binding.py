@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libsfe.so")
 OK, EINVAL, ENOMEM, ECUDA, ELIMIT = 0, -1, -2, -3, -4
 YDROP_INF = 0x7FFFFFFF
 PRUNE_LAG = 32
-WANT_CIGAR, SCORE_ONLY, NO_BINNING, BLOCK_KERNEL, NO_BLOCK_KERNEL = 1, 0, 2, 4, 8
+WANT_CIGAR, SCORE_ONLY, NO_BINNING, BLOCK_KERNEL, NO_BLOCK_KERNEL, CIGAR_KEPT_ONLY = 1, 0, 2, 4, 8, 16
 ST_TB_OVERFLOW, ST_CIGAR_OVERFLOW, ST_WIDE, ST_SCORE_LIMIT, ST_BAD_ANCHOR, ST_BAND_LIMIT, ST_INTERNAL, ST_SKIPPED = 1, 2, 4, 8, 16, 32, 64, 128
 OP_M, OP_I, OP_D = 0, 1, 2
 

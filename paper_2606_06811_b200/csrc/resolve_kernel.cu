@@ -357,6 +357,43 @@ __global__ void spec_finish_kernel(const SpecState *st, long long *n_accepted_io
     if (threadIdx.x == 0) *n_accepted_io = st->overflow ? -st->nacc : st->nacc;
 }
 
+// SFE_CIGAR_KEPT_ONLY: the kept anchors, in anchor order, for the final traceback batch (single warp), and the scatter back.
+__global__ void spec_gather_kept_kernel(const sfe_anchor *anchors, const uint8_t *keep, long long n, sfe_anchor *kept_anchors,
+                                        long long *kept_idx, long long *n_kept)
+{
+    const int lane = threadIdx.x & 31;
+    long long w = 0;
+    for (long long base = 0; base < n; base += 32) {
+        const long long i = base + lane;
+        const bool k = i < n && keep[i] == 1;
+        const unsigned m = __ballot_sync(FULL, k);
+        if (k) { const long long d = w + __popc(m & ((1u << lane) - 1)); kept_anchors[d] = anchors[i]; kept_idx[d] = i; }
+        w += __popc(m);
+    }
+    if (lane == 0) *n_kept = w;
+}
+
+__global__ void spec_scatter_kept_kernel(const sfe_result *kres, const long long *kept_idx, long long nk, sfe_result *results)
+{
+    const long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (k < nk) results[kept_idx[k]] = kres[k];
+}
+
+int sfe_launch_spec_gather_kept(const sfe_anchor *anchors, const uint8_t *keep, long long n, sfe_anchor *kept_anchors,
+                                long long *kept_idx, long long *n_kept, cudaStream_t st)
+{
+    spec_gather_kept_kernel<<<1, 32, 0, st>>>(anchors, keep, n, kept_anchors, kept_idx, n_kept);
+    SFE_LAUNCH_CHECK();
+}
+
+int sfe_launch_spec_scatter_kept(const sfe_result *kres, const long long *kept_idx, long long nk, sfe_result *results, cudaStream_t st)
+{
+    if (nk <= 0) return SFE_OK;
+    const int bs = 256;
+    spec_scatter_kept_kernel<<<(unsigned)((nk + bs - 1) / bs), bs, 0, st>>>(kres, kept_idx, nk, results);
+    SFE_LAUNCH_CHECK();
+}
+
 int sfe_launch_spec_prepare(const sfe_anchor *anchors, long long n, long long *blkmin, void *state, const sfe_box *accepted,
                             const long long *n_accepted, sfe_box *act, cudaStream_t st)
 {

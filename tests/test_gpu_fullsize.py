@@ -137,14 +137,14 @@ def test_config4_full(sfe_big, oracle):
         check_cigar(w, i, res[i], out["cigar"])
 
 
-def _speculate_full(sfe, w, K, cigar_cap):
+def _speculate_full(sfe, w, K, cigar_cap, flags=B.WANT_CIGAR | B.CIGAR_KEPT_ONLY):
     import torch
     dev = sfe.device
     tp = sfe.pack(torch.from_numpy(w.target_ascii().copy()).to(dev), with_rc=False)
     qp = sfe.pack(torch.from_numpy(w.query_ascii().copy()).to(dev), with_rc=True)
     n = len(w.anchors)
     o = sfe.speculate(tp[:2], len(w.target), qp, len(w.query), B._dev(B.make_pairs(w.pairs), dev), len(w.pairs),
-                      B._dev(B.make_anchors(w.anchors), dev), n, B.scoring(), K, B.WANT_CIGAR, cigar_cap)
+                      B._dev(B.make_anchors(w.anchors), dev), n, B.scoring(), K, flags, cigar_cap)
     torch.cuda.synchronize()
     return dict(results=B.results_to_numpy(o["results"], n), keep=o["keep"].cpu().numpy()[:n],
                 stats=o["stats"].cpu().numpy().view(B.STATS_DT)[0], n_accepted=int(o["n_accepted"].item()),
@@ -165,13 +165,16 @@ def _check_speculated(w, out, seed, n_sample):
         check_cigar(w, int(i), res[i], out["cigar"])
     ok = ~skipped & (bad == 0)
     for i in sample_indices(res, n, n_sample, seed, ok):
-        H.assert_anchor_equal(out, w, i)
+        # bench configuration (SFE_CIGAR_KEPT_ONLY): ops exist for the kept anchors; score / box / cells for every extended one
+        H.assert_anchor_equal(out, w, i, want_cigar=bool(keep[i] == 1))
+    assert (res["n_ops"][keep != 1] == 0).all()
 
 
 def test_config3_full_windowed(sfe_big, oracle):
-    """configs[2] (10 Mbp, 50,000 dense anchors, extensions of 10^4..10^5 rows) through sfe_speculate."""
+    """configs[2] (10 Mbp, 50,000 dense anchors, extensions of 10^4..10^5 rows) through sfe_speculate, as bench.py runs it:
+    K = 256, score-only windows, CIGARs for the kept anchors from one final traceback batch."""
     w = W.config3()
-    out = _speculate_full(sfe_big, w, 1024, 1 << 26)
+    out = _speculate_full(sfe_big, w, 256, 1 << 26)
     _check_speculated(w, out, 3, 24)
     assert int((out["keep"] == 0).sum()) > 0.9 * len(w.anchors)        # "most are subsumed under serial order"
 

@@ -290,3 +290,21 @@ def test_resolve_random_boxes(sfe, oracle, seed, n, spread):
     st = stats.cpu().numpy().view(B.STATS_DT)[0]
     assert (int(st["n_kept"]), int(st["n_covered"]), int(st["n_below"])) == (int((state == 1).sum()), int((state == 0).sum()), int((state == 2).sum()))
     assert int(st["cells_covered"]) == 7 * int((state == 0).sum())
+
+
+def test_speculate_cigar_for_kept_only(sfe, oracle):
+    """SFE_CIGAR_KEPT_ONLY: windows speculate score-only, the kept anchors get their CIGAR from one traceback batch at the
+    end.  Same kept set and the same score / box / cells for every extended anchor as the all-CIGAR run; kept anchors are
+    bit-exact against the oracle incl. the ops; everybody else carries no ops."""
+    w = W.config2(t_len=60_000, n_segments=30, per_seg=8, n_decoys=40, min_len=150, max_len=700)
+    full = _speculate(sfe, w, 32)
+    ko = _speculate(sfe, w, 32, flags=B.WANT_CIGAR | B.CIGAR_KEPT_ONLY)
+    assert ko["keep"].tolist() == full["keep"].tolist()
+    for f in ("score", "score_fwd", "score_bwd", "tstart", "tend", "qstart", "qend", "cells", "status"):
+        assert (ko["results"][f] == full["results"][f]).all(), f
+    kept = ko["keep"] == 1
+    assert (ko["results"]["n_ops"][~kept] == 0).all() and (ko["results"]["cigar_off"][~kept] == -1).all()
+    assert (ko["results"]["n_ops"][kept] == full["results"]["n_ops"][kept]).all()
+    assert ko["cigar_used"] == int(ko["results"]["n_ops"][kept].sum())
+    for i in np.nonzero(kept)[0]:
+        H.assert_anchor_equal(ko, w, int(i))
