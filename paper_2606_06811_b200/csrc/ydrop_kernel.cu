@@ -408,7 +408,13 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
                 if (!first_al) { first_al = al; first_g = t0; }
                 last_al = al; last_g = t0;
             }
-            if (!__any_sync(FULL, al != 0) && cs + t0 + 16 > prevR + 1) { t0 += 16; break; }
+            // End of the strip.  A cell needs an alive predecessor: left = my previous step, up / diagonal = the lane above
+            // SK / SK + 1 steps earlier (lane 0: the boundary row, dead beyond column prevR + 1).  So SK + 1 consecutive steps
+            // in which no lane has an alive cell, with lane 0 already past prevR + 1, prove that nothing can come alive any
+            // more -- no need to run a whole dead group to find out.  anyal: bit 15 - k = some lane alive in step k.
+            const uint32_t anyal = __reduce_or_sync(FULL, al);
+            const int tz = __ffs(anyal | 0x10000u) - 1;     // trailing all-dead steps of this group (0 .. 16)
+            if (tz >= SK + 1 && cs + t0 + 16 - (SK + 1) > prevR + 1) { t0 += 16; break; }
             if (t0 + 16 >= G::MAX_STEPS - 16 * (SK - 1)) { t0 += 16; bail = true; break; }
         }
         const int first = first_al ? cs - SK * lane + first_g + __clz(first_al) - 16 : 0x7fffffff;
