@@ -346,7 +346,7 @@ def main():
                        "R_unit": "lane-instr/clk/SM at sm_max_mhz", "n_sm": n_sm, "f_mhz_used": fmax,
                        "f_mhz_sampled": f_mhz, "peak_source": "measured by sfe_probe_int_issue in this run",
                        "tb_bytes_per_step": info0["tb_bytes"], "tb_gbs": info0["tb_bytes"] * args.steps / (kernel_us * 1e-6) / 1e9 if kernel_us else None,
-                       "lane_efficiency": cells_step / (32.0 * info0["steps"]) if info0["steps"] else None}}
+                       "lane_efficiency": cells_step / (32.0 * info0["steps"]) if info0["steps"] and window == 0 else None}}
 
     oc, osec, od = oracle_sample(w, args.cpu_seconds)
     cpu = {"value": oc / osec / 1e9, "unit": "GCUPS", "cores": 1, "kind": "oracle",
