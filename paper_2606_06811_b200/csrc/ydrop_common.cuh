@@ -5,6 +5,7 @@
 #include "sfe_internal.cuh"
 
 #define FULL 0xffffffffu
+#define SFE_SPIN_LIMIT (1 << 22)       // iterations a ring operation waits for its partner (normally a handful)
 
 // PRMT with the sign-replicate selector mode (bit 3 of a selector nibble), which __byte_perm masks off
 static __device__ __forceinline__ int prmt_sx(uint32_t lo, uint32_t hi, uint32_t sel)
@@ -71,10 +72,12 @@ static __device__ __forceinline__ int chunk_pop(int32_t *ring, SfeFreeRing *st, 
     if (a <= 0) return -1;
     volatile int32_t *slot = ring + (h % (unsigned long long)n_chunks);
     int id = -1;
-    do {
+    for (int spin = 0; spin < SFE_SPIN_LIMIT; spin++) {     // bounded: a hang must be impossible, whatever happened to the pusher
         if (lane == 0) id = *slot;
         id = __shfl_sync(FULL, id, 0);
-    } while (id < 0);
+        if (id >= 0) break;
+    }
+    if (id < 0) return -1;                                  // treated like an empty arena: score-only now, re-run later
     if (lane == 0) *slot = -1;
     return id;
 }
@@ -83,11 +86,13 @@ static __device__ __forceinline__ void chunk_push(int32_t *ring, SfeFreeRing *st
     unsigned long long t = 0;
     if (lane == 0) t = atomicAdd(&st->tail, 1ULL);
     int32_t *slot = ring + (t % (unsigned long long)n_chunks);
-    int old = -1;
-    do {                                                   // the pop that owns this slot may not have emptied it yet
+    int old = 0;
+    for (int spin = 0; spin < SFE_SPIN_LIMIT; spin++) {     // the pop that owns this slot may not have emptied it yet
         if (lane == 0) old = atomicCAS(slot, -1, id);
         old = __shfl_sync(FULL, old, 0);
-    } while (old != -1);
+        if (old == -1) break;
+    }
+    if (old != -1) return;                                  // give the chunk up (capacity leak) rather than wait for ever
     if (lane == 0) atomicAdd((unsigned long long *)&st->avail, 1ULL);
 }
 
