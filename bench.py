@@ -25,7 +25,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 SCRATCH_GB = {"c1": 2, "c2": 16, "c4": 24, "c3": 32, "c3s": 24, "c5s": 32, "c5": 48}   # traceback arena (chunks are recycled)
-DEFAULT_WINDOW = {"c3": 256, "c3s": 256, "c5s": 64, "c5": 64}   # Algorithm 3's K for the dense-anchor workloads; others: one batch
+DEFAULT_WINDOW = {"c3": 16384, "c3s": 16384, "c5s": 1024, "c5": 1024}   # Algorithm 3's K for the dense-anchor workloads; others: one batch
 
 
 def make_workload(name):

@@ -113,7 +113,7 @@ static __device__ bool block_walk(const YdParams &p, BkShared &sh, const int end
             const int pos = jx - sh.dir_c0[k];
             valid = pos >= 0 && pos < 8 * sh.dir_nw[k];
             if (valid) {
-                nib = (sh.walk[(sh.dir_base[k] - base0) + (pos >> 3)] >> (4 * (pos & 7))) & 15u;
+                nib = (sh.walk[(sh.dir_base[k] - base0) + (pos >> 3)] >> (16 * ((pos >> 2) & 1) + 4 * (3 - (pos & 3)))) & 15u;
             }
         }
         // nib: bit3 = H not from M, bit2 = H not from E, bit1 = E extended, bit0 = F extended (R11)
@@ -186,11 +186,14 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
     unsigned long long cells = 0;
     int rows_done = 0, max_width = 0;
     bool wide = false;
-    uint32_t srow_nxt = 0u;                               // row 0: every substitution score is 0 (R8: H(0,0) = 0 enters as M)
+    uint32_t srow32 = 0u;                                 // lane l: packed scores of query row (i & ~31) + l (row 0: all 0, R8)
 
     for (int i = 0; i <= g.n; i++) {
-        const uint32_t srow_lo = srow_nxt;
-        if (i < g.n) srow_nxt = p.srow[sfe_base(g.qc, g.qm, g.q0 + (long long)g.d * (i + 1))];   // prefetched for the next row
+        if ((i & 31) == 0) {                              // one load per lane per 32 rows instead of one per thread per row
+            const int r = i + lane;
+            srow32 = (r == 0 || r > g.n) ? 0u : p.srow[sfe_base(g.qc, g.qm, g.q0 + (long long)g.d * r)];
+        }
+        const uint32_t srow_lo = __shfl_sync(FULL, srow32, i & 31);
         const int T = p.ydrop_inf ? SFE_T_INF : (i >= 32 ? sh.cum[(i - 32) & 63] : 0) - p.Y;    // R4, Lambda = 32
         // ---- my columns in this row's window ----
         const int q = ((tid * BK_CPT) - ws) & (BK_WIN - 1);       // window position of my first column
@@ -213,8 +216,7 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
             const int s = prmt_sx(srow_lo, srow_hi, sel[k]);
             M[k] = Hd + s + OX;
             E[k] = __viaddmax_s32(Eu[k], -X, Hu[k]);
-            Ht[k] = max(M[k], E[k]);
-            if (c0 + k > g.m) Ht[k] = SFE_NEG;
+            Ht[k] = max(M[k], E[k]);                      // (columns beyond m: overridden on H below; their H~ only feeds columns further right)
             const int a = Ht[k] - OX + X * (q + k + 1);   // a_p = H~ - O + X p
             pa[k] = k == 0 ? a : max(pa[k - 1], a);
         }
@@ -234,7 +236,7 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
         // final H of the column left of my first one (for "F extended", R11)
         int lpre = max(lpre_in, carry);
         if (lane == 0 && rank > 0) { lHt = sh.tht[rank - 1]; lpre = max(sh.tex[rank - 1], carry_prev); }
-        int Hprev = q == 0 ? SFE_NEG : max(lHt, q == 1 ? SFE_NEG : lpre - X * (q - 1));
+        int Hprev = q == 0 ? SFE_NEG : max(lHt, lpre - X * (q - 1));   // (q == 1: lpre = BK_NINF)
         uint32_t nibs = 0;
         int hmax = SFE_NEG, hcol = 0x7fffffff, cl = 0x7fffffff, cr = -1;
         int Hc[BK_CPT], ph[BK_CPT];
@@ -242,13 +244,15 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
         for (int k = 0; k < BK_CPT; k++) {
             const int pk = q + k;
             const int pre = k == 0 ? pre0 : max(pre0, pa[k - 1]);
-            const int F = pk == 0 ? SFE_NEG : pre - X * pk;
+            const int F = pre - X * pk;                   // window position 0: pre = BK_NINF (nothing to its left)
             int H = max(Ht[k], F);
             if (c0 + k > g.m) H = SFE_NEG;
-            if (TB) {
-                const int Hgl = pk == 0 ? SFE_NEG : Hprev - OX;
-                const uint32_t nib = ((M[k] < H) ? 8u : 0u) | ((E[k] < H) ? 4u : 0u) | ((Hu[k] < E[k]) ? 2u : 0u) | ((Hgl < F) ? 1u : 0u);
-                nibs |= nib << (4 * k);
+            if (TB) {                                     // sign bits shifted in, newest nibble lowest: column k ends at bits 4(3-k)..
+                const int Hgl = Hprev - OX;
+                nibs = __funnelshift_l((uint32_t)(M[k] - H), nibs, 1);
+                nibs = __funnelshift_l((uint32_t)(E[k] - H), nibs, 1);
+                nibs = __funnelshift_l((uint32_t)(Hu[k] - E[k]), nibs, 1);
+                nibs = __funnelshift_l((uint32_t)(Hgl - F), nibs, 1);
             }
             Hprev = H;
             Hc[k] = H;

@@ -172,15 +172,15 @@ def _check_speculated(w, out, seed, n_sample):
 
 def test_config3_full_windowed(sfe_big, oracle):
     """configs[2] (10 Mbp, 50,000 dense anchors, extensions of 10^4..10^5 rows) through sfe_speculate, as bench.py runs it:
-    K = 256, score-only windows, CIGARs for the kept anchors from one final traceback batch."""
+    K = 16384, score-only windows, CIGARs for the kept anchors from one final traceback batch."""
     w = W.config3()
-    out = _speculate_full(sfe_big, w, 256, 1 << 26)
+    out = _speculate_full(sfe_big, w, 16384, 1 << 26)
     _check_speculated(w, out, 3, 24)
     assert int((out["keep"] == 0).sum()) > 0.9 * len(w.anchors)        # "most are subsumed under serial order"
 
 
 def test_config5_scaled_windowed(sfe_big, oracle):
-    """configs[4] at 1/10 scale (10 Mbp with N runs and segmental duplications, 100,000 anchors), K = 64."""
+    """configs[4] at 1/10 scale (10 Mbp with N runs and segmental duplications, 100,000 anchors), K = 1024 as bench.py."""
     w = W.config5(t_len=10_000_000, n_anchors=100_000)
-    out = _speculate_full(sfe_big, w, 64, 1 << 26)
+    out = _speculate_full(sfe_big, w, 1024, 1 << 26)
     _check_speculated(w, out, 5, 24)
