@@ -7,8 +7,8 @@ The oracle cannot run 10^10..10^12 cells, so at full size the CUDA path is check
       against the sequences with the R12 rule, reproduces the reported score and consumes exactly
       the box; the keep flags satisfy the in-order containment rule (R17/R18) given the reported
       boxes; the counters add up.
-C1 is covered in full by test_gpu_parity.py.  C5 runs at 1/10 scale (10 Mbp, 100,000 anchors: SURVEY 8(d)
-allows the prefix-scale run; the full 1 M anchors take minutes per pass)."""
+C1 is covered in full by test_gpu_parity.py.  C5 runs at 1/10 scale and at full size (100 Mbp, 1,000,000 anchors;
+~90 s of GPU time per pass)."""
 import numpy as np
 import pytest
 
@@ -184,3 +184,12 @@ def test_config5_scaled_windowed(sfe_big, oracle):
     w = W.config5(t_len=10_000_000, n_anchors=100_000)
     out = _speculate_full(sfe_big, w, 1024, 1 << 26)
     _check_speculated(w, out, 5, 24)
+
+
+def test_config5_full_windowed(sfe_big, oracle):
+    """configs[4] at FULL size (100 Mbp, 1,000,000 anchors, N runs, segmental duplications, decoys), K = 1024 as bench.py:
+    resolve rule over all anchors, every kept CIGAR rescored, a sample + the largest extensions against the oracle."""
+    w = W.config5()
+    out = _speculate_full(sfe_big, w, 1024, 1 << 27)
+    _check_speculated(w, out, 55, 16)
+    assert int((out["keep"] == 1).sum()) > 1000
