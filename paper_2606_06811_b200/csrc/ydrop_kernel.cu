@@ -108,9 +108,7 @@ struct TbWriter {
     {
         // One fence per half: this warp's record stores must have landed before a chunk changes owner.
         // (A gpu-scope fence also invalidates the SM's L1, so it is not done per chunk.)
-#ifndef SFE_DBG_NOFENCE
         __threadfence();
-#endif
         __syncwarp();
         int c = cur_chunk;
         while (c >= 0) {
