@@ -87,3 +87,23 @@ def test_workload_generators():
     assert (np.diff(mu.t_idx) > 0).all() and (np.diff(mu.q_idx) > 0).all()
     ident = (src[mu.t_idx] == mu.seq[mu.q_idx]).mean()
     assert 0.86 < ident < 0.94
+
+
+def test_binding_constants_match_header():
+    """Flags, status bits, op codes and error codes of the Python binding are the header's #defines / enum values."""
+    src = open(os.path.join(ROOT, "include", "sfe.h")).read()
+    defs = {m.group(1): int(m.group(2), 0) for m in re.finditer(r"#define\s+(SFE_[A-Z_0-9]+)\s+(0x[0-9a-fA-F]+|\d+)u?\b", src)}
+    enum = {m.group(1): int(m.group(2)) for m in re.finditer(r"\b(SFE_E?[A-Z]+)\s*=\s*(-?\d+)", src)}
+    pairs = {"SFE_WANT_CIGAR": B.WANT_CIGAR, "SFE_SCORE_ONLY": B.SCORE_ONLY, "SFE_NO_BINNING": B.NO_BINNING,
+             "SFE_BLOCK_KERNEL": B.BLOCK_KERNEL, "SFE_NO_BLOCK_KERNEL": B.NO_BLOCK_KERNEL, "SFE_CIGAR_KEPT_ONLY": B.CIGAR_KEPT_ONLY,
+             "SFE_ST_TB_OVERFLOW": B.ST_TB_OVERFLOW, "SFE_ST_CIGAR_OVERFLOW": B.ST_CIGAR_OVERFLOW, "SFE_ST_WIDE": B.ST_WIDE,
+             "SFE_ST_SCORE_LIMIT": B.ST_SCORE_LIMIT, "SFE_ST_BAD_ANCHOR": B.ST_BAD_ANCHOR, "SFE_ST_BAND_LIMIT": B.ST_BAND_LIMIT,
+             "SFE_ST_INTERNAL": B.ST_INTERNAL, "SFE_ST_SKIPPED": B.ST_SKIPPED, "SFE_OP_M": B.OP_M, "SFE_OP_I": B.OP_I,
+             "SFE_OP_D": B.OP_D, "SFE_YDROP_INF": B.YDROP_INF, "SFE_PRUNE_LAG": B.PRUNE_LAG}
+    for name, val in pairs.items():
+        assert defs[name] == val, name
+    for name, val in {"SFE_OK": B.OK, "SFE_EINVAL": B.EINVAL, "SFE_ENOMEM": B.ENOMEM, "SFE_ECUDA": B.ECUDA, "SFE_ELIMIT": B.ELIMIT}.items():
+        assert enum[name] == val, name
+    # status bits are distinct single bits
+    st = [v for k, v in defs.items() if k.startswith("SFE_ST_")]
+    assert len(set(st)) == len(st) and all(v & (v - 1) == 0 for v in st)
