@@ -325,7 +325,8 @@ def main():
         return
 
     # roofline of the dominant kernel (integer issue)
-    hl = sassinfo.hot_loop(traceback=bool(flags & B.WANT_CIGAR))
+    tb_loop = bool(flags & B.WANT_CIGAR) and not kept_only       # kept-only windows run the score-only loop
+    hl = sassinfo.hot_loop(traceback=tb_loop)
     r_alu, _ = sfe.probe_int_issue(1, 20000); r_dpx, _ = sfe.probe_int_issue(2, 20000)
     r_fma, _ = sfe.probe_int_issue(3, 20000); r_mix, _ = sfe.probe_int_issue(0, 20000)
     f_mhz = clocks.get("sm_mhz") or 1965.0
@@ -339,7 +340,7 @@ def main():
     peak_gcups = n_sm * fmax * 1e6 / cyc_per_cell / 1e9
     k_gcups = cells_step * args.steps / (kernel_us * 1e-6) / 1e9 if kernel_us > 0 else None
     roof = {"bound": "alu", "achieved": k_gcups, "peak": peak_gcups, "unit": "GCUPS", "frac": (k_gcups / peak_gcups) if k_gcups else None,
-            "traffic": None, "kernel": "ydrop_kernel<%s>" % ("traceback" if flags & B.WANT_CIGAR else "score-only"),
+            "traffic": None, "kernel": "ydrop_kernel<%s>" % ("traceback" if tb_loop else "score-only"),
             "kernel_share_of_step": kernel_us * 1e-3 / ms,
             "detail": {"instr_per_cell_sass": hl["per_cell"], "alu_per_cell": hl["alu"], "dpx_per_cell": hl["dpx"], "fma_per_cell": hl["fma"],
                        "lsu_per_cell": hl["lsu"], "R_alu": r_alu, "R_dpx": r_dpx, "R_imad": r_fma, "R_mixed": r_mix,
