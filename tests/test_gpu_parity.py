@@ -308,3 +308,48 @@ def test_speculate_cigar_for_kept_only(sfe, oracle):
     assert ko["cigar_used"] == int(ko["results"]["n_ops"][kept].sum())
     for i in np.nonzero(kept)[0]:
         H.assert_anchor_equal(ko, w, int(i))
+
+
+def test_degenerate_calls(sfe, oracle):
+    """Boundary behaviour of the C ABI: zero anchors, anchors outside their pair / with an unknown pair / on the - strand
+    without reverse-complement planes (SFE_ST_BAD_ANCHOR, nothing computed, no fault), invalid arguments (error codes)."""
+    import ctypes as C
+    import torch
+    dev = sfe.device
+    L = B.lib()
+    T = W.randseq(3, 500); Q = T.copy()
+    w = _wl(T, Q, [(10, 10, 0, 1)])
+    tp = sfe.pack(torch.from_numpy(w.target_ascii().copy()).to(dev), with_rc=False)
+    qp = sfe.pack(torch.from_numpy(w.query_ascii().copy()).to(dev), with_rc=True)
+    pairs = B._dev(B.make_pairs(np.array([[0, 500, 0, 500], [100, 200, 100, 200]], np.int64)), dev)
+    sc = B.scoring()
+    # zero anchors: every entry point returns OK and touches nothing
+    res, pool, used = sfe.ydrop_batch(tp[:2], 500, qp, 500, pairs, 2, None, 0, sc)
+    keep = sfe.resolve(None, None, 0, 3000, None, 0, None)
+    o = sfe.speculate(tp[:2], 500, qp, 500, pairs, 2, None, 0, sc, 8)
+    torch.cuda.synchronize()
+    assert int(used.item()) == 0
+    # bad anchors next to a good one
+    A = np.array([(10, 10, 0, 1), (600, 10, 0, 1), (10, 10, 7, 1), (50, 50, 1, 1), (150, 150, 1, 1), (-1, 5, 0, 1)], np.int64)
+    res, pool, used = sfe.ydrop_batch(tp[:2], 500, qp, 500, pairs, 2, B._dev(B.make_anchors(A), dev), len(A), sc)
+    torch.cuda.synchronize()
+    r = B.results_to_numpy(res, len(A))
+    bad = (r["status"] & B.ST_BAD_ANCHOR) != 0
+    assert bad.tolist() == [False, True, True, True, False, True]
+    assert (r["score"][bad] == 0).all() and (r["n_ops"][bad] == 0).all() and (r["cells"][bad] == 0).all()
+    assert int(r["score"][0]) == oracle.extend_anchor(T, Q, 10, 10, oracle.scoring())[0].score
+    assert int(r["score"][4]) == oracle.extend_anchor(T, Q, 150, 150, oracle.scoring(), t_lim=(100, 200), q_lim=(100, 200))[0].score
+    # - strand anchors without reverse-complement planes
+    Am = np.array([(10, 10, 0, -1)], np.int64)
+    res, pool, used = sfe.ydrop_batch(tp[:2], 500, qp[:2], 500, pairs, 2, B._dev(B.make_anchors(Am), dev), 1, sc)
+    torch.cuda.synchronize()
+    assert int(B.results_to_numpy(res, 1)["status"][0]) & B.ST_BAD_ANCHOR
+    # invalid arguments are refused with error codes, not faults
+    assert L.sfe_ydrop_batch(sfe.h, None, None, 500, None, None, None, None, 500, None, 2, None, 5, C.byref(sc), 1, None, None, 0, None) == B.EINVAL
+    bad_sc = B.scoring(prune_lag=7)
+    with pytest.raises(B.SfeError):
+        sfe.ydrop_batch(tp[:2], 500, qp, 500, pairs, 2, B._dev(B.make_anchors(A), dev), len(A), bad_sc)
+    with pytest.raises(B.SfeError):
+        sfe.ydrop_batch(tp[:2], 500, qp, 500, pairs, 2, B._dev(B.make_anchors(A), dev), len(A), B.scoring(gap_extend=0))
+    with pytest.raises(B.SfeError):
+        sfe.speculate(tp[:2], 500, qp, 500, pairs, 2, B._dev(B.make_anchors(A), dev), len(A), sc, 0)
