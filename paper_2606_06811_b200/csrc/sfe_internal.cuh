@@ -14,11 +14,12 @@
 #define SFE_OOB_SCORE 0xE0000000u       // substitution "score" of a column beyond the target end (-2^29)
 
 // ---- shared-memory geometry of one warp -------------------------
-// A strip is 32 consecutive DP rows, one per lane, swept left to right; lane l is one column
+// A strip is 32 consecutive DP rows, one per lane, swept left to right; lane l is SK (1 or 2) columns
 // behind lane l-1.  Messages (H-(O+X) gated by alive, E) travel lane l -> l+1 through a tiny
 // exchange area; the last lane's messages go to the boundary ring that lane 0 of the NEXT strip
-// reads.  Everything is laid out in 8 "rows", one per step of an unrolled group of 8 steps, so
-// that every access in the unrolled loop is base + immediate.
+// reads.  Everything is laid out in 8 "rows"; step k of an unrolled group of 16 steps uses row k & 7
+// (and, in the ring, segment base + (k >> 3)), so that every access in the unrolled loop is
+// base + immediate.
 // The ring capacity is a template parameter: 2^10 columns in shared memory for the normal kernel,
 // 2^16 columns in global memory (L2) for the wide-band kernel that re-runs the rare halves whose
 // strip exceeds the shared-memory window.

@@ -1,19 +1,21 @@
-// ydrop_kernel.cu -- the warp-systolic Y-drop gapped extension (SURVEY 8(a) a3-a7).
+// ydrop_kernel.cu -- the warp-systolic Y-drop gapped extension (SURVEY 8(a) a3-a8).
 //
 // One warp = one one-sided extension ("anchor-half").  The paper's kernel
 // (Fig. 8) gives each thread one line of the DP matrix and passes neighbour values
 // between threads; this kernel keeps that systolic idea but is organised for sm_100a:
 //   * rows are processed in strips of 32 (lane l owns row 32 s + l), each lane sweeping its row
-//     left to right one column behind the lane above, so that 32 lanes stay busy whatever the
-//     width of the live band is (the band is 0..~700 columns wide and changes every row);
+//     left to right SK columns behind the lane above (SK = 1, or 2 for the longest tickets), so that
+//     32 lanes stay busy whatever the width of the live band is (0..~700 columns, changing every row);
 //   * per cell: PRMT score lookup from a packed int8 row, IADD3, two VIADDMNMX (E, F), one
 //     VIMNMX3 (H) -- the Blackwell DPX instructions -- plus compare/select for the Y-drop prune;
 //   * lane-to-lane messages and the strip-to-strip boundary row go through a 10 KiB per-warp
-//     shared-memory area laid out so that every access of the 8x unrolled loop is base+immediate;
-//   * 4 traceback bits per cell are packed 8 cells to a word and written as one coalesced 128 B
-//     record per warp per 8 steps into the HBM arena (R11);
+//     shared-memory area laid out so that every access of the 16x unrolled loop is base+immediate;
+//   * 4 traceback bits per cell are packed 8 cells to a word and written as one coalesced 256 B
+//     record per warp per 16 steps into the recycled HBM arena (R11);
 //   * rows are pruned with the row-lagged threshold T(r) = best(rows <= r - 32) - ydrop (R4),
-//     which is exactly what is final when row r starts in this schedule.
+//     which is exactly what is final when row r starts in this schedule;
+//   * when the half is done the same warp walks its traceback (walk_traceback: 32 path cells per
+//     ballot), stages the run-length ops and gives its chunks back to the free ring (a8).
 // Dead cells are gated only on the diagonal/open edge (R6 lemma).
 #include "sfe_internal.cuh"
 #include "ydrop_common.cuh"
