@@ -25,6 +25,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 SCRATCH_GB = {"c1": 2, "c2": 16, "c4": 24, "c3": 32, "c3s": 24, "c5s": 32, "c5": 48}   # traceback arena (chunks are recycled)
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE ydrop_kernel<traceback> launch, from an `ncu --set full` capture of the
+# default run (profiles/r1_04_final_round1.md, "full C2 launch"): 0.768 GB read + 15.376 GB written.  Algorithmic bytes of
+# the same launch = the traceback records, `roofline.detail.tb_bytes_per_step` (15.8 GB): no wasted re-reads.
+NCU_TRAFFIC_BYTES = {("c2", "cigar", 0, "auto"): 16_144_609_424}
 DEFAULT_WINDOW = {"c3": 16384, "c3s": 16384, "c5s": 1024, "c5": 1024}   # Algorithm 3's K for the dense-anchor workloads; others: one batch
 
 
@@ -340,7 +344,7 @@ def main():
     peak_gcups = n_sm * fmax * 1e6 / cyc_per_cell / 1e9
     k_gcups = cells_step * args.steps / (kernel_us * 1e-6) / 1e9 if kernel_us > 0 else None
     roof = {"bound": "alu", "achieved": k_gcups, "peak": peak_gcups, "unit": "GCUPS", "frac": (k_gcups / peak_gcups) if k_gcups else None,
-            "traffic": None, "kernel": "ydrop_kernel<%s>" % ("traceback" if tb_loop else "score-only"),
+            "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.flags, window, args.kernel)) if not args.limit_anchors else None, "kernel": "ydrop_kernel<%s>" % ("traceback" if tb_loop else "score-only"),
             "kernel_share_of_step": kernel_us * 1e-3 / ms,
             "detail": {"instr_per_cell_sass": hl["per_cell"], "alu_per_cell": hl["alu"], "dpx_per_cell": hl["dpx"], "fma_per_cell": hl["fma"],
                        "lsu_per_cell": hl["lsu"], "R_alu": r_alu, "R_dpx": r_dpx, "R_imad": r_fma, "R_mixed": r_mix,
