@@ -37,17 +37,24 @@ static __device__ __forceinline__ bool box_has(const sfe_box &b, long long t, lo
 // parallel.  Rounds <= kept reaching candidates (none for disjoint boxes such as C4's); the non-reaching
 // candidates are kept iff nothing covered them.  Returns the kept mask; cov is updated for every live lane
 // (candidate or below tau: R17 is tested before R16).
-static __device__ unsigned decide_block(bool live, bool cand, bool &cov, const sfe_box &mine, long long tp, long long qp, int strand,
+static __device__ unsigned decide_block(bool valid, bool live, bool cand, bool &cov, const sfe_box &mine, long long tp, long long qp, int strand,
                                         int lane)
 {
     __shared__ sfe_box sb[32];
     __syncwarp();
     sb[lane] = mine;
-    long long suf = live ? tp : 0x7fffffffffffffffLL;             // inclusive suffix minimum of tpos over live lanes
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const long long y = __shfl_down_sync(FULL, suf, o); if (lane + o < 32 && y < suf) suf = y; }
-    long long after = __shfl_down_sync(FULL, suf, 1);
+    // `after` = a lower bound of the tpos of every later live lane.  Sorted block (the normal case): the next lane's tpos;
+    // otherwise the exact suffix minimum over live lanes.  (A smaller bound only adds rounds, never changes a decision.)
+    const long long tpv = valid ? tp : 0x7fffffffffffffffLL;      // (covered lanes count too: still a lower bound)
+    long long after = __shfl_down_sync(FULL, tpv, 1);
     if (lane == 31) after = 0x7fffffffffffffffLL;
+    if (!__all_sync(FULL, after >= tpv)) {                        // not sorted: the block's anchors are not in position order
+        long long suf = live ? tp : 0x7fffffffffffffffLL;         // inclusive suffix minimum of tpos over live lanes
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const long long y = __shfl_down_sync(FULL, suf, o); if (lane + o < 32 && y < suf) suf = y; }
+        after = __shfl_down_sync(FULL, suf, 1);
+        if (lane == 31) after = 0x7fffffffffffffffLL;
+    }
     const unsigned reach = __ballot_sync(FULL, cand && mine.tend >= after);
     unsigned covm = 0;
     for (unsigned m = reach; m; m &= m - 1) {
@@ -139,7 +146,7 @@ __global__ void resolve_kernel(const sfe_anchor *anchors, const sfe_result *resu
         for (long long k = ns; k < nact; k++) { const sfe_box b = act[k]; cov = cov || box_has(b, tp, qp, strand); }
         cov = cov && valid;
         const bool live = valid && !cov, cand = live && commit && score >= min_score;
-        const unsigned kmask = decide_block(live, cand, cov, mine, tp, qp, strand, lane);
+        const unsigned kmask = decide_block(valid, live, cand, cov, mine, tp, qp, strand, lane);
         const bool kept = (kmask >> lane) & 1u;
         if (kept) {                                               // append the kept boxes in lane order
             const long long r = __popc(kmask & ((1u << lane) - 1));
@@ -313,7 +320,7 @@ __global__ void spec_commit_kernel(SpecState *st, const sfe_anchor *win_anchors,
         for (long long k = 0; k < nloc; k++) { const sfe_box b = local[k]; cov = cov || box_has(b, tp, qp, strand); }
         cov = cov && valid;
         const bool live = valid && !cov, cand = live && score >= min_score;
-        const unsigned kmask = decide_block(live, cand, cov, mine, tp, qp, strand, lane);
+        const unsigned kmask = decide_block(valid, live, cand, cov, mine, tp, qp, strand, lane);
         const bool kept = (kmask >> lane) & 1u;
         if (kept) {
             const long long r = __popc(kmask & ((1u << lane) - 1));

@@ -262,13 +262,17 @@ def test_speculate_config1_windows(sfe, oracle):
     assert out["keep"].tolist() == full["keep"].tolist()
 
 
-@pytest.mark.parametrize("seed,n,spread", [(1, 1000, 40), (2, 5000, 400), (3, 257, 5), (4, 4096, 3000)])
+@pytest.mark.parametrize("seed,n,spread", [(1, 1000, 40), (2, 5000, 400), (3, 257, 5), (4, 4096, 3000), (5, 1500, 60)])
 def test_resolve_random_boxes(sfe, oracle, seed, n, spread):
     """sfe_resolve alone on synthetic (score, box) records: dense chains of mutually covering boxes, below-tau
     anchors inside kept boxes (covered, not 'below': R17 is tested before R16), both strands, unsorted ties."""
     import torch
     rng = np.random.default_rng(seed)
-    tpos = np.sort(rng.integers(0, n * spread // 8 + 50, n)); qpos = tpos + rng.integers(-30, 30, n)
+    tpos = np.sort(rng.integers(0, n * spread // 8 + 50, n))
+    if seed == 5:                                   # anchor order need not be position order: locally shuffled
+        for a in range(0, n - 40, 40):
+            rng.shuffle(tpos[a:a + 40])
+    qpos = tpos + rng.integers(-30, 30, n)
     strand = np.where(rng.random(n) < 0.3, -1, 1)
     anchors = np.stack([tpos, qpos, np.zeros(n, np.int64), strand], 1).astype(np.int64)
     score = rng.integers(2000, 4500, n)
