@@ -17,8 +17,13 @@
  * loops over explicit cells, no blocking, no fusion, no reordering.
  *
  * Pins (tests/test_oracle_pins.py): SURVEY Appendix A worked examples (tests/golden),
- * ydrop = infinity against a brute-force full Gotoh DP, closed forms, CIGAR rescoring and
- * the other invariants of SURVEY 8(c) P1..P7.  No function here is "parity unpinned".
+ * ydrop = infinity against a brute-force full Gotoh DP (10^5 trials) and cell by cell against an
+ * independent numpy DP, closed forms (incl. lag > n == constant threshold), CIGAR rescoring and
+ * the other invariants of SURVEY 8(c) P1..P7, hand-worked tie-break examples for R11 (E / F open
+ * on ties, E over F), the four closed box edges of R17, the mirrored query limits of R15, the
+ * matrix orientation [query][target] and tau's inclusiveness.  Single-token mutations of every
+ * rule turn a pin red, except three that are provably equivalent.
+ * No function here is "parity unpinned".
  */
 #include <stdint.h>
 #include <stdlib.h>
@@ -80,8 +85,9 @@ static int32_t pair_score(const osfe_scoring *sc, uint8_t a, uint8_t b)
  * anchor.  ops (may be NULL) receives up to ops_cap run-length ops in origin -> end order;
  * out->n_ops is the number needed.  Returns 0, or -1 if out of memory.
  * ------------------------------------------------------------------------------------------ */
-static int ext_onesided_alloc(const uint8_t *q, int64_t n, const uint8_t *t, int64_t m,
-                              const osfe_scoring *sc, osfe_half *out, uint32_t **ops_out)
+static int ext_onesided_cells(const uint8_t *q, int64_t n, const uint8_t *t, int64_t m,
+                              const osfe_scoring *sc, osfe_half *out, uint32_t **ops_out,
+                              int32_t *cellH, uint8_t *cellA)
 {
     const int32_t O = sc->gap_open, X = sc->gap_extend, OX = O + X;
     const int inf = (sc->ydrop == OSFE_YDROP_INF);
@@ -167,6 +173,8 @@ static int ext_onesided_alloc(const uint8_t *q, int64_t n, const uint8_t *t, int
                 }
             }
             Hc[k] = H; Ec[k] = E; Ac[k] = (uint8_t)alive; Fprev = F;
+            if (cellH) cellH[i * (m + 1) + j] = H;        /* inspection only (pin P5): no effect on the DP */
+            if (cellA) cellA[i * (m + 1) + j] = (uint8_t)alive;
             if (pused == pcap) { pcap *= 2; ptr = realloc(ptr, pcap); if (!ptr) return -1; }
             ptr[pused++] = p;
             if (alive) {
@@ -238,6 +246,21 @@ static int ext_onesided_alloc(const uint8_t *q, int64_t n, const uint8_t *t, int
     free(rev); free(Hp); free(Ep); free(Hc); free(Ec); free(Ap); free(Ac);
     free(row_off); free(row_c0); free(best_upto); free(ptr);
     return 0;
+}
+
+static int ext_onesided_alloc(const uint8_t *q, int64_t n, const uint8_t *t, int64_t m,
+                              const osfe_scoring *sc, osfe_half *out, uint32_t **ops_out)
+{
+    return ext_onesided_cells(q, n, t, m, sc, out, ops_out, NULL, NULL);
+}
+
+/* The same extension, also writing every VISITED cell's H and alive flag into dense (n+1) x (m+1)
+ * arrays the caller pre-filled (cells never visited keep the caller's fill).  Used only by pin P5
+ * ("every alive cell's H is <= its unpruned Gotoh value"). */
+int osfe_ext_onesided_cells(const uint8_t *q, int64_t n, const uint8_t *t, int64_t m,
+                            const osfe_scoring *sc, osfe_half *out, int32_t *cellH, uint8_t *cellA)
+{
+    return ext_onesided_cells(q, n, t, m, sc, out, NULL, cellH, cellA);
 }
 
 int osfe_ext_onesided(const uint8_t *q, int64_t n, const uint8_t *t, int64_t m,

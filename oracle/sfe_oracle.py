@@ -170,6 +170,18 @@ def ext_onesided(q, t, sc: Scoring, want_ops: bool = True) -> HalfOut:
     return HalfOut(h.score, h.end_i, h.end_j, h.cells, h.rows, h.max_width, ops)
 
 
+def ext_onesided_cells(q, t, sc: Scoring):
+    """One-sided extension that also returns dense (n+1) x (m+1) arrays with every visited cell's H and alive flag
+    (cells never visited: H = -2**31, alive 0).  Inspection only (pin P5)."""
+    q = _u8(q); t = _u8(t)
+    h = Half()
+    H = np.full((len(q) + 1, len(t) + 1), -2**31, np.int32); A = np.zeros((len(q) + 1, len(t) + 1), np.uint8)
+    rc = lib().osfe_ext_onesided_cells(_p(q), C.c_int64(len(q)), _p(t), C.c_int64(len(t)), C.byref(sc), C.byref(h),
+                                       _p(H, C.c_int32), _p(A))
+    assert rc == 0
+    return HalfOut(h.score, h.end_i, h.end_j, h.cells, h.rows, h.max_width, []), H, A
+
+
 def gotoh_bruteforce(q, t, sc: Scoring):
     q = _u8(q); t = _u8(t)
     s = C.c_int32(); ei = C.c_int64(); ej = C.c_int64()

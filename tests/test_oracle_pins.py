@@ -88,21 +88,28 @@ def test_p1_a17_overrun(oracle):
 
 
 def test_p2_ydrop_inf_equals_bruteforce(oracle):
-    """R27: with pruning off, score and end cell equal the textbook Gotoh DP (first max)."""
+    """R27: with pruning off, score and end cell equal the textbook Gotoh DP (first max).  SURVEY P2: random pairs
+    <= 12 x 12, >= 10^5 trials (100,000 here; each at lag 0, every 8th also at lag 32)."""
     rng = np.random.default_rng(12345)
-    for trial in range(3000):
-        n, m = rng.integers(0, 13, 2)
-        alpha = 5 if trial % 3 == 0 else 4          # include N sometimes
-        q = rng.integers(0, alpha, n).astype(np.uint8); t = rng.integers(0, alpha, m).astype(np.uint8)
+    N = 100_000
+    nm = rng.integers(0, 13, (N, 2)); seqs = rng.integers(0, 5, (N, 2, 12)).astype(np.uint8); aux = rng.integers(0, 1 << 30, (N, 4))
+    for trial in range(N):
+        n, m = int(nm[trial, 0]), int(nm[trial, 1])
+        q = seqs[trial, 0, :n].copy(); t = seqs[trial, 1, :m].copy()
+        if trial % 3:                                # N only sometimes
+            q[q == 4] = 0; t[t == 4] = 1
         if trial % 2:                                # make them related so gaps/matches matter
             t = np.resize(q, m).astype(np.uint8) if n else t
             if m:
-                t[rng.integers(0, m)] = rng.integers(0, 4)
-        go, ge = (400, 30) if trial % 4 else (int(rng.integers(0, 60)) + 1, int(rng.integers(1, 20)))
-        for lag in (0, 32):
+                t[aux[trial, 0] % m] = aux[trial, 1] % 4
+        go, ge = (400, 30) if trial % 4 else (int(aux[trial, 2] % 60), int(aux[trial, 3] % 19) + 1)
+        bf = None
+        for lag in ((0, 32) if trial % 8 == 0 else (0,)):
             sc = oracle.scoring(ydrop=oracle.YDROP_INF, prune_lag=lag, gap_open=go, gap_extend=ge)
+            if bf is None:
+                bf = oracle.gotoh_bruteforce(q, t, sc)
             h = oracle.ext_onesided(q, t, sc, want_ops=False)
-            assert (h.score, h.end_i, h.end_j) == oracle.gotoh_bruteforce(q, t, sc)
+            assert (h.score, h.end_i, h.end_j) == bf, (trial, q, t, go, ge)
             assert h.cells == (n + 1) * (m + 1)
 
 
@@ -135,11 +142,58 @@ def test_p3_closed_forms(oracle):
                 best, bi = s, k + 1
         assert (h.score, h.end_i, h.end_j) == (best, bi, bi)
         assert h.cigar == (f"{bi}M" if bi else "")
-    # lag >= n: the threshold is the constant -Y, so lag n and lag 10 n agree
-    q = W.randseq(11, 80); t = W.randseq(12, 90)
-    h1 = oracle.ext_onesided(q, t, oracle.scoring(prune_lag=81, ydrop=2000))
-    h2 = oracle.ext_onesided(q, t, oracle.scoring(prune_lag=800, ydrop=2000))
-    assert (h1.score, h1.cells, h1.cigar) == (h2.score, h2.cells, h2.cigar)
+
+
+def _gotoh_const_threshold(q, t, sub, n_score, O, X, thr):
+    """Independent textbook Gotoh over the whole rectangle in which a cell is dead iff it has no alive predecessor
+    or H < thr (a CONSTANT), dead cells feeding nothing.  Returns (best, end_i, end_j, cells, H, alive) with
+    cells = sum over rows of (last alive - first alive + 1); thr = None disables the threshold."""
+    NEG = -(1 << 40)
+    n, m = len(q), len(t)
+    H = np.full((n + 1, m + 1), NEG, np.int64); E = H.copy(); F = H.copy(); A = np.zeros((n + 1, m + 1), bool)
+    H[0, 0] = 0; A[0, 0] = True
+    best = (0, 0, 0)
+    for i in range(n + 1):
+        for j in range(m + 1):
+            if i == 0 and j == 0:
+                continue
+            e = f = d = NEG
+            if i and A[i - 1, j]:
+                e = max(H[i - 1, j] - O - X, E[i - 1, j] - X)
+            if j and A[i, j - 1]:
+                f = max(H[i, j - 1] - O - X, F[i, j - 1] - X)
+            if i and j and A[i - 1, j - 1]:
+                a, b = int(q[i - 1]), int(t[j - 1])
+                d = H[i - 1, j - 1] + (n_score if a > 3 or b > 3 else sub[a][b])
+            h = max(d, e, f)
+            E[i, j] = e; F[i, j] = f; H[i, j] = h
+            if h > NEG // 2 and (thr is None or h >= thr):
+                A[i, j] = True
+                if h > best[0]:
+                    best = (int(h), i, j)
+    cells = 0
+    for i in range(n + 1):
+        c = np.nonzero(A[i])[0]
+        if len(c):
+            cells += int(c[-1] - c[0] + 1)
+    return best + (cells, H, A)
+
+
+def test_p3_lag_beyond_rows_is_constant_threshold(oracle):
+    """R4 closed form: with lag > n no row ever sees a best, so T is the constant -Y: the result equals the plain
+    Gotoh DP in which cells below -Y (and their descendants through dead-only routes) do not exist."""
+    rng = np.random.default_rng(4242)
+    for trial in range(150):
+        n, m = (int(x) for x in rng.integers(1, 28, 2))
+        q = rng.integers(0, 4, n).astype(np.uint8)
+        t = np.resize(q, m).astype(np.uint8); t[rng.random(m) < 0.35] = rng.integers(0, 4)
+        if trial % 3 == 0:
+            t = rng.integers(0, 4, m).astype(np.uint8)
+        Y = int(rng.choice([150, 450, 700, 1500]))
+        ref = _gotoh_const_threshold(q, t, oracle.HOXD70, -100, 400, 30, -Y)
+        for lag in (n + 1, 10 * n + 7):
+            h = oracle.ext_onesided(q, t, oracle.scoring(prune_lag=lag, ydrop=Y), want_ops=False)
+            assert (h.score, h.end_i, h.end_j, h.cells) == ref[:4], (trial, lag)
 
 
 def _mutated_pair(seed, n, p_sub, p_indel):
@@ -189,6 +243,131 @@ def test_p5_upper_bound(oracle):
             for Y in (100, 500, 2000):
                 h = oracle.ext_onesided(q, t, oracle.scoring(ydrop=Y, prune_lag=lag), want_ops=False)
                 assert 0 <= h.score <= bf
+
+
+def test_p5_cellwise_bound_and_unpruned_equality(oracle):
+    """SURVEY P5 on small inputs, cell by cell (through the oracle's inspection entry point): every ALIVE cell's H is
+    <= its unpruned Gotoh value for any finite (Y, lag); with ydrop = infinity every cell equals it (R27) -- the
+    unpruned table comes from the independent numpy DP above, not from the oracle."""
+    rng = np.random.default_rng(31337)
+    for trial in range(120):
+        n, m = (int(x) for x in rng.integers(1, 22, 2))
+        q = rng.integers(0, 5 if trial % 4 == 0 else 4, n).astype(np.uint8)
+        t = np.resize(q, m).astype(np.uint8); t[rng.random(m) < 0.25] = rng.integers(0, 4)
+        go, ge = ((400, 30), (0, 5), (37, 11))[trial % 3]
+        sub = oracle.HOXD70 if trial % 2 else MM
+        ref = _gotoh_const_threshold(q, t, sub, -100, go, ge, None)
+        Href = ref[4]
+        for lag in (0, 1, 32):
+            sc = oracle.scoring(sub=sub, gap_open=go, gap_extend=ge, ydrop=oracle.YDROP_INF, prune_lag=lag)
+            h, H, A = oracle.ext_onesided_cells(q, t, sc)
+            assert A.all() and (H.astype(np.int64) == Href).all(), (trial, lag)
+            assert (h.score, h.end_i, h.end_j) == ref[:3]
+            for Y in (60, 300, 1200):
+                sc = oracle.scoring(sub=sub, gap_open=go, gap_extend=ge, ydrop=Y, prune_lag=lag)
+                h, H, A = oracle.ext_onesided_cells(q, t, sc)
+                al = A.astype(bool)
+                assert al[0, 0] and (H.astype(np.int64)[al] <= Href[al]).all(), (trial, lag, Y)
+                assert h.score == int(H[al].max()) and 0 <= h.score <= ref[0]
+                assert h.cells == sum(int(c[-1] - c[0] + 1) for c in (np.nonzero(r)[0] for r in al) if len(c))
+
+
+@pytest.mark.parametrize("row", _rows("tiebreak_examples.txt"), ids=lambda r: r[0])
+def test_p1_tiebreak_examples(oracle, row):
+    """R11: E opens on ties, F opens on ties, H-source priority E over F (hand-worked)."""
+    cid, q, t, score, ei, ej, cigar, wrong = row
+    sc = oracle.scoring(sub=MM, gap_open=0, gap_extend=5, ydrop=1000, prune_lag=0)
+    h = oracle.ext_onesided(oracle.codes(q), oracle.codes(t), sc)
+    assert (h.score, h.end_i, h.end_j, h.cigar) == (int(score), int(ei), int(ej), cigar)
+    assert cigar != wrong
+    # both candidate CIGARs are optimal alignments (the rule picks among equals): rescoring gives the same score
+    for c in (cigar, wrong):
+        import re
+        ops = [(int(a), "MID".index(b)) for a, b in re.findall(r"(\d+)([MID])", c)]
+        assert oracle.rescore(oracle.codes(q), oracle.codes(t), ops, sc) == (int(score), len(q), len(t))
+
+
+def test_r17_closed_box_edges(oracle):
+    """R17: containment is a point-in-closed-box test on all four edges, same strand (tests/golden/resolver_edges.txt)."""
+    with open(os.path.join(GOLD, "resolver_edges.txt")) as f:
+        rows = [ln.split()[:4] for ln in f if ln.strip() and not ln.startswith("#")]
+    anchors = [(10, 10, 0, 1)] + [(int(r[0]), int(r[1]), 0, int(r[2])) for r in rows]
+    scores = [5000] + [100] * len(rows)
+    boxes = [(5, 15, 6, 14)] + [(a[0], a[0], a[1], a[1]) for a in anchors[1:]]
+    state, acc = oracle.resolve(anchors, scores, boxes, 3000)
+    assert state[0] == 1 and acc == [(5, 15, 6, 14, 1)]
+    assert state[1:].tolist() == [int(r[3]) for r in rows]
+    # the same edges as boxes carried in from an earlier window (R26)
+    state2, _ = oracle.resolve(anchors[1:], scores[1:], boxes[1:], 3000, accepted=[(5, 15, 6, 14, 1)])
+    assert state2.tolist() == [int(r[3]) for r in rows]
+    # through Algorithm 1 itself on the Appendix-A pair: the first anchor's alignment (1268) has box [0,20] x [0,18];
+    # anchors exactly on its corners are covered and never extended (with an open interval they would be kept:
+    # the whole alignment is reachable from either corner)
+    T = oracle.codes("ACGTACGTTTGGCCAGTCAT"); Q = oracle.codes("ACGTACGTGGCCAGTCAT")
+    sc = oracle.scoring(prune_lag=0, min_score=500)
+    r = oracle.serial_loop(T, Q, W.revcomp(Q), [(0, 20, 0, 18)], [(14, 12, 0, 1), (20, 18, 0, 1), (0, 0, 0, 1), (20, 0, 0, 1)], sc)
+    assert list(r["state"]) == [1, 0, 0, 0] and r["n_extended"] == 1
+    for K in (1, 2, 4):
+        sp = oracle.speculative_loop(T, Q, W.revcomp(Q), [(0, 20, 0, 18)], [(14, 12, 0, 1), (20, 18, 0, 1), (0, 0, 0, 1), (20, 0, 0, 1)], sc, K)
+        assert list(sp["state"]) == [1, 0, 0, 0]
+
+
+def test_r15_minus_strand_subrange_pair(oracle):
+    """R15 / R9: for a - strand anchor the pair's query interval [q_begin, q_end) is mirrored into the reverse-
+    complement frame, [q_len - q_end, q_len - q_begin); the target interval is not.  Qrc = T (Q = revcomp(T)), so an
+    anchor on the main diagonal extends as pure matches until a LIMIT stops it: score = sum of s(x,x) over the bases
+    inside the limits (closed form), CIGAR kM + kM, box = the limits.  A pair whose mirror is not the identity."""
+    T = W.randseq(77, 40); Q = W.revcomp(T)
+    assert (W.revcomp(Q) == T).all()
+    diag = lambda lo, hi: sum(oracle.HOXD70[int(x)][int(x)] for x in T[lo:hi])
+    sc = oracle.scoring(min_score=0)
+    # (pair, anchor, limits that apply in the rc frame)
+    cases = [((0, 40, 10, 26), (20, 20), (0, 40, 14, 30)),        # query interval mirrored: [40-26, 40-10) = [14, 30)
+             ((0, 40, 0, 9), (33, 33), (0, 40, 31, 40)),          # [31, 40): touches the end of the rc frame
+             ((16, 27, 10, 26), (20, 20), (16, 27, 14, 30)),      # target limits bite first (not mirrored)
+             ((0, 40, 12, 12 + 1), (27, 27), (0, 40, 27, 28))]    # one-base interval [27, 28)
+    for pair, (tp, qp), (tb, te, qb, qe) in cases:
+        lo = max(tb - tp, qb - qp); hi = min(te - tp, qe - qp)           # diagonal run inside the limits, relative to the anchor
+        r = oracle.serial_loop(T, Q, T.copy(), [pair], [(tp, qp, 0, -1)], sc)
+        res = r["results"][0]
+        assert r["state"][0] == 1
+        assert (res.score_bwd, res.score_fwd) == (diag(tp + lo, tp), diag(tp, tp + hi)), (pair, res.score_bwd, res.score_fwd)
+        assert (res.tstart, res.tend, res.qstart, res.qend) == (tp + lo, tp + hi, qp + lo, qp + hi)
+        # the same through the two-sided entry point with explicit rc-frame limits, incl. the CIGAR
+        r2, ops = oracle.extend_anchor(T, T, tp, qp, sc, t_lim=(tb, te), q_lim=(qb, qe))
+        assert r2.score == res.score and oracle.cigar_str(ops) == (f"{-lo}M" if lo else "") + (f"{hi}M" if hi else "")
+    # + strand control: the interval is used as given
+    r = oracle.serial_loop(T, T.copy(), W.revcomp(T), [(0, 40, 10, 26)], [(20, 20, 0, 1)], sc)
+    res = r["results"][0]
+    assert (res.qstart, res.qend, res.score) == (10, 26, diag(10, 26))
+
+
+def test_r3_substitution_matrix_orientation(oracle):
+    """R3 / R13: sub[a][b] is indexed [query base][target base] (HOXD70 is symmetric, so only an asymmetric matrix can
+    tell).  s(A over C) = +7, s(C over A) = -50, matches +10: q = A, t = C scores 7 with 1M; q = C, t = A scores nothing.
+    q = AC vs t = CC: (1,1) = s(A,C) = 7, (2,2) = 7 + s(C,C) = 17 -> 2M, 17."""
+    sub = [[10, 7, -50, -50], [-50, 10, -50, -50], [-50, -50, 10, -50], [-50, -50, -50, 10]]
+    sc = oracle.scoring(sub=sub, gap_open=20, gap_extend=5, ydrop=1000, prune_lag=0)
+    h = oracle.ext_onesided(oracle.codes("A"), oracle.codes("C"), sc); assert (h.score, h.cigar) == (7, "1M")
+    h = oracle.ext_onesided(oracle.codes("C"), oracle.codes("A"), sc); assert (h.score, h.cigar) == (0, "")
+    h = oracle.ext_onesided(oracle.codes("AC"), oracle.codes("CC"), sc); assert (h.score, h.end_i, h.end_j, h.cigar) == (17, 2, 2, "2M")
+    ops = [(2, oracle.OP_M)]
+    assert oracle.rescore(oracle.codes("AC"), oracle.codes("CC"), ops, sc)[0] == 17
+    assert oracle.gotoh_bruteforce(oracle.codes("AC"), oracle.codes("CC"), oracle.scoring(sub=sub, gap_open=20, gap_extend=5))[0] == 17
+
+
+def test_r16_tau_is_inclusive(oracle):
+    """PAPER.md:62 / 143: Score(a) >= tau commits.  The Appendix-A alignment scores exactly 1268: tau = 1268 keeps it
+    (and it masks the second anchor), tau = 1269 does not (state 2, masks nothing: R18), in Alg. 1, Alg. 3 and resolve."""
+    T = oracle.codes("ACGTACGTTTGGCCAGTCAT"); Q = oracle.codes("ACGTACGTGGCCAGTCAT")
+    A = [(14, 12, 0, 1), (10, 10, 0, 1)]
+    for tau, exp in ((1268, [1, 0]), (1269, [2, 2])):
+        sc = oracle.scoring(prune_lag=0, min_score=tau)
+        assert list(oracle.serial_loop(T, Q, W.revcomp(Q), [(0, 20, 0, 18)], A, sc)["state"]) == exp
+        for K in (1, 2):
+            assert list(oracle.speculative_loop(T, Q, W.revcomp(Q), [(0, 20, 0, 18)], A, sc, K)["state"]) == exp
+        st, _ = oracle.resolve(A, [1268, 840], [(0, 20, 0, 18), (0, 20, 0, 18)], tau)
+        assert st.tolist() == exp
 
 
 def test_p6_resolver_order_examples(oracle):
