@@ -4,14 +4,18 @@
 A "step" is one pass of the whole hot path over one batch: sfe_pack (target, query + reverse
 complement) -> sfe_ydrop_batch (binning, persistent queue, systolic Y-drop DP with traceback,
 CIGAR emission) -> sfe_resolve, on device-resident inputs (`value`), and the same through
-sfe_extend_host with pinned HOST buffers (`e2e`).  Default workload = BASELINE.json configs[1]
-(C2, divergent cross-species regime, 25,000 anchors); --workload c4 is the kernel
-microbenchmark (configs[3]).  The path does not shard (BASELINE.json: one GPU, no collectives):
---gpus N runs N independent replicas ("replicas only"), value = sum over ranks.
+sfe_extend_host with pinned HOST buffers (`e2e`).  Default workload = BASELINE.json configs[3]
+(C4: 65,536 independent pairs, the kernel microbenchmark SURVEY 8(d) names for "headline GCUPS and
+roofline fraction"); the same line carries `c5_e2e`: Algorithm 3 end to end (sfe_speculate) on
+configs[4] (C5, the chromosome-scale pair; see --c5).  --workload c1|c2|c3|c5|c3s|c5s select the others.
+The path does not shard (BASELINE.json: one GPU, no collectives): --gpus N runs N independent
+replicas ("replicas only"), value = sum over ranks.
 
 --impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload.
 """
 import argparse
+import glob
+import hashlib
 import json
 import os
 import subprocess
@@ -25,11 +29,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 SCRATCH_GB = {"c1": 2, "c2": 16, "c4": 24, "c3": 32, "c3s": 24, "c5s": 32, "c5": 48}   # traceback arena (chunks are recycled)
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE ydrop_kernel<traceback> launch, from an `ncu --set full` capture of the
-# default run (profiles/r1_04_final_round1.md, "full C2 launch"): 0.768 GB read + 15.376 GB written.  Algorithmic bytes of
-# the same launch = the traceback records, `roofline.detail.tb_bytes_per_step` (15.8 GB): no wasted re-reads.
-NCU_TRAFFIC_BYTES = {("c2", "cigar", 0, "auto"): 16_144_609_424}
 DEFAULT_WINDOW = {"c3": 16384, "c3s": 16384, "c5s": 1024, "c5": 1024}   # Algorithm 3's K for the dense-anchor workloads; others: one batch
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.csv")      # written by hand from `ncu --set full` captures (see ncu_traffic.md)
 
 
 def make_workload(name):
@@ -47,8 +48,34 @@ def make_workload(name):
     if name == "c3s":
         return W.config3(t_len=1_000_000, n_anchors=5_000), "configs[2] scaled 1/10: 1 Mbp, 5,000 anchors (prefix-scale run)"
     if name == "c5s":
-        return W.config5(t_len=10_000_000, n_anchors=100_000), "configs[4] scaled 1/10: 10 Mbp, 100,000 anchors"
+        return W.config5(t_len=10_000_000, n_anchors=100_000), "configs[4] scaled 1/10: 10 Mbp, 100,000 anchors (the prefix-scale run SURVEY 8(d) allows)"
     raise SystemExit(f"unknown workload {name}")
+
+
+def source_hash():
+    """sha256 over the CUDA sources and the header: what an ncu capture was taken of (git is not on the GPU box)."""
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2606_06811_b200", "csrc", "*.cu*")) + [os.path.join(ROOT, "include", "sfe.h")]):
+        h.update(os.path.basename(f).encode()); h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload, flags, window, kernel):
+    """roofline.traffic = dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel from an
+    `ncu --set full` capture, recorded in profiles/ncu_traffic.csv together with the hash of the sources it was
+    taken of.  A capture of other sources, or of another configuration, is not reported: null plus the reason."""
+    import csv
+    key = f"{workload}/{flags}/{window}/{kernel}"
+    try:
+        rows = [r for r in csv.DictReader(ln for ln in open(TRAFFIC_FILE) if not ln.startswith("#")) if r.get("key") == key]
+    except OSError:
+        return None, "no capture recorded (profiles/ncu_traffic.csv missing)"
+    if not rows:
+        return None, f"no capture for {key}"
+    ent = rows[-1]
+    if ent.get("source_hash") != source_hash():
+        return None, f"capture is of sources {ent.get('source_hash')}, this run is {source_hash()} (stale: re-capture)"
+    return int(ent["dram_bytes_read"]) + int(ent["dram_bytes_write"]), ent.get("profile")
 
 
 class ClockSampler:
@@ -93,27 +120,76 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_sample(w, budget_s):
-    """The oracle as it stands, one thread, on a strided sample of the workload's anchors until
+# ---- CPU legs (the oracle as it stands; SURVEY 8(d) "Timing the oracle beside it") -------------------------------
+def _oracle_one(w, qrc, sc, i):
+    from oracle import sfe_oracle as O
+    a = w.anchors[i]; p = w.pairs[int(a[2])]
+    qlim = (int(p[2]), int(p[3])) if a[3] > 0 else (len(w.query) - int(p[3]), len(w.query) - int(p[2]))
+    r, _ = O.extend_anchor(w.target, w.query if a[3] > 0 else qrc, int(a[0]), int(a[1]), sc,
+                           t_lim=(int(p[0]), int(p[1])), q_lim=qlim, want_ops=True)
+    return r.cells
+
+
+def strided_order(n):
+    stride = max(1, n // 4096)
+    return [i for s in range(stride) for i in range(s, n, stride)]
+
+
+def oracle_sample(w, budget_s, indices=None):
+    """The oracle, ONE thread, two-sided extension with CIGAR over a strided sample of the anchors (or `indices`) until
     ~budget_s seconds of CPU work are done.  Returns (cells, seconds, n_anchors_done)."""
     from oracle import sfe_oracle as O
     O.lib()
     sc = O.scoring()
-    n = len(w.anchors)
     qrc = w.query_rc
-    stride = max(1, n // 4096)
-    order = [i for s in range(stride) for i in range(s, n, stride)]
+    order = strided_order(len(w.anchors)) if indices is None else list(indices)
     cells = 0; done = 0
     t0 = time.perf_counter()
     for i in order:
-        a = w.anchors[i]; p = w.pairs[int(a[2])]
-        qlim = (int(p[2]), int(p[3])) if a[3] > 0 else (len(w.query) - int(p[3]), len(w.query) - int(p[2]))
-        r, _ = O.extend_anchor(w.target, w.query if a[3] > 0 else qrc, int(a[0]), int(a[1]), sc,
-                               t_lim=(int(p[0]), int(p[1])), q_lim=qlim, want_ops=True)
-        cells += r.cells; done += 1
+        cells += _oracle_one(w, qrc, sc, i); done += 1
         if time.perf_counter() - t0 > budget_s:
             break
     return cells, time.perf_counter() - t0, done
+
+
+def oracle_parallel(w, budget_s, indices=None):
+    """The same extensions on ALL host cores: a thread pool over anchors (the ctypes call releases the GIL), the analogue
+    of the paper's 32-core prototype.  Returns (cells, seconds, n_done, cores)."""
+    from concurrent.futures import ThreadPoolExecutor
+    from oracle import sfe_oracle as O
+    O.lib()
+    sc = O.scoring()
+    qrc = w.query_rc
+    cores = max(1, os.cpu_count() or 1)
+    order = strided_order(len(w.anchors)) if indices is None else list(indices)
+    cells = 0; done = 0; pos = 0
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=cores) as ex:
+        while pos < len(order) and time.perf_counter() - t0 < budget_s:
+            chunk = order[pos:pos + 4 * cores]; pos += len(chunk)
+            for c in ex.map(lambda i: _oracle_one(w, qrc, sc, i), chunk):
+                cells += c; done += 1
+    return cells, time.perf_counter() - t0, done, cores
+
+
+def oracle_serial_prefix(w, budget_s):
+    """Algorithm 1 as the oracle runs it, one thread, on growing PREFIXES of the anchor list until one
+    call takes about budget_s.  Returns dict(anchors, extended, kept, cells, seconds)."""
+    from oracle import sfe_oracle as O
+    O.lib()
+    sc = O.scoring()
+    qrc = w.query_rc
+    n = len(w.anchors)
+    m = min(n, 16)
+    best = None
+    while True:
+        t0 = time.perf_counter()
+        r = O.serial_loop(w.target, w.query, qrc, w.pairs, w.anchors[:m], sc, want_results=False)
+        dt = time.perf_counter() - t0
+        best = dict(anchors=m, extended=int(r["n_extended"]), kept=int(r["n_kept"]), cells=int(r["cells"]), seconds=dt)
+        if m >= n or dt > budget_s / 3:
+            return best
+        m = min(n, int(m * max(2.0, min(8.0, 0.6 * budget_s / max(dt, 1e-3)))))
 
 
 def run_reference(args):
@@ -153,13 +229,63 @@ def aggregate_replicas(ms, cells, world, device):
     return float(t.item()), float(c.item())
 
 
+class Job:
+    """One workload resident on the device + the step that runs the hot path over it."""
+
+    def __init__(self, sfe, w, dev, flags, window, cigar_cap):
+        import torch
+        from paper_2606_06811_b200 import binding as B
+        self.B = B; self.sfe = sfe; self.w = w; self.dev = dev; self.flags = flags; self.window = window
+        self.n = len(w.anchors)
+        self.t_ascii = torch.from_numpy(w.target_ascii().copy()).to(dev)
+        self.q_ascii = torch.from_numpy(w.query_ascii().copy()).to(dev)
+        self.anchors_np = B.make_anchors(w.anchors); self.pairs_np = B.make_pairs(w.pairs)
+        self.anchors = B._dev(self.anchors_np, dev); self.pairs = B._dev(self.pairs_np, dev)
+        self.acc = torch.zeros((self.n + 1) * B.BOX_DT.itemsize, dtype=torch.uint8, device=dev)
+        self.nacc = torch.zeros(1, dtype=torch.int64, device=dev)
+        self.stats = torch.zeros(B.STATS_DT.itemsize, dtype=torch.uint8, device=dev)
+        self.cigar_cap = cigar_cap
+        self.sc = B.scoring()
+        self.state = {}
+
+    def step(self, K=None, flags=None):
+        B = self.B; w = self.w; sfe = self.sfe
+        K = self.window if K is None else K
+        flags = self.flags if flags is None else flags
+        self.nacc.zero_(); self.stats.zero_()
+        tp = sfe.pack(self.t_ascii, with_rc=False)
+        qp = sfe.pack(self.q_ascii, with_rc=True)
+        self.state.update(tp=tp, qp=qp)
+        if K > 0:
+            o = sfe.speculate(tp[:2], len(w.target), qp, len(w.query), self.pairs, len(w.pairs), self.anchors, self.n, self.sc, K, flags,
+                              self.cigar_cap, accepted_dev=self.acc, n_accepted_dev=self.nacc, stats_dev=self.stats)
+            self.state.update(res=o["results"], keep=o["keep"])
+        else:
+            res, pool, used = sfe.ydrop_batch(tp[:2], len(w.target), qp, len(w.query), self.pairs, len(w.pairs), self.anchors, self.n,
+                                              self.sc, flags, self.cigar_cap)
+            keep = sfe.resolve(self.anchors, res, self.n, self.sc.min_score, self.acc, self.n + 1, self.nacc, self.stats)
+            self.state.update(res=res, keep=keep)
+
+    def stats_dict(self):
+        st = self.stats.cpu().numpy().view(self.B.STATS_DT)[0]
+        return {k: int(st[k]) for k in self.B.STATS_DT.names}
+
+
+def summarize_pass(st, ms):
+    ext = st["n_extended"]
+    return {"ms": ms, "gcups": st["cells_total"] / (ms * 1e-3) / 1e9, "kept": st["n_kept"], "kept_per_s": st["n_kept"] / (ms * 1e-3),
+            "extended": ext, "windows": st["n_windows"], "cells": st["cells_total"],
+            "waste_ext": (1.0 - (st["n_kept"] + st["n_below"]) / ext) if ext else None,
+            "waste_cells": (st["cells_covered"] / st["cells_total"]) if st["cells_total"] else None}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c4", "c3", "c3s", "c5s", "c5"])
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c4", "c3", "c3s", "c5s", "c5"])
     ap.add_argument("--window", type=int, default=-1, help="Algorithm 3's K (sfe_speculate); 0 = one batch over all anchors; -1 = workload default")
     ap.add_argument("--kernel", default="auto", choices=["auto", "block", "systolic"],
                     help="block: the cooperative-warps kernel (one CTA per half) for every half; auto / systolic: one warp per half")
@@ -167,11 +293,15 @@ def main():
                     help="windowed workloads: CIGARs for every extended anchor, or (SFE_CIGAR_KEPT_ONLY) score-only windows + one "
                          "traceback batch over the kept anchors; auto = kept for windowed workloads")
     ap.add_argument("--fidelity", action="store_true",
-                    help="R4 fidelity report: one extra pass at prune_lag = 0 (serial-order pruning, block kernel) compared with the timed Lambda = 32 results")
+                    help="R4 fidelity report: prune_lag = 0 (serial-order pruning, block kernel) against the Lambda = 32 results; "
+                         "one-batch workloads in full, windowed ones on a seeded sample of their extended anchors")
     ap.add_argument("--sweep-k", default="", help="comma-separated K values: one extra timed pass each (PAPER.md:163, Fig. 3)")
     ap.add_argument("--flags", default="cigar", choices=["cigar", "score"])
-    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--cpu-seconds", type=float, default=10.0, help="budget of EACH CPU leg (1-core serial loop, all-core extensions)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--c5", default="auto", choices=["auto", "full", "prefix", "off"],
+                    help="the c5_e2e key of the default (c4) line: Algorithm 3 end to end on configs[4]; prefix = the 10 Mbp / "
+                         "100,000-anchor prefix-scale run SURVEY 8(d) allows; auto = prefix")
     ap.add_argument("--limit-anchors", type=int, default=0, help="profiling aid: keep every k-th anchor so that N remain")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -190,7 +320,9 @@ def main():
     dev = torch.device("cuda", local)
     entry.build()
 
+    t_gen = time.perf_counter()
     w, desc = make_workload(args.workload)
+    t_gen = time.perf_counter() - t_gen
     if args.limit_anchors and args.limit_anchors < len(w.anchors):
         w.anchors = w.anchors[:: len(w.anchors) // args.limit_anchors][: args.limit_anchors]
         desc += f" [profiling subset: {len(w.anchors)} anchors]"
@@ -200,43 +332,13 @@ def main():
     free_b, _ = torch.cuda.mem_get_info(dev)
     scratch = min(SCRATCH_GB[args.workload] << 30, int(free_b * 0.6))
     sfe = B.Sfe(local, scratch)
-    sc = B.scoring()
-
-    # device-resident inputs
-    t_ascii = torch.from_numpy(w.target_ascii().copy()).to(dev)
-    q_ascii = torch.from_numpy(w.query_ascii().copy()).to(dev)
-    anchors_np = B.make_anchors(w.anchors); pairs_np = B.make_pairs(w.pairs)
-    anchors = B._dev(anchors_np, dev); pairs = B._dev(pairs_np, dev)
-    acc = torch.zeros((n + 1) * B.BOX_DT.itemsize, dtype=torch.uint8, device=dev)
-    nacc = torch.zeros(1, dtype=torch.int64, device=dev)
-    stats = torch.zeros(B.STATS_DT.itemsize, dtype=torch.uint8, device=dev)
-    cigar_cap = max(1 << 26 if DEFAULT_WINDOW.get(args.workload, 0) or args.window > 0 else 1 << 20, 96 * n)
-    state = {}
 
     window = DEFAULT_WINDOW.get(args.workload, 0) if args.window < 0 else args.window
     kept_only = window > 0 and args.flags == "cigar" and args.cigar_for in ("auto", "kept")
     if kept_only:
         flags |= B.CIGAR_KEPT_ONLY
-
-    def step(K=None):
-        K = window if K is None else K
-        nacc.zero_(); stats.zero_()
-        tp = sfe.pack(t_ascii, with_rc=False)
-        qp = sfe.pack(q_ascii, with_rc=True)
-        if K > 0:
-            o = sfe.speculate(tp[:2], len(w.target), qp, len(w.query), pairs, len(w.pairs), anchors, n, sc, K, flags, cigar_cap,
-                              accepted_dev=acc, n_accepted_dev=nacc, stats_dev=stats)
-            state.update(res=o["results"], keep=o["keep"])
-        else:
-            res, pool, used = sfe.ydrop_batch(tp[:2], len(w.target), qp, len(w.query), pairs, len(w.pairs), anchors, n, sc, flags,
-                                              cigar_cap)
-            keep = sfe.resolve(anchors, res, n, sc.min_score, acc, n + 1, nacc, stats)
-            state.update(res=res, keep=keep)
-
-    def launches_of(info, n_windows, K):
-        # pack x3; per Y-drop pass: tickets x3, ydrop, select_wide, ydrop_wide, join, scan, emit (+ select_overflow on re-runs);
-        # one batch: block_min + resolve; windows: prepare x3, scan + commit per window, finish
-        return 3 + 9 * info["launches"] + (info["launches"] - max(1, n_windows)) + ((3 + 2 * n_windows + 1) if K > 0 else 2)
+    cigar_cap = max(1 << 26 if window > 0 else 1 << 20, 96 * n)
+    job = Job(sfe, w, dev, flags, window, cigar_cap)
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -245,25 +347,24 @@ def main():
         torch.cuda.synchronize(dev)
 
     for _ in range(max(3, args.warmup)):
-        step()
+        job.step()
     barrier()
     info0 = sfe.last_batch_info()
-    st = stats.cpu().numpy().view(B.STATS_DT)[0]
-    cells_step = int(st["cells_total"]); kept_step = int(st["n_kept"]); covered_step = int(st["n_covered"])
-    cells_cov = int(st["cells_covered"]); ext_step = int(st["n_extended"]); below_step = int(st["n_below"]); windows_step = int(st["n_windows"])
+    st0 = job.stats_dict()
+    cells_step = st0["cells_total"]; kept_step = st0["n_kept"]
 
     sampler = ClockSampler(local)
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-    kernel_us = 0.0; launches = 0
+    kernel_us = 0.0
     barrier()
+    launches0 = B.launch_counter()
     e0.record()
     for _ in range(args.steps):
-        step()
-        inf = sfe.last_batch_info()
-        kernel_us += inf["ydrop_kernel_us"]
-        launches += launches_of(inf, windows_step, window)
+        job.step()
+        kernel_us += sfe.last_batch_info()["ydrop_kernel_us"]
     e1.record()
     barrier()
+    launches = B.launch_counter() - launches0          # counted at the launch sites (sfe_launch_counter), not derived
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop()
     ms, tot_cells = aggregate_replicas(ms, cells_step * args.steps, world, dev)
@@ -275,53 +376,106 @@ def main():
         t_host = torch.from_numpy(w.target_ascii().copy()).pin_memory().numpy()
         q_host = torch.from_numpy(w.query_ascii().copy()).pin_memory().numpy()
         for _ in range(2):
-            ho = sfe.extend_host(t_host, q_host, pairs_np, anchors_np, sc, flags, cigar_cap, window)
+            ho = sfe.extend_host(t_host, q_host, job.pairs_np, job.anchors_np, job.sc, flags, cigar_cap, window)
         barrier()
         t0 = time.perf_counter()
         for _ in range(args.steps):
-            ho = sfe.extend_host(t_host, q_host, pairs_np, anchors_np, sc, flags, cigar_cap, window)
+            ho = sfe.extend_host(t_host, q_host, job.pairs_np, job.anchors_np, job.sc, flags, cigar_cap, window)
         torch.cuda.synchronize(dev)
         dt = time.perf_counter() - t0
-        h2d = len(t_host) + len(q_host) + anchors_np.nbytes + pairs_np.nbytes
+        h2d = len(t_host) + len(q_host) + job.anchors_np.nbytes + job.pairs_np.nbytes
         d2h = n * B.RESULT_DT.itemsize + n + 4 * int(ho["cigar_used"]) + B.STATS_DT.itemsize + 8
         e2e_cells = int(ho["stats"]["cells_total"]) * args.steps * world
         e2e = {"value": e2e_cells / dt / 1e9, "unit": "GCUPS", "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": 1e3 * dt / args.steps, "kept_per_s": int(ho["stats"]["n_kept"]) * args.steps / dt}
+        del t_host, q_host
 
     # f4: batch-size sweep (Fig. 3): one timed pass per K, same inputs
     sweep = []
     for K in [int(x) for x in args.sweep_k.split(",") if x.strip()]:
-        step(K); torch.cuda.synchronize(dev)
+        job.step(K); torch.cuda.synchronize(dev)
         k0 = torch.cuda.Event(enable_timing=True); k1 = torch.cuda.Event(enable_timing=True)
-        k0.record(); step(K); k1.record(); torch.cuda.synchronize(dev)
-        s2 = stats.cpu().numpy().view(B.STATS_DT)[0]; kms = k0.elapsed_time(k1)
-        sweep.append({"k": K, "ms": kms, "gcups": float(s2["cells_total"]) / (kms * 1e-3) / 1e9, "windows": int(s2["n_windows"]),
-                      "extended": int(s2["n_extended"]), "kept": int(s2["n_kept"]),
-                      "waste_ext": 1.0 - (int(s2["n_kept"]) + int(s2["n_below"])) / max(1, int(s2["n_extended"])),
-                      "waste_cells": float(s2["cells_covered"]) / max(1.0, float(s2["cells_total"])),
-                      "kept_per_s": int(s2["n_kept"]) / (kms * 1e-3)})
+        k0.record(); job.step(K); k1.record(); torch.cuda.synchronize(dev)
+        d = summarize_pass(job.stats_dict(), k0.elapsed_time(k1)); d["k"] = K
+        sweep.append(d)
 
     # R4 fidelity: how often does the row-lagged threshold (Lambda = 32) change a result of Lambda = 0?
     fidelity = None
-    if args.fidelity and window == 0:
-        step(); torch.cuda.synchronize(dev)
-        r32 = B.results_to_numpy(state["res"], n); k32 = state["keep"].cpu().numpy()[:n]
-        sc0 = B.scoring(prune_lag=0)
-        f0 = torch.cuda.Event(enable_timing=True); f1 = torch.cuda.Event(enable_timing=True)
-        tp = sfe.pack(t_ascii, with_rc=False); qp = sfe.pack(q_ascii, with_rc=True)
-        nacc.zero_(); stats.zero_()
-        f0.record()
-        res0, pool0, used0 = sfe.ydrop_batch(tp[:2], len(w.target), qp, len(w.query), pairs, len(w.pairs), anchors, n, sc0,
-                                             B.WANT_CIGAR | B.BLOCK_KERNEL, cigar_cap)
-        keep0 = sfe.resolve(anchors, res0, n, sc0.min_score, acc, n + 1, nacc, stats)
-        f1.record(); torch.cuda.synchronize(dev)
-        r0 = B.results_to_numpy(res0, n); k0 = keep0.cpu().numpy()[:n]
+    if args.fidelity:
+        job.step(); torch.cuda.synchronize(dev)
+        r_all = B.results_to_numpy(job.state["res"], n); k_all = job.state["keep"].cpu().numpy()[:n]
         box = lambda r: np.stack([r["tstart"], r["tend"], r["qstart"], r["qend"]], 1)
-        fidelity = {"anchors": n, "ms_lag0_block_kernel": f0.elapsed_time(f1),
-                    "score_differs": int((r0["score"] != r32["score"]).sum()), "box_differs": int((box(r0) != box(r32)).any(1).sum()),
-                    "n_ops_differs": int((r0["n_ops"] != r32["n_ops"]).sum()), "keep_differs": int((k0 != k32).sum()),
-                    "kept_lag0": int((k0 == 1).sum()), "kept_lag32": int((k32 == 1).sum()),
+        sc0 = B.scoring(prune_lag=0)
+        tp, qp = job.state["tp"], job.state["qp"]
+        f0 = torch.cuda.Event(enable_timing=True); f1 = torch.cuda.Event(enable_timing=True)
+        if window == 0:
+            job.nacc.zero_(); job.stats.zero_()
+            f0.record()
+            res0, _, _ = sfe.ydrop_batch(tp[:2], len(w.target), qp, len(w.query), job.pairs, len(w.pairs), job.anchors, n, sc0,
+                                         B.WANT_CIGAR | B.BLOCK_KERNEL, cigar_cap)
+            keep0 = sfe.resolve(job.anchors, res0, n, sc0.min_score, job.acc, n + 1, job.nacc, job.stats)
+            f1.record(); torch.cuda.synchronize(dev)
+            r0 = B.results_to_numpy(res0, n); k0 = keep0.cpu().numpy()[:n]; r32 = r_all
+            extra = {"anchors": n, "keep_differs": int((k0 != k_all).sum()), "kept_lag0": int((k0 == 1).sum()), "kept_lag32": int((k_all == 1).sum()),
+                     "n_ops_differs": int((r0["n_ops"] != r32["n_ops"]).sum())}
+        else:
+            # windowed workloads: a seeded sample of the anchors the speculative run extended (kept ones first), the same
+            # anchors as ONE batch at Lambda = 0 on the block kernel; compared with their Lambda = 32 results of the timed path
+            ext = np.nonzero((r_all["status"] & np.uint32(B.ST_SKIPPED)) == 0)[0]
+            rng = np.random.default_rng(4)
+            kept_i = ext[k_all[ext] == 1]; other = ext[k_all[ext] != 1]
+            pick = np.sort(np.concatenate([rng.choice(kept_i, min(len(kept_i), 200), replace=False),
+                                           rng.choice(other, min(len(other), 1800), replace=False)]))
+            sub = B._dev(job.anchors_np[pick], dev)
+            f0.record()
+            res0, _, _ = sfe.ydrop_batch(tp[:2], len(w.target), qp, len(w.query), job.pairs, len(w.pairs), sub, len(pick), sc0,
+                                         B.SCORE_ONLY | B.BLOCK_KERNEL, 0)
+            f1.record(); torch.cuda.synchronize(dev)
+            r0 = B.results_to_numpy(res0, len(pick)); r32 = r_all[pick]
+            extra = {"anchors": int(len(pick)), "sample": f"{int(len(pick))} of {len(ext)} extended anchors (seeded; {min(len(kept_i), 200)} kept)",
+                     "below_tau_flips": int(((r0["score"] >= job.sc.min_score) != (r32["score"] >= job.sc.min_score)).sum())}
+        fidelity = {"ms_lag0_block_kernel": f0.elapsed_time(f1), "score_differs": int((r0["score"] != r32["score"]).sum()),
+                    "box_differs": int((box(r0) != box(r32)).any(1).sum()),
                     "cells_lag32_over_lag0": float(r32["cells"].sum()) / max(1.0, float(r0["cells"].sum()))}
+        fidelity.update(extra)
+
+    # c5_e2e: Algorithm 3 end to end on the chromosome-scale config, in the same line (default run only)
+    c5 = None
+    if args.workload == "c4" and args.c5 != "off" and not args.limit_anchors:
+        del job
+        sfe.close(); torch.cuda.empty_cache()
+        name5 = "c5" if args.c5 == "full" else "c5s"
+        tg = time.perf_counter(); w5, desc5 = make_workload(name5); tg = time.perf_counter() - tg
+        free_b, _ = torch.cuda.mem_get_info(dev)
+        sfe5 = B.Sfe(local, min(SCRATCH_GB[name5] << 30, int(free_b * 0.6)))
+        K5 = DEFAULT_WINDOW[name5]
+        f5 = B.WANT_CIGAR | B.CIGAR_KEPT_ONLY
+        cap5 = max(1 << 26, 96 * len(w5.anchors))
+        job5 = Job(sfe5, w5, dev, f5, K5, cap5)
+        job5.step(); torch.cuda.synchronize(dev)                       # warm-up pass
+        a0 = torch.cuda.Event(enable_timing=True); a1 = torch.cuda.Event(enable_timing=True)
+        a0.record(); job5.step(); a1.record(); torch.cuda.synchronize(dev)
+        c5 = summarize_pass(job5.stats_dict(), a0.elapsed_time(a1))
+        c5.update({"workload": f"{name5}: {desc5}", "anchors": len(w5.anchors), "window_k": K5, "cigar_for": "kept", "generation_s": tg,
+                   "path": "sfe_pack x2 -> sfe_speculate (phase 1 scan, phase 2 Y-drop windows, phase 3 commit, all on the device) "
+                           "-> one traceback batch over the kept anchors; device-resident inputs, CUDA events"})
+        t_host = torch.from_numpy(w5.target_ascii().copy()).pin_memory().numpy()
+        q_host = torch.from_numpy(w5.query_ascii().copy()).pin_memory().numpy()
+        t0 = time.perf_counter()
+        ho = sfe5.extend_host(t_host, q_host, job5.pairs_np, job5.anchors_np, job5.sc, f5, cap5, K5)
+        torch.cuda.synchronize(dev)
+        dt = time.perf_counter() - t0
+        c5["host_e2e"] = {"ms": 1e3 * dt, "gcups": int(ho["stats"]["cells_total"]) / dt / 1e9, "kept_per_s": int(ho["stats"]["n_kept"]) / dt,
+                          "h2d_bytes": int(len(t_host) + len(q_host) + job5.anchors_np.nbytes + job5.pairs_np.nbytes),
+                          "d2h_bytes": int(len(w5.anchors) * (B.RESULT_DT.itemsize + 1) + 4 * int(ho["cigar_used"]))}
+        # Algorithm 1 as the oracle runs it, one thread, on a prefix of the same anchor list ("LASTZ-like serial seconds")
+        if rank == 0:
+            sp = oracle_serial_prefix(w5, args.cpu_seconds)
+            sp["gcups"] = sp["cells"] / sp["seconds"] / 1e9
+            c5["cpu_serial_alg1"] = sp
+        del t_host, q_host, job5
+        sfe5.close()
+        sfe = B.Sfe(local, 1 << 30)                                    # for the probes below
 
     if rank != 0:
         if world > 1:
@@ -342,33 +496,49 @@ def main():
     r_alu_pipe = min(r_alu, r_dpx)
     cyc_per_cell = max(hl["alu"] / r_alu_pipe, hl["fma"] / r_fma, hl["per_cell"] / max(r_mix, r_alu, r_dpx))
     peak_gcups = n_sm * fmax * 1e6 / cyc_per_cell / 1e9
+    # SURVEY 8(d)'s literal formula: N_SM x R x f / I with I = ALL SASS instructions per cell, R = the measured mixed issue rate
+    peak_issue = n_sm * fmax * 1e6 * max(r_mix, r_alu, r_dpx) / hl["per_cell"] / 1e9
     k_gcups = cells_step * args.steps / (kernel_us * 1e-6) / 1e9 if kernel_us > 0 else None
+    traffic, traffic_note = (None, "profiling subset") if args.limit_anchors else ncu_traffic(args.workload, args.flags, window, args.kernel)
     roof = {"bound": "alu", "achieved": k_gcups, "peak": peak_gcups, "unit": "GCUPS", "frac": (k_gcups / peak_gcups) if k_gcups else None,
-            "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.flags, window, args.kernel)) if not args.limit_anchors else None, "kernel": "ydrop_kernel<%s>" % ("traceback" if tb_loop else "score-only"),
+            "frac_issue": (k_gcups / peak_issue) if k_gcups else None, "peak_issue": peak_issue,
+            "traffic": traffic, "traffic_source": traffic_note, "kernel": "ydrop_kernel<%s>" % ("traceback" if tb_loop else "score-only"),
             "kernel_share_of_step": kernel_us * 1e-3 / ms,
             "detail": {"instr_per_cell_sass": hl["per_cell"], "alu_per_cell": hl["alu"], "dpx_per_cell": hl["dpx"], "fma_per_cell": hl["fma"],
                        "lsu_per_cell": hl["lsu"], "R_alu": r_alu, "R_dpx": r_dpx, "R_imad": r_fma, "R_mixed": r_mix,
                        "R_unit": "lane-instr/clk/SM at sm_max_mhz", "n_sm": n_sm, "f_mhz_used": fmax,
                        "f_mhz_sampled": f_mhz, "peak_source": "measured by sfe_probe_int_issue in this run",
-                       "tb_bytes_per_step": info0["tb_bytes"], "tb_gbs": info0["tb_bytes"] * args.steps / (kernel_us * 1e-6) / 1e9 if kernel_us else None,
+                       "frac_is": "pipe-bound reading: the ALU pipe's instructions per cell over its measured rate",
+                       "frac_issue_is": "SURVEY 8(d) literal: all SASS instructions per cell over the measured mixed issue rate",
+                       "source_hash": source_hash(),
+                       "algorithmic_bytes_per_step": 0.5 * cells_step, "tb_bytes_per_step": info0["tb_bytes"],
+                       "tb_gbs": info0["tb_bytes"] * args.steps / (kernel_us * 1e-6) / 1e9 if kernel_us else None,
                        "lane_efficiency": cells_step / (32.0 * info0["steps"]) if info0["steps"] and window == 0 else None}}
 
+    # CPU legs: (1) one thread; for a one-batch workload without coverage this IS Algorithm 1's serial work; (2) all cores
     oc, osec, od = oracle_sample(w, args.cpu_seconds)
+    pc, psec, pd, cores = oracle_parallel(w, args.cpu_seconds)
+    sp = oracle_serial_prefix(w, args.cpu_seconds)
     cpu = {"value": oc / osec / 1e9, "unit": "GCUPS", "cores": 1, "kind": "oracle",
-           "sample": f"{od} of {n} anchors (strided), two-sided extension with CIGAR, {osec:.1f} s"}
+           "sample": f"{od} of {n} anchors (strided), two-sided extension with CIGAR, {osec:.1f} s",
+           "parallel": {"value": pc / psec / 1e9, "unit": "GCUPS", "cores": cores, "kind": "oracle",
+                        "sample": f"{pd} of {n} anchors (strided; the extensions the GPU computed), thread pool over anchors, {psec:.1f} s"},
+           "serial_alg1": {"seconds": sp["seconds"], "anchors": sp["anchors"], "extended": sp["extended"], "kept": sp["kept"], "cells": sp["cells"],
+                           "gcups": sp["cells"] / sp["seconds"] / 1e9, "cores": 1,
+                           "sample": f"Algorithm 1 on the first {sp['anchors']} of {n} anchors, 1 thread"}}
 
     line = {"metric": "ydrop_gcups", "value": gcups, "unit": "GCUPS", "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
             "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "window_k": window, "kernel": args.kernel, "cigar_for": "kept" if kept_only else ("all" if args.flags == "cigar" else "none"),
-                       "l2": "inputs+traceback per step exceed L2 (126 MB)",
+                       "l2": "inputs+traceback per step exceed L2 (126 MB)", "generation_s": t_gen,
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "scoring": "HOXD70/400/30/ydrop 9400/lag 32/tau 3000"},
             "kept_alignments_per_s": kept_step * args.steps * world / (ms * 1e-3),
             "kept": kept_step, "cells_per_step": cells_step,
-            "extended": ext_step, "windows": windows_step,
-            "speculation_waste": {"ext": 1.0 - (kept_step + below_step) / ext_step if ext_step else None,
-                                  "cells": cells_cov / cells_step if cells_step else None},
-            "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roof, "cpu_baseline": cpu,
+            "extended": st0["n_extended"], "windows": st0["n_windows"],
+            "speculation_waste": {"ext": 1.0 - (kept_step + st0["n_below"]) / st0["n_extended"] if st0["n_extended"] else None,
+                                  "cells": st0["cells_covered"] / cells_step if cells_step else None},
+            "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roof, "cpu_baseline": cpu, "c5_e2e": c5,
             "batch_info": info0, "k_sweep": sweep or None, "lag0_fidelity": fidelity}
     print(json.dumps(line))
     if world > 1:

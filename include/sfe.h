@@ -57,7 +57,8 @@ enum {
 #define SFE_ST_TB_OVERFLOW 1u         /* traceback arena exhausted even when run alone: no CIGAR */
 #define SFE_ST_CIGAR_OVERFLOW 2u      /* cigar pool too small: ops not written (n_ops is valid)   */
 #define SFE_ST_WIDE 4u                /* informational: a half took the wide-band (global ring) path */
-#define SFE_ST_SCORE_LIMIT 8u         /* R25: |score| would exceed 2^29                           */
+#define SFE_ST_SCORE_LIMIT 8u         /* R25: a half's running best reached 2^29 - 2^22: the half was STOPPED there (its score,
+                                         end and box are those of the truncated extension; no CIGAR).  Split the pair.  */
 #define SFE_ST_BAD_ANCHOR 16u         /* anchor outside its pair's limits: nothing computed          */
 #define SFE_ST_BAND_LIMIT 32u         /* live band wider than 65,344 columns: half not computed      */
 #define SFE_ST_INTERNAL 64u           /* traceback walk did not reach the origin (a library bug)     */
@@ -116,8 +117,11 @@ typedef struct sfe_stats {
 int sfe_create(sfe_ctx **ctx, int device, void *cuda_stream, size_t scratch_bytes);
 int sfe_destroy(sfe_ctx *ctx);
 const char *sfe_strerror(int code);
-/* file:line and CUDA runtime message of the most recent SFE_ECUDA (process-wide, for diagnosis) */
+/* file:line and CUDA runtime message of the most recent SFE_ECUDA seen by the CALLING HOST THREAD (for diagnosis) */
 const char *sfe_last_error_detail(void);
+/* cumulative number of CUDA kernel launches this library has enqueued from the calling host thread (every launch
+ * site counts itself); bench.py reports the difference over its timed region as gpu_launches. */
+int64_t sfe_launch_counter(void);
 
 /* a1 Pack (R13, R14): ASCII (device) -> 2-bit code plane (base k in byte k/4, bits 2(k%4)..; A0 C1
  * G2 T3, N stored as 0) and 1-bit N-mask plane (base k in byte k/8, bit k%8).  If rc_codes2_dev
@@ -148,7 +152,10 @@ int sfe_ydrop_batch(sfe_ctx *ctx, const uint8_t *t_codes2_dev, const uint8_t *t_
  * keep_dev[i] = 0 covered, 1 kept, 2 below min_score.  accepted_dev / *n_accepted_dev carry the
  * boxes kept in earlier windows in and the extended list out.  With results_dev == NULL this
  * is the phase-1 "is masked" filter: keep_dev[i] = 0 covered, 1 not covered,
- * nothing appended.  stats_dev (may be NULL) is accumulated, not reset. */
+ * nothing appended.  stats_dev (may be NULL) is accumulated, not reset.
+ * Deviation from SURVEY 8(b), which sketches `sfe_result *accepted_dev`: the accepted set is an array of sfe_box
+ * (40 B: the box and its strand).  The rule reads nothing else of a kept result, the strand is not a field of
+ * sfe_result, and a driver that carries the set between windows / calls moves 40 B per kept alignment, not 72. */
 int sfe_resolve(sfe_ctx *ctx, const sfe_anchor *anchors_dev, const sfe_result *results_dev, int64_t n,
                 int32_t min_score, sfe_box *accepted_dev, int64_t accepted_cap, int64_t *n_accepted_dev,
                 uint8_t *keep_dev, sfe_stats *stats_dev);
@@ -197,21 +204,26 @@ int sfe_speculate_host(sfe_ctx *ctx, const char *t_ascii_host, int64_t t_len, co
  * sfe_ydrop_batch on this ctx: [0] kernel launches, [1] halves run, [2] halves re-run after a
  * traceback overflow, [3] traceback bytes written, [4] DP steps (warp wavefronts) executed,
  * [5] halves that took the wide path, [6] device time of the Y-drop kernel launches in microseconds
- * (CUDA events on the ctx stream; synchronises on the last one), [7] halves computed by the block kernel. */
+ * (CUDA events on the ctx stream; synchronises on the last one), [7] halves computed by the block kernel,
+ * [8] traceback chunks dropped or pops abandoned by the free-chunk ring's bounded waits (a capacity leak that should never
+ * happen: 0 in every test), [9..11] reserved (0). */
+#define SFE_INFO_N 12
 int sfe_probe_int_issue(sfe_ctx *ctx, int mix, int iters, double *lane_ops_per_clk_per_sm, double *elapsed_ms);
 
 /* Per-half profile of the most recent sfe_ydrop_batch on this ctx (Fig. 5: the
  * spread of per-anchor extension runtimes is what defeats static load balancing).  Entry 2a is the
  * forward half of anchor a, 2a+1 the backward half.  cycles = SM clock cycles from ticket to
- * result (DP + traceback walk), steps = warp wavefronts, smid / wslot = where it ran.  Copies
- * min(n, 2 * n_anchors) entries to profile_host; synchronises the stream. */
+ * result (DP + traceback walk), steps = warp wavefronts, smid / wslot = where it ran; status = the half's status
+ * bits plus, for the tests' stratified sampling, 0x800 computed by the block kernel, 0x1000 ran with the lane skew
+ * of 2 (a reserved, longest-first ticket), 0x2000 a skew-2 attempt outgrew its window and the half was re-run with
+ * skew 1.  Copies min(n, 2 * n_anchors) entries to profile_host; synchronises the stream. */
 typedef struct {
     int64_t cells, cycles;
     int32_t steps, n_strips, max_steps, n_ops;
     uint32_t smid, wslot, status, reserved;
 } sfe_half_profile;
 int sfe_last_half_profile(sfe_ctx *ctx, int64_t n, sfe_half_profile *profile_host);
-int sfe_last_batch_info(sfe_ctx *ctx, int64_t info[8]);
+int sfe_last_batch_info(sfe_ctx *ctx, int64_t info[SFE_INFO_N]);
 
 #ifdef __cplusplus
 }

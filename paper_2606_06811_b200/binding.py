@@ -21,9 +21,12 @@ PRUNE_LAG = 32
 WANT_CIGAR, SCORE_ONLY, NO_BINNING, BLOCK_KERNEL, NO_BLOCK_KERNEL, CIGAR_KEPT_ONLY = 1, 0, 2, 4, 8, 16
 ST_TB_OVERFLOW, ST_CIGAR_OVERFLOW, ST_WIDE, ST_SCORE_LIMIT, ST_BAD_ANCHOR, ST_BAND_LIMIT, ST_INTERNAL, ST_SKIPPED = 1, 2, 4, 8, 16, 32, 64, 128
 OP_M, OP_I, OP_D = 0, 1, 2
+INFO_N = 12
+ST_SKEW2, ST_SKEW_RETRY, ST_BLOCK = 0x1000, 0x2000, 0x800      # profile-only bits of sfe_half_profile.status (internal)
 
 EXPORTS = ("sfe_create", "sfe_destroy", "sfe_strerror", "sfe_last_error_detail", "sfe_pack", "sfe_ydrop_batch", "sfe_resolve",
-           "sfe_speculate", "sfe_extend_host", "sfe_speculate_host", "sfe_probe_int_issue", "sfe_last_batch_info", "sfe_last_half_profile")
+           "sfe_speculate", "sfe_extend_host", "sfe_speculate_host", "sfe_probe_int_issue", "sfe_last_batch_info", "sfe_last_half_profile",
+           "sfe_launch_counter")
 
 
 class Scoring(C.Structure):
@@ -70,6 +73,7 @@ def lib():
         _lib.sfe_strerror.restype = C.c_char_p
         _lib.sfe_strerror.argtypes = [C.c_int]
         _lib.sfe_last_error_detail.restype = C.c_char_p
+        _lib.sfe_launch_counter.restype = C.c_int64
         vp, i64, i32, u32 = C.c_void_p, C.c_int64, C.c_int32, C.c_uint32
         _lib.sfe_create.argtypes = [C.POINTER(vp), C.c_int, vp, C.c_size_t]
         _lib.sfe_destroy.argtypes = [vp]
@@ -269,10 +273,15 @@ class Sfe:
         return out[:n_halves]
 
     def last_batch_info(self):
-        a = (C.c_int64 * 8)()
+        a = (C.c_int64 * INFO_N)()
         _check(lib().sfe_last_batch_info(self.h, a), "sfe_last_batch_info")
-        keys = ("launches", "halves", "halves_rerun", "tb_bytes", "steps", "wide", "ydrop_kernel_us", "block_halves")
+        keys = ("launches", "halves", "halves_rerun", "tb_bytes", "steps", "wide", "ydrop_kernel_us", "block_halves", "ring_drops")
         return dict(zip(keys, list(a)))
+
+
+def launch_counter() -> int:
+    """Kernel launches enqueued so far by this thread through libsfe (sfe_launch_counter)."""
+    return int(lib().sfe_launch_counter())
 
 
 def results_to_numpy(results_dev, n) -> np.ndarray:

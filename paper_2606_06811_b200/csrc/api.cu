@@ -36,6 +36,7 @@ int sfe_launch_spec_gather_kept(const sfe_anchor *anchors, const uint8_t *keep, 
                                 long long *kept_idx, long long *n_kept, cudaStream_t st);
 int sfe_launch_spec_scatter_kept(const sfe_result *kres, const long long *kept_idx, long long nk, sfe_result *results, cudaStream_t st);
 int sfe_launch_ring_init(int32_t *ring, SfeFreeRing *st, int n_chunks, cudaStream_t stream);
+int sfe_ydrop_init_device(void);
 
 struct DevBuf {                       // grow-only device scratch
     void *p = nullptr; size_t cap = 0;
@@ -62,12 +63,15 @@ struct sfe_ctx {
     long long *state_host;            // pinned, 8 words
     // host-API staging
     DevBuf h_tascii, h_qascii, h_t2, h_tm, h_q2, h_qm, h_r2, h_rm, h_pairs, h_anchors, h_results, h_keep, h_cigar, h_acc, h_small;
-    long long info[8]; long long n_profile;
+    long long info[SFE_INFO_N]; long long n_profile;
     cudaEvent_t ev0, ev1; bool ev_pending;
     double kernel_us;
 };
 
-static char g_err_detail[512] = "";
+thread_local long long sfe_tls_launches = 0;
+extern "C" int64_t sfe_launch_counter(void) { return (int64_t)sfe_tls_launches; }
+
+static thread_local char g_err_detail[512] = "";      // per host thread: contexts driven from different threads do not race
 void sfe_note_cuda_error(cudaError_t e, const char *file, int line)
 {
     snprintf(g_err_detail, sizeof g_err_detail, "%s:%d: %s", file, line, cudaGetErrorString(e));
@@ -120,6 +124,7 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
         return SFE_ENOMEM;
     }
     if (sfe_launch_ring_init(c->free_ring, c->ring_state, c->n_chunks, c->stream) != SFE_OK) { sfe_destroy(c); return SFE_ECUDA; }
+    if (sfe_ydrop_init_device() != SFE_OK) { sfe_destroy(c); return SFE_ECUDA; }      // function attributes are per device
     *out = c;
     return SFE_OK;
 }
@@ -181,17 +186,17 @@ extern "C" int sfe_probe_int_issue(sfe_ctx *c, int mix, int iters, double *lane_
     return SFE_OK;
 }
 
-extern "C" int sfe_last_batch_info(sfe_ctx *c, int64_t info[8])
+extern "C" int sfe_last_batch_info(sfe_ctx *c, int64_t info[SFE_INFO_N])
 {
     if (!c || !info) return SFE_EINVAL;
     harvest_kernel_time(c);
     c->info[6] = (long long)(c->kernel_us + 0.5);
     if (c->info[4] == 0) {   // score-only batches do not read the counters back inside the call
         if (cudaMemcpyAsync(c->counters_host, c->counters, CNT_N * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream) == cudaSuccess &&
-            cudaStreamSynchronize(c->stream) == cudaSuccess) { c->info[4] = (long long)c->counters_host[CNT_STEPS]; c->info[5] = (long long)c->counters_host[CNT_WIDE]; c->info[7] = (long long)c->counters_host[CNT_BLOCK_HALVES]; }
+            cudaStreamSynchronize(c->stream) == cudaSuccess) { c->info[4] = (long long)c->counters_host[CNT_STEPS]; c->info[5] = (long long)c->counters_host[CNT_WIDE]; c->info[7] = (long long)c->counters_host[CNT_BLOCK_HALVES]; c->info[8] = (long long)c->counters_host[CNT_RING_DROPS]; }
         else cudaGetLastError();
     }
-    for (int k = 0; k < 8; k++) info[k] = c->info[k];
+    for (int k = 0; k < SFE_INFO_N; k++) info[k] = c->info[k];
     return SFE_OK;
 }
 
@@ -335,6 +340,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
         c->info[4] += (long long)c->counters_host[CNT_STEPS];
         c->info[5] += (long long)c->counters_host[CNT_WIDE];
         c->info[7] += (long long)c->counters_host[CNT_BLOCK_HALVES];
+        c->info[8] += (long long)c->counters_host[CNT_RING_DROPS];
         const long long n_over = (long long)c->counters_host[CNT_OVERFLOW];
         if (n_over == 0) break;
         // no progress possible: the anchors that overflowed were already running alone

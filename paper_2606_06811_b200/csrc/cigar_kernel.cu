@@ -25,7 +25,7 @@ __global__ void join_kernel(const sfe_anchor *anchors, const sfe_half *halves, l
     r.qstart = an.qpos - b.end_i; r.qend = an.qpos + f.end_i;
     r.cells = f.cells + b.cells;
     r.cigar_off = -1; r.n_ops = 0; r.n_ops_back = 0;
-    if (want_cigar && !(st & (SFE_ST_PASS_OVERFLOW | SFE_ST_BAD_ANCHOR | SFE_ST_BAND_LIMIT | SFE_ST_INTERNAL))) {
+    if (want_cigar && !(st & (SFE_ST_PASS_OVERFLOW | SFE_ST_BAD_ANCHOR | SFE_ST_BAND_LIMIT | SFE_ST_SCORE_LIMIT | SFE_ST_INTERNAL))) {
         r.n_ops_back = b.n_ops; r.n_ops = b.n_ops + f.n_ops;
     }
     r.status = (st & 0xffu) | ((st & SFE_ST_PASS_OVERFLOW) ? SFE_ST_TB_OVERFLOW : 0u) |
@@ -107,7 +107,7 @@ int sfe_launch_join(const sfe_anchor *anchors, const sfe_half *halves, long long
 {
     if (n_sel <= 0) return SFE_OK;
     const int bs = 128;
-    join_kernel<<<(unsigned)((n_sel + bs - 1) / bs), bs, 0, st>>>(anchors, halves, n, sel, n_sel, want_cigar, results);
+    SFE_KL join_kernel<<<(unsigned)((n_sel + bs - 1) / bs), bs, 0, st>>>(anchors, halves, n, sel, n_sel, want_cigar, results);
     SFE_LAUNCH_CHECK();
 }
 
@@ -115,10 +115,10 @@ int sfe_launch_scan_emit(const sfe_half *halves, long long n, const long long *s
                          sfe_result *results, uint32_t *cigar_pool, long long cap, long long *pool_used, cudaStream_t st)
 {
     if (n <= 0) return SFE_OK;
-    scan_offsets_kernel<<<1, 1024, 0, st>>>(results, n, pool_used, cap);
+    SFE_KL scan_offsets_kernel<<<1, 1024, 0, st>>>(results, n, pool_used, cap);
     if (n_sel > 0) {
         const int bs = 256;                                   // 8 anchors per block, one warp each
-        emit_kernel<<<(unsigned)((n_sel * 32 + bs - 1) / bs), bs, 0, st>>>(halves, n, sel, n_sel, stage, results, cigar_pool);
+        SFE_KL emit_kernel<<<(unsigned)((n_sel * 32 + bs - 1) / bs), bs, 0, st>>>(halves, n, sel, n_sel, stage, results, cigar_pool);
     }
     SFE_LAUNCH_CHECK();
 }

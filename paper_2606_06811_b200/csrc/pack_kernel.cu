@@ -59,7 +59,7 @@ int sfe_launch_pack(const char *ascii, long long len, uint8_t *codes2, uint8_t *
     const long long nthreads = (len + 31) / 32;
     const int bs = 256;
     const unsigned nb = (unsigned)((nthreads + bs - 1) / bs);
-    pack_fwd_kernel<<<nb, bs, 0, st>>>(ascii, len, codes2, nmask);
-    if (rc_codes2 && rc_nmask) pack_rc_kernel<<<nb, bs, 0, st>>>(ascii, len, rc_codes2, rc_nmask);
+    SFE_KL pack_fwd_kernel<<<nb, bs, 0, st>>>(ascii, len, codes2, nmask);
+    if (rc_codes2 && rc_nmask) SFE_KL pack_rc_kernel<<<nb, bs, 0, st>>>(ascii, len, rc_codes2, rc_nmask);
     SFE_LAUNCH_CHECK();
 }

@@ -1,5 +1,5 @@
-// queue_probe_kernels.cu -- a3: length-binned ticket order for the persistent work queue, the
-// overflow re-run selection, and the integer-issue microbenchmark used for the roofline (8(d)).
+// queue_kernels.cu -- a3: length-binned ticket order for the persistent work queue, the free-chunk ring of the
+// traceback arena and the overflow re-run selection.
 #include "sfe_internal.cuh"
 
 
@@ -61,12 +61,12 @@ int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe
     if (n <= 0) return SFE_OK;
     const int bs = 256;
     const unsigned nb = (unsigned)((n + bs - 1) / bs);
-    if (!binned) iota_tickets_kernel<<<nb, bs, 0, st>>>(tickets, n);
+    if (!binned) SFE_KL iota_tickets_kernel<<<nb, bs, 0, st>>>(tickets, n);
     else {
         if (cudaMemsetAsync(hist, 0, 64 * sizeof(unsigned int), st) != cudaSuccess) return SFE_ECUDA;
-        bin_count_kernel<<<nb, bs, 0, st>>>(anchors, n_anchors, pairs, n_pairs, q_len, hist);
-        bin_offsets_kernel<<<1, 32, 0, st>>>(hist);
-        bin_scatter_kernel<<<nb, bs, 0, st>>>(anchors, n_anchors, pairs, n_pairs, q_len, hist, tickets);
+        SFE_KL bin_count_kernel<<<nb, bs, 0, st>>>(anchors, n_anchors, pairs, n_pairs, q_len, hist);
+        SFE_KL bin_offsets_kernel<<<1, 32, 0, st>>>(hist);
+        SFE_KL bin_scatter_kernel<<<nb, bs, 0, st>>>(anchors, n_anchors, pairs, n_pairs, q_len, hist, tickets);
     }
     SFE_LAUNCH_CHECK();
 }
@@ -82,7 +82,7 @@ __global__ void ring_init_kernel(int32_t *ring, SfeFreeRing *st, int n_chunks)
 int sfe_launch_ring_init(int32_t *ring, SfeFreeRing *st, int n_chunks, cudaStream_t stream)
 {
     const int bs = 256;
-    ring_init_kernel<<<(unsigned)((n_chunks + bs - 1) / bs), bs, 0, stream>>>(ring, st, n_chunks);
+    SFE_KL ring_init_kernel<<<(unsigned)((n_chunks + bs - 1) / bs), bs, 0, stream>>>(ring, st, n_chunks);
     SFE_LAUNCH_CHECK();
 }
 
@@ -116,52 +116,6 @@ int sfe_launch_select_overflow(const sfe_half *halves, long long n_anchors, long
                                unsigned long long *counters, int n_chunks, cudaStream_t st)
 {
     const int bs = 256;
-    select_overflow_kernel<<<(unsigned)((n_anchors + bs - 1) / bs), bs, 0, st>>>(halves, n_anchors, sel, tickets, counters, n_chunks);
-    SFE_LAUNCH_CHECK();
-}
-
-// ---- integer-issue microbenchmark ---------------------------------------------------------------------
-// Register-only loops of independent chains, one kernel per opcode mix, at full occupancy.  Each
-// iteration issues OPS instructions per thread (checked against cuobjdump: DESIGN.md "Roofline").
-#define PROBE_CHAINS 8
-template <int MIX>
-__global__ void __launch_bounds__(256) probe_kernel(int iters, int seed, int *sink)
-{
-    int a[PROBE_CHAINS], b[PROBE_CHAINS];
-#pragma unroll
-    for (int c = 0; c < PROBE_CHAINS; c++) { a[c] = seed + threadIdx.x * (c + 1); b[c] = seed ^ (c * 77 + blockIdx.x); }
-    const int k1 = seed | 1, k2 = seed + 3;
-    for (int it = 0; it < iters; it++) {
-#pragma unroll
-        for (int c = 0; c < PROBE_CHAINS; c++) {
-            if (MIX == 1) {            // ALU pipe only: SHF + LOP3 (an add.s32 would become IMAD.IADD on the FMA pipe)
-                asm volatile("shf.l.wrap.b32 %0, %0, %1, 3;" : "+r"(a[c]) : "r"(b[c]));
-                asm volatile("xor.b32 %0, %0, %1;" : "+r"(b[c]) : "r"(a[c]));
-            } else if (MIX == 2) {     // DPX: VIADDMNMX + VIMNMX3
-                a[c] = __viaddmax_s32(a[c], k1, b[c]);
-                b[c] = __vimax3_s32(b[c], a[c], k2);
-            } else if (MIX == 3) {     // FMA pipe: IMAD
-                asm volatile("mad.lo.s32 %0, %0, %1, %2;" : "+r"(a[c]) : "r"(k1), "r"(b[c]));
-                asm volatile("mad.lo.s32 %0, %0, %1, %2;" : "+r"(b[c]) : "r"(k2), "r"(a[c]));
-            } else {                   // mixed: one ALU/DPX op + one IMAD (both pipes busy)
-                a[c] = __viaddmax_s32(a[c], k1, b[c]);
-                asm volatile("mad.lo.s32 %0, %0, %1, %2;" : "+r"(b[c]) : "r"(k2), "r"(a[c]));
-            }
-        }
-    }
-    int r = 0;
-#pragma unroll
-    for (int c = 0; c < PROBE_CHAINS; c++) r ^= a[c] ^ b[c];
-    if (r == 0x7fffabcd) *sink = r;
-}
-
-int sfe_launch_probe(int mix, int iters, int blocks, int *sink, cudaStream_t st)
-{
-    switch (mix) {
-    case 1: probe_kernel<1><<<blocks, 256, 0, st>>>(iters, 12345, sink); break;
-    case 2: probe_kernel<2><<<blocks, 256, 0, st>>>(iters, 12345, sink); break;
-    case 3: probe_kernel<3><<<blocks, 256, 0, st>>>(iters, 12345, sink); break;
-    default: probe_kernel<0><<<blocks, 256, 0, st>>>(iters, 12345, sink); break;
-    }
+    SFE_KL select_overflow_kernel<<<(unsigned)((n_anchors + bs - 1) / bs), bs, 0, st>>>(halves, n_anchors, sel, tickets, counters, n_chunks);
     SFE_LAUNCH_CHECK();
 }

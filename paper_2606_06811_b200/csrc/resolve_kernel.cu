@@ -43,6 +43,7 @@ static __device__ unsigned decide_block(bool valid, bool live, bool cand, bool &
     __shared__ sfe_box sb[32];
     __syncwarp();
     sb[lane] = mine;
+    __syncwarp();                                                 // the boxes are read by other lanes below
     // `after` = a lower bound of the tpos of every later live lane.  Sorted block (the normal case): the next lane's tpos;
     // otherwise the exact suffix minimum over live lanes.  (A smaller bound only adds rounds, never changes a decision.)
     const long long tpv = valid ? tp : 0x7fffffffffffffffLL;      // (covered lanes count too: still a lower bound)
@@ -186,8 +187,8 @@ int sfe_launch_resolve(const sfe_anchor *anchors, const sfe_result *results, lon
 {
     if (n <= 0) return SFE_OK;
     const int bs = 256;
-    block_min_kernel<<<(unsigned)((n + bs - 1) / bs), bs, 0, st>>>(anchors, n, blkmin);
-    resolve_kernel<<<1, 32, 0, st>>>(anchors, results, n, min_score, accepted, accepted_cap, n_accepted_io, keep, stats, blkmin, act);
+    SFE_KL block_min_kernel<<<(unsigned)((n + bs - 1) / bs), bs, 0, st>>>(anchors, n, blkmin);
+    SFE_KL resolve_kernel<<<1, 32, 0, st>>>(anchors, results, n, min_score, accepted, accepted_cap, n_accepted_io, keep, stats, blkmin, act);
     SFE_LAUNCH_CHECK();
 }
 
@@ -389,7 +390,7 @@ __global__ void spec_scatter_kept_kernel(const sfe_result *kres, const long long
 int sfe_launch_spec_gather_kept(const sfe_anchor *anchors, const uint8_t *keep, long long n, sfe_anchor *kept_anchors,
                                 long long *kept_idx, long long *n_kept, cudaStream_t st)
 {
-    spec_gather_kept_kernel<<<1, 32, 0, st>>>(anchors, keep, n, kept_anchors, kept_idx, n_kept);
+    SFE_KL spec_gather_kept_kernel<<<1, 32, 0, st>>>(anchors, keep, n, kept_anchors, kept_idx, n_kept);
     SFE_LAUNCH_CHECK();
 }
 
@@ -397,7 +398,7 @@ int sfe_launch_spec_scatter_kept(const sfe_result *kres, const long long *kept_i
 {
     if (nk <= 0) return SFE_OK;
     const int bs = 256;
-    spec_scatter_kept_kernel<<<(unsigned)((nk + bs - 1) / bs), bs, 0, st>>>(kres, kept_idx, nk, results);
+    SFE_KL spec_scatter_kept_kernel<<<(unsigned)((nk + bs - 1) / bs), bs, 0, st>>>(kres, kept_idx, nk, results);
     SFE_LAUNCH_CHECK();
 }
 
@@ -405,9 +406,9 @@ int sfe_launch_spec_prepare(const sfe_anchor *anchors, long long n, long long *b
                             const long long *n_accepted, sfe_box *act, cudaStream_t st)
 {
     const int bs = 256;
-    block_min_kernel<<<(unsigned)((n + bs - 1) / bs), bs, 0, st>>>(anchors, n, blkmin);
-    suffix_min_kernel<<<1, 32, 0, st>>>(blkmin, (n + 31) >> 5);
-    spec_init_kernel<<<1, 32, 0, st>>>((SpecState *)state, accepted, n_accepted, act);
+    SFE_KL block_min_kernel<<<(unsigned)((n + bs - 1) / bs), bs, 0, st>>>(anchors, n, blkmin);
+    SFE_KL suffix_min_kernel<<<1, 32, 0, st>>>(blkmin, (n + 31) >> 5);
+    SFE_KL spec_init_kernel<<<1, 32, 0, st>>>((SpecState *)state, accepted, n_accepted, act);
     SFE_LAUNCH_CHECK();
 }
 
@@ -415,7 +416,7 @@ int sfe_launch_spec_scan(void *state, const sfe_anchor *anchors, long long n, co
                          long long *win_idx, sfe_anchor *win_anchors, uint8_t *keep, sfe_result *results, sfe_stats *stats,
                          cudaStream_t st)
 {
-    spec_scan_kernel<<<1, 32, 0, st>>>((SpecState *)state, anchors, n, blkmin, K, act, win_idx, win_anchors, keep, results, stats);
+    SFE_KL spec_scan_kernel<<<1, 32, 0, st>>>((SpecState *)state, anchors, n, blkmin, K, act, win_idx, win_anchors, keep, results, stats);
     SFE_LAUNCH_CHECK();
 }
 
@@ -423,13 +424,13 @@ int sfe_launch_spec_commit(void *state, const sfe_anchor *win_anchors, const sfe
                            const long long *blkmin, int min_score, sfe_box *accepted, long long accepted_cap, sfe_box *act,
                            sfe_box *local, uint8_t *keep, sfe_result *results, sfe_stats *stats, cudaStream_t st)
 {
-    spec_commit_kernel<<<1, 32, 0, st>>>((SpecState *)state, win_anchors, wres, win_idx, blkmin, min_score, accepted, accepted_cap,
+    SFE_KL spec_commit_kernel<<<1, 32, 0, st>>>((SpecState *)state, win_anchors, wres, win_idx, blkmin, min_score, accepted, accepted_cap,
                                          act, local, keep, results, stats);
     SFE_LAUNCH_CHECK();
 }
 
 int sfe_launch_spec_finish(const void *state, long long *n_accepted_io, cudaStream_t st)
 {
-    spec_finish_kernel<<<1, 32, 0, st>>>((const SpecState *)state, n_accepted_io);
+    SFE_KL spec_finish_kernel<<<1, 32, 0, st>>>((const SpecState *)state, n_accepted_io);
     SFE_LAUNCH_CHECK();
 }

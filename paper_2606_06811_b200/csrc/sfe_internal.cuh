@@ -11,6 +11,11 @@
 #define SFE_ST_PASS_OVERFLOW 0x100u   // internal: the traceback arena ran out during this pass; the anchor is re-run
 #define SFE_ST_OPS_OVERFLOW 0x400u    // internal: the ops arena ran out; reported as SFE_ST_CIGAR_OVERFLOW
 #define SFE_ST_BLOCK 0x800u           // internal: computed by the row-synchronous block kernel
+#define SFE_ST_SKEW2 0x1000u          // internal (profile only): the half ran with the lane skew of 2 (reserved ticket)
+#define SFE_ST_SKEW_RETRY 0x2000u     // internal (profile only): a skew-2 strip outgrew the window; re-run with skew 1
+// R25: scores stay below 2^29 (inactive-row threshold, SFE_T_INF, the out-of-bounds score and SFE_NEG arithmetic all rely on
+// it).  The running best is tested once per strip / per row; it can rise by at most 32 rows x 127 between two tests.
+#define SFE_SCORE_LIMIT ((1 << 29) - (1 << 22))
 #define SFE_OOB_SCORE 0xE0000000u       // substitution "score" of a column beyond the target end (-2^29)
 
 // ---- shared-memory geometry of one warp -------------------------
@@ -74,7 +79,7 @@ struct sfe_half {                 // result of one one-sided extension (a7)
     uint32_t smid, wslot;         // SM and hardware warp slot that ran it
 };
 
-enum { CNT_TICKET = 0, CNT_UNUSED1, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_OPS, CNT_MAXNEED, CNT_CLASS0, CNT_CLASS1, CNT_CLASS2, CNT_CLASS3, CNT_BLOCK_HALVES, CNT_N = 16 };
+enum { CNT_TICKET = 0, CNT_RING_DROPS, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_OPS, CNT_MAXNEED, CNT_CLASS0, CNT_CLASS1, CNT_CLASS2, CNT_CLASS3, CNT_BLOCK_HALVES, CNT_N = 16 };
 
 struct SfeFreeRing {              // persistent across launches: every half returns its chunks before it ends
     unsigned long long head;      // pops issued
@@ -120,7 +125,11 @@ static __device__ __forceinline__ int sfe_base(const uint8_t *codes2, const uint
     return n ? 4 : c;
 }
 
-// last CUDA failure (file:line + runtime message), readable through sfe_last_error_detail()
+// kernel launches enqueued by the calling host thread (read through sfe_launch_counter); SFE_KL prefixes every launch
+extern thread_local long long sfe_tls_launches;
+#define SFE_KL (++sfe_tls_launches),
+
+// last CUDA failure of the calling host thread (file:line + runtime message), readable through sfe_last_error_detail()
 void sfe_note_cuda_error(cudaError_t e, const char *file, int line);
 #define SFE_CUDA_CHECK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { sfe_note_cuda_error(e_, __FILE__, __LINE__); return SFE_ECUDA; } } while (0)
 #define SFE_LAUNCH_CHECK() do { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) { sfe_note_cuda_error(e_, __FILE__, __LINE__); return SFE_ECUDA; } return SFE_OK; } while (0)

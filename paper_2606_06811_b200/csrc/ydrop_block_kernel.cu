@@ -185,7 +185,7 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
     for (int k = 0; k < BK_CPT; k++) { Hu[k] = SFE_NEG; Eu[k] = SFE_NEG; sel[k] = 0x8880u; }
     unsigned long long cells = 0;
     int rows_done = 0, max_width = 0;
-    bool wide = false;
+    bool wide = false, limit = false;
     uint32_t srow32 = 0u;                                 // lane l: packed scores of query row (i & ~31) + l (row 0: all 0, R8)
 
     for (int i = 0; i <= g.n; i++) {
@@ -194,6 +194,7 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
             srow32 = (r == 0 || r > g.n) ? 0u : p.srow[sfe_base(g.qc, g.qm, g.q0 + (long long)g.d * r)];
         }
         const uint32_t srow_lo = __shfl_sync(FULL, srow32, i & 31);
+        if (i >= 32 && sh.cum[(i - 32) & 63] >= SFE_SCORE_LIMIT) { limit = true; break; }    // R25 (block-uniform: one shared word)
         const int T = p.ydrop_inf ? SFE_T_INF : (i >= 32 ? sh.cum[(i - 32) & 63] : 0) - p.Y;    // R4, Lambda = 32
         // ---- my columns in this row's window ----
         const int q = ((tid * BK_CPT) - ws) & (BK_WIN - 1);       // window position of my first column
@@ -309,7 +310,7 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
             if (wpos + nw + 2 > BK_CHUNK_WORDS) {         // next chunk (uniform decision)
                 if (warp == 0) {
                     if (cur_chunk >= 0 && lane == 0) p.pool[(size_t)cur_chunk * BK_CHUNK_WORDS] = (uint32_t)wpos;
-                    const int nc = chunk_pop(p.free_ring, p.ring_state, p.n_chunks, lane);
+                    const int nc = chunk_pop(p.free_ring, p.ring_state, p.n_chunks, &p.counters[CNT_RING_DROPS], lane);
                     if (lane == 0) { sh.new_chunk = nc; if (nc >= 0) p.chunk_prev[nc] = cur_chunk; }
                 }
                 __syncthreads();
@@ -345,11 +346,12 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
     if (TB && cur_chunk >= 0 && tid == 0) p.pool[(size_t)cur_chunk * BK_CHUNK_WORDS] = (uint32_t)wpos;
 
     out.score = sh.best; out.end_i = sh.best_i; out.end_j = sh.best_j; out.cells = cells;
-    out.status = (wide ? (LAG0 ? SFE_ST_BAND_LIMIT : SFE_ST_WIDE_PENDING) : 0u) | ((TB && !tb_ok) ? SFE_ST_PASS_OVERFLOW : 0u) | SFE_ST_BLOCK;
+    out.status = (wide ? (LAG0 ? SFE_ST_BAND_LIMIT : SFE_ST_WIDE_PENDING) : 0u) | ((TB && !tb_ok) ? SFE_ST_PASS_OVERFLOW : 0u) | SFE_ST_BLOCK |
+                 (limit ? SFE_ST_SCORE_LIMIT : 0u);
     out.n_strips = rows_done; out.n_rec = (int)(n_words >> 6); out.steps = rows_done; out.max_steps = max_width;
     // ---- a8: warp 0 walks the row log and stages the ops; then the chunks go back to the ring ----
     if (warp == 0) {
-        if (TB && tb_ok && !wide) {
+        if (TB && tb_ok && !wide && !limit) {
             bool ops_ok = true;
             if (!block_walk(p, sh, sh.best_i, sh.best_j, sh.best_chunk, sh.best_wpos, lane, out.ops_seg, out.n_ops, ops_ok))
                 out.status |= SFE_ST_INTERNAL;
@@ -359,7 +361,7 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
             __threadfence();
             __syncwarp();
             int cc = cur_chunk;
-            while (cc >= 0) { const int prev = __ldcg(p.chunk_prev + cc); chunk_push(p.free_ring, p.ring_state, p.n_chunks, cc, lane); cc = prev; }
+            while (cc >= 0) { const int prev = __ldcg(p.chunk_prev + cc); chunk_push(p.free_ring, p.ring_state, p.n_chunks, cc, &p.counters[CNT_RING_DROPS], lane); cc = prev; }
         }
         unsigned smid, wslot;
         asm("mov.u32 %0, %%smid;" : "=r"(smid));
@@ -398,11 +400,11 @@ int sfe_launch_ydrop_block(const YdParams &p, bool want_tb, int n_sm, cudaStream
     long long blocks = p.n_tickets < 2LL * n_sm ? p.n_tickets : 2LL * n_sm;      // two CTAs of 8 warps per SM
     if (blocks < 1) blocks = 1;
     if (p.lag0) {
-        if (want_tb) ydrop_block_kernel<true, true><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
-        else ydrop_block_kernel<false, true><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
+        if (want_tb) SFE_KL ydrop_block_kernel<true, true><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
+        else SFE_KL ydrop_block_kernel<false, true><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
     } else {
-        if (want_tb) ydrop_block_kernel<true, false><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
-        else ydrop_block_kernel<false, false><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
+        if (want_tb) SFE_KL ydrop_block_kernel<true, false><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
+        else SFE_KL ydrop_block_kernel<false, false><<<(unsigned)blocks, BK_THREADS, 0, st>>>(p);
     }
     SFE_LAUNCH_CHECK();
 }

@@ -60,7 +60,7 @@ static __device__ __forceinline__ bool half_setup(const YdParams &p, const int h
 // lane-divergent region makes ptxas clone the whole DP loop with real WARPSYNCs).  Both spins wait
 // for one bounded action of another resident warp (the matching push / pop has already reserved the
 // slot), never for work.
-static __device__ __forceinline__ int chunk_pop(int32_t *ring, SfeFreeRing *st, int n_chunks, int lane)
+static __device__ __forceinline__ int chunk_pop(int32_t *ring, SfeFreeRing *st, int n_chunks, unsigned long long *drops, int lane)
 {
     long long a = 0; unsigned long long h = 0;
     if (lane == 0) {
@@ -70,18 +70,17 @@ static __device__ __forceinline__ int chunk_pop(int32_t *ring, SfeFreeRing *st, 
     }
     a = __shfl_sync(FULL, a, 0);
     if (a <= 0) return -1;
-    volatile int32_t *slot = ring + (h % (unsigned long long)n_chunks);
+    int32_t *slot = ring + (h % (unsigned long long)n_chunks);
     int id = -1;
     for (int spin = 0; spin < SFE_SPIN_LIMIT; spin++) {     // bounded: a hang must be impossible, whatever happened to the pusher
-        if (lane == 0) id = *slot;
-        id = __shfl_sync(FULL, id, 0);
+        if (lane == 0) id = atomicExch(slot, -1);           // take the id and empty the slot in ONE step: a delayed pop can never
+        id = __shfl_sync(FULL, id, 0);                      // read an id that a later lap's pop also reads
         if (id >= 0) break;
     }
-    if (id < 0) return -1;                                  // treated like an empty arena: score-only now, re-run later
-    if (lane == 0) *slot = -1;
+    if (id < 0 && lane == 0) atomicAdd(drops, 1ULL);        // treated like an empty arena: score-only now, re-run later (counted)
     return id;
 }
-static __device__ __forceinline__ void chunk_push(int32_t *ring, SfeFreeRing *st, int n_chunks, int id, int lane)
+static __device__ __forceinline__ void chunk_push(int32_t *ring, SfeFreeRing *st, int n_chunks, int id, unsigned long long *drops, int lane)
 {
     unsigned long long t = 0;
     if (lane == 0) t = atomicAdd(&st->tail, 1ULL);
@@ -92,7 +91,7 @@ static __device__ __forceinline__ void chunk_push(int32_t *ring, SfeFreeRing *st
         old = __shfl_sync(FULL, old, 0);
         if (old == -1) break;
     }
-    if (old != -1) return;                                  // give the chunk up (capacity leak) rather than wait for ever
+    if (old != -1) { if (lane == 0) atomicAdd(drops, 1ULL); return; }   // give the chunk up (capacity leak, counted) rather than wait for ever
     if (lane == 0) atomicAdd((unsigned long long *)&st->avail, 1ULL);
 }
 

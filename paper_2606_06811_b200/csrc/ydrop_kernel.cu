@@ -87,7 +87,7 @@ static __device__ __forceinline__ void fill_bnd_neg(char *wbase, int lo, int hi,
 }
 
 struct TbWriter {
-    uint32_t *pool; int32_t *chunk_prev; int32_t *ring; SfeFreeRing *ring_state; int n_chunks;
+    uint32_t *pool; int32_t *chunk_prev; int32_t *ring; SfeFreeRing *ring_state; int n_chunks; unsigned long long *drops;
     uint32_t *ptr;          // this lane's word pair of the next record
     int left;               // records left in the current chunk
     int cur_chunk; int nrec; bool ok;
@@ -95,7 +95,7 @@ struct TbWriter {
     {
         if (!ok) return;
         if (left == 0) {
-            const int c = chunk_pop(ring, ring_state, n_chunks, lane);
+            const int c = chunk_pop(ring, ring_state, n_chunks, drops, lane);
             if (c < 0) { ok = false; return; }
             if (lane == 0) chunk_prev[c] = cur_chunk;
             cur_chunk = c;
@@ -115,7 +115,7 @@ struct TbWriter {
         int c = cur_chunk;
         while (c >= 0) {
             const int prev = __ldcg(chunk_prev + c);        // same address in every lane
-            chunk_push(ring, ring_state, n_chunks, c, lane);
+            chunk_push(ring, ring_state, n_chunks, c, drops, lane);
             c = prev;
         }
         cur_chunk = -1;
@@ -295,7 +295,7 @@ static __device__ bool walk_traceback(const YdParams &p, TbReader &rd, const int
 template <bool TB, int RL2, bool GLOBAL, int SK>
 // Returns false only when SK == 2 and a strip outgrew the shared-memory window (skew 2 needs 31 more steps per strip):
 // nothing has been published then, and the caller runs the half again with SK == 1.
-static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, char *wk, const int lane)
+static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, char *wk, const int lane, const uint32_t mode_bits)
 {
     typedef RingGeom<RL2> G;
     uint16_t *selring = (uint16_t *)(wsm + 8 * G::ROW_STRIDE);
@@ -314,7 +314,7 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
 
     const int OX = p.OX, X = p.X;
     TbWriter tb;
-    tb.pool = p.pool; tb.chunk_prev = p.chunk_prev; tb.ring = p.free_ring; tb.ring_state = p.ring_state; tb.n_chunks = p.n_chunks;
+    tb.pool = p.pool; tb.chunk_prev = p.chunk_prev; tb.ring = p.free_ring; tb.ring_state = p.ring_state; tb.n_chunks = p.n_chunks; tb.drops = &p.counters[CNT_RING_DROPS];
     tb.cur_chunk = -1; tb.nrec = 0; tb.ok = TB; tb.ptr = nullptr; tb.left = 0;
 
     int best = 0, best_i = 0, best_j = 0;     // lane-local first maximum
@@ -324,7 +324,7 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
     int bnd_valid = 0;                         // boundary ring holds row (r0-1) for columns < bnd_valid
     int sel_hi = -32 * SK;                     // selector ring is filled for columns < sel_hi (lane 31 starts at column -31 SK)
     int total_steps = 0, max_steps = 0, last_hdr = -1, n_strips = 0;
-    bool wide = false;
+    bool wide = false, limit = false;
 
     for (int s = 0;; s++) {
         const int r0 = s * 32;
@@ -425,6 +425,7 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
         if (last >= 0) cells += (unsigned long long)(last - first + 1);
         if (best > best_before) { best_i = r; best_j = cs + best_t - SK * lane; }
         cumB = cumA; cumA = best;
+        if (__any_sync(FULL, best >= SFE_SCORE_LIMIT)) { limit = true; break; }   // R25: one test per strip
         const int L31 = __shfl_sync(FULL, first, 31), R31 = __shfl_sync(FULL, last, 31);
         if (R31 < 0) break;                                 // last row of the strip has no alive cell
         bnd_valid = cs + t0 - 31 * SK;                      // lane 31 wrote columns cs-31 SK .. cs+t0-31 SK-1
@@ -453,9 +454,9 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
     out.score = bs; out.end_i = bi; out.end_j = bj; out.cells = cells;
     // normal kernel: a bail-out is re-run by the wide kernel; wide kernel: a bail-out is final (band limit)
     out.status = (wide ? (GLOBAL ? (SFE_ST_WIDE | SFE_ST_BAND_LIMIT) : SFE_ST_WIDE_PENDING) : (GLOBAL ? SFE_ST_WIDE : 0u)) |
-                 ((TB && !tb.ok) ? SFE_ST_PASS_OVERFLOW : 0u);
+                 ((TB && !tb.ok) ? SFE_ST_PASS_OVERFLOW : 0u) | (limit ? SFE_ST_SCORE_LIMIT : 0u) | mode_bits;
     out.n_strips = n_strips; out.n_rec = tb.nrec;
-    if (TB && tb.ok && !wide) {                             // a8: walk the pointers now, stage the run-length ops
+    if (TB && tb.ok && !wide && !limit) {                             // a8: walk the pointers now, stage the run-length ops
         TbReader rd;
         rd.pool = p.pool; rd.chunk_prev = p.chunk_prev; rd.chunk = tb.cur_chunk; rd.ord = (tb.nrec - 1) / SFE_CHUNK_RECS;
         rd.last_chunk = rd.chunk; rd.last_ord = rd.ord; rd.nrec = tb.nrec; rd.bad = false;
@@ -516,8 +517,9 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kerne
             if (lo + (long long)tk >= hi) break;
             // the reserved (longest) tickets run with a lane skew of 2: a shorter dependent step, a few more idle steps
             bool done = false;
-            if (phase == 0 && SFE_LONG_SKEW == 2) done = extend_half<TB, SFE_RING_LOG2, false, SFE_LONG_SKEW>(p, p.tickets[lo + tk], wsm, wsm, lane);
-            if (!done) extend_half<TB, SFE_RING_LOG2, false, 1>(p, p.tickets[lo + tk], wsm, wsm, lane);
+            const bool long_skew = phase == 0 && SFE_LONG_SKEW == 2;
+            if (long_skew) done = extend_half<TB, SFE_RING_LOG2, false, SFE_LONG_SKEW>(p, p.tickets[lo + tk], wsm, wsm, lane, SFE_ST_SKEW2);
+            if (!done) extend_half<TB, SFE_RING_LOG2, false, 1>(p, p.tickets[lo + tk], wsm, wsm, lane, long_skew ? SFE_ST_SKEW_RETRY : 0u);
             __syncwarp();
         }
     }
@@ -546,12 +548,21 @@ __global__ void __launch_bounds__(32) ydrop_wide_kernel(const YdParams p)
         if (lane == 0) tk = atomicAdd(&p.counters[CNT_WIDE_TICKET], 1ULL);
         tk = __shfl_sync(FULL, tk, 0);
         if ((long long)tk >= n) break;
-        extend_half<TB, SFE_WIDE_RING_LOG2, true, 1>(p, p.wide_tickets[tk], wsm, wk, lane);
+        extend_half<TB, SFE_WIDE_RING_LOG2, true, 1>(p, p.wide_tickets[tk], wsm, wk, lane, 0u);
         __syncwarp();
     }
 }
 
 int sfe_launch_ydrop_block(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st);
+
+// Function attributes are per DEVICE: sfe_create calls this after cudaSetDevice, for every context.
+int sfe_ydrop_init_device(void)
+{
+    const int smem = (SFE_BLOCK_THREADS / 32) * SFE_WARP_SMEM;
+    SFE_CUDA_CHECK(cudaFuncSetAttribute(ydrop_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    SFE_CUDA_CHECK(cudaFuncSetAttribute(ydrop_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    return SFE_OK;
+}
 
 // use_block: the whole pass goes to the row-synchronous block kernel (ydrop_block_kernel.cu) instead of the
 // warp-systolic one; either way halves whose band outgrew the window are re-run by the wide kernel.
@@ -563,12 +574,6 @@ int sfe_launch_ydrop(const YdParams &p, bool want_tb, bool use_block, int n_sm, 
     } else {
         const int warps_per_block = SFE_BLOCK_THREADS / 32;
         const size_t smem = (size_t)warps_per_block * SFE_WARP_SMEM;
-        static bool attr_done = false;
-        if (!attr_done) {
-            if (cudaFuncSetAttribute(ydrop_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SFE_ECUDA;
-            if (cudaFuncSetAttribute(ydrop_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SFE_ECUDA;
-            attr_done = true;
-        }
         int bps = 0;
         if (want_tb) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<true>, SFE_BLOCK_THREADS, smem);
         else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<false>, SFE_BLOCK_THREADS, smem);
@@ -580,12 +585,12 @@ int sfe_launch_ydrop(const YdParams &p, bool want_tb, bool use_block, int n_sm, 
         const long long need = (p.n_tickets + warps_per_block - 1) / warps_per_block;
         if (blocks > need) blocks = need;
         if (blocks < 1) blocks = 1;
-        if (want_tb) ydrop_kernel<true><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
-        else ydrop_kernel<false><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
+        if (want_tb) SFE_KL ydrop_kernel<true><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
+        else SFE_KL ydrop_kernel<false><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
     }
     const int bs = 256;
-    select_wide_kernel<<<(unsigned)((p.n_tickets + bs - 1) / bs), bs, 0, st>>>(p);
-    if (want_tb) ydrop_wide_kernel<true><<<SFE_WIDE_WARPS, 32, 0, st>>>(p);
-    else ydrop_wide_kernel<false><<<SFE_WIDE_WARPS, 32, 0, st>>>(p);
+    SFE_KL select_wide_kernel<<<(unsigned)((p.n_tickets + bs - 1) / bs), bs, 0, st>>>(p);
+    if (want_tb) SFE_KL ydrop_wide_kernel<true><<<SFE_WIDE_WARPS, 32, 0, st>>>(p);
+    else SFE_KL ydrop_wide_kernel<false><<<SFE_WIDE_WARPS, 32, 0, st>>>(p);
     SFE_LAUNCH_CHECK();
 }

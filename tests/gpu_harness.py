@@ -56,6 +56,32 @@ def assert_anchor_equal(out, w, i, want_cigar=True, **sc_kw):
     return r
 
 
+def oracle_many(w, indices, **sc_kw):
+    """oracle_anchor for many anchors on all host cores (ctypes releases the GIL during the C call)."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    O.lib()
+    with ThreadPoolExecutor(max_workers=max(1, os.cpu_count() or 1)) as ex:
+        return list(ex.map(lambda i: oracle_anchor(w, int(i), **sc_kw), indices))
+
+
+def assert_anchors_equal(out, w, indices, want_cigar=True, **sc_kw):
+    """assert_anchor_equal over many anchors, the oracle side run in parallel.  want_cigar: bool or a callable(i)."""
+    indices = [int(i) for i in indices]
+    for i, (r, ops) in zip(indices, oracle_many(w, indices, **sc_kw)):
+        g = out["results"][i]
+        got = (int(g["score"]), int(g["score_fwd"]), int(g["score_bwd"]), int(g["tstart"]), int(g["tend"]), int(g["qstart"]),
+               int(g["qend"]), int(g["cells"]))
+        exp = (r.score, r.score_fwd, r.score_bwd, r.tstart, r.tend, r.qstart, r.qend, r.cells)
+        assert got == exp, (i, tuple(w.anchors[i]), got, exp, int(g["status"]))
+        wc = want_cigar(i) if callable(want_cigar) else want_cigar
+        if wc:
+            assert not (int(g["status"]) & (B.ST_TB_OVERFLOW | B.ST_CIGAR_OVERFLOW | B.ST_BAD_ANCHOR)), (i, int(g["status"]))
+            assert (int(g["n_ops"]), int(g["n_ops_back"])) == (r.n_ops, r.n_ops_back), i
+            assert B.ops_list(out["cigar"], int(g["cigar_off"]), int(g["n_ops"])) == ops, i
+    return len(indices)
+
+
 def assert_resolve_equal(out, w, **sc_kw):
     """kept set / covered / below of the GPU resolver == Algorithm 1 run by the oracle."""
     ser = O.serial_loop(w.target, w.query, w.query_rc, w.pairs, w.anchors, O.scoring(**sc_kw), want_results=False)

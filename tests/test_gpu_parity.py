@@ -357,3 +357,134 @@ def test_degenerate_calls(sfe, oracle):
         sfe.ydrop_batch(tp[:2], 500, qp, 500, pairs, 2, B._dev(B.make_anchors(A), dev), len(A), B.scoring(gap_extend=0))
     with pytest.raises(B.SfeError):
         sfe.speculate(tp[:2], 500, qp, 500, pairs, 2, B._dev(B.make_anchors(A), dev), len(A), sc, 0)
+
+
+@pytest.mark.parametrize("kernel", ["systolic", "block"])
+def test_minus_strand_subrange_pairs(sfe, oracle, kernel):
+    """R15 on the GPU (half_setup's mirrored branch): - strand anchors in pairs whose query interval is NOT the whole
+    query, so the mirror [q_len - q_end, q_len - q_begin) differs from the interval itself.  First the closed form of
+    tests/test_oracle_pins.py::test_r15_minus_strand_subrange_pair (Q = revcomp(T): pure matches up to the limits), then
+    mutated sequences with random sub-range pairs on both strands against the oracle, element by element."""
+    kflag = B.BLOCK_KERNEL if kernel == "block" else B.NO_BLOCK_KERNEL
+    T = W.randseq(77, 40); Q = W.revcomp(T)
+    diag = lambda lo, hi: sum(B.HOXD70[int(x)][int(x)] for x in T[lo:hi])
+    cases = [((0, 40, 10, 26), (20, 20), (0, 40, 14, 30)), ((0, 40, 0, 9), (33, 33), (0, 40, 31, 40)),
+             ((16, 27, 10, 26), (20, 20), (16, 27, 14, 30)), ((0, 40, 12, 13), (27, 27), (0, 40, 27, 28))]
+    w = _wl(T, Q, [(tp, qp, k, -1) for k, (_, (tp, qp), _) in enumerate(cases)], [c[0] for c in cases])
+    out = H.gpu_run(sfe, w, flags=B.WANT_CIGAR | kflag, min_score=0)
+    for k, (_, (tp, qp), (tb, te, qb, qe)) in enumerate(cases):
+        lo = max(tb - tp, qb - qp); hi = min(te - tp, qe - qp)
+        g = out["results"][k]
+        assert int(g["status"]) & 0xff == 0
+        assert (int(g["score_bwd"]), int(g["score_fwd"])) == (diag(tp + lo, tp), diag(tp, tp + hi)), k
+        assert (int(g["tstart"]), int(g["tend"]), int(g["qstart"]), int(g["qend"])) == (tp + lo, tp + hi, qp + lo, qp + hi), k
+        exp_ops = ([(-lo, B.OP_M)] if lo else []) + ([(hi, B.OP_M)] if hi else [])
+        assert B.ops_list(out["cigar"], int(g["cigar_off"]), int(g["n_ops"])) == exp_ops, k
+        H.assert_anchor_equal(out, w, k, min_score=0)
+    # mutated sequences, half the segments reverse-complemented, each anchor in its own random sub-range pair
+    w2 = W.config2(t_len=50_000, n_segments=24, per_seg=5, n_decoys=20, min_len=200, max_len=700)
+    rng = np.random.default_rng(15)
+    qlen = len(w2.query)
+    pairs, anchors = [], []
+    for a in w2.anchors:
+        tp, qp, strand = int(a[0]), int(a[1]), int(a[3])
+        qf = qp if strand > 0 else qlen - qp                        # the anchor's corner in the forward query frame
+        t0 = max(0, tp - int(rng.integers(0, 400))); t1 = min(len(w2.target), tp + int(rng.integers(0, 400)))
+        q0 = max(0, qf - int(rng.integers(0, 400))); q1 = min(qlen, qf + int(rng.integers(0, 400)))
+        anchors.append((tp, qp, len(pairs), strand)); pairs.append((t0, t1, q0, q1))
+    w3 = W.Workload("subrange", w2.target, w2.query, np.array(pairs, np.int64), np.array(anchors, np.int64))
+    assert int((w3.anchors[:, 3] < 0).sum()) > 20
+    out = H.gpu_run(sfe, w3, flags=B.WANT_CIGAR | kflag)
+    assert not (out["results"]["status"] & np.uint32(B.ST_BAD_ANCHOR)).any()
+    assert H.assert_anchors_equal(out, w3, range(len(w3.anchors))) == len(anchors)
+    H.assert_resolve_equal(out, w3)
+
+
+def test_no_binning_equals_binned(sfe, oracle):
+    """SFE_NO_BINNING (tickets in anchor order, no reserved longest-first segment): the same results as the binned
+    queue, bit for bit, and equal to the oracle."""
+    w = W.config2(t_len=80_000, n_segments=40, per_seg=4, n_decoys=40, min_len=100, max_len=700)
+    a = H.gpu_run(sfe, w)
+    b = H.gpu_run(sfe, w, flags=B.WANT_CIGAR | B.NO_BINNING)
+    assert (a["results"] == b["results"]).all() and a["keep"].tolist() == b["keep"].tolist()
+    assert a["cigar_used"] == b["cigar_used"] and (a["cigar"][: a["cigar_used"]] == b["cigar"][: b["cigar_used"]]).all()
+    prof = sfe.last_half_profile(2 * len(w.anchors))
+    assert not (prof["status"] & (B.ST_SKEW2 | B.ST_SKEW_RETRY)).any()          # no reserved tickets without binning
+    H.assert_anchors_equal(b, w, range(len(w.anchors)))
+    H.assert_resolve_equal(b, w)
+    c = H.gpu_run(sfe, w, flags=B.SCORE_ONLY | B.NO_BINNING)
+    for f in ("score", "tstart", "tend", "qstart", "qend", "cells"):
+        assert (c["results"][f] == a["results"][f]).all()
+
+
+@pytest.mark.parametrize("kernel", ["systolic", "block"])
+def test_score_limit_is_flagged(sfe, oracle, kernel):
+    """R25: a half whose running best reaches 2^29 - 2^22 is stopped and flagged SFE_ST_SCORE_LIMIT instead of running
+    into the 2^29 sentinels.  An all-match C/G pair scores exactly 100 per row (closed form, pin P3), so the limit
+    532,676,608 is crossed after 5,326,767 rows: a 5.2 Mbp pair stays below it (score = 100 * length, no flag), a
+    5.6 Mbp pair trips it.  Score-only (the traceback of such a half would be > 1.5 GB)."""
+    import torch
+    LIMIT = (1 << 29) - (1 << 22)
+    kflag = B.BLOCK_KERNEL if kernel == "block" else B.NO_BLOCK_KERNEL
+    for n, tripped in ((5_200_000, False), (5_600_000, True)):
+        T = np.tile(np.array([1, 2], np.uint8), n // 2)
+        w = _wl(T, T.copy(), [(0, 0, 0, 1)])
+        out = H.gpu_run(sfe, w, flags=B.SCORE_ONLY | kflag)
+        g = out["results"][0]
+        assert bool(int(g["status"]) & B.ST_SCORE_LIMIT) == tripped
+        assert int(g["score_bwd"]) == 0 and int(g["score_fwd"]) == 100 * (int(g["qend"]) - int(g["qstart"]))
+        assert int(g["tend"]) == int(g["qend"]) and int(g["tstart"]) == int(g["qstart"]) == 0
+        if tripped:
+            assert LIMIT <= int(g["score"]) < LIMIT + (1 << 22)
+        else:
+            assert int(g["score"]) == 100 * n and int(g["qend"]) == n
+    # with traceback asked for, a flagged anchor carries no CIGAR (like SFE_ST_BAND_LIMIT)
+    if kernel == "systolic":
+        s2 = B.Sfe(0, 8 << 30)
+        try:
+            T = np.tile(np.array([1, 2], np.uint8), 2_800_000)
+            out = H.gpu_run(s2, _wl(T, T.copy(), [(0, 0, 0, 1), (5_599_000, 5_599_000, 0, 1)]), flags=B.WANT_CIGAR | kflag)
+            g = out["results"]
+            assert int(g["status"][0]) & B.ST_SCORE_LIMIT and int(g["n_ops"][0]) == 0 and int(g["cigar_off"][0]) == -1
+            assert int(g["status"][1]) & B.ST_SCORE_LIMIT and int(g["score_fwd"][1]) == 100_000
+        finally:
+            s2.close()
+            torch.cuda.empty_cache()
+
+
+def test_two_contexts_on_two_devices(oracle):
+    """Function attributes (dynamic shared memory) are set per device in sfe_create: a context on a second GPU of the same
+    process must run.  Skipped on a single-GPU box; there the same code path runs for a second context on device 0."""
+    import torch
+    w = W.config1(n_segments=3, seg_len=500, slot=1200, per_seg=2)
+    devs = [0, 1] if torch.cuda.device_count() > 1 else [0, 0]
+    ctxs = [B.Sfe(d, 256 << 20) for d in devs]
+    try:
+        outs = []
+        for d, s in zip(devs, ctxs):
+            with torch.cuda.device(d):
+                outs.append(s.extend_host(w.target_ascii(), w.query_ascii(), B.make_pairs(w.pairs), B.make_anchors(w.anchors), B.scoring()))
+        assert (outs[0]["results"] == outs[1]["results"]).all() and outs[0]["keep"].tolist() == outs[1]["keep"].tolist()
+        r, _ = oracle.extend_anchor(w.target, w.query, int(w.anchors[0][0]), int(w.anchors[0][1]), oracle.scoring())
+        assert int(outs[1]["results"]["score"][0]) == r.score
+    finally:
+        for s in ctxs:
+            s.close()
+
+
+def test_tiny_arena_many_short_halves(oracle):
+    """Free-chunk ring under churn: 4 chunks (the minimum) shared by thousands of short halves -- every pop / push goes
+    through the same few slots many laps over.  Results stay bit-exact, nothing is dropped (info ring_drops == 0)."""
+    import __graft_entry__ as entry
+    entry.build()
+    s = B.Sfe(0, 4 * 65536)
+    try:
+        w = W.config2(t_len=120_000, n_segments=60, per_seg=10, n_decoys=600, min_len=100, max_len=300)
+        out = H.gpu_run(s, w)
+        assert out["info"]["ring_drops"] == 0
+        bad = out["results"]["status"] & np.uint32(B.ST_TB_OVERFLOW | B.ST_INTERNAL)
+        assert not bad.any()
+        H.assert_anchors_equal(out, w, range(0, len(w.anchors), 3))
+        H.assert_resolve_equal(out, w)
+    finally:
+        s.close()
