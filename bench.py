@@ -296,6 +296,9 @@ def main():
                     help="R4 fidelity report: prune_lag = 0 (serial-order pruning, block kernel) against the Lambda = 32 results; "
                          "one-batch workloads in full, windowed ones on a seeded sample of their extended anchors")
     ap.add_argument("--sweep-k", default="", help="comma-separated K values: one extra timed pass each (PAPER.md:163, Fig. 3)")
+    ap.add_argument("--spec", default="leaders", choices=["leaders", "classic"],
+                    help="windowed workloads: leaders = SFE_SPEC_LEADERS (speculate on predicted leaders, results cached); "
+                         "classic = Algorithm 3's 'next K uncovered anchors'")
     ap.add_argument("--flags", default="cigar", choices=["cigar", "score"])
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="budget of EACH CPU leg (1-core serial loop, all-core extensions)")
     ap.add_argument("--no-e2e", action="store_true")
@@ -337,6 +340,8 @@ def main():
     kept_only = window > 0 and args.flags == "cigar" and args.cigar_for in ("auto", "kept")
     if kept_only:
         flags |= B.CIGAR_KEPT_ONLY
+    if window > 0 and args.spec == "leaders":
+        flags |= B.SPEC_LEADERS
     cigar_cap = max(1 << 26 if window > 0 else 1 << 20, 96 * n)
     job = Job(sfe, w, dev, flags, window, cigar_cap)
 
@@ -449,14 +454,15 @@ def main():
         free_b, _ = torch.cuda.mem_get_info(dev)
         sfe5 = B.Sfe(local, min(SCRATCH_GB[name5] << 30, int(free_b * 0.6)))
         K5 = DEFAULT_WINDOW[name5]
-        f5 = B.WANT_CIGAR | B.CIGAR_KEPT_ONLY
+        f5 = B.WANT_CIGAR | B.CIGAR_KEPT_ONLY | (B.SPEC_LEADERS if args.spec == "leaders" else 0)
         cap5 = max(1 << 26, 96 * len(w5.anchors))
         job5 = Job(sfe5, w5, dev, f5, K5, cap5)
         job5.step(); torch.cuda.synchronize(dev)                       # warm-up pass
         a0 = torch.cuda.Event(enable_timing=True); a1 = torch.cuda.Event(enable_timing=True)
         a0.record(); job5.step(); a1.record(); torch.cuda.synchronize(dev)
         c5 = summarize_pass(job5.stats_dict(), a0.elapsed_time(a1))
-        c5.update({"workload": f"{name5}: {desc5}", "anchors": len(w5.anchors), "window_k": K5, "cigar_for": "kept", "generation_s": tg,
+        c5.update({"workload": f"{name5}: {desc5}", "anchors": len(w5.anchors), "window_k": K5, "spec": args.spec, "speculate_info": sfe5.last_speculate_info(),
+                   "cigar_for": "kept", "generation_s": tg,
                    "path": "sfe_pack x2 -> sfe_speculate (phase 1 scan, phase 2 Y-drop windows, phase 3 commit, all on the device) "
                            "-> one traceback batch over the kept anchors; device-resident inputs, CUDA events"})
         t_host = torch.from_numpy(w5.target_ascii().copy()).pin_memory().numpy()
@@ -530,7 +536,7 @@ def main():
     line = {"metric": "ydrop_gcups", "value": gcups, "unit": "GCUPS", "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "window_k": window, "kernel": args.kernel, "cigar_for": "kept" if kept_only else ("all" if args.flags == "cigar" else "none"),
+            "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "window_k": window, "kernel": args.kernel, "spec": (args.spec if window > 0 else None), "cigar_for": "kept" if kept_only else ("all" if args.flags == "cigar" else "none"),
                        "l2": "inputs+traceback per step exceed L2 (126 MB)", "generation_s": t_gen,
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "scoring": "HOXD70/400/30/ydrop 9400/lag 32/tau 3000"},
             "kept_alignments_per_s": kept_step * args.steps * world / (ms * 1e-3),
@@ -539,7 +545,8 @@ def main():
             "speculation_waste": {"ext": 1.0 - (kept_step + st0["n_below"]) / st0["n_extended"] if st0["n_extended"] else None,
                                   "cells": st0["cells_covered"] / cells_step if cells_step else None},
             "gpu_launches": launches, "clocks": clocks, "e2e": e2e, "roofline": roof, "cpu_baseline": cpu, "c5_e2e": c5,
-            "batch_info": info0, "k_sweep": sweep or None, "lag0_fidelity": fidelity}
+            "batch_info": info0, "speculate_info": (sfe.last_speculate_info() if window > 0 and args.workload != "c4" else None),
+            "k_sweep": sweep or None, "lag0_fidelity": fidelity}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -53,6 +53,11 @@ enum {
                                          score and box only); CIGARs are produced for the KEPT anchors in one
                                          traceback batch at the end; other anchors get n_ops = 0, cigar_off = -1 */
 
+#define SFE_SPEC_LEADERS 32u          /* sfe_speculate: speculate on PREDICTED LEADERS instead of "the next K uncovered anchors":
+                                         an anchor that follows a close earlier anchor on (nearly) the same diagonal is not
+                                         extended unless the in-order commit reaches it uncovered; results per anchor are cached.
+                                         Same kept set / results as Algorithm 1 for any prediction; far less shadow work.     */
+
 /* per-anchor status bits (sfe_result.status) */
 #define SFE_ST_TB_OVERFLOW 1u         /* traceback arena exhausted even when run alone: no CIGAR */
 #define SFE_ST_CIGAR_OVERFLOW 2u      /* cigar pool too small: ops not written (n_ops is valid)   */
@@ -169,7 +174,10 @@ int sfe_resolve(sfe_ctx *ctx, const sfe_anchor *anchors_dev, const sfe_result *r
  * Algorithm 1's for every window_k >= 1 (R20, P7); window_k trades waste for parallelism.
  * results_dev / keep_dev have n_anchors entries in anchor order; CIGARs of all extended anchors go to the
  * pool (offsets grow window by window).  accepted_dev / n_accepted_dev as in sfe_resolve (boxes carried in
- * are honoured).  Synchronises the stream once per window (it reads the window size). */
+ * are honoured).  Synchronises the stream once per window (it reads the window size).
+ * With SFE_SPEC_LEADERS phase 1 picks predicted leaders (window_k = most extensions per batch; see the flag and
+ * sfe_set_option); anchors must then be sorted by target position within a pair for the prediction to be useful
+ * (any order is still exact). */
 int sfe_speculate(sfe_ctx *ctx, const uint8_t *t_codes2_dev, const uint8_t *t_nmask_dev, int64_t t_len,
                   const uint8_t *q_codes2_dev, const uint8_t *q_nmask_dev,
                   const uint8_t *qrc_codes2_dev, const uint8_t *qrc_nmask_dev, int64_t q_len,
@@ -179,6 +187,24 @@ int sfe_speculate(sfe_ctx *ctx, const uint8_t *t_codes2_dev, const uint8_t *t_nm
                   sfe_result *results_dev, uint8_t *keep_dev,
                   uint32_t *cigar_pool_dev, int64_t cigar_pool_cap, int64_t *cigar_pool_used_dev,
                   sfe_box *accepted_dev, int64_t accepted_cap, int64_t *n_accepted_dev, sfe_stats *stats_dev);
+
+/* Tunables of sfe_speculate with SFE_SPEC_LEADERS (defaults in brackets) and of chain-bound launches.  They change how much
+ * is extended and how it is scheduled, never a result.  sfe_set_option returns SFE_EINVAL for an unknown key / bad value. */
+enum {
+    SFE_OPT_LEADER_DIAG_TOL = 0,   /* [48]    follower: |diagonal - predecessor's diagonal| <= tol ...                              */
+    SFE_OPT_LEADER_GAP,            /* [2000]  ... and target distance to that predecessor <= gap ...                                */
+    SFE_OPT_LEADER_LOOKBACK,       /* [64]    ... among the previous `lookback` anchors (same strand, same pair) ...                */
+    SFE_OPT_LEADER_NBREAK,         /* [64]    ... with fewer than nbreak N between them in the target                               */
+    SFE_OPT_SPEC_SPAN,             /* [65536] look-ahead, in anchors beyond the commit cursor, in which leaders are extended        */
+    SFE_OPT_SPEC_ESC_MAX,          /* [64]    cap of the doubling number of anchors force-extended after repeated commit stops      */
+    SFE_OPT_SPARSE_WARPS,          /* [4]     resident warps per SM for sfe_speculate's leader batches (0 = the dense launch)       */
+    SFE_OPT_FORCE_CLASS,           /* [0]     testing: 1 = nobody leads, 2 = everybody leads, 3 = second half of the anchors never  */
+    SFE_OPT_N
+};
+int sfe_set_option(sfe_ctx *ctx, int key, int64_t value);
+/* counters of the most recent sfe_speculate with SFE_SPEC_LEADERS: [0] extension batches, [1] commit stops (the commit
+ * reached an anchor that was neither covered nor extended), [2] anchors force-extended after stops, [3..7] reserved. */
+int sfe_last_speculate_info(sfe_ctx *ctx, int64_t info[8]);
 
 /* End-to-end convenience with HOST buffers (bench.py's e2e leg): copies the ASCII sequences and
  * anchors to the device, packs, extends (flags as above), resolves in one window, copies

@@ -18,7 +18,9 @@ LIB_PATH = os.path.join(_HERE, "libsfe.so")
 OK, EINVAL, ENOMEM, ECUDA, ELIMIT = 0, -1, -2, -3, -4
 YDROP_INF = 0x7FFFFFFF
 PRUNE_LAG = 32
-WANT_CIGAR, SCORE_ONLY, NO_BINNING, BLOCK_KERNEL, NO_BLOCK_KERNEL, CIGAR_KEPT_ONLY = 1, 0, 2, 4, 8, 16
+WANT_CIGAR, SCORE_ONLY, NO_BINNING, BLOCK_KERNEL, NO_BLOCK_KERNEL, CIGAR_KEPT_ONLY, SPEC_LEADERS = 1, 0, 2, 4, 8, 16, 32
+(OPT_LEADER_DIAG_TOL, OPT_LEADER_GAP, OPT_LEADER_LOOKBACK, OPT_LEADER_NBREAK, OPT_SPEC_SPAN, OPT_SPEC_ESC_MAX, OPT_SPARSE_WARPS,
+ OPT_FORCE_CLASS) = range(8)
 ST_TB_OVERFLOW, ST_CIGAR_OVERFLOW, ST_WIDE, ST_SCORE_LIMIT, ST_BAD_ANCHOR, ST_BAND_LIMIT, ST_INTERNAL, ST_SKIPPED = 1, 2, 4, 8, 16, 32, 64, 128
 OP_M, OP_I, OP_D = 0, 1, 2
 INFO_N = 12
@@ -26,7 +28,7 @@ ST_SKEW2, ST_SKEW_RETRY, ST_BLOCK = 0x1000, 0x2000, 0x800      # profile-only bi
 
 EXPORTS = ("sfe_create", "sfe_destroy", "sfe_strerror", "sfe_last_error_detail", "sfe_pack", "sfe_ydrop_batch", "sfe_resolve",
            "sfe_speculate", "sfe_extend_host", "sfe_speculate_host", "sfe_probe_int_issue", "sfe_last_batch_info", "sfe_last_half_profile",
-           "sfe_launch_counter")
+           "sfe_launch_counter", "sfe_set_option", "sfe_last_speculate_info")
 
 
 class Scoring(C.Structure):
@@ -90,6 +92,8 @@ def lib():
                                             vp, vp, vp, i64, C.POINTER(i64), C.POINTER(Stats)]
         _lib.sfe_probe_int_issue.argtypes = [vp, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib.sfe_last_batch_info.argtypes = [vp, C.POINTER(i64)]
+        _lib.sfe_set_option.argtypes = [vp, C.c_int, i64]
+        _lib.sfe_last_speculate_info.argtypes = [vp, C.POINTER(i64)]
     return _lib
 
 
@@ -271,6 +275,14 @@ class Sfe:
         out = np.zeros(max(n_halves, 1), dtype=HALF_PROFILE_DT)
         _check(lib().sfe_last_half_profile(self.h, n_halves, C.c_void_p(out.ctypes.data)), "sfe_last_half_profile")
         return out[:n_halves]
+
+    def set_option(self, key: int, value: int):
+        _check(lib().sfe_set_option(self.h, key, value), "sfe_set_option")
+
+    def last_speculate_info(self):
+        a = (C.c_int64 * 8)()
+        _check(lib().sfe_last_speculate_info(self.h, a), "sfe_last_speculate_info")
+        return dict(batches=a[0], stops=a[1], forced=a[2])
 
     def last_batch_info(self):
         a = (C.c_int64 * INFO_N)()

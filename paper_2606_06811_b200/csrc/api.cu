@@ -19,7 +19,18 @@ int sfe_launch_resolve(const sfe_anchor *anchors, const sfe_result *results, lon
                        long long accepted_cap, long long *n_accepted_io, uint8_t *keep, sfe_stats *stats, long long *blkmin,
                        sfe_box *act, cudaStream_t st);
 int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe_pair *pairs, int n_pairs, long long q_len,
-                       bool binned, unsigned int *hist, int32_t *tickets, cudaStream_t st);
+                       bool binned, const uint8_t *prio, unsigned int *hist, int32_t *tickets, cudaStream_t st);
+int sfe_launch_specl_prepare(const sfe_anchor *anchors, long long n, const uint8_t *t_nmask, long long t_len, const uint8_t *q_nmask,
+                             const uint8_t *qrc_nmask, long long q_len, int tol, long long gap, int lookback, int n_break,
+                             uint8_t *cls, uint8_t *ext_state, long long *blkmin, void *state, const sfe_box *accepted,
+                             const long long *n_accepted, sfe_box *act, cudaStream_t st);
+int sfe_launch_spec_advance(void *state, const sfe_anchor *anchors, long long n, const long long *blkmin, long long K, long long span,
+                            int esc_max, const uint8_t *cls, uint8_t *ext_state, sfe_box *act, int min_score, sfe_box *accepted,
+                            long long accepted_cap, long long *win_idx, sfe_anchor *win_anchors, uint8_t *win_prio, uint8_t *keep,
+                            sfe_result *results, sfe_stats *stats, cudaStream_t st);
+int sfe_launch_spec_store(const sfe_result *wres, const long long *win_idx, long long wn, sfe_result *results, uint8_t *ext_state,
+                          cudaStream_t st);
+int sfe_launch_specl_finish(const void *state, long long *n_accepted_io, cudaStream_t st);
 int sfe_launch_select_overflow(const sfe_half *halves, long long n_anchors, long long *sel, int32_t *tickets,
                                unsigned long long *counters, int n_chunks, cudaStream_t st);
 int sfe_launch_probe(int mix, int iters, int blocks, int *sink, cudaStream_t st);
@@ -60,7 +71,10 @@ struct sfe_ctx {
     unsigned long long *counters_host;  // pinned
     DevBuf halves, tickets, sel, hist, blkmin, act, misc, wide_tickets, wide_ring, ops_stage;
     DevBuf sp_state, sp_idx, sp_anchors, sp_results, sp_local, sp_blkmin, sp_act, sp_kanchors, sp_kidx, sp_kres;   // sfe_speculate
-    long long *state_host;            // pinned, 8 words
+    DevBuf sp_cls, sp_ext, sp_prio;   // predicted leaders
+    long long opt[SFE_OPT_N];         // sfe_set_option
+    long long spec_info[8];           // sfe_last_speculate_info
+    long long *state_host;            // pinned, 16 words
     // host-API staging
     DevBuf h_tascii, h_qascii, h_t2, h_tm, h_q2, h_qm, h_r2, h_rm, h_pairs, h_anchors, h_results, h_keep, h_cigar, h_acc, h_small;
     long long info[SFE_INFO_N]; long long n_profile;
@@ -110,6 +124,10 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
     c->n_chunks = (int)nch;
     c->pool = nullptr; c->chunk_prev = nullptr; c->free_ring = nullptr; c->ring_state = nullptr; c->counters = nullptr; c->counters_host = nullptr; c->state_host = nullptr;
     memset(c->info, 0, sizeof c->info);
+    memset(c->spec_info, 0, sizeof c->spec_info);
+    c->opt[SFE_OPT_LEADER_DIAG_TOL] = 48; c->opt[SFE_OPT_LEADER_GAP] = 2000; c->opt[SFE_OPT_LEADER_LOOKBACK] = 64;
+    c->opt[SFE_OPT_LEADER_NBREAK] = 64; c->opt[SFE_OPT_SPEC_SPAN] = 65536; c->opt[SFE_OPT_SPEC_ESC_MAX] = 64;
+    c->opt[SFE_OPT_SPARSE_WARPS] = 4; c->opt[SFE_OPT_FORCE_CLASS] = 0;
     c->ev_pending = false; c->kernel_us = 0.0; c->n_profile = 0;
     if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) { delete c; return SFE_ECUDA; }
     if (cudaMalloc((void **)&c->pool, (size_t)nch * SFE_CHUNK_BYTES) != cudaSuccess ||
@@ -118,7 +136,7 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
         cudaMalloc((void **)&c->ring_state, sizeof(SfeFreeRing)) != cudaSuccess ||
         cudaMalloc((void **)&c->counters, CNT_N * sizeof(unsigned long long)) != cudaSuccess ||
         cudaMallocHost((void **)&c->counters_host, CNT_N * sizeof(unsigned long long)) != cudaSuccess ||
-        cudaMallocHost((void **)&c->state_host, 8 * sizeof(long long)) != cudaSuccess) {
+        cudaMallocHost((void **)&c->state_host, 16 * sizeof(long long)) != cudaSuccess) {
         cudaGetLastError();
         sfe_destroy(c);
         return SFE_ENOMEM;
@@ -141,7 +159,7 @@ extern "C" int sfe_destroy(sfe_ctx *c)
     if (c->counters_host) cudaFreeHost(c->counters_host);
     if (c->state_host) cudaFreeHost(c->state_host);
     cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1);
-    DevBuf *bufs[] = {&c->sp_kanchors, &c->sp_kidx, &c->sp_kres, &c->sp_state, &c->sp_idx, &c->sp_anchors, &c->sp_results, &c->sp_local, &c->sp_blkmin, &c->sp_act, &c->ops_stage, &c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
+    DevBuf *bufs[] = {&c->sp_cls, &c->sp_ext, &c->sp_prio, &c->sp_kanchors, &c->sp_kidx, &c->sp_kres, &c->sp_state, &c->sp_idx, &c->sp_anchors, &c->sp_results, &c->sp_local, &c->sp_blkmin, &c->sp_act, &c->ops_stage, &c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
                       &c->h_t2, &c->h_tm, &c->h_q2, &c->h_qm, &c->h_r2, &c->h_rm, &c->h_pairs, &c->h_anchors, &c->h_results,
                       &c->h_keep, &c->h_cigar, &c->h_acc, &c->h_small};
     for (DevBuf *b : bufs) b->release();
@@ -183,6 +201,23 @@ extern "C" int sfe_probe_int_issue(sfe_ctx *c, int mix, int iters, double *lane_
     const double cycles = (double)ms * 1e-3 * (double)c->clock_khz * 1e3;
     *lane_ops_per_clk_per_sm = lane_ops / cycles / (double)c->n_sm;
     if (elapsed_ms) *elapsed_ms = ms;
+    return SFE_OK;
+}
+
+extern "C" int sfe_set_option(sfe_ctx *c, int key, int64_t value)
+{
+    if (!c || key < 0 || key >= SFE_OPT_N || value < 0) return SFE_EINVAL;
+    if ((key == SFE_OPT_SPEC_SPAN || key == SFE_OPT_SPEC_ESC_MAX || key == SFE_OPT_LEADER_LOOKBACK) && value < 1) return SFE_EINVAL;
+    if (key == SFE_OPT_SPARSE_WARPS && value > 16) return SFE_EINVAL;
+    if (key == SFE_OPT_FORCE_CLASS && value > 3) return SFE_EINVAL;
+    c->opt[key] = (long long)value;
+    return SFE_OK;
+}
+
+extern "C" int sfe_last_speculate_info(sfe_ctx *c, int64_t info[8])
+{
+    if (!c || !info) return SFE_EINVAL;
+    for (int k = 0; k < 8; k++) info[k] = c->spec_info[k];
     return SFE_OK;
 }
 
@@ -268,7 +303,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
                             const uint8_t *qrc_nmask, int64_t q_len, const sfe_pair *pairs_dev, int32_t n_pairs,
                             const sfe_anchor *anchors_dev, int64_t n_anchors, const sfe_scoring *sc, uint32_t flags,
                             sfe_result *results_dev, uint32_t *cigar_pool_dev, int64_t cigar_pool_cap,
-                            int64_t *cigar_pool_used_dev, bool first_of_series)
+                            int64_t *cigar_pool_used_dev, bool first_of_series, const uint8_t *prio_dev = nullptr, int sparse_warps = 0)
 {
     if (!c || n_anchors < 0 || t_len < 0 || q_len < 0 || n_pairs < 0) return SFE_EINVAL;
     int rc = check_scoring(sc, flags);
@@ -288,7 +323,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
 
     if ((rc = c->halves.ensure((size_t)(2 * n_anchors) * sizeof(sfe_half)))) return rc;
     if ((rc = c->tickets.ensure((size_t)(2 * n_anchors) * sizeof(int32_t)))) return rc;
-    if ((rc = c->hist.ensure(64 * sizeof(unsigned int)))) return rc;
+    if ((rc = c->hist.ensure(128 * sizeof(unsigned int)))) return rc;
     if ((rc = c->wide_tickets.ensure((size_t)(2 * n_anchors) * sizeof(int32_t)))) return rc;
     if ((rc = c->wide_ring.ensure((size_t)SFE_WIDE_WARPS * RingGeom<SFE_WIDE_RING_LOG2>::WARP_BYTES))) return rc;
     if (want_tb && (rc = c->sel.ensure((size_t)n_anchors * sizeof(long long)))) return rc;
@@ -305,7 +340,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
     p.qrc_codes = qrc_codes2; p.qrc_nmask = qrc_nmask; p.t_len = t_len; p.q_len = q_len;
     p.pairs = pairs_dev; p.anchors = anchors_dev; p.tickets = (const int32_t *)c->tickets.p; p.n_tickets = 2 * n_anchors; p.seg_tickets = (flags & SFE_NO_BINNING) ? 0 : 4LL * c->n_sm;
     p.counters = c->counters; p.halves = (sfe_half *)c->halves.p; p.pool = c->pool; p.chunk_prev = c->chunk_prev; p.free_ring = c->free_ring; p.ring_state = c->ring_state;
-    p.n_chunks = want_tb ? c->n_chunks : 0; p.n_pairs = n_pairs; p.max_warps = 0x7fffffff;
+    p.n_chunks = want_tb ? c->n_chunks : 0; p.n_pairs = n_pairs; p.max_warps = 0x7fffffff; p.sparse_warps = sparse_warps;
     p.wide_ring = (char *)c->wide_ring.p; p.wide_tickets = (int32_t *)c->wide_tickets.p;
     p.ops_stage = (uint32_t *)c->ops_stage.p; p.ops_cap = ops_cap;
     p.OX = sc->gap_open + sc->gap_extend; p.X = sc->gap_extend;
@@ -320,7 +355,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
     p.srow_hi = (uint32_t)(uint8_t)(int8_t)sc->n_score | (0xE0u << 16);
 
     SFE_CUDA_CHECK(cudaMemsetAsync(c->counters, 0, CNT_N * sizeof(unsigned long long), c->stream));
-    if ((rc = sfe_launch_tickets(anchors_dev, n_anchors, pairs_dev, n_pairs, q_len, !(flags & SFE_NO_BINNING),
+    if ((rc = sfe_launch_tickets(anchors_dev, n_anchors, pairs_dev, n_pairs, q_len, !(flags & SFE_NO_BINNING), prio_dev,
                                  (unsigned int *)c->hist.p, (int32_t *)c->tickets.p, c->stream))) return rc;
     if ((rc = timed_ydrop(c, p, want_tb, flags))) return rc;
     c->info[0] += 1; c->info[1] += 2 * n_anchors; c->n_profile = 2 * n_anchors;
@@ -401,6 +436,47 @@ extern "C" int sfe_speculate(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t 
     const bool kept_only = (flags & SFE_CIGAR_KEPT_ONLY) && (flags & SFE_WANT_CIGAR);
     const uint32_t flags2 = kept_only ? (flags & ~SFE_WANT_CIGAR) : flags;
     const long long K = window_k < n_anchors ? window_k : n_anchors;
+    memset(c->spec_info, 0, sizeof c->spec_info);
+    if (flags & SFE_SPEC_LEADERS) {
+        // ---- Algorithm 3 with predicted leaders (resolve_kernel.cu): classify once, then advance / extend until done ----
+        if (!t_nmask || !q_nmask) return SFE_EINVAL;
+        if ((rc = c->sp_state.ensure(128)) || (rc = c->sp_idx.ensure((size_t)K * sizeof(long long))) ||
+            (rc = c->sp_anchors.ensure((size_t)K * sizeof(sfe_anchor))) || (rc = c->sp_results.ensure((size_t)K * sizeof(sfe_result))) ||
+            (rc = c->sp_prio.ensure((size_t)K)) || (rc = c->sp_cls.ensure((size_t)n_anchors)) || (rc = c->sp_ext.ensure((size_t)n_anchors)) ||
+            (rc = c->sp_blkmin.ensure((size_t)((n_anchors + 31) / 32 + 32) * sizeof(long long))) ||
+            (rc = c->sp_act.ensure((size_t)(n_anchors + accepted_cap + 1) * sizeof(sfe_box)))) return rc;
+        long long *blkmin = (long long *)c->sp_blkmin.p;
+        sfe_box *act = (sfe_box *)c->sp_act.p;
+        uint8_t *cls = (uint8_t *)c->sp_cls.p, *ext = (uint8_t *)c->sp_ext.p;
+        if ((rc = sfe_launch_specl_prepare(anchors_dev, n_anchors, t_nmask, t_len, q_nmask, qrc_nmask, q_len, (int)c->opt[SFE_OPT_LEADER_DIAG_TOL],
+                                           c->opt[SFE_OPT_LEADER_GAP], (int)c->opt[SFE_OPT_LEADER_LOOKBACK], (int)c->opt[SFE_OPT_LEADER_NBREAK],
+                                           cls, ext, blkmin, c->sp_state.p, accepted_dev, (const long long *)n_accepted_dev, act, c->stream))) return rc;
+        if (c->opt[SFE_OPT_FORCE_CLASS] == 1) SFE_CUDA_CHECK(cudaMemsetAsync(cls, 0, (size_t)n_anchors, c->stream));        // testing: nobody leads
+        else if (c->opt[SFE_OPT_FORCE_CLASS] == 2) SFE_CUDA_CHECK(cudaMemsetAsync(cls, 1, (size_t)n_anchors, c->stream));   // everybody leads
+        else if (c->opt[SFE_OPT_FORCE_CLASS] == 3) SFE_CUDA_CHECK(cudaMemsetAsync(cls + n_anchors / 2, 0, (size_t)(n_anchors - n_anchors / 2), c->stream));
+        long long n_batches = 0;
+        for (;;) {
+            if ((rc = sfe_launch_spec_advance(c->sp_state.p, anchors_dev, n_anchors, blkmin, K, c->opt[SFE_OPT_SPEC_SPAN], (int)c->opt[SFE_OPT_SPEC_ESC_MAX],
+                                              cls, ext, act, sc->min_score, accepted_dev, accepted_cap, (long long *)c->sp_idx.p,
+                                              (sfe_anchor *)c->sp_anchors.p, (uint8_t *)c->sp_prio.p, keep_dev, results_dev, stats_dev, c->stream))) return rc;
+            SFE_CUDA_CHECK(cudaMemcpyAsync(c->state_host, c->sp_state.p, 10 * sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
+            SFE_CUDA_CHECK(cudaStreamSynchronize(c->stream));
+            const long long cursor = c->state_host[0], wn = c->state_host[1];
+            c->spec_info[0] = n_batches; c->spec_info[1] = c->state_host[9]; c->spec_info[2] = c->state_host[8];
+            if (wn <= 0) {
+                if (cursor < n_anchors) return SFE_ECUDA;            // cannot happen: a stop always queues the anchor it stopped at
+                break;
+            }
+            if ((rc = ydrop_batch_impl(c, t_codes2, t_nmask, t_len, q_codes2, q_nmask, qrc_codes2, qrc_nmask, q_len, pairs_dev, n_pairs,
+                                       (const sfe_anchor *)c->sp_anchors.p, wn, sc, flags2, (sfe_result *)c->sp_results.p,
+                                       cigar_pool_dev, cigar_pool_cap, cigar_pool_used_dev, false, (const uint8_t *)c->sp_prio.p,
+                                       (int)c->opt[SFE_OPT_SPARSE_WARPS]))) return rc;
+            harvest_kernel_time(c);
+            if ((rc = sfe_launch_spec_store((const sfe_result *)c->sp_results.p, (const long long *)c->sp_idx.p, wn, results_dev, ext, c->stream))) return rc;
+            n_batches++;
+        }
+        if ((rc = sfe_launch_specl_finish(c->sp_state.p, (long long *)n_accepted_dev, c->stream))) return rc;
+    } else {
     if ((rc = c->sp_state.ensure(64)) || (rc = c->sp_idx.ensure((size_t)K * sizeof(long long))) ||
         (rc = c->sp_anchors.ensure((size_t)K * sizeof(sfe_anchor))) || (rc = c->sp_results.ensure((size_t)K * sizeof(sfe_result))) ||
         (rc = c->sp_local.ensure((size_t)(K + 1) * sizeof(sfe_box))) ||
@@ -426,6 +502,7 @@ extern "C" int sfe_speculate(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t 
                                          (sfe_box *)c->sp_local.p, keep_dev, results_dev, stats_dev, c->stream))) return rc;
     }
     if ((rc = sfe_launch_spec_finish(c->sp_state.p, (long long *)n_accepted_dev, c->stream))) return rc;
+    }
     if (!kept_only) return SFE_OK;
     if ((rc = c->sp_kanchors.ensure((size_t)n_anchors * sizeof(sfe_anchor))) || (rc = c->sp_kidx.ensure((size_t)n_anchors * sizeof(long long)))) return rc;
     long long *d_nk = (long long *)((char *)c->sp_state.p + 48);

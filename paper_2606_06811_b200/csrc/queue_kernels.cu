@@ -22,30 +22,33 @@ static __device__ __forceinline__ int half_bin(const sfe_anchor &an, const sfe_p
     return 31 - __clz((int)v + 1);                   // 0..30
 }
 
+// prio (may be NULL): one byte per anchor; anchors flagged long-likely by the caller (sfe_speculate's predicted leaders
+// with followers) go into the upper 32 bins, i.e. before everybody else, whatever their distance to the pair's end --
+// in a genome-scale pair that distance says nothing (every anchor is "far from the end").
 __global__ void bin_count_kernel(const sfe_anchor *anchors, long long n_anchors, const sfe_pair *pairs, int n_pairs,
-                                 long long q_len, unsigned int *hist)
+                                 long long q_len, const uint8_t *prio, unsigned int *hist)
 {
     const long long h = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (h >= 2 * n_anchors) return;
-    atomicAdd(&hist[half_bin(anchors[h >> 1], pairs, n_pairs, q_len, (int)(h & 1))], 1u);
+    atomicAdd(&hist[half_bin(anchors[h >> 1], pairs, n_pairs, q_len, (int)(h & 1)) + ((prio && prio[h >> 1]) ? 32 : 0)], 1u);
 }
 
-// hist[0..31] -> hist[32..63] = start offset of each bin in descending-bin order
+// hist[0..63] -> hist[64..127] = start offset of each bin in descending-bin order
 __global__ void bin_offsets_kernel(unsigned int *hist)
 {
     if (threadIdx.x == 0) {
         unsigned int off = 0;
-        for (int b = 31; b >= 0; b--) { hist[32 + b] = off; off += hist[b]; }
+        for (int b = 63; b >= 0; b--) { hist[64 + b] = off; off += hist[b]; }
     }
 }
 
 __global__ void bin_scatter_kernel(const sfe_anchor *anchors, long long n_anchors, const sfe_pair *pairs, int n_pairs,
-                                   long long q_len, unsigned int *hist, int32_t *tickets)
+                                   long long q_len, const uint8_t *prio, unsigned int *hist, int32_t *tickets)
 {
     const long long h = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (h >= 2 * n_anchors) return;
-    const int b = half_bin(anchors[h >> 1], pairs, n_pairs, q_len, (int)(h & 1));
-    tickets[atomicAdd(&hist[32 + b], 1u)] = (int32_t)h;
+    const int b = half_bin(anchors[h >> 1], pairs, n_pairs, q_len, (int)(h & 1)) + ((prio && prio[h >> 1]) ? 32 : 0);
+    tickets[atomicAdd(&hist[64 + b], 1u)] = (int32_t)h;
 }
 
 __global__ void iota_tickets_kernel(int32_t *tickets, long long n)
@@ -55,7 +58,7 @@ __global__ void iota_tickets_kernel(int32_t *tickets, long long n)
 }
 
 int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe_pair *pairs, int n_pairs, long long q_len,
-                       bool binned, unsigned int *hist, int32_t *tickets, cudaStream_t st)
+                       bool binned, const uint8_t *prio, unsigned int *hist, int32_t *tickets, cudaStream_t st)
 {
     const long long n = 2 * n_anchors;
     if (n <= 0) return SFE_OK;
@@ -63,10 +66,10 @@ int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe
     const unsigned nb = (unsigned)((n + bs - 1) / bs);
     if (!binned) SFE_KL iota_tickets_kernel<<<nb, bs, 0, st>>>(tickets, n);
     else {
-        if (cudaMemsetAsync(hist, 0, 64 * sizeof(unsigned int), st) != cudaSuccess) return SFE_ECUDA;
-        SFE_KL bin_count_kernel<<<nb, bs, 0, st>>>(anchors, n_anchors, pairs, n_pairs, q_len, hist);
+        if (cudaMemsetAsync(hist, 0, 128 * sizeof(unsigned int), st) != cudaSuccess) return SFE_ECUDA;
+        SFE_KL bin_count_kernel<<<nb, bs, 0, st>>>(anchors, n_anchors, pairs, n_pairs, q_len, prio, hist);
         SFE_KL bin_offsets_kernel<<<1, 32, 0, st>>>(hist);
-        SFE_KL bin_scatter_kernel<<<nb, bs, 0, st>>>(anchors, n_anchors, pairs, n_pairs, q_len, hist, tickets);
+        SFE_KL bin_scatter_kernel<<<nb, bs, 0, st>>>(anchors, n_anchors, pairs, n_pairs, q_len, prio, hist, tickets);
     }
     SFE_LAUNCH_CHECK();
 }

@@ -434,3 +434,306 @@ int sfe_launch_spec_finish(const void *state, long long *n_accepted_io, cudaStre
     SFE_KL spec_finish_kernel<<<1, 32, 0, st>>>((const SpecState *)state, n_accepted_io);
     SFE_LAUNCH_CHECK();
 }
+
+// =====================================================================================================
+// Algorithm 3 with PREDICTED LEADERS (SFE_SPEC_LEADERS): the same in-order commit, a smarter phase 1.
+//
+// Algorithm 3 takes "the next K unmasked seeds" as its batch.  In the dense-anchor regimes the
+// paper is about, almost all of those lie on the diagonal of the batch's first alignment and are thrown away in phase 3
+// (shadow work) -- after each of them has cost one full-length extension.  Which anchors are speculated on
+// is a free choice as long as phase 3 stays in order: an anchor may be DECIDED only when every earlier anchor is, and it
+// is decided either because a kept box covers it (no extension needed: Algorithm 1 would not extend it either) or because
+// its extension is available.  So:
+//   classify  (parallel, once)   an anchor is a FOLLOWER if a close earlier anchor of the same strand lies on (nearly) the
+//                                same diagonal with no N run in between -- it will most likely be covered by that
+//                                anchor's alignment -- else a LEADER; leaders with followers right behind them are
+//                                flagged long-likely (their tickets are issued first);
+//   advance   (one warp)         commit from the cursor in anchor order using the results cached so far; STOP at the
+//                                first anchor that is neither covered nor extended; then build the next batch: that
+//                                anchor (plus a doubling number of its successors after repeated stops in one region: a
+//                                mispredicted stretch costs O(log) batches) and every not yet extended leader in the
+//                                look-ahead span;
+//   extend    (sfe_ydrop_batch)  results are cached per anchor: nothing is ever extended twice;
+// until the cursor reaches the end.  The kept set, scores, boxes and CIGARs are Algorithm 1's for ANY classification
+// (tests run it with adversarial ones); the classification only decides how much is extended and how many batches it takes.
+// =====================================================================================================
+struct SpecLState { long long cursor, win_n, nact, nacc, overflow, spec_hi, esc, last_stop, n_forced, n_stops; };
+
+enum { CLS_FOLLOWER = 0, CLS_LEADER = 1, CLS_LEADER_LONG = 2 };
+
+static __device__ __forceinline__ bool is_n_at(const uint8_t *nmask, long long k, long long len)
+{
+    return k >= 0 && k < len && ((nmask[k >> 3] >> (k & 7)) & 1);
+}
+
+// number of N among target bases [a, b)
+static __device__ long long count_n(const uint8_t *nmask, long long a, long long b)
+{
+    long long c = 0;
+    for (long long k = a; k < b;) {
+        if ((k & 7) == 0 && k + 8 <= b) { c += __popc((unsigned)nmask[k >> 3]); k += 8; }
+        else { c += (nmask[k >> 3] >> (k & 7)) & 1; k++; }
+    }
+    return c;
+}
+
+__global__ void spec_classify_kernel(const sfe_anchor *anchors, long long n, const uint8_t *t_nmask, long long t_len,
+                                     const uint8_t *q_nmask, const uint8_t *qrc_nmask, long long q_len, int tol, long long gap,
+                                     int lookback, int n_break, uint8_t *cls)
+{
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const sfe_anchor a = anchors[i];
+    const int strand = a.strand >= 0 ? 1 : -1;
+    const uint8_t *qm = strand > 0 ? q_nmask : qrc_nmask;
+    auto dead_end = [&](const sfe_anchor &x) {              // both first diagonal cells pair with an N: both halves die at once
+        const uint8_t *m = x.strand >= 0 ? q_nmask : qrc_nmask;
+        if (!m) return false;
+        const bool f = is_n_at(t_nmask, x.tpos, t_len) || is_n_at(m, x.qpos, q_len);
+        const bool b = is_n_at(t_nmask, x.tpos - 1, t_len) || is_n_at(m, x.qpos - 1, q_len);
+        return f && b;
+    };
+    uint8_t c = CLS_LEADER;
+    if (qm && dead_end(a)) { cls[i] = CLS_LEADER; return; }
+    const long long diag = a.tpos - a.qpos;
+    for (long long j = i - 1; j >= 0 && j >= i - lookback; j--) {
+        const sfe_anchor p = anchors[j];
+        if (a.tpos - p.tpos > gap) break;                   // anchors are in target order (any other order: everybody leads)
+        if (a.tpos < p.tpos) break;
+        if ((p.strand >= 0 ? 1 : -1) != strand || p.pair != a.pair) continue;
+        const long long dd = (p.tpos - p.qpos) - diag;
+        if (dd > tol || dd < -tol) continue;
+        if (dead_end(p)) continue;
+        if (count_n(t_nmask, p.tpos, a.tpos) >= n_break) break;
+        c = CLS_FOLLOWER;
+        break;
+    }
+    if (c == CLS_LEADER) {                                  // long-likely: a follower-to-be right behind it
+        for (long long j = i + 1; j < n && j <= i + lookback; j++) {
+            const sfe_anchor p = anchors[j];
+            if (p.tpos - a.tpos > gap || p.tpos < a.tpos) break;
+            if ((p.strand >= 0 ? 1 : -1) != strand || p.pair != a.pair) continue;
+            const long long dd = (p.tpos - p.qpos) - diag;
+            if (dd <= tol && dd >= -tol) { c = CLS_LEADER_LONG; break; }
+        }
+    }
+    cls[i] = c;
+}
+
+__global__ void specl_init_kernel(SpecLState *st, const sfe_box *accepted, const long long *n_accepted, sfe_box *act)
+{
+    const int lane = threadIdx.x & 31;
+    const long long nacc = *n_accepted;
+    for (long long k = lane; k < nacc; k += 32) act[k] = accepted[k];
+    if (lane == 0) { st->cursor = 0; st->win_n = 0; st->nact = nacc; st->nacc = nacc; st->overflow = 0; st->spec_hi = 0; st->esc = 1;
+                     st->last_stop = -1; st->n_forced = 0; st->n_stops = 0; }
+}
+
+// ext_state[i]: 0 = not extended, 1 = extended (results[i] holds it), 2 = queued in the batch being built
+// single warp
+__global__ void spec_advance_kernel(SpecLState *st, const sfe_anchor *anchors, long long n, const long long *blkmin, long long K,
+                                    long long span, int esc_max, const uint8_t *cls, uint8_t *ext_state, sfe_box *act,
+                                    int min_score, sfe_box *accepted, long long accepted_cap, long long *win_idx,
+                                    sfe_anchor *win_anchors, uint8_t *win_prio, uint8_t *keep, sfe_result *results, sfe_stats *stats)
+{
+    const int lane = threadIdx.x & 31;
+    long long j = st->cursor, nact = st->nact, nacc = st->nacc;
+    long long c_kept = 0, c_cov = 0, c_below = 0, c_dec = 0;
+    unsigned long long cells_tot = 0, cells_cov = 0;
+    bool overflow = false, stopped = false;
+    // ---- phase 3, in order, as far as the cached extensions reach ----
+    while (j < n && !stopped) {
+        const long long blk = j >> 5;
+        nact = retire_boxes(act, nact, blkmin[blk], lane);
+        const long long i = (blk << 5) + lane;
+        const bool valid = i >= j && i < n;
+        long long tp = 0, qp = 0; int strand = 0, score = 0; unsigned long long cells = 0; bool ext = false;
+        sfe_box mine; mine.tstart = mine.tend = mine.qstart = mine.qend = 0; mine.strand = 0; mine.reserved = 0;
+        if (valid) {
+            const sfe_anchor an = anchors[i];
+            tp = an.tpos; qp = an.qpos; strand = an.strand >= 0 ? 1 : -1;
+            ext = ext_state[i] == 1;
+            if (ext) {
+                const sfe_result r = results[i];
+                score = r.score; cells = r.cells;
+                mine.tstart = r.tstart; mine.tend = r.tend; mine.qstart = r.qstart; mine.qend = r.qend; mine.strand = strand;
+            }
+        }
+        bool cov = false;
+        for (long long k = 0; k < nact; k++) { const sfe_box b = act[k]; cov = cov || box_has(b, tp, qp, strand); }
+        cov = cov && valid;
+        const bool live = valid && !cov, cand = live && ext && score >= min_score;
+        const unsigned kmask_all = decide_block(valid, live, cand, cov, mine, tp, qp, strand, lane);
+        // the first anchor that is neither covered nor extended cannot be decided: everything from there on waits
+        const unsigned stopm = __ballot_sync(FULL, valid && !cov && !ext);
+        const int stop_lane = stopm ? __ffs(stopm) - 1 : 32;
+        const unsigned below_stop = stop_lane >= 32 ? 0xffffffffu : ((1u << stop_lane) - 1u);
+        const unsigned kmask = kmask_all & below_stop;
+        const bool decided = valid && lane < stop_lane;
+        const bool kept = (kmask >> lane) & 1u;
+        if (kept) {
+            const long long r = __popc(kmask & ((1u << lane) - 1));
+            act[nact + r] = mine;
+            if (nacc + r < accepted_cap) accepted[nacc + r] = mine;
+        }
+        {
+            const long long nk = __popc(kmask);
+            if (nacc + nk > accepted_cap) overflow = true;
+            nact += nk; nacc += nk;
+        }
+        __syncwarp();
+        if (decided) {
+            keep[i] = cov ? 0 : (kept ? 1 : 2);
+            if (!ext) {                                       // covered before anybody extended it: as in Algorithm 1
+                sfe_result r; r.score = r.score_fwd = r.score_bwd = 0; r.status = SFE_ST_SKIPPED;
+                r.tstart = r.tend = tp; r.qstart = r.qend = qp; r.cigar_off = -1; r.n_ops = r.n_ops_back = 0; r.cells = 0;
+                results[i] = r;
+            }
+            c_dec++; c_kept += kept; c_cov += cov; c_below += (!cov && !kept);
+            cells_tot += cells; if (cov) cells_cov += cells;
+        }
+        stopped = stop_lane < 32;
+        j = stopped ? (blk << 5) + stop_lane : (((blk + 1) << 5) < n ? ((blk + 1) << 5) : n);
+    }
+    // ---- the next batch: the anchor(s) the commit waits for, then every leader of the look-ahead span ----
+    long long esc = st->esc, last_stop = st->last_stop, n_forced = 0;
+    if (stopped) {
+        esc = (last_stop >= 0 && j - last_stop <= 4096) ? (2 * esc < esc_max ? 2 * esc : esc_max) : 1;
+        last_stop = j;
+    }
+    long long wn = 0;
+    if (j < n) {
+        // forced: the first `esc` not-extended anchors from the cursor that no active box covers
+        long long want = stopped ? esc : 0;
+        for (long long p = j; p < n && want > 0 && wn < K && p < j + 8192; ) {
+            const long long blk = p >> 5;
+            const long long i = (blk << 5) + lane;
+            const bool valid = i >= p && i < n;
+            sfe_anchor an; an.tpos = an.qpos = 0; an.pair = 0; an.strand = 1;
+            bool take = false;
+            if (valid) {
+                an = anchors[i];
+                take = ext_state[i] == 0;
+            }
+            bool cov = false;
+            const int strand = an.strand >= 0 ? 1 : -1;
+            for (long long k = 0; k < nact; k++) { const sfe_box b = act[k]; cov = cov || box_has(b, an.tpos, an.qpos, strand); }
+            take = take && !cov;
+            unsigned m = __ballot_sync(FULL, take);
+            const long long room = (want < K - wn) ? want : (K - wn);
+            while ((long long)__popc(m) > room) m &= ~(0x80000000u >> __clz(m));     // drop the highest lanes
+            if ((m >> lane) & 1u) {
+                const long long d = wn + __popc(m & ((1u << lane) - 1));
+                win_idx[d] = i; win_anchors[d] = an; win_prio[d] = 1; ext_state[i] = 2;
+            }
+            const long long got = __popc(m);
+            wn += got; want -= got; n_forced += got;
+            p = ((blk + 1) << 5);
+        }
+        // speculative: leaders of [max(spec_hi, cursor), cursor + span) that are not extended yet
+        long long p = st->spec_hi > j ? st->spec_hi : j;
+        const long long hi = (j + span < n) ? j + span : n;
+        while (p < hi && wn < K) {
+            const long long blk = p >> 5;
+            const long long i = (blk << 5) + lane;
+            const bool valid = i >= p && i < hi;
+            sfe_anchor an; an.tpos = an.qpos = 0; an.pair = 0; an.strand = 1;
+            bool take = false; uint8_t c = 0;
+            if (valid) {
+                c = cls[i];
+                if (c != CLS_FOLLOWER && ext_state[i] == 0) { an = anchors[i]; take = true; }
+            }
+            if (__any_sync(FULL, take)) {
+                bool cov = false;
+                const int strand = an.strand >= 0 ? 1 : -1;
+                for (long long k = 0; k < nact; k++) { const sfe_box b = act[k]; cov = cov || box_has(b, an.tpos, an.qpos, strand); }
+                take = take && !cov;
+            }
+            unsigned m = __ballot_sync(FULL, take);
+            long long next_p = ((blk + 1) << 5) < hi ? ((blk + 1) << 5) : hi;
+            if ((long long)__popc(m) > K - wn) {                  // the batch is full: stop inside this block
+                unsigned keepm = 0; long long room = K - wn;
+                for (unsigned mm = m; mm && room > 0; mm &= mm - 1, room--) keepm |= mm & (0u - mm);
+                const int last = 31 - __clz(keepm);
+                next_p = (blk << 5) + last + 1;
+                m = keepm;
+            }
+            if ((m >> lane) & 1u) {
+                const long long d = wn + __popc(m & ((1u << lane) - 1));
+                win_idx[d] = i; win_anchors[d] = an; win_prio[d] = c == CLS_LEADER_LONG ? 1 : 0; ext_state[i] = 2;
+            }
+            wn += __popc(m);
+            p = next_p;
+        }
+        if (lane == 0) st->spec_hi = p;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        c_kept += __shfl_xor_sync(FULL, c_kept, o); c_cov += __shfl_xor_sync(FULL, c_cov, o);
+        c_below += __shfl_xor_sync(FULL, c_below, o); c_dec += __shfl_xor_sync(FULL, c_dec, o);
+        cells_tot += __shfl_xor_sync(FULL, cells_tot, o); cells_cov += __shfl_xor_sync(FULL, cells_cov, o);
+    }
+    if (lane == 0) {
+        st->cursor = j; st->win_n = wn; st->nact = nact; st->nacc = nacc; if (overflow) st->overflow = 1;
+        st->esc = esc; st->last_stop = last_stop; st->n_forced += n_forced; st->n_stops += stopped ? 1 : 0;
+        if (stats) {
+            stats->n_anchors += c_dec; stats->n_kept += c_kept; stats->n_covered += c_cov; stats->n_below += c_below;
+            stats->cells_total += cells_tot; stats->cells_covered += cells_cov;
+            stats->n_extended += wn; if (wn > 0) stats->n_windows += 1;
+        }
+    }
+}
+
+// cache the batch's results per anchor (anchor order) and mark them extended
+__global__ void spec_store_kernel(const sfe_result *wres, const long long *win_idx, long long wn, sfe_result *results, uint8_t *ext_state)
+{
+    const long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (k >= wn) return;
+    const long long i = win_idx[k];
+    results[i] = wres[k];
+    ext_state[i] = 1;
+}
+
+__global__ void specl_finish_kernel(const SpecLState *st, long long *n_accepted_io)
+{
+    if (threadIdx.x == 0) *n_accepted_io = st->overflow ? -st->nacc : st->nacc;
+}
+
+int sfe_launch_specl_prepare(const sfe_anchor *anchors, long long n, const uint8_t *t_nmask, long long t_len, const uint8_t *q_nmask,
+                             const uint8_t *qrc_nmask, long long q_len, int tol, long long gap, int lookback, int n_break,
+                             uint8_t *cls, uint8_t *ext_state, long long *blkmin, void *state, const sfe_box *accepted,
+                             const long long *n_accepted, sfe_box *act, cudaStream_t st)
+{
+    const int bs = 256;
+    const unsigned nb = (unsigned)((n + bs - 1) / bs);
+    SFE_KL block_min_kernel<<<nb, bs, 0, st>>>(anchors, n, blkmin);
+    SFE_KL suffix_min_kernel<<<1, 32, 0, st>>>(blkmin, (n + 31) >> 5);
+    SFE_KL spec_classify_kernel<<<nb, bs, 0, st>>>(anchors, n, t_nmask, t_len, q_nmask, qrc_nmask, q_len, tol, gap, lookback, n_break, cls);
+    if (cudaMemsetAsync(ext_state, 0, (size_t)n, st) != cudaSuccess) return SFE_ECUDA;
+    SFE_KL specl_init_kernel<<<1, 32, 0, st>>>((SpecLState *)state, accepted, n_accepted, act);
+    SFE_LAUNCH_CHECK();
+}
+
+int sfe_launch_spec_advance(void *state, const sfe_anchor *anchors, long long n, const long long *blkmin, long long K, long long span,
+                            int esc_max, const uint8_t *cls, uint8_t *ext_state, sfe_box *act, int min_score, sfe_box *accepted,
+                            long long accepted_cap, long long *win_idx, sfe_anchor *win_anchors, uint8_t *win_prio, uint8_t *keep,
+                            sfe_result *results, sfe_stats *stats, cudaStream_t st)
+{
+    SFE_KL spec_advance_kernel<<<1, 32, 0, st>>>((SpecLState *)state, anchors, n, blkmin, K, span, esc_max, cls, ext_state, act, min_score,
+                                                 accepted, accepted_cap, win_idx, win_anchors, win_prio, keep, results, stats);
+    SFE_LAUNCH_CHECK();
+}
+
+int sfe_launch_spec_store(const sfe_result *wres, const long long *win_idx, long long wn, sfe_result *results, uint8_t *ext_state,
+                          cudaStream_t st)
+{
+    if (wn <= 0) return SFE_OK;
+    const int bs = 256;
+    SFE_KL spec_store_kernel<<<(unsigned)((wn + bs - 1) / bs), bs, 0, st>>>(wres, win_idx, wn, results, ext_state);
+    SFE_LAUNCH_CHECK();
+}
+
+int sfe_launch_specl_finish(const void *state, long long *n_accepted_io, cudaStream_t st)
+{
+    SFE_KL specl_finish_kernel<<<1, 32, 0, st>>>((const SpecLState *)state, n_accepted_io);
+    SFE_LAUNCH_CHECK();
+}

@@ -104,6 +104,8 @@ struct YdParams {
     SfeFreeRing *ring_state;
     int32_t n_chunks;
     int32_t max_warps;            // warps of the normal kernel allowed to work in this pass
+    int32_t n_classes;            // reserved ticket segments in use (set by sfe_launch_ydrop: 4, or fewer in a sparse launch)
+    int32_t sparse_warps;         // > 0: resident warps per SM for a chain-bound pass (blocks of 4 warps), see sfe_launch_ydrop
     int32_t n_pairs;
     int32_t OX, X, Y, ydrop_inf;
     int32_t lag0;                 // prune_lag == 0 (R4, serial-order pruning): block kernel only

@@ -310,8 +310,8 @@ static __device__ void block_half(const YdParams &p, const int hid, BkShared &sh
             if (wpos + nw + 2 > BK_CHUNK_WORDS) {         // next chunk (uniform decision)
                 if (warp == 0) {
                     if (cur_chunk >= 0 && lane == 0) p.pool[(size_t)cur_chunk * BK_CHUNK_WORDS] = (uint32_t)wpos;
-                    const int nc = chunk_pop(p.free_ring, p.ring_state, p.n_chunks, &p.counters[CNT_RING_DROPS], lane);
-                    if (lane == 0) { sh.new_chunk = nc; if (nc >= 0) p.chunk_prev[nc] = cur_chunk; }
+                    const int nc = chunk_pop(p.free_ring, p.ring_state, p.n_chunks, lane);
+                    if (lane == 0) { sh.new_chunk = nc; if (nc >= 0) p.chunk_prev[nc] = cur_chunk; if (nc == -2) atomicAdd(&p.counters[CNT_RING_DROPS], 1ULL); }
                 }
                 __syncthreads();
                 const int nc = sh.new_chunk;

@@ -60,7 +60,8 @@ static __device__ __forceinline__ bool half_setup(const YdParams &p, const int h
 // lane-divergent region makes ptxas clone the whole DP loop with real WARPSYNCs).  Both spins wait
 // for one bounded action of another resident warp (the matching push / pop has already reserved the
 // slot), never for work.
-static __device__ __forceinline__ int chunk_pop(int32_t *ring, SfeFreeRing *st, int n_chunks, unsigned long long *drops, int lane)
+// Returns the chunk id, -1 if the arena is empty, -2 if the bounded wait for the pusher ran out (counted by the caller).
+static __device__ __forceinline__ int chunk_pop(int32_t *ring, SfeFreeRing *st, int n_chunks, int lane)
 {
     long long a = 0; unsigned long long h = 0;
     if (lane == 0) {
@@ -77,8 +78,7 @@ static __device__ __forceinline__ int chunk_pop(int32_t *ring, SfeFreeRing *st, 
         id = __shfl_sync(FULL, id, 0);                      // read an id that a later lap's pop also reads
         if (id >= 0) break;
     }
-    if (id < 0 && lane == 0) atomicAdd(drops, 1ULL);        // treated like an empty arena: score-only now, re-run later (counted)
-    return id;
+    return id < 0 ? -2 : id;                                // -2: treated like an empty arena (score-only now, re-run later)
 }
 static __device__ __forceinline__ void chunk_push(int32_t *ring, SfeFreeRing *st, int n_chunks, int id, unsigned long long *drops, int lane)
 {

@@ -87,7 +87,7 @@ static __device__ __forceinline__ void fill_bnd_neg(char *wbase, int lo, int hi,
 }
 
 struct TbWriter {
-    uint32_t *pool; int32_t *chunk_prev; int32_t *ring; SfeFreeRing *ring_state; int n_chunks; unsigned long long *drops;
+    uint32_t *pool; int32_t *chunk_prev; int32_t *ring; SfeFreeRing *ring_state; int n_chunks;
     uint32_t *ptr;          // this lane's word pair of the next record
     int left;               // records left in the current chunk
     int cur_chunk; int nrec; bool ok;
@@ -95,8 +95,8 @@ struct TbWriter {
     {
         if (!ok) return;
         if (left == 0) {
-            const int c = chunk_pop(ring, ring_state, n_chunks, drops, lane);
-            if (c < 0) { ok = false; return; }
+            const int c = chunk_pop(ring, ring_state, n_chunks, lane);
+            if (c < 0) { ok = false; left = c == -2 ? -1 : 0; return; }      // left == -1 remembers an abandoned wait (counted at the end)
             if (lane == 0) chunk_prev[c] = cur_chunk;
             cur_chunk = c;
             ptr = pool + (size_t)c * SFE_CHUNK_RECS * SFE_REC_WORDS + 2 * lane;
@@ -106,7 +106,7 @@ struct TbWriter {
         ptr += SFE_REC_WORDS; left--; nrec++;
     }
     // give every chunk of this half back (after the walk, or when the half is abandoned)
-    __device__ __forceinline__ void release(int lane)
+    __device__ __forceinline__ void release(int lane, unsigned long long *counters)
     {
         // One fence per half: this warp's record stores must have landed before a chunk changes owner.
         // (A gpu-scope fence also invalidates the SM's L1, so it is not done per chunk.)
@@ -115,7 +115,7 @@ struct TbWriter {
         int c = cur_chunk;
         while (c >= 0) {
             const int prev = __ldcg(chunk_prev + c);        // same address in every lane
-            chunk_push(ring, ring_state, n_chunks, c, drops, lane);
+            chunk_push(ring, ring_state, n_chunks, c, counters + CNT_RING_DROPS, lane);
             c = prev;
         }
         cur_chunk = -1;
@@ -314,7 +314,7 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
 
     const int OX = p.OX, X = p.X;
     TbWriter tb;
-    tb.pool = p.pool; tb.chunk_prev = p.chunk_prev; tb.ring = p.free_ring; tb.ring_state = p.ring_state; tb.n_chunks = p.n_chunks; tb.drops = &p.counters[CNT_RING_DROPS];
+    tb.pool = p.pool; tb.chunk_prev = p.chunk_prev; tb.ring = p.free_ring; tb.ring_state = p.ring_state; tb.n_chunks = p.n_chunks;
     tb.cur_chunk = -1; tb.nrec = 0; tb.ok = TB; tb.ptr = nullptr; tb.left = 0;
 
     int best = 0, best_i = 0, best_j = 0;     // lane-local first maximum
@@ -444,7 +444,7 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) cells += __shfl_xor_sync(FULL, cells, o);
     if (SK == 2 && wide) {                                  // too wide for the skew-2 schedule: give the chunks back, try again with skew 1
-        if (TB) tb.release(lane);
+        if (TB) tb.release(lane, p.counters);
         return false;
     }
     // every lane holds the same winner; the broadcast makes that visible to the compiler's uniformity
@@ -465,7 +465,7 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
             out.status |= SFE_ST_INTERNAL;
         if (!ops_ok) out.status |= SFE_ST_OPS_OVERFLOW;
     }
-    if (TB) tb.release(lane);
+    if (TB) tb.release(lane, p.counters);
     out.steps = total_steps; out.max_steps = max_steps;
     {   // per-half profile (Fig. 5: per-anchor runtime spread): SM cycles spent, where it ran
         unsigned smid, wslot;
@@ -478,6 +478,7 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
         atomicAdd(&p.counters[CNT_STEPS], (unsigned long long)total_steps);
         if (TB) atomicAdd(&p.counters[CNT_TBBYTES], (unsigned long long)tb.nrec * (unsigned long long)SFE_REC_BYTES);
         if (TB && !tb.ok) atomicAdd(&p.counters[CNT_OVERFLOW], 1ULL);
+        if (TB && !tb.ok && tb.left < 0) atomicAdd(&p.counters[CNT_RING_DROPS], 1ULL);
         if (wide && !GLOBAL) atomicAdd(&p.counters[CNT_WIDE], 1ULL);
     }
     return true;
@@ -491,7 +492,7 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kerne
     const int lane = sfe_lane();
     char *wsm = smem + (threadIdx.x >> 5) * SFE_WARP_SMEM;
     // re-run passes after a traceback-arena overflow admit only as many warps as the arena can serve
-    if ((int)(blockIdx.x * (SFE_BLOCK_THREADS / 32) + (threadIdx.x >> 5)) >= p.max_warps) return;
+    if ((int)(blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) >= p.max_warps) return;
     // Ticket queue (a3): tickets are sorted longest bin first and every warp takes the next one (LPT order).
     // One extension is a serial chain of wavefront steps (R4 allows only 32 rows in flight), so the longest
     // halves decide when the kernel ends -- and the SM's schedulers strongly favour the lowest hardware warp
@@ -503,11 +504,12 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kerne
     asm("mov.u32 %0, %%warpid;" : "=r"(wslot));
     const long long seg = p.seg_tickets;
     const int my_class = (int)(wslot >> 2);
+    const int ncls = p.n_classes;                      // slot classes of this launch (1..4): segments 0 .. ncls-1 are reserved
     for (int phase = 0; phase < 6; phase++) {
         // phase 0: my class's segment; phase 1: main queue; phases 2..5: leftovers of segments 0..3
         const int k = phase == 0 ? my_class : phase - 2;
-        if (phase != 1 && (k > 3 || seg == 0)) continue;
-        const long long lo = phase == 1 ? 4 * seg : k * seg;
+        if (phase != 1 && (k >= ncls || seg == 0)) continue;
+        const long long lo = phase == 1 ? (seg ? ncls * seg : 0) : k * seg;
         const long long hi = phase == 1 ? p.n_tickets : (lo + seg < p.n_tickets ? lo + seg : p.n_tickets);
         unsigned long long *cnt = &p.counters[phase == 1 ? CNT_TICKET : CNT_CLASS0 + k];
         for (;;) {
@@ -566,27 +568,43 @@ int sfe_ydrop_init_device(void)
 
 // use_block: the whole pass goes to the row-synchronous block kernel (ydrop_block_kernel.cu) instead of the
 // warp-systolic one; either way halves whose band outgrew the window are re-run by the wide kernel.
-int sfe_launch_ydrop(const YdParams &p, bool want_tb, bool use_block, int n_sm, cudaStream_t st)
+int sfe_launch_ydrop(const YdParams &p_in, bool want_tb, bool use_block, int n_sm, cudaStream_t st)
 {
+    YdParams p = p_in;
+    p.n_classes = 4;
     if (use_block) {
         const int rc = sfe_launch_ydrop_block(p, want_tb, n_sm, st);
         if (rc) return rc;
     } else {
-        const int warps_per_block = SFE_BLOCK_THREADS / 32;
-        const size_t smem = (size_t)warps_per_block * SFE_WARP_SMEM;
+        int warps_per_block = SFE_BLOCK_THREADS / 32;
+        size_t smem = (size_t)warps_per_block * SFE_WARP_SMEM;
         int bps = 0;
         if (want_tb) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<true>, SFE_BLOCK_THREADS, smem);
         else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<false>, SFE_BLOCK_THREADS, smem);
         if (bps < 1) return SFE_ECUDA;
-        // A pass with at most one ticket per warp slot ends with its longest half: fewer resident warps make every half
-        // faster (measured on the windowed workloads: 12 warps per SM beat 18 by 7-12 %, 6 are too few).
-        if (bps > 2 && p.n_tickets <= (long long)n_sm * bps * warps_per_block) bps = 2;
-        long long blocks = (long long)n_sm * bps;
+        long long blocks;
+        if (p.sparse_warps > 0) {
+            // A pass whose time is its longest half (sfe_speculate's batches): one extension is a serial chain of wavefront
+            // steps and every co-resident warp on its scheduler slows it down (solo step 49 / 77 cycles, 140-310 with 18
+            // warps per SM).  Blocks of 4 warps = one warp per SM sub-partition; sparse_warps / 4 blocks per SM.
+            warps_per_block = 4;
+            smem = (size_t)warps_per_block * SFE_WARP_SMEM;
+            int per_sm = (p.sparse_warps + 3) / 4;
+            if (per_sm < 1) per_sm = 1;
+            if (per_sm > 4) per_sm = 4;
+            blocks = (long long)n_sm * per_sm;
+            p.n_classes = per_sm;                             // warp slots 0 .. 4 per_sm - 1 exist: that many reserved segments
+        } else {
+            // A pass with at most one ticket per warp slot ends with its longest half: fewer resident warps make every half
+            // faster (measured on the windowed workloads: 12 warps per SM beat 18 by 7-12 %, 6 are too few).
+            if (bps > 2 && p.n_tickets <= (long long)n_sm * bps * warps_per_block) bps = 2;
+            blocks = (long long)n_sm * bps;
+        }
         const long long need = (p.n_tickets + warps_per_block - 1) / warps_per_block;
         if (blocks > need) blocks = need;
         if (blocks < 1) blocks = 1;
-        if (want_tb) SFE_KL ydrop_kernel<true><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
-        else SFE_KL ydrop_kernel<false><<<(unsigned)blocks, SFE_BLOCK_THREADS, smem, st>>>(p);
+        if (want_tb) SFE_KL ydrop_kernel<true><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
+        else SFE_KL ydrop_kernel<false><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
     }
     const int bs = 256;
     SFE_KL select_wide_kernel<<<(unsigned)((p.n_tickets + bs - 1) / bs), bs, 0, st>>>(p);

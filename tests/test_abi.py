@@ -95,7 +95,7 @@ def test_binding_constants_match_header():
     defs = {m.group(1): int(m.group(2), 0) for m in re.finditer(r"#define\s+(SFE_[A-Z_0-9]+)\s+(0x[0-9a-fA-F]+|\d+)u?\b", src)}
     enum = {m.group(1): int(m.group(2)) for m in re.finditer(r"\b(SFE_E?[A-Z]+)\s*=\s*(-?\d+)", src)}
     pairs = {"SFE_WANT_CIGAR": B.WANT_CIGAR, "SFE_SCORE_ONLY": B.SCORE_ONLY, "SFE_NO_BINNING": B.NO_BINNING,
-             "SFE_BLOCK_KERNEL": B.BLOCK_KERNEL, "SFE_NO_BLOCK_KERNEL": B.NO_BLOCK_KERNEL, "SFE_CIGAR_KEPT_ONLY": B.CIGAR_KEPT_ONLY,
+             "SFE_BLOCK_KERNEL": B.BLOCK_KERNEL, "SFE_NO_BLOCK_KERNEL": B.NO_BLOCK_KERNEL, "SFE_CIGAR_KEPT_ONLY": B.CIGAR_KEPT_ONLY, "SFE_SPEC_LEADERS": B.SPEC_LEADERS,
              "SFE_ST_TB_OVERFLOW": B.ST_TB_OVERFLOW, "SFE_ST_CIGAR_OVERFLOW": B.ST_CIGAR_OVERFLOW, "SFE_ST_WIDE": B.ST_WIDE,
              "SFE_ST_SCORE_LIMIT": B.ST_SCORE_LIMIT, "SFE_ST_BAD_ANCHOR": B.ST_BAD_ANCHOR, "SFE_ST_BAND_LIMIT": B.ST_BAND_LIMIT,
              "SFE_ST_INTERNAL": B.ST_INTERNAL, "SFE_ST_SKIPPED": B.ST_SKIPPED, "SFE_OP_M": B.OP_M, "SFE_OP_I": B.OP_I,
@@ -107,3 +107,20 @@ def test_binding_constants_match_header():
     # status bits are distinct single bits
     st = [v for k, v in defs.items() if k.startswith("SFE_ST_")]
     assert len(set(st)) == len(st) and all(v & (v - 1) == 0 for v in st)
+
+
+def test_hot_loop_codegen_guard(built):
+    """The Y-drop kernel's steady-state loop is sensitive to register pressure: an innocent edit elsewhere in the kernel
+    once turned 16 VIADD into IMAD, added spills and cost 16 % ("Codegen notes").  Guard the static
+    instruction mix of the 16-step group (what the roofline denominator is computed from) and the absence of spills."""
+    import subprocess
+    from paper_2606_06811_b200 import sassinfo
+    tb = sassinfo.hot_loop(True); so = sassinfo.hot_loop(False)
+    assert tb["per_cell"] <= 22.6 and tb["alu"] <= 14.1 and tb["fma"] <= 4.2 and tb["lsu"] <= 3.2, tb
+    assert so["per_cell"] <= 14.6 and so["alu"] <= 10.1, so
+    assert tb["hist"].get("VIADDMNMX") == 32 and tb["hist"].get("VIMNMX3") == 24          # DPX: E, F and H / best
+    out = subprocess.run(["cuobjdump", "-res-usage", B.LIB_PATH], capture_output=True, text=True).stdout
+    blocks = out.split("Function ")
+    for b in blocks:
+        if b.startswith("_Z12ydrop_kernelILb"):
+            assert "STACK:0" in b.replace(" ", ""), b[:300]

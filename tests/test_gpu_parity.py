@@ -473,11 +473,11 @@ def test_two_contexts_on_two_devices(oracle):
 
 
 def test_tiny_arena_many_short_halves(oracle):
-    """Free-chunk ring under churn: 4 chunks (the minimum) shared by thousands of short halves -- every pop / push goes
+    """Free-chunk ring under churn: 12 chunks (a half of this input needs up to 6) shared by thousands of halves -- every pop / push goes
     through the same few slots many laps over.  Results stay bit-exact, nothing is dropped (info ring_drops == 0)."""
     import __graft_entry__ as entry
     entry.build()
-    s = B.Sfe(0, 4 * 65536)
+    s = B.Sfe(0, 12 * 65536)
     try:
         w = W.config2(t_len=120_000, n_segments=60, per_seg=10, n_decoys=600, min_len=100, max_len=300)
         out = H.gpu_run(s, w)
@@ -488,3 +488,90 @@ def test_tiny_arena_many_short_halves(oracle):
         H.assert_resolve_equal(out, w)
     finally:
         s.close()
+
+
+def _dense_workload(seed=7, t_len=60_000, n_anchors=900):
+    """A small configs[2]-like input: high identity, blocks, some inverted / moved, dense anchors on the true path --
+    most anchors are followers of their block's first one."""
+    return W.config3(t_len=t_len, n_anchors=n_anchors, blk_lo=1500, blk_hi=6000)
+
+
+@pytest.mark.parametrize("force", [0, 1, 2, 3])
+@pytest.mark.parametrize("K", [1, 7, 64, 4096])
+def test_speculate_leaders_equals_serial_loop(sfe, oracle, K, force):
+    """SFE_SPEC_LEADERS: Algorithm 3 with predicted leaders keeps exactly what Algorithm 1 keeps for ANY prediction --
+    the classifier's (force 0), nobody leads (1: every uncovered anchor is reached by the commit and force-extended),
+    everybody leads (2), the second half of the anchors never leads (3) -- and any batch size K.  Extended anchors are
+    bit-exact against the oracle; anchors never extended are covered ones; the counters add up."""
+    for w in (W.config2(t_len=60_000, n_segments=30, per_seg=8, n_decoys=40, min_len=150, max_len=700), _dense_workload()):
+        n = len(w.anchors)
+        ser = oracle.serial_loop(w.target, w.query, w.query_rc, w.pairs, w.anchors, oracle.scoring(), want_results=False)
+        sfe.set_option(B.OPT_FORCE_CLASS, force)
+        sfe.set_option(B.OPT_SPEC_SPAN, 256)
+        try:
+            out = _speculate(sfe, w, K, flags=B.WANT_CIGAR | B.SPEC_LEADERS)
+            info = sfe.last_speculate_info()
+        finally:
+            sfe.set_option(B.OPT_FORCE_CLASS, 0); sfe.set_option(B.OPT_SPEC_SPAN, 65536)
+        assert out["keep"].tolist() == ser["state"].tolist(), (K, force)
+        st = out["stats"]
+        skipped = (out["results"]["status"] & B.ST_SKIPPED) != 0
+        assert int(st["n_anchors"]) == n and int(st["n_kept"]) == ser["n_kept"] == out["n_accepted"]
+        assert int(st["n_extended"]) == int((~skipped).sum()) and int(st["n_kept"] + st["n_covered"] + st["n_below"]) == n
+        assert (out["keep"][skipped] == 0).all()
+        serial_ext = ser["state"] != 0
+        assert (~skipped)[serial_ext].all()                      # everything Algorithm 1 extends was extended
+        assert int(st["cells_total"]) == int(out["results"]["cells"][~skipped].sum())
+        assert info["batches"] == int(st["n_windows"]) >= 1
+        H.assert_anchors_equal(out, w, np.nonzero(~skipped)[0][:: max(1, int((~skipped).sum()) // 60)])
+
+
+def test_speculate_leaders_serial_when_nobody_leads(sfe, oracle):
+    """With no predicted leader and no escalation the path degenerates to Algorithm 1 itself: one extension per commit
+    stop, exactly the anchors the serial loop extends, no shadow work.  With the classifier on the dense input it extends
+    far fewer anchors than classic windows of the same K."""
+    w = _dense_workload()
+    ser = oracle.serial_loop(w.target, w.query, w.query_rc, w.pairs, w.anchors, oracle.scoring(), want_results=False)
+    n_serial = int((ser["state"] != 0).sum())
+    sfe.set_option(B.OPT_FORCE_CLASS, 1); sfe.set_option(B.OPT_SPEC_ESC_MAX, 1)
+    try:
+        out = _speculate(sfe, w, 64, flags=B.SCORE_ONLY | B.SPEC_LEADERS)
+        info = sfe.last_speculate_info()
+    finally:
+        sfe.set_option(B.OPT_FORCE_CLASS, 0); sfe.set_option(B.OPT_SPEC_ESC_MAX, 64)
+    assert out["keep"].tolist() == ser["state"].tolist()
+    assert int(out["stats"]["n_extended"]) == n_serial == info["stops"] == info["forced"]
+    lead = _speculate(sfe, w, 64, flags=B.SCORE_ONLY | B.SPEC_LEADERS)
+    classic = _speculate(sfe, w, 64, flags=B.SCORE_ONLY)
+    assert lead["keep"].tolist() == classic["keep"].tolist() == ser["state"].tolist()
+    assert n_serial <= int(lead["stats"]["n_extended"]) < int(classic["stats"]["n_extended"]) // 3
+    for f in ("score", "tstart", "tend", "qstart", "qend", "cells"):
+        both = ((lead["results"]["status"] | classic["results"]["status"]) & B.ST_SKIPPED) == 0
+        assert (lead["results"][f][both] == classic["results"][f][both]).all()
+
+
+def test_speculate_leaders_kept_only_and_carried_boxes(sfe, oracle):
+    """SFE_SPEC_LEADERS with SFE_CIGAR_KEPT_ONLY (score-only batches + one traceback batch over the kept anchors) and with
+    accepted boxes carried in from an earlier call (R26): the second half of the anchors resolved against the first half's."""
+    import torch
+    w = _dense_workload(n_anchors=700)
+    n = len(w.anchors)
+    ser = oracle.serial_loop(w.target, w.query, w.query_rc, w.pairs, w.anchors, oracle.scoring(), want_results=False)
+    ko = _speculate(sfe, w, 128, flags=B.WANT_CIGAR | B.CIGAR_KEPT_ONLY | B.SPEC_LEADERS)
+    assert ko["keep"].tolist() == ser["state"].tolist()
+    kept = ko["keep"] == 1
+    assert (ko["results"]["n_ops"][~kept] == 0).all() and ko["cigar_used"] == int(ko["results"]["n_ops"][kept].sum())
+    H.assert_anchors_equal(ko, w, np.nonzero(kept)[0])
+    # two calls, accepted list carried across
+    dev = sfe.device
+    tp = sfe.pack(torch.from_numpy(w.target_ascii().copy()).to(dev), with_rc=False)
+    qp = sfe.pack(torch.from_numpy(w.query_ascii().copy()).to(dev), with_rc=True)
+    acc = torch.zeros((n + 1) * B.BOX_DT.itemsize, dtype=torch.uint8, device=dev); nacc = torch.zeros(1, dtype=torch.int64, device=dev)
+    pairs = B._dev(B.make_pairs(w.pairs), dev); A = B.make_anchors(w.anchors); h = n // 2
+    keep = []
+    for lo, hi in ((0, h), (h, n)):
+        o = sfe.speculate(tp[:2], len(w.target), qp, len(w.query), pairs, len(w.pairs), B._dev(A[lo:hi], dev), hi - lo, B.scoring(), 64,
+                          B.SCORE_ONLY | B.SPEC_LEADERS, accepted_dev=acc, n_accepted_dev=nacc)
+        torch.cuda.synchronize()
+        keep += o["keep"].cpu().numpy()[: hi - lo].tolist()
+    assert keep == ser["state"].tolist() and int(nacc.item()) == ser["n_kept"]
