@@ -29,7 +29,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 SCRATCH_GB = {"c1": 2, "c2": 16, "c4": 24, "c3": 32, "c3s": 24, "c5s": 32, "c5": 48}   # traceback arena (chunks are recycled)
-DEFAULT_WINDOW = {"c3": 16384, "c3s": 16384, "c5s": 1024, "c5": 1024}   # Algorithm 3's K for the dense-anchor workloads; others: one batch
+DEFAULT_WINDOW = {"c3": 16384, "c3s": 16384, "c5s": 1024, "c5": 1024}   # classic Algorithm 3: K for the dense-anchor workloads; others: one batch
+LEADER_WINDOW = 262144                                                  # --spec leaders: most extensions per batch
 TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.csv")      # written by hand from `ncu --set full` captures (see ncu_traffic.md)
 
 
@@ -337,7 +338,11 @@ def main():
     sfe = B.Sfe(local, scratch)
 
     window = DEFAULT_WINDOW.get(args.workload, 0) if args.window < 0 else args.window
-    kept_only = window > 0 and args.flags == "cigar" and args.cigar_for in ("auto", "kept")
+    if args.window < 0 and window > 0 and args.spec == "leaders":
+        window = LEADER_WINDOW
+    # CIGARs for the kept anchors only (score-only speculation + one traceback batch) pays when most extensions are thrown
+    # away (classic windows); with predicted leaders nearly every extension is kept or cheap: trace back while extending
+    kept_only = window > 0 and args.flags == "cigar" and (args.cigar_for == "kept" or (args.cigar_for == "auto" and args.spec == "classic"))
     if kept_only:
         flags |= B.CIGAR_KEPT_ONLY
     if window > 0 and args.spec == "leaders":
@@ -453,8 +458,8 @@ def main():
         tg = time.perf_counter(); w5, desc5 = make_workload(name5); tg = time.perf_counter() - tg
         free_b, _ = torch.cuda.mem_get_info(dev)
         sfe5 = B.Sfe(local, min(SCRATCH_GB[name5] << 30, int(free_b * 0.6)))
-        K5 = DEFAULT_WINDOW[name5]
-        f5 = B.WANT_CIGAR | B.CIGAR_KEPT_ONLY | (B.SPEC_LEADERS if args.spec == "leaders" else 0)
+        K5 = LEADER_WINDOW if args.spec == "leaders" else DEFAULT_WINDOW[name5]
+        f5 = B.WANT_CIGAR | (B.SPEC_LEADERS if args.spec == "leaders" else B.CIGAR_KEPT_ONLY)
         cap5 = max(1 << 26, 96 * len(w5.anchors))
         job5 = Job(sfe5, w5, dev, f5, K5, cap5)
         job5.step(); torch.cuda.synchronize(dev)                       # warm-up pass
@@ -462,7 +467,7 @@ def main():
         a0.record(); job5.step(); a1.record(); torch.cuda.synchronize(dev)
         c5 = summarize_pass(job5.stats_dict(), a0.elapsed_time(a1))
         c5.update({"workload": f"{name5}: {desc5}", "anchors": len(w5.anchors), "window_k": K5, "spec": args.spec, "speculate_info": sfe5.last_speculate_info(),
-                   "cigar_for": "kept", "generation_s": tg,
+                   "cigar_for": "all extended" if args.spec == "leaders" else "kept", "generation_s": tg,
                    "path": "sfe_pack x2 -> sfe_speculate (phase 1 scan, phase 2 Y-drop windows, phase 3 commit, all on the device) "
                            "-> one traceback batch over the kept anchors; device-resident inputs, CUDA events"})
         t_host = torch.from_numpy(w5.target_ascii().copy()).pin_memory().numpy()

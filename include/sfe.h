@@ -195,15 +195,20 @@ enum {
     SFE_OPT_LEADER_GAP,            /* [2000]  ... and target distance to that predecessor <= gap ...                                */
     SFE_OPT_LEADER_LOOKBACK,       /* [64]    ... among the previous `lookback` anchors (same strand, same pair) ...                */
     SFE_OPT_LEADER_NBREAK,         /* [64]    ... with fewer than nbreak N between them in the target                               */
-    SFE_OPT_SPEC_SPAN,             /* [65536] look-ahead, in anchors beyond the commit cursor, in which leaders are extended        */
-    SFE_OPT_SPEC_ESC_MAX,          /* [64]    cap of the doubling number of anchors force-extended after repeated commit stops      */
+    SFE_OPT_SPEC_SPAN,             /* [2^20]  look-ahead, in anchors beyond the commit cursor, in which leaders are extended        */
+    SFE_OPT_SPEC_ESC_MAX,          /* [64]    cap of the doubling number of anchors force-extended after repeated commit stops;
+                                              1 = exactly one anchor per stop, no cold-diagonal sweep either                        */
     SFE_OPT_SPARSE_WARPS,          /* [4]     resident warps per SM for sfe_speculate's leader batches (0 = the dense launch)       */
     SFE_OPT_FORCE_CLASS,           /* [0]     testing: 1 = nobody leads, 2 = everybody leads, 3 = second half of the anchors never  */
+    SFE_OPT_PROMOTE_REACH,         /* [65536] after a batch, followers within this target distance of an extended anchor that will  
+                                              not cover them (it scored below tau, or they lie beyond its box) become leaders       */
     SFE_OPT_N
 };
 int sfe_set_option(sfe_ctx *ctx, int key, int64_t value);
 /* counters of the most recent sfe_speculate with SFE_SPEC_LEADERS: [0] extension batches, [1] commit stops (the commit
- * reached an anchor that was neither covered nor extended), [2] anchors force-extended after stops, [3..7] reserved. */
+ * reached an anchor that was neither covered nor extended), [2] anchors force-extended after stops, [3] stops on a
+ * cold diagonal (its extended predecessor scored below tau: every anchor of that diagonal ahead is taken at once),
+ * [4] followers promoted to leaders after a batch showed that the anchor they follow will not cover them, [5..7] reserved. */
 int sfe_last_speculate_info(sfe_ctx *ctx, int64_t info[8]);
 
 /* End-to-end convenience with HOST buffers (bench.py's e2e leg): copies the ASCII sequences and

@@ -25,12 +25,16 @@ int sfe_launch_specl_prepare(const sfe_anchor *anchors, long long n, const uint8
                              uint8_t *cls, uint8_t *ext_state, long long *blkmin, void *state, const sfe_box *accepted,
                              const long long *n_accepted, sfe_box *act, cudaStream_t st);
 int sfe_launch_spec_advance(void *state, const sfe_anchor *anchors, long long n, const long long *blkmin, long long K, long long span,
-                            int esc_max, const uint8_t *cls, uint8_t *ext_state, sfe_box *act, int min_score, sfe_box *accepted,
+                            int esc_max, int tol, long long gap, int lookback, const uint8_t *cls, uint8_t *ext_state, sfe_box *act, int min_score, sfe_box *accepted,
                             long long accepted_cap, long long *win_idx, sfe_anchor *win_anchors, uint8_t *win_prio, uint8_t *keep,
-                            sfe_result *results, sfe_stats *stats, cudaStream_t st);
+                            sfe_result *results, sfe_stats *stats, const int32_t *plist, cudaStream_t st);
 int sfe_launch_spec_store(const sfe_result *wres, const long long *win_idx, long long wn, sfe_result *results, uint8_t *ext_state,
                           cudaStream_t st);
 int sfe_launch_specl_finish(const void *state, long long *n_accepted_io, cudaStream_t st);
+int sfe_launch_spec_promote(const sfe_result *wres, const long long *win_idx, long long wn, const sfe_anchor *anchors, long long n,
+                            int min_score, int tol, long long reach, int max_ahead, const uint8_t *ext_state, uint8_t *cls, void *state,
+                            int32_t *plist, cudaStream_t st);
+int sfe_launch_len_bins(const sfe_result *res, long long n, uint8_t *prio, cudaStream_t st);
 int sfe_launch_select_overflow(const sfe_half *halves, long long n_anchors, long long *sel, int32_t *tickets,
                                unsigned long long *counters, int n_chunks, cudaStream_t st);
 int sfe_launch_probe(int mix, int iters, int blocks, int *sink, cudaStream_t st);
@@ -71,7 +75,7 @@ struct sfe_ctx {
     unsigned long long *counters_host;  // pinned
     DevBuf halves, tickets, sel, hist, blkmin, act, misc, wide_tickets, wide_ring, ops_stage;
     DevBuf sp_state, sp_idx, sp_anchors, sp_results, sp_local, sp_blkmin, sp_act, sp_kanchors, sp_kidx, sp_kres;   // sfe_speculate
-    DevBuf sp_cls, sp_ext, sp_prio;   // predicted leaders
+    DevBuf sp_cls, sp_ext, sp_prio, sp_plist;   // predicted leaders
     long long opt[SFE_OPT_N];         // sfe_set_option
     long long spec_info[8];           // sfe_last_speculate_info
     long long *state_host;            // pinned, 16 words
@@ -126,8 +130,8 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
     memset(c->info, 0, sizeof c->info);
     memset(c->spec_info, 0, sizeof c->spec_info);
     c->opt[SFE_OPT_LEADER_DIAG_TOL] = 48; c->opt[SFE_OPT_LEADER_GAP] = 2000; c->opt[SFE_OPT_LEADER_LOOKBACK] = 64;
-    c->opt[SFE_OPT_LEADER_NBREAK] = 64; c->opt[SFE_OPT_SPEC_SPAN] = 65536; c->opt[SFE_OPT_SPEC_ESC_MAX] = 64;
-    c->opt[SFE_OPT_SPARSE_WARPS] = 4; c->opt[SFE_OPT_FORCE_CLASS] = 0;
+    c->opt[SFE_OPT_LEADER_NBREAK] = 64; c->opt[SFE_OPT_SPEC_SPAN] = 1 << 20; c->opt[SFE_OPT_SPEC_ESC_MAX] = 64;
+    c->opt[SFE_OPT_SPARSE_WARPS] = 4; c->opt[SFE_OPT_FORCE_CLASS] = 0; c->opt[SFE_OPT_PROMOTE_REACH] = 65536;
     c->ev_pending = false; c->kernel_us = 0.0; c->n_profile = 0;
     if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) { delete c; return SFE_ECUDA; }
     if (cudaMalloc((void **)&c->pool, (size_t)nch * SFE_CHUNK_BYTES) != cudaSuccess ||
@@ -159,7 +163,7 @@ extern "C" int sfe_destroy(sfe_ctx *c)
     if (c->counters_host) cudaFreeHost(c->counters_host);
     if (c->state_host) cudaFreeHost(c->state_host);
     cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1);
-    DevBuf *bufs[] = {&c->sp_cls, &c->sp_ext, &c->sp_prio, &c->sp_kanchors, &c->sp_kidx, &c->sp_kres, &c->sp_state, &c->sp_idx, &c->sp_anchors, &c->sp_results, &c->sp_local, &c->sp_blkmin, &c->sp_act, &c->ops_stage, &c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
+    DevBuf *bufs[] = {&c->sp_cls, &c->sp_ext, &c->sp_prio, &c->sp_plist, &c->sp_kanchors, &c->sp_kidx, &c->sp_kres, &c->sp_state, &c->sp_idx, &c->sp_anchors, &c->sp_results, &c->sp_local, &c->sp_blkmin, &c->sp_act, &c->ops_stage, &c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
                       &c->h_t2, &c->h_tm, &c->h_q2, &c->h_qm, &c->h_r2, &c->h_rm, &c->h_pairs, &c->h_anchors, &c->h_results,
                       &c->h_keep, &c->h_cigar, &c->h_acc, &c->h_small};
     for (DevBuf *b : bufs) b->release();
@@ -442,7 +446,7 @@ extern "C" int sfe_speculate(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t 
         if (!t_nmask || !q_nmask) return SFE_EINVAL;
         if ((rc = c->sp_state.ensure(128)) || (rc = c->sp_idx.ensure((size_t)K * sizeof(long long))) ||
             (rc = c->sp_anchors.ensure((size_t)K * sizeof(sfe_anchor))) || (rc = c->sp_results.ensure((size_t)K * sizeof(sfe_result))) ||
-            (rc = c->sp_prio.ensure((size_t)K)) || (rc = c->sp_cls.ensure((size_t)n_anchors)) || (rc = c->sp_ext.ensure((size_t)n_anchors)) ||
+            (rc = c->sp_prio.ensure((size_t)K)) || (rc = c->sp_cls.ensure((size_t)n_anchors + 8)) || (rc = c->sp_plist.ensure((size_t)n_anchors * sizeof(int32_t))) || (rc = c->sp_ext.ensure((size_t)n_anchors)) ||
             (rc = c->sp_blkmin.ensure((size_t)((n_anchors + 31) / 32 + 32) * sizeof(long long))) ||
             (rc = c->sp_act.ensure((size_t)(n_anchors + accepted_cap + 1) * sizeof(sfe_box)))) return rc;
         long long *blkmin = (long long *)c->sp_blkmin.p;
@@ -457,12 +461,13 @@ extern "C" int sfe_speculate(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t 
         long long n_batches = 0;
         for (;;) {
             if ((rc = sfe_launch_spec_advance(c->sp_state.p, anchors_dev, n_anchors, blkmin, K, c->opt[SFE_OPT_SPEC_SPAN], (int)c->opt[SFE_OPT_SPEC_ESC_MAX],
-                                              cls, ext, act, sc->min_score, accepted_dev, accepted_cap, (long long *)c->sp_idx.p,
-                                              (sfe_anchor *)c->sp_anchors.p, (uint8_t *)c->sp_prio.p, keep_dev, results_dev, stats_dev, c->stream))) return rc;
-            SFE_CUDA_CHECK(cudaMemcpyAsync(c->state_host, c->sp_state.p, 10 * sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
+                                              (int)c->opt[SFE_OPT_LEADER_DIAG_TOL], c->opt[SFE_OPT_LEADER_GAP], (int)c->opt[SFE_OPT_LEADER_LOOKBACK], cls, ext, act, sc->min_score, accepted_dev, accepted_cap, (long long *)c->sp_idx.p,
+                                              (sfe_anchor *)c->sp_anchors.p, (uint8_t *)c->sp_prio.p, keep_dev, results_dev, stats_dev, (const int32_t *)c->sp_plist.p, c->stream))) return rc;
+            SFE_CUDA_CHECK(cudaMemcpyAsync(c->state_host, c->sp_state.p, 13 * sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
             SFE_CUDA_CHECK(cudaStreamSynchronize(c->stream));
             const long long cursor = c->state_host[0], wn = c->state_host[1];
-            c->spec_info[0] = n_batches; c->spec_info[1] = c->state_host[9]; c->spec_info[2] = c->state_host[8];
+            c->spec_info[0] = n_batches; c->spec_info[1] = c->state_host[9]; c->spec_info[2] = c->state_host[8]; c->spec_info[3] = c->state_host[10];
+            c->spec_info[4] = c->state_host[12];
             if (wn <= 0) {
                 if (cursor < n_anchors) return SFE_ECUDA;            // cannot happen: a stop always queues the anchor it stopped at
                 break;
@@ -473,6 +478,9 @@ extern "C" int sfe_speculate(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t 
                                        (int)c->opt[SFE_OPT_SPARSE_WARPS]))) return rc;
             harvest_kernel_time(c);
             if ((rc = sfe_launch_spec_store((const sfe_result *)c->sp_results.p, (const long long *)c->sp_idx.p, wn, results_dev, ext, c->stream))) return rc;
+            if (c->opt[SFE_OPT_SPEC_ESC_MAX] > 1 && c->opt[SFE_OPT_FORCE_CLASS] == 0 &&
+                (rc = sfe_launch_spec_promote((const sfe_result *)c->sp_results.p, (const long long *)c->sp_idx.p, wn, anchors_dev, n_anchors, sc->min_score,
+                                              (int)c->opt[SFE_OPT_LEADER_DIAG_TOL], c->opt[SFE_OPT_PROMOTE_REACH], 8192, ext, cls, c->sp_state.p, (int32_t *)c->sp_plist.p, c->stream))) return rc;
             n_batches++;
         }
         if ((rc = sfe_launch_specl_finish(c->sp_state.p, (long long *)n_accepted_dev, c->stream))) return rc;
@@ -511,10 +519,18 @@ extern "C" int sfe_speculate(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t 
     SFE_CUDA_CHECK(cudaStreamSynchronize(c->stream));
     const long long nk = c->state_host[0];
     if (nk <= 0) return SFE_OK;
-    if ((rc = c->sp_kres.ensure((size_t)nk * sizeof(sfe_result)))) return rc;
+    if ((rc = c->sp_kres.ensure((size_t)nk * sizeof(sfe_result))) || (rc = c->sp_prio.ensure((size_t)nk))) return rc;
+    // The kept anchors' extensions are known (score-only): their tickets are binned by the TRUE span, longest first, and --
+    // the pass being as long as its longest half -- run with the sparse residency of the leader batches.
+    const bool lead = (flags & SFE_SPEC_LEADERS) != 0;
+    if (lead) {
+        if ((rc = sfe_launch_spec_scatter_kept(results_dev, (const long long *)c->sp_kidx.p, -nk, (sfe_result *)c->sp_kres.p, c->stream))) return rc;
+        if ((rc = sfe_launch_len_bins((const sfe_result *)c->sp_kres.p, nk, (uint8_t *)c->sp_prio.p, c->stream))) return rc;
+    }
     if ((rc = ydrop_batch_impl(c, t_codes2, t_nmask, t_len, q_codes2, q_nmask, qrc_codes2, qrc_nmask, q_len, pairs_dev, n_pairs,
                                (const sfe_anchor *)c->sp_kanchors.p, nk, sc, flags, (sfe_result *)c->sp_kres.p,
-                               cigar_pool_dev, cigar_pool_cap, cigar_pool_used_dev, false))) return rc;
+                               cigar_pool_dev, cigar_pool_cap, cigar_pool_used_dev, false, lead ? (const uint8_t *)c->sp_prio.p : nullptr,
+                               lead ? (int)c->opt[SFE_OPT_SPARSE_WARPS] : 0))) return rc;
     harvest_kernel_time(c);
     return sfe_launch_spec_scatter_kept((const sfe_result *)c->sp_kres.p, (const long long *)c->sp_kidx.p, nk, results_dev, c->stream);
 }

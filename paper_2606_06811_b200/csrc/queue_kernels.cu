@@ -22,15 +22,17 @@ static __device__ __forceinline__ int half_bin(const sfe_anchor &an, const sfe_p
     return 31 - __clz((int)v + 1);                   // 0..30
 }
 
-// prio (may be NULL): one byte per anchor; anchors flagged long-likely by the caller (sfe_speculate's predicted leaders
-// with followers) go into the upper 32 bins, i.e. before everybody else, whatever their distance to the pair's end --
-// in a genome-scale pair that distance says nothing (every anchor is "far from the end").
+// prio (may be NULL): one byte per anchor.  0 = bin by the proxy.  p > 0 = bin 31 + p, i.e. before every proxy-binned
+// ticket and ordered among themselves by p: sfe_speculate passes 1 for predicted leaders with followers ("long-likely";
+// in a genome-scale pair the distance to the pair's end says nothing: every anchor is far from it) and
+// 1 + floor(log2(span)) for the kept anchors' traceback batch, whose extensions are already known.
 __global__ void bin_count_kernel(const sfe_anchor *anchors, long long n_anchors, const sfe_pair *pairs, int n_pairs,
                                  long long q_len, const uint8_t *prio, unsigned int *hist)
 {
     const long long h = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (h >= 2 * n_anchors) return;
-    atomicAdd(&hist[half_bin(anchors[h >> 1], pairs, n_pairs, q_len, (int)(h & 1)) + ((prio && prio[h >> 1]) ? 32 : 0)], 1u);
+    const int pb = prio ? prio[h >> 1] : 0;
+    atomicAdd(&hist[pb ? min(63, 31 + pb) : half_bin(anchors[h >> 1], pairs, n_pairs, q_len, (int)(h & 1))], 1u);
 }
 
 // hist[0..63] -> hist[64..127] = start offset of each bin in descending-bin order
@@ -47,7 +49,8 @@ __global__ void bin_scatter_kernel(const sfe_anchor *anchors, long long n_anchor
 {
     const long long h = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (h >= 2 * n_anchors) return;
-    const int b = half_bin(anchors[h >> 1], pairs, n_pairs, q_len, (int)(h & 1)) + ((prio && prio[h >> 1]) ? 32 : 0);
+    const int pb = prio ? prio[h >> 1] : 0;
+    const int b = pb ? min(63, 31 + pb) : half_bin(anchors[h >> 1], pairs, n_pairs, q_len, (int)(h & 1));
     tickets[atomicAdd(&hist[64 + b], 1u)] = (int32_t)h;
 }
 

@@ -394,8 +394,41 @@ int sfe_launch_spec_gather_kept(const sfe_anchor *anchors, const uint8_t *keep, 
     SFE_LAUNCH_CHECK();
 }
 
+__global__ void spec_gather_results_kernel(const sfe_result *results, const long long *kept_idx, long long nk, sfe_result *kres)
+{
+    const long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (k < nk) kres[k] = results[kept_idx[k]];
+}
+
+// one byte per anchor for sfe_launch_tickets: 1 + floor(log2(span)) of an extension that is already known
+__global__ void len_bins_kernel(const sfe_result *res, long long n, uint8_t *prio)
+{
+    const long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    long long span = res[k].tend - res[k].tstart;
+    const long long qs = res[k].qend - res[k].qstart;
+    if (qs > span) span = qs;
+    if (span < 1) span = 1;
+    if (span > 0x3fffffff) span = 0x3fffffff;
+    prio[k] = (uint8_t)(1 + (31 - __clz((int)span)));
+}
+
+int sfe_launch_len_bins(const sfe_result *res, long long n, uint8_t *prio, cudaStream_t st)
+{
+    if (n <= 0) return SFE_OK;
+    const int bs = 256;
+    SFE_KL len_bins_kernel<<<(unsigned)((n + bs - 1) / bs), bs, 0, st>>>(res, n, prio);
+    SFE_LAUNCH_CHECK();
+}
+
+// nk > 0: results[kept_idx[k]] = kres[k];  nk < 0: the other way round for -nk entries (first argument = results)
 int sfe_launch_spec_scatter_kept(const sfe_result *kres, const long long *kept_idx, long long nk, sfe_result *results, cudaStream_t st)
 {
+    if (nk < 0) {
+        const int bs = 256;
+        SFE_KL spec_gather_results_kernel<<<(unsigned)((-nk + bs - 1) / bs), bs, 0, st>>>(kres, kept_idx, -nk, results);
+        SFE_LAUNCH_CHECK();
+    }
     if (nk <= 0) return SFE_OK;
     const int bs = 256;
     SFE_KL spec_scatter_kept_kernel<<<(unsigned)((nk + bs - 1) / bs), bs, 0, st>>>(kres, kept_idx, nk, results);
@@ -457,9 +490,10 @@ int sfe_launch_spec_finish(const void *state, long long *n_accepted_io, cudaStre
 // until the cursor reaches the end.  The kept set, scores, boxes and CIGARs are Algorithm 1's for ANY classification
 // (tests run it with adversarial ones); the classification only decides how much is extended and how many batches it takes.
 // =====================================================================================================
-struct SpecLState { long long cursor, win_n, nact, nacc, overflow, spec_hi, esc, last_stop, n_forced, n_stops; };
+struct SpecLState { long long cursor, win_n, nact, nacc, overflow, spec_hi, esc, last_stop, n_forced, n_stops, n_cold, plist_rd;
+                    unsigned long long plist_n; };
 
-enum { CLS_FOLLOWER = 0, CLS_LEADER = 1, CLS_LEADER_LONG = 2 };
+enum { CLS_FOLLOWER = 0, CLS_LEADER = 1, CLS_LEADER_LONG = 2, CLS_PROMOTED = 3 };
 
 static __device__ __forceinline__ bool is_n_at(const uint8_t *nmask, long long k, long long len)
 {
@@ -526,15 +560,16 @@ __global__ void specl_init_kernel(SpecLState *st, const sfe_box *accepted, const
     const long long nacc = *n_accepted;
     for (long long k = lane; k < nacc; k += 32) act[k] = accepted[k];
     if (lane == 0) { st->cursor = 0; st->win_n = 0; st->nact = nacc; st->nacc = nacc; st->overflow = 0; st->spec_hi = 0; st->esc = 1;
-                     st->last_stop = -1; st->n_forced = 0; st->n_stops = 0; }
+                     st->last_stop = -1; st->n_forced = 0; st->n_stops = 0; st->n_cold = 0; st->plist_rd = 0; st->plist_n = 0ULL; }
 }
 
 // ext_state[i]: 0 = not extended, 1 = extended (results[i] holds it), 2 = queued in the batch being built
 // single warp
 __global__ void spec_advance_kernel(SpecLState *st, const sfe_anchor *anchors, long long n, const long long *blkmin, long long K,
-                                    long long span, int esc_max, const uint8_t *cls, uint8_t *ext_state, sfe_box *act,
+                                    long long span, int esc_max, int tol, long long gap, int lookback, const uint8_t *cls, uint8_t *ext_state, sfe_box *act,
                                     int min_score, sfe_box *accepted, long long accepted_cap, long long *win_idx,
-                                    sfe_anchor *win_anchors, uint8_t *win_prio, uint8_t *keep, sfe_result *results, sfe_stats *stats)
+                                    sfe_anchor *win_anchors, uint8_t *win_prio, uint8_t *keep, sfe_result *results, sfe_stats *stats,
+                                    const int32_t *plist)
 {
     const int lane = threadIdx.x & 31;
     long long j = st->cursor, nact = st->nact, nacc = st->nacc;
@@ -597,14 +632,40 @@ __global__ void spec_advance_kernel(SpecLState *st, const sfe_anchor *anchors, l
     }
     // ---- the next batch: the anchor(s) the commit waits for, then every leader of the look-ahead span ----
     long long esc = st->esc, last_stop = st->last_stop, n_forced = 0;
+    bool cold = false; long long cdiag = 0; int cstrand = 0;
     if (stopped) {
         esc = (last_stop >= 0 && j - last_stop <= 4096) ? (2 * esc < esc_max ? 2 * esc : esc_max) : 1;
         last_stop = j;
+        // Cold diagonal: the nearest EXTENDED predecessor on the stop anchor's diagonal came out below tau (it masks
+        // nothing, R18), so the anchors behind it on that diagonal are not covered either and will most likely score the
+        // same: false homology, repeats, a diagonal through N runs.  Their extensions are short and independent of one
+        // another -- take every one of them in the look-ahead at once instead of one commit stop each.
+        const sfe_anchor sa = anchors[j];
+        cdiag = sa.tpos - sa.qpos; cstrand = sa.strand >= 0 ? 1 : -1;
+        long long best_d = 0x7fffffffffffffffLL; int best_below = 0;
+        for (long long base = j - 1; base >= 0 && base > j - 1 - lookback; base -= 32) {
+            const long long x = base - lane;
+            long long d = 0x7fffffffffffffffLL; int below = 0;
+            if (x >= 0 && x > j - 1 - lookback && ext_state[x] == 1) {
+                const sfe_anchor pa = anchors[x];
+                const long long dd = (pa.tpos - pa.qpos) - cdiag;
+                if ((pa.strand >= 0 ? 1 : -1) == cstrand && pa.pair == sa.pair && dd <= tol && dd >= -tol && sa.tpos - pa.tpos <= gap && sa.tpos >= pa.tpos) {
+                    d = j - x; below = results[x].score < min_score;
+                }
+            }
+            for (int o = 16; o > 0; o >>= 1) {
+                const long long od = __shfl_xor_sync(FULL, d, o); const int ob = __shfl_xor_sync(FULL, below, o);
+                if (od < d) { d = od; below = ob; }
+            }
+            if (d < best_d) { best_d = d; best_below = below; }
+        }
+        cold = esc_max > 1 && best_d != 0x7fffffffffffffffLL && best_below;      // esc_max == 1: no escalation of any kind
     }
     long long wn = 0;
     if (j < n) {
-        // forced: the first `esc` not-extended anchors from the cursor that no active box covers
-        long long want = stopped ? esc : 0;
+        // forced: the first `esc` not-extended anchors from the cursor that no active box covers -- or, on a cold diagonal,
+        // every not-extended anchor of that diagonal in the next 8192
+        long long want = stopped ? (cold ? K : esc) : 0;
         for (long long p = j; p < n && want > 0 && wn < K && p < j + 8192; ) {
             const long long blk = p >> 5;
             const long long i = (blk << 5) + lane;
@@ -614,6 +675,10 @@ __global__ void spec_advance_kernel(SpecLState *st, const sfe_anchor *anchors, l
             if (valid) {
                 an = anchors[i];
                 take = ext_state[i] == 0;
+                if (cold) {
+                    const long long dd = (an.tpos - an.qpos) - cdiag;
+                    take = take && (an.strand >= 0 ? 1 : -1) == cstrand && dd <= 2 * tol && dd >= -2 * tol;
+                }
             }
             bool cov = false;
             const int strand = an.strand >= 0 ? 1 : -1;
@@ -624,11 +689,48 @@ __global__ void spec_advance_kernel(SpecLState *st, const sfe_anchor *anchors, l
             while ((long long)__popc(m) > room) m &= ~(0x80000000u >> __clz(m));     // drop the highest lanes
             if ((m >> lane) & 1u) {
                 const long long d = wn + __popc(m & ((1u << lane) - 1));
-                win_idx[d] = i; win_anchors[d] = an; win_prio[d] = 1; ext_state[i] = 2;
+                win_idx[d] = i; win_anchors[d] = an; win_prio[d] = cold ? 0 : 1; ext_state[i] = 2;
             }
             const long long got = __popc(m);
             wn += got; want -= got; n_forced += got;
             p = ((blk + 1) << 5);
+        }
+        // promoted followers (spec_promote_kernel's list; any order): those still ahead of the cursor and not extended yet
+        {
+            long long rd = st->plist_rd;
+            const long long pn = (long long)st->plist_n;
+            while (rd < pn && wn < K) {
+                const long long x = rd + lane;
+                long long i = -1;
+                sfe_anchor an; an.tpos = an.qpos = 0; an.pair = 0; an.strand = 1;
+                bool take = false;
+                if (x < pn) {
+                    i = plist[x];
+                    if (i >= j && i < j + span && ext_state[i] == 0) { an = anchors[i]; take = true; }
+                }
+                if (__any_sync(FULL, take)) {
+                    bool cov = false;
+                    const int strand = an.strand >= 0 ? 1 : -1;
+                    for (long long k = 0; k < nact; k++) { const sfe_box b = act[k]; cov = cov || box_has(b, an.tpos, an.qpos, strand); }
+                    take = take && !cov;
+                }
+                unsigned m = __ballot_sync(FULL, take);
+                long long adv = 32;
+                if ((long long)__popc(m) > K - wn) {               // the batch is full: stop inside this group of 32
+                    unsigned keepm = 0; long long room = K - wn;
+                    for (unsigned mm = m; mm && room > 0; mm &= mm - 1, room--) keepm |= mm & (0u - mm);
+                    adv = 31 - __clz(keepm) + 1;
+                    m = keepm;
+                }
+                if ((m >> lane) & 1u) {
+                    const long long d = wn + __popc(m & ((1u << lane) - 1));
+                    win_idx[d] = i; win_anchors[d] = an; win_prio[d] = 0; ext_state[i] = 2;
+                }
+                wn += __popc(m);
+                rd += adv;
+            }
+            if (rd > pn) rd = pn;
+            if (lane == 0) st->plist_rd = rd;
         }
         // speculative: leaders of [max(spec_hi, cursor), cursor + span) that are not extended yet
         long long p = st->spec_hi > j ? st->spec_hi : j;
@@ -674,7 +776,7 @@ __global__ void spec_advance_kernel(SpecLState *st, const sfe_anchor *anchors, l
     }
     if (lane == 0) {
         st->cursor = j; st->win_n = wn; st->nact = nact; st->nacc = nacc; if (overflow) st->overflow = 1;
-        st->esc = esc; st->last_stop = last_stop; st->n_forced += n_forced; st->n_stops += stopped ? 1 : 0;
+        st->esc = esc; st->last_stop = last_stop; st->n_forced += n_forced; st->n_stops += stopped ? 1 : 0; st->n_cold += cold ? 1 : 0;
         if (stats) {
             stats->n_anchors += c_dec; stats->n_kept += c_kept; stats->n_covered += c_cov; stats->n_below += c_below;
             stats->cells_total += cells_tot; stats->cells_covered += cells_cov;
@@ -691,6 +793,42 @@ __global__ void spec_store_kernel(const sfe_result *wres, const long long *win_i
     const long long i = win_idx[k];
     results[i] = wres[k];
     ext_state[i] = 1;
+}
+
+// After a batch: anchors the classifier called followers are promoted to leaders where the result of the anchor they
+// follow shows that they will NOT be covered by it -- it scored below tau (R18: it masks nothing; a cold diagonal), or
+// they lie beyond its box (an alignment that stopped right at its own anchor, e.g. at the edge of an N run: every later
+// anchor of that diagonal starts another one).  They are extended together in the next batch instead of costing one
+// commit stop each.  Parallel over the batch; scans ahead while the target distance is within `reach`.
+__global__ void spec_promote_kernel(const sfe_result *wres, const long long *win_idx, long long wn, const sfe_anchor *anchors,
+                                    long long n, int min_score, int tol, long long reach, int max_ahead, const uint8_t *ext_state,
+                                    uint8_t *cls, SpecLState *st, int32_t *plist)
+{
+    const long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (k >= wn) return;
+    const long long i = win_idx[k];
+    const sfe_result r = wres[k];
+    const sfe_anchor a = anchors[i];
+    const bool below = r.score < min_score;
+    const long long diag = a.tpos - a.qpos;
+    const int strand = a.strand >= 0 ? 1 : -1;
+    for (long long j = i + 1; j < n && j <= i + max_ahead; j++) {
+        const sfe_anchor f = anchors[j];
+        if (f.tpos - a.tpos > reach || f.tpos < a.tpos) break;
+        if ((f.strand >= 0 ? 1 : -1) != strand || f.pair != a.pair) continue;
+        const long long dd = (f.tpos - f.qpos) - diag;
+        if (dd > 2 * tol || dd < -2 * tol) continue;
+        const uint8_t cj = cls[j];
+        // the next leader / extended anchor of this diagonal owns whatever follows it
+        if (cj == CLS_LEADER || cj == CLS_LEADER_LONG || ext_state[j] != 0) break;
+        if (cj == CLS_PROMOTED) continue;
+        if (below || f.tpos > r.tend || f.qpos > r.qend || f.tpos < r.tstart || f.qpos < r.qstart) {
+            // claim the byte (FOLLOWER = 0 -> PROMOTED = 3) in its 32-bit word; the first claimer appends the anchor to the list
+            const unsigned sh = 8u * (unsigned)(j & 3);
+            const unsigned old = atomicOr((unsigned *)(cls + (j & ~3LL)), (unsigned)CLS_PROMOTED << sh);
+            if (((old >> sh) & 0xffu) == CLS_FOLLOWER) plist[atomicAdd(&st->plist_n, 1ULL)] = (int32_t)j;
+        }
+    }
 }
 
 __global__ void specl_finish_kernel(const SpecLState *st, long long *n_accepted_io)
@@ -714,12 +852,12 @@ int sfe_launch_specl_prepare(const sfe_anchor *anchors, long long n, const uint8
 }
 
 int sfe_launch_spec_advance(void *state, const sfe_anchor *anchors, long long n, const long long *blkmin, long long K, long long span,
-                            int esc_max, const uint8_t *cls, uint8_t *ext_state, sfe_box *act, int min_score, sfe_box *accepted,
+                            int esc_max, int tol, long long gap, int lookback, const uint8_t *cls, uint8_t *ext_state, sfe_box *act, int min_score, sfe_box *accepted,
                             long long accepted_cap, long long *win_idx, sfe_anchor *win_anchors, uint8_t *win_prio, uint8_t *keep,
-                            sfe_result *results, sfe_stats *stats, cudaStream_t st)
+                            sfe_result *results, sfe_stats *stats, const int32_t *plist, cudaStream_t st)
 {
-    SFE_KL spec_advance_kernel<<<1, 32, 0, st>>>((SpecLState *)state, anchors, n, blkmin, K, span, esc_max, cls, ext_state, act, min_score,
-                                                 accepted, accepted_cap, win_idx, win_anchors, win_prio, keep, results, stats);
+    SFE_KL spec_advance_kernel<<<1, 32, 0, st>>>((SpecLState *)state, anchors, n, blkmin, K, span, esc_max, tol, gap, lookback, cls, ext_state, act, min_score,
+                                                 accepted, accepted_cap, win_idx, win_anchors, win_prio, keep, results, stats, plist);
     SFE_LAUNCH_CHECK();
 }
 
@@ -729,6 +867,17 @@ int sfe_launch_spec_store(const sfe_result *wres, const long long *win_idx, long
     if (wn <= 0) return SFE_OK;
     const int bs = 256;
     SFE_KL spec_store_kernel<<<(unsigned)((wn + bs - 1) / bs), bs, 0, st>>>(wres, win_idx, wn, results, ext_state);
+    SFE_LAUNCH_CHECK();
+}
+
+int sfe_launch_spec_promote(const sfe_result *wres, const long long *win_idx, long long wn, const sfe_anchor *anchors, long long n,
+                            int min_score, int tol, long long reach, int max_ahead, const uint8_t *ext_state, uint8_t *cls, void *state,
+                            int32_t *plist, cudaStream_t st)
+{
+    if (wn <= 0) return SFE_OK;
+    const int bs = 128;
+    SFE_KL spec_promote_kernel<<<(unsigned)((wn + bs - 1) / bs), bs, 0, st>>>(wres, win_idx, wn, anchors, n, min_score, tol, reach, max_ahead, ext_state, cls,
+                                                                              (SpecLState *)state, plist);
     SFE_LAUNCH_CHECK();
 }
 

@@ -512,7 +512,7 @@ def test_speculate_leaders_equals_serial_loop(sfe, oracle, K, force):
             out = _speculate(sfe, w, K, flags=B.WANT_CIGAR | B.SPEC_LEADERS)
             info = sfe.last_speculate_info()
         finally:
-            sfe.set_option(B.OPT_FORCE_CLASS, 0); sfe.set_option(B.OPT_SPEC_SPAN, 65536)
+            sfe.set_option(B.OPT_FORCE_CLASS, 0); sfe.set_option(B.OPT_SPEC_SPAN, 1 << 20)
         assert out["keep"].tolist() == ser["state"].tolist(), (K, force)
         st = out["stats"]
         skipped = (out["results"]["status"] & B.ST_SKIPPED) != 0
