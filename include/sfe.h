@@ -46,9 +46,10 @@ enum {
 #define SFE_WANT_CIGAR 1u             /* spill traceback pointers to HBM and emit CIGARs         */
 #define SFE_SCORE_ONLY 0u             /* scores, boxes and cell counts only                      */
 #define SFE_NO_BINNING 2u             /* tickets in anchor order (default: longest-first bins)   */
-#define SFE_BLOCK_KERNEL 4u           /* every half on the cooperative-warps kernel (one CTA per half, rows in order,
-                                         block-wide prefix maximum for F; same results)  */
-#define SFE_NO_BLOCK_KERNEL 8u        /* overrides SFE_BLOCK_KERNEL                               */
+#define SFE_BLOCK_KERNEL 4u           /* every half on a cooperative-warps kernel (one CTA per half, rows in order, prefix
+                                         maximum for F; same results).  By default only the longest
+                                         tickets of a pass go there, beside the warp-systolic kernel                       */
+#define SFE_NO_BLOCK_KERNEL 8u        /* warp-systolic kernel only (overrides SFE_BLOCK_KERNEL and the default split)     */
 #define SFE_CIGAR_KEPT_ONLY 16u       /* sfe_speculate with SFE_WANT_CIGAR: windows run score-only (the commit rule needs
                                          score and box only); CIGARs are produced for the KEPT anchors in one
                                          traceback batch at the end; other anchors get n_ops = 0, cigar_off = -1 */
@@ -202,6 +203,9 @@ enum {
     SFE_OPT_FORCE_CLASS,           /* [0]     testing: 1 = nobody leads, 2 = everybody leads, 3 = second half of the anchors never  */
     SFE_OPT_PROMOTE_REACH,         /* [65536] after a batch, followers within this target distance of an extended anchor that will  
                                               not cover them (it scored below tau, or they lie beyond its box) become leaders       */
+    SFE_OPT_ROW_KERNEL_CAP,        /* [2^20]  most priority tickets (long-likely leaders, known long extensions) a pass hands to the
+                                              cooperative row kernel, one CTA per half; 0 = never use it beside the systolic kernel  */
+    SFE_OPT_ROW_KERNEL_SCORE_ONLY, /* [0]     1 = also in score-only passes (there the systolic chain is currently the faster one)   */
     SFE_OPT_N
 };
 int sfe_set_option(sfe_ctx *ctx, int key, int64_t value);

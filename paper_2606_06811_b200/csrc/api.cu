@@ -8,7 +8,8 @@
 
 
 // launchers defined next to their kernels
-int sfe_launch_ydrop(const YdParams &p, bool want_tb, bool use_block, int n_sm, cudaStream_t st);
+int sfe_launch_ydrop(const YdParams &p, bool want_tb, bool use_block, int n_sm, cudaStream_t st, cudaStream_t aux,
+                     cudaEvent_t ev_fork, cudaEvent_t ev_join);
 int sfe_launch_join(const sfe_anchor *anchors, const sfe_half *halves, long long n, const long long *sel, long long n_sel,
                     int want_cigar, sfe_result *results, cudaStream_t st);
 int sfe_launch_scan_emit(const sfe_half *halves, long long n, const long long *sel, long long n_sel, const uint32_t *stage,
@@ -19,7 +20,8 @@ int sfe_launch_resolve(const sfe_anchor *anchors, const sfe_result *results, lon
                        long long accepted_cap, long long *n_accepted_io, uint8_t *keep, sfe_stats *stats, long long *blkmin,
                        sfe_box *act, cudaStream_t st);
 int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe_pair *pairs, int n_pairs, long long q_len,
-                       bool binned, const uint8_t *prio, unsigned int *hist, int32_t *tickets, cudaStream_t st);
+                       bool binned, const uint8_t *prio, unsigned int *hist, int32_t *tickets, unsigned long long *counters,
+                       long long cap_prio, long long cap_plain, cudaStream_t st);
 int sfe_launch_specl_prepare(const sfe_anchor *anchors, long long n, const uint8_t *t_nmask, long long t_len, const uint8_t *q_nmask,
                              const uint8_t *qrc_nmask, long long q_len, int tol, long long gap, int lookback, int n_break,
                              uint8_t *cls, uint8_t *ext_state, long long *blkmin, void *state, const sfe_box *accepted,
@@ -83,6 +85,7 @@ struct sfe_ctx {
     DevBuf h_tascii, h_qascii, h_t2, h_tm, h_q2, h_qm, h_r2, h_rm, h_pairs, h_anchors, h_results, h_keep, h_cigar, h_acc, h_small;
     long long info[SFE_INFO_N]; long long n_profile;
     cudaEvent_t ev0, ev1; bool ev_pending;
+    cudaStream_t aux; cudaEvent_t ev_fork, ev_join;     // the cooperative row kernel runs beside the systolic one
     double kernel_us;
 };
 
@@ -131,9 +134,12 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
     memset(c->spec_info, 0, sizeof c->spec_info);
     c->opt[SFE_OPT_LEADER_DIAG_TOL] = 48; c->opt[SFE_OPT_LEADER_GAP] = 2000; c->opt[SFE_OPT_LEADER_LOOKBACK] = 64;
     c->opt[SFE_OPT_LEADER_NBREAK] = 64; c->opt[SFE_OPT_SPEC_SPAN] = 1 << 20; c->opt[SFE_OPT_SPEC_ESC_MAX] = 64;
-    c->opt[SFE_OPT_SPARSE_WARPS] = 4; c->opt[SFE_OPT_FORCE_CLASS] = 0; c->opt[SFE_OPT_PROMOTE_REACH] = 65536;
+    c->opt[SFE_OPT_SPARSE_WARPS] = 4; c->opt[SFE_OPT_FORCE_CLASS] = 0; c->opt[SFE_OPT_PROMOTE_REACH] = 65536; c->opt[SFE_OPT_ROW_KERNEL_CAP] = 1 << 20; c->opt[SFE_OPT_ROW_KERNEL_SCORE_ONLY] = 0;
     c->ev_pending = false; c->kernel_us = 0.0; c->n_profile = 0;
-    if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) { delete c; return SFE_ECUDA; }
+    if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&c->aux, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); delete c; return SFE_ECUDA; }
     if (cudaMalloc((void **)&c->pool, (size_t)nch * SFE_CHUNK_BYTES) != cudaSuccess ||
         cudaMalloc((void **)&c->chunk_prev, (size_t)nch * sizeof(int32_t)) != cudaSuccess ||
         cudaMalloc((void **)&c->free_ring, (size_t)nch * sizeof(int32_t)) != cudaSuccess ||
@@ -162,7 +168,8 @@ extern "C" int sfe_destroy(sfe_ctx *c)
     if (c->counters) cudaFree(c->counters);
     if (c->counters_host) cudaFreeHost(c->counters_host);
     if (c->state_host) cudaFreeHost(c->state_host);
-    cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1);
+    cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1); cudaEventDestroy(c->ev_fork); cudaEventDestroy(c->ev_join);
+    if (c->aux) { cudaStreamSynchronize(c->aux); cudaStreamDestroy(c->aux); }
     DevBuf *bufs[] = {&c->sp_cls, &c->sp_ext, &c->sp_prio, &c->sp_plist, &c->sp_kanchors, &c->sp_kidx, &c->sp_kres, &c->sp_state, &c->sp_idx, &c->sp_anchors, &c->sp_results, &c->sp_local, &c->sp_blkmin, &c->sp_act, &c->ops_stage, &c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
                       &c->h_t2, &c->h_tm, &c->h_q2, &c->h_qm, &c->h_r2, &c->h_rm, &c->h_pairs, &c->h_anchors, &c->h_results,
                       &c->h_keep, &c->h_cigar, &c->h_acc, &c->h_small};
@@ -279,7 +286,7 @@ static int timed_ydrop(sfe_ctx *c, const YdParams &p, bool want_tb, uint32_t fla
 {
     harvest_kernel_time(c);
     SFE_CUDA_CHECK(cudaEventRecord(c->ev0, c->stream));
-    const int rc = sfe_launch_ydrop(p, want_tb, pick_block_kernel(c, p.n_tickets, flags), c->n_sm, c->stream);
+    const int rc = sfe_launch_ydrop(p, want_tb, pick_block_kernel(c, p.n_tickets, flags), c->n_sm, c->stream, c->aux, c->ev_fork, c->ev_join);
     if (rc) return rc;
     SFE_CUDA_CHECK(cudaEventRecord(c->ev1, c->stream));
     c->ev_pending = true;
@@ -359,8 +366,13 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
     p.srow_hi = (uint32_t)(uint8_t)(int8_t)sc->n_score | (0xE0u << 16);
 
     SFE_CUDA_CHECK(cudaMemsetAsync(c->counters, 0, CNT_N * sizeof(unsigned long long), c->stream));
+    // the longest tickets go to the cooperative row kernel (one CTA per half) unless the caller pinned the kernel choice
+    const bool row_split = !(flags & (SFE_BLOCK_KERNEL | SFE_NO_BLOCK_KERNEL | SFE_NO_BINNING)) && sc->prune_lag == SFE_PRUNE_LAG &&
+                           c->opt[SFE_OPT_ROW_KERNEL_CAP] > 0 && (want_tb || c->opt[SFE_OPT_ROW_KERNEL_SCORE_ONLY]);
+    p.row_split = row_split ? 1 : 0;
     if ((rc = sfe_launch_tickets(anchors_dev, n_anchors, pairs_dev, n_pairs, q_len, !(flags & SFE_NO_BINNING), prio_dev,
-                                 (unsigned int *)c->hist.p, (int32_t *)c->tickets.p, c->stream))) return rc;
+                                 (unsigned int *)c->hist.p, (int32_t *)c->tickets.p, c->counters, row_split ? c->opt[SFE_OPT_ROW_KERNEL_CAP] : 0,
+                                 row_split ? c->n_sm / 2 : 0, c->stream))) return rc;
     if ((rc = timed_ydrop(c, p, want_tb, flags))) return rc;
     c->info[0] += 1; c->info[1] += 2 * n_anchors; c->n_profile = 2 * n_anchors;
     if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, nullptr, n_anchors, want_tb, results_dev, c->stream))) return rc;

@@ -54,6 +54,23 @@ __global__ void bin_scatter_kernel(const sfe_anchor *anchors, long long n_anchor
     tickets[atomicAdd(&hist[64 + b], 1u)] = (int32_t)h;
 }
 
+// How many of the longest-first tickets go to the cooperative row kernel (ydrop_row_kernel.cu): the priority bins
+// (32..63: long-likely leaders / known long extensions) if there are any, up to cap_prio; else whole proxy bins from the top
+// while they hold at most cap_plain tickets and promise at least 2^min_bin rows.  One CTA works on one such half.
+__global__ void row_split_kernel(const unsigned int *hist, unsigned long long *counters, unsigned int cap_prio, unsigned int cap_plain,
+                                 int min_bin)
+{
+    if (threadIdx.x != 0) return;
+    unsigned int n = 0;
+    for (int b = 63; b >= 32; b--) n += hist[b];
+    if (n > 0) { counters[CNT_ROW_N] = n < cap_prio ? n : cap_prio; return; }
+    for (int b = 31; b >= min_bin; b--) {
+        if (n + hist[b] > cap_plain) break;
+        n += hist[b];
+    }
+    counters[CNT_ROW_N] = n;
+}
+
 __global__ void iota_tickets_kernel(int32_t *tickets, long long n)
 {
     const long long h = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -61,7 +78,8 @@ __global__ void iota_tickets_kernel(int32_t *tickets, long long n)
 }
 
 int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe_pair *pairs, int n_pairs, long long q_len,
-                       bool binned, const uint8_t *prio, unsigned int *hist, int32_t *tickets, cudaStream_t st)
+                       bool binned, const uint8_t *prio, unsigned int *hist, int32_t *tickets, unsigned long long *counters,
+                       long long cap_prio, long long cap_plain, cudaStream_t st)
 {
     const long long n = 2 * n_anchors;
     if (n <= 0) return SFE_OK;
@@ -73,6 +91,7 @@ int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe
         SFE_KL bin_count_kernel<<<nb, bs, 0, st>>>(anchors, n_anchors, pairs, n_pairs, q_len, prio, hist);
         SFE_KL bin_offsets_kernel<<<1, 32, 0, st>>>(hist);
         SFE_KL bin_scatter_kernel<<<nb, bs, 0, st>>>(anchors, n_anchors, pairs, n_pairs, q_len, prio, hist, tickets);
+        if (cap_prio > 0 || cap_plain > 0) SFE_KL row_split_kernel<<<1, 32, 0, st>>>(hist, counters, (unsigned int)cap_prio, (unsigned int)cap_plain, 12);
     }
     SFE_LAUNCH_CHECK();
 }

@@ -79,7 +79,8 @@ struct sfe_half {                 // result of one one-sided extension (a7)
     uint32_t smid, wslot;         // SM and hardware warp slot that ran it
 };
 
-enum { CNT_TICKET = 0, CNT_RING_DROPS, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_OPS, CNT_MAXNEED, CNT_CLASS0, CNT_CLASS1, CNT_CLASS2, CNT_CLASS3, CNT_BLOCK_HALVES, CNT_N = 16 };
+enum { CNT_TICKET = 0, CNT_RING_DROPS, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_OPS, CNT_MAXNEED, CNT_CLASS0, CNT_CLASS1, CNT_CLASS2, CNT_CLASS3, CNT_BLOCK_HALVES,
+       CNT_ROW_N, CNT_ROW_TICKET, CNT_N = 24 };
 
 struct SfeFreeRing {              // persistent across launches: every half returns its chunks before it ends
     unsigned long long head;      // pops issued
@@ -104,6 +105,8 @@ struct YdParams {
     SfeFreeRing *ring_state;
     int32_t n_chunks;
     int32_t max_warps;            // warps of the normal kernel allowed to work in this pass
+    int32_t row_all;              // row kernel: 1 = every ticket, 0 = the first counters[CNT_ROW_N] (the longest)
+    int32_t row_split;            // systolic kernel: 1 = skip the first counters[CNT_ROW_N] tickets (the row kernel takes them)
     int32_t n_classes;            // reserved ticket segments in use (set by sfe_launch_ydrop: 4, or fewer in a sparse launch)
     int32_t sparse_warps;         // > 0: resident warps per SM for a chain-bound pass (blocks of 4 warps), see sfe_launch_ydrop
     int32_t n_pairs;

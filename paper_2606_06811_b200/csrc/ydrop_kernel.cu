@@ -505,11 +505,14 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kerne
     const long long seg = p.seg_tickets;
     const int my_class = (int)(wslot >> 2);
     const int ncls = p.n_classes;                      // slot classes of this launch (1..4): segments 0 .. ncls-1 are reserved
+    // the first counters[CNT_ROW_N] tickets (the longest) belong to the cooperative row kernel launched beside this one
+    const long long base = p.row_split ? (long long)*((volatile unsigned long long *)&p.counters[CNT_ROW_N]) : 0;
     for (int phase = 0; phase < 6; phase++) {
         // phase 0: my class's segment; phase 1: main queue; phases 2..5: leftovers of segments 0..3
         const int k = phase == 0 ? my_class : phase - 2;
         if (phase != 1 && (k >= ncls || seg == 0)) continue;
-        const long long lo = phase == 1 ? (seg ? ncls * seg : 0) : k * seg;
+        const long long lo0 = base + (phase == 1 ? (seg ? ncls * seg : 0) : k * seg);
+        const long long lo = lo0 < p.n_tickets ? lo0 : p.n_tickets;
         const long long hi = phase == 1 ? p.n_tickets : (lo + seg < p.n_tickets ? lo + seg : p.n_tickets);
         unsigned long long *cnt = &p.counters[phase == 1 ? CNT_TICKET : CNT_CLASS0 + k];
         for (;;) {
@@ -556,6 +559,7 @@ __global__ void __launch_bounds__(32) ydrop_wide_kernel(const YdParams p)
 }
 
 int sfe_launch_ydrop_block(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st);
+int sfe_launch_ydrop_row(const YdParams &p, bool want_tb, long long grid, cudaStream_t st);
 
 // Function attributes are per DEVICE: sfe_create calls this after cudaSetDevice, for every context.
 int sfe_ydrop_init_device(void)
@@ -568,14 +572,30 @@ int sfe_ydrop_init_device(void)
 
 // use_block: the whole pass goes to the row-synchronous block kernel (ydrop_block_kernel.cu) instead of the
 // warp-systolic one; either way halves whose band outgrew the window are re-run by the wide kernel.
-int sfe_launch_ydrop(const YdParams &p_in, bool want_tb, bool use_block, int n_sm, cudaStream_t st)
+// use_block: every half on a cooperative kernel (the row kernel; Lambda = 0: the first block kernel).  Otherwise the
+// warp-systolic kernel, and -- row_split -- the row kernel beside it on `aux` for the first counters[CNT_ROW_N] (longest)
+// tickets; fork / join through the two events.
+int sfe_launch_ydrop(const YdParams &p_in, bool want_tb, bool use_block, int n_sm, cudaStream_t st, cudaStream_t aux,
+                     cudaEvent_t ev_fork, cudaEvent_t ev_join)
 {
     YdParams p = p_in;
     p.n_classes = 4;
+    const bool split = !use_block && p.row_split && aux != nullptr;
+    if (!split) p.row_split = 0;
     if (use_block) {
-        const int rc = sfe_launch_ydrop_block(p, want_tb, n_sm, st);
+        int rc;
+        if (p.lag0) rc = sfe_launch_ydrop_block(p, want_tb, n_sm, st);
+        else { p.row_all = 1; rc = sfe_launch_ydrop_row(p, want_tb, p.n_tickets < 2LL * n_sm ? p.n_tickets : 2LL * n_sm, st); }
         if (rc) return rc;
     } else {
+        if (split) {                                              // launched FIRST so that its CTAs get their SM resources
+            SFE_CUDA_CHECK(cudaEventRecord(ev_fork, st));
+            SFE_CUDA_CHECK(cudaStreamWaitEvent(aux, ev_fork, 0));
+            p.row_all = 0;
+            const int rc = sfe_launch_ydrop_row(p, want_tb, p.n_tickets < (long long)n_sm ? p.n_tickets : (long long)n_sm, aux);
+            if (rc) return rc;
+            SFE_CUDA_CHECK(cudaEventRecord(ev_join, aux));
+        }
         int warps_per_block = SFE_BLOCK_THREADS / 32;
         size_t smem = (size_t)warps_per_block * SFE_WARP_SMEM;
         int bps = 0;
@@ -605,6 +625,7 @@ int sfe_launch_ydrop(const YdParams &p_in, bool want_tb, bool use_block, int n_s
         if (blocks < 1) blocks = 1;
         if (want_tb) SFE_KL ydrop_kernel<true><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
         else SFE_KL ydrop_kernel<false><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
+        if (split) SFE_CUDA_CHECK(cudaStreamWaitEvent(st, ev_join, 0));
     }
     const int bs = 256;
     SFE_KL select_wide_kernel<<<(unsigned)((p.n_tickets + bs - 1) / bs), bs, 0, st>>>(p);

@@ -1,0 +1,431 @@
+// ydrop_row_kernel.cu -- cooperative warps per anchor-half, second design ("8 warps
+// per anchor-half ... kernel wall time / 3.3"), for the LONG halves whose serial chain bounds a pass.
+//
+// Why a second kernel.  With the row-lagged threshold (R4, Lambda = 32) at most 32 rows of one extension can be in flight:
+// the warp-systolic kernel turns a half of n rows into ~ n/32 (W + 62) dependent wavefront steps, measured 1,016 cycles per
+// row score-only and 2,270 with traceback on a 580 k-row half of configs[4] (profiles/r2_*), whatever else the GPU does.
+// The parallelism that is left is ALONG a row: one CTA per half, rows strictly in order, every thread owns RK_C consecutive
+// columns of a 1024-column window.  The first cooperative kernel (ydrop_block_kernel.cu, kept for Lambda = 0) spent ~700
+// instructions per thread per row and two block barriers on that and was slower than the chain it should replace.  Here:
+//   * ONE block barrier per row (the exchange of the warps' F carries); the diagonal hand-off between neighbouring warps
+//     is an 8-byte {value, row} word that the reader polls (it is there by the time it is needed);
+//   * F(i,j) = max_{j'<j} (H~(i,j') - O - X (j - j')), H~ = max(M, E): a sequential max-plus chain over the thread's own
+//     columns (DPX VIADDMNMX), one shuffle scan per warp (shfl_up returns the caller's own value out of range, so a max
+//     scan needs no predicate), one 4-entry combine across warps;
+//   * everything that is not needed for the next row is LAGGED: per-row maxima (for T of row i + 32), alive bounds (cell
+//     count, end of the half, window position) go to shared-memory rings and are folded every 16 rows;
+//   * the column -> (warp, lane, slot) map is fixed modulo the window, so a traceback row is a fixed 512-byte record the
+//     walk can address without any directory, and a thread's 8 nibbles are exactly one coalesced 32-bit store;
+//   * the "F extended" bit is stored with the cell the gap run CONTINUES FROM (F(i,j) - X > H(i,j) - (O+X): the cell's own
+//     values) instead of the cell it arrives at, so no final H crosses a thread boundary within a row.
+// Exactness (same argument as ydrop_block_kernel.cu): E depends on the column above only; the prefix maximum over H~ equals
+// the recurrence over H because a gap opened from an H that came from F never beats extending that F (O >= 0); by the R6
+// lemma cells that are dead or outside the window (which starts at or left of the first alive column of an older row; that
+// column never moves left) contribute nothing an alive cell, its H or a pointer on an alive path depends on.  Score, end
+// cell (first maximum, R7), cell count (R28) and CIGAR (R11, R12) are the oracle's at Lambda = 32: same tests as ydrop_kernel.
+#include "ydrop_common.cuh"
+
+#define RK_NW 4                              // warps per CTA: one per SM sub-partition
+#define RK_C 8                               // columns per thread
+#define RK_THREADS (32 * RK_NW)
+#define RK_WCOLS (32 * RK_C)                 // columns per warp (256): the window moves in steps of this
+#define RK_WIN (RK_THREADS * RK_C)           // 1024
+#define RK_ROW_WORDS RK_THREADS              // traceback record of a row: one word (8 nibbles) per thread = 512 B
+#define RK_CHUNK_ROWS (SFE_CHUNK_BYTES / (4 * RK_ROW_WORDS))     // 128 rows per 64-KiB chunk
+#define RK_NINF (-(1 << 30) - (1 << 28))     // identity of the max-plus scans: the decay terms (< 2^27) fit below it, and H - O - F with
+                                             // H < 2^29 (R25) stays inside int32
+#define RK_FOLD 16                           // rows between two folds of the lagged statistics
+#define RK_POLL_LIMIT (1 << 22)
+
+struct RkShared {
+    unsigned long long edge[RK_NW];          // by warp: {row << 32 | gated H - OX of its last column after that row}: ONE 8-byte word
+    int carry[2][RK_NW];                     // by row parity, warp: F leaving the warp to the right (before the decay)
+    int rmax[64][RK_NW];                     // by row & 63, warp: max H of the row (any cell: a dead one never raises the best)
+    int rlo[64][RK_NW], rhi[64][RK_NW];      // first / last alive column of the row in the warp's block (lo > hi: none)
+    int new_chunk;
+    int fail_row;                            // row in which a bounded wait ran out (never expected; -1 = none): SFE_ST_INTERNAL
+    int wide_row;                            // row in which the window's last column held an alive cell (-1 = none): the band outgrew it
+    int red_s[RK_NW], red_i[RK_NW], red_j[RK_NW];
+    uint32_t opsbuf[SFE_WALK_OPS];
+};
+
+// exclusive prefix over the warps LEFT of rank `rho` in the window of the carries published for this row:
+//   max_{rho' < rho} carry[rho'] - Dw (rho - 1 - rho'),  Dw = X * RK_WCOLS
+static __device__ __forceinline__ int warp_carry_in(const int *carry, int rho, int wsb, int Dw, int lane)
+{
+    int v = RK_NINF;
+    if (lane < RK_NW) {
+        const int r = (lane - wsb) & (RK_NW - 1);                 // rank of warp `lane`
+        if (r < rho) v = carry[lane] - Dw * (rho - 1 - r);
+    }
+    return __reduce_max_sync(FULL, v);
+}
+
+// ---- a8: walk the fixed-size row records from the end cell to the origin (warp 0; every lane holds the same state) ----
+// Nibble of cell (i, j): word (j mod RK_WIN) / RK_C of row i's record, bits 4 (RK_C - 1 - j mod RK_C) ..:
+//   bit3 = H not from M, bit2 = H not from E, bit1 = E extended (R11), bit0 = the F of the NEXT column extends this cell's F.
+static __device__ bool row_walk(const YdParams &p, RkShared &sh, const int end_i, const int end_j, int chunk, const int lane,
+                                uint32_t &ops_seg, int &n_ops, bool &ops_ok)
+{
+    OpsWriter ow;
+    ow.buf = sh.opsbuf; ow.stage = p.ops_stage; ow.used = &p.counters[CNT_OPS]; ow.cap = p.ops_cap;
+    ow.nbuf = 0; ow.nops = 0; ow.cur_op = -1; ow.run = 0; ow.prev_seg = SFE_NO_SEG; ow.ok = true;
+    ops_seg = SFE_NO_SEG; n_ops = 0; ops_ok = true;
+    if (end_i == 0 && end_j == 0) return true;
+    if (chunk < 0) return false;
+    // `chunk` holds the rows of ordinal `ord`; the chain runs backwards through chunk_prev
+    int ord = end_i / RK_CHUNK_ROWS;
+    int prev = __ldcg(p.chunk_prev + chunk);
+    int i = end_i, j = end_j, state = 0;
+    long long guard = 3LL * ((long long)end_i + end_j) + 64;
+    auto nibble = [&](int r, int c) -> uint32_t {
+        const int o = r / RK_CHUNK_ROWS;
+        const int ch = o == ord ? chunk : prev;                  // 32 consecutive rows span at most two chunks
+        const uint32_t w = __ldcg(p.pool + (size_t)ch * (SFE_CHUNK_BYTES / 4) + (size_t)(r - o * RK_CHUNK_ROWS) * RK_ROW_WORDS +
+                                  ((c & (RK_WIN - 1)) / RK_C));
+        return (w >> (4 * (RK_C - 1 - (c & (RK_C - 1))))) & 15u;
+    };
+    while (!(i == 0 && j == 0 && state == 0)) {
+        if (--guard < 0) return false;
+        while (i / RK_CHUNK_ROWS < ord) {                        // the walk left the current chunk's rows
+            chunk = prev; ord--;
+            if (chunk < 0) return false;
+            prev = __ldcg(p.chunk_prev + chunk);
+        }
+        if (prev < 0 && ord > 0) return false;
+        if (state == 2) {
+            // F: emit D, go left; the run continues while the cell we arrive at says "my F is extended into the next column"
+            const int jx = j - 1 - lane;
+            const bool valid = jx >= 0;
+            uint32_t nib = 0;
+            if (valid) nib = nibble(i, jx);
+            const uint32_t stop = __ballot_sync(FULL, !(valid && (nib & 1u)));
+            const int pstop = stop ? __ffs(stop) - 1 : 32;       // cells j-1 .. j-pstop continue; the run was opened at j-1-pstop
+            const int cnt = pstop < 32 ? pstop + 1 : 32;
+            ow.emit(SFE_OP_D, cnt, lane);
+            j -= cnt;
+            if (pstop < 32) state = 0;
+            if (j < 0) return false;
+            continue;
+        }
+        // H (diagonal) or E (up): lane x examines the x-th cell from (i, j) in the current direction
+        const int dj = state == 1 ? 0 : 1;
+        const int ix = i - lane, jx = j - lane * dj;
+        const bool valid = ix >= 0 && jx >= 0 && ix / RK_CHUNK_ROWS >= ord - 1;
+        uint32_t nib = 0;
+        if (valid) nib = nibble(ix, jx);
+        const bool cont = state == 0 ? !(nib & 8u) : (nib & 2u) != 0;
+        const bool origin = ix == 0 && jx == 0;
+        const uint32_t stop = __ballot_sync(FULL, !(valid && cont) || origin);
+        const uint32_t vmask = __ballot_sync(FULL, valid);
+        const int pstop = stop ? __ffs(stop) - 1 : 32;
+        const bool stop_valid = pstop < 32 && ((vmask >> pstop) & 1u);
+        if (pstop == 0 && !stop_valid) return false;
+        if (state == 0) {
+            ow.emit(SFE_OP_M, pstop, lane);
+            i -= pstop; j -= pstop;
+            if (stop_valid && !(i == 0 && j == 0)) {
+                const uint32_t nb = __shfl_sync(FULL, nib, pstop);
+                state = (nb & 4u) ? 2 : 1;
+            }
+        } else {
+            const int cnt = stop_valid ? pstop + 1 : pstop;
+            ow.emit(SFE_OP_I, cnt, lane);
+            i -= cnt;
+            if (stop_valid) state = 0;
+        }
+    }
+    if (ow.cur_op >= 0) ow.push(lane);
+    ow.flush(lane);
+    ops_seg = ow.prev_seg; n_ops = ow.nops; ops_ok = ow.ok;
+    return true;
+}
+
+template <bool TB>
+static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
+{
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    sfe_half out;
+    out.score = 0; out.end_i = 0; out.end_j = 0; out.status = 0; out.cells = 0;
+    out.ops_seg = SFE_NO_SEG; out.n_ops = 0; out.n_strips = 0; out.n_rec = 0; out.steps = 0; out.max_steps = 0;
+    out.cycles = 0; out.smid = 0; out.wslot = 0;
+    const long long clk0 = clock64();
+    HalfGeom g;
+    if (!half_setup(p, hid, g)) {
+        out.status = SFE_ST_BAD_ANCHOR;
+        if (tid == 0) p.halves[hid] = out;
+        return;
+    }
+    const int OX = p.OX, X = p.X, O = p.OX - p.X;
+    const int D = X * RK_C, Dw = X * RK_WCOLS;
+    const uint32_t srow_hi = p.srow_hi;
+
+    if (tid < RK_NW) { sh.edge[tid] = 0xffffffff00000000ULL | (unsigned)SFE_NEG; sh.carry[0][tid] = RK_NINF; sh.carry[1][tid] = RK_NINF; }
+    if (tid == 0) { sh.fail_row = -1; sh.wide_row = -1; sh.new_chunk = -1; }
+    __syncthreads();
+
+    int ws = 0, ws_prev = 0;                              // window start of this / the previous row (multiples of RK_WCOLS)
+    int myc0 = -1;                                        // first of my RK_C columns
+    int Hu[RK_C], Eu[RK_C];                               // previous row of my columns: gated H - OX, E
+    uint32_t sel[RK_C];
+#pragma unroll
+    for (int k = 0; k < RK_C; k++) { Hu[k] = SFE_NEG; Eu[k] = SFE_NEG; sel[k] = 0x8880u; }
+    int best = 0, best_i = 0, best_j = 0;                 // thread-local first maximum (my cells are visited in row-major order)
+    int cumbest = 0;                                      // best over alive cells of rows <= i - 32 (uniform)
+    unsigned long long cells = 0;                         // folded rows (uniform)
+    int folded = 0;                                       // rows < folded have been folded (uniform)
+    int rows_done = 0, max_width = 0, last_lo = 0;
+    bool wide = false, limit = false, done = false;
+    uint32_t srow32 = 0u;
+    int cur_chunk = -1;                                   // traceback chunk of the current 128 rows (uniform)
+    bool tb_ok = TB;
+    long long n_words = 0;
+
+    // fold the statistics of rows [folded, upto): cells, first dead row, newest alive bounds.  Uniform: every warp reads the
+    // same shared-memory rings (written >= 16 block barriers ago).  Returns false when a row without an alive cell was found.
+    auto fold = [&](int upto, int &new_lo, int &new_hi) -> bool {
+        bool alive_all = true;
+        while (folded < upto) {
+            const int r = folded + lane;
+            int lo = 0x7fffffff, hi = -1;
+            if (r < upto) {
+#pragma unroll
+                for (int w = 0; w < RK_NW; w++) { lo = min(lo, sh.rlo[r & 63][w]); hi = max(hi, sh.rhi[r & 63][w]); }
+            }
+            const unsigned nb = r < upto ? 1u : 0u;
+            const unsigned deadm = __ballot_sync(FULL, nb && hi < lo);
+            const int nrows = min(32, upto - folded);
+            const int ndead_first = deadm ? __ffs(deadm) - 1 : nrows;            // rows before the first dead one count
+            const int width = (nb && lane < ndead_first) ? hi - lo + 1 : 0;
+            unsigned long long wsum = (unsigned long long)width;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) wsum += __shfl_xor_sync(FULL, wsum, o);
+            cells += wsum;
+            max_width = max(max_width, __reduce_max_sync(FULL, width));
+            if (ndead_first > 0) {
+                new_lo = __shfl_sync(FULL, lo, ndead_first - 1); new_hi = __shfl_sync(FULL, hi, ndead_first - 1);
+                rows_done = folded + ndead_first;
+            }
+            if (deadm) { alive_all = false; folded = 0x7fffffff; break; }        // everything after the first dead row is dead
+            folded += nrows;
+        }
+        return alive_all;
+    };
+
+    int i = 0;
+    for (; i <= g.n; i++) {
+        // ---- lagged housekeeping, every RK_FOLD rows: rows [i - 32, i - 16) ----
+        if ((i & (RK_FOLD - 1)) == 0 && i >= 2 * RK_FOLD) {
+            int nlo = last_lo, nhi = -1;
+            if (!fold(i - RK_FOLD, nlo, nhi)) { done = true; break; }
+            last_lo = nlo;
+            const int nws = nlo & ~(RK_WCOLS - 1);                // the first alive column never moves left: a stale one is safe
+            // the last alive column grows by at most one per row: rows up to the next fold stay below nhi + 2 RK_FOLD + 1
+            if (nhi + 2 * RK_FOLD + 2 >= nws + RK_WIN) { wide = true; break; }
+            ws_prev = ws; ws = nws;
+        } else ws_prev = ws;
+        if ((i & 31) == 0) {
+            const int r = i + lane;
+            srow32 = (r == 0 || r > g.n) ? 0u : p.srow[sfe_base(g.qc, g.qm, g.q0 + (long long)g.d * r)];
+        }
+        const uint32_t srow_lo = __shfl_sync(FULL, srow32, i & 31);
+        // ---- R4: T(i) = best(rows <= i - 32) - ydrop ----
+        if (i >= 32) {
+            const int rm = lane < RK_NW ? sh.rmax[(i - 32) & 63][lane] : SFE_NEG;
+            cumbest = max(cumbest, __reduce_max_sync(FULL, rm));
+            if (cumbest >= SFE_SCORE_LIMIT) { limit = true; break; }              // R25
+        }
+        const int T = p.ydrop_inf ? SFE_T_INF : cumbest - p.Y;
+        // ---- my columns in this row's window ----
+        const int wsb = ws / RK_WCOLS;
+        const int q = ((tid * RK_C) - ws) & (RK_WIN - 1);         // window position of my first column
+        const int c0 = ws + q;
+        const int rho = (warp - wsb) & (RK_NW - 1);               // my warp's rank in the window
+        if (c0 != myc0) {
+            myc0 = c0;
+#pragma unroll
+            for (int k = 0; k < RK_C; k++) { Hu[k] = SFE_NEG; Eu[k] = SFE_NEG; sel[k] = col_selector(g, c0 + k); }
+        }
+        // ---- traceback chunk of rows i .. i + 127 (popped by warp 0 before the barrier, read by everybody after it) ----
+        const bool new_chunk_row = TB && tb_ok && (i % RK_CHUNK_ROWS) == 0;
+        if (new_chunk_row && warp == 0) {
+            const int nc = chunk_pop(p.free_ring, p.ring_state, p.n_chunks, lane);
+            if (lane == 0) {
+                sh.new_chunk = nc;
+                if (nc >= 0) p.chunk_prev[nc] = cur_chunk;
+                if (nc == -2) atomicAdd(&p.counters[CNT_RING_DROPS], 1ULL);
+            }
+        }
+        // ---- diagonal of my first column: the left neighbour's previous-row value ----
+        int Hd0 = __shfl_up_sync(FULL, Hu[RK_C - 1], 1);
+        if (lane == 0) {
+            Hd0 = SFE_NEG;
+            if (i > 0 && q != 0 && c0 - 1 - ws_prev < RK_WIN) {   // column c0 - 1 was inside the previous row's window
+                volatile unsigned long long *e = &sh.edge[(warp - 1) & (RK_NW - 1)];
+                unsigned long long v = *e;
+                for (int spin = 0; (int)(v >> 32) != i - 1 && spin < RK_POLL_LIMIT; spin++) v = *e;
+                if ((int)(v >> 32) != i - 1) sh.fail_row = i;     // (readers act on it from this row's barrier on)
+                Hd0 = (int)(unsigned)v;
+            }
+        }
+        if (i == 0 && c0 == 0) Hd0 = -OX;                         // the origin (R8)
+        // ---- phase A: M, E, H~ and the in-thread F chain ----
+        int M[RK_C], E[RK_C], Ht[RK_C], gl[RK_C];                 // gl[k]: F entering column k from my own columns left of it
+        int gk = RK_NINF;
+#pragma unroll
+        for (int k = 0; k < RK_C; k++) {
+            const int Hd = k == 0 ? Hd0 : Hu[k - 1];
+            const int s = prmt_sx(srow_lo, srow_hi, sel[k]);
+            M[k] = Hd + s + OX;
+            E[k] = __viaddmax_s32(Eu[k], -X, Hu[k]);
+            Ht[k] = max(M[k], E[k]);
+            gl[k] = gk;
+            gk = __viaddmax_s32(gk, -X, Ht[k] - OX);
+        }
+        // ---- F across the threads of the warp: y = x + D lane, prefix maximum, exclusive ----
+        int y = gk + D * lane;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) y = max(y, __shfl_up_sync(FULL, y, o));      // out-of-range lanes get their own value back
+        if (lane == 31) sh.carry[i & 1][warp] = y - D * 31;        // F leaving the warp (entering the next warp's first column)
+        int yex = __shfl_up_sync(FULL, y, 1);
+        if (lane == 0) yex = RK_NINF;
+        const int fin_warp = yex - D * lane + D;                   // F entering my first column from my warp's lanes left of me
+        __syncthreads();                                                                   // the one barrier of the row
+        // both flags carry the row they were raised in: a fast warp's later write is ignored by a slow reader, so every
+        // thread leaves the loop in the same row (a non-uniform exit would hang the next barrier)
+        { const int fr = sh.fail_row; if (fr >= 0 && fr <= i) break; }
+        { const int wr = sh.wide_row; if (wr >= 0 && wr < i) { wide = true; break; } }
+        const int win = warp_carry_in(sh.carry[i & 1], rho, wsb, Dw, lane);                // F entering my warp from the left
+        const int Fin = max(fin_warp, win - D * lane);
+        if (new_chunk_row) {
+            const int nc = sh.new_chunk;
+            if (nc < 0) tb_ok = false; else cur_chunk = nc;
+        }
+        // ---- phase C: F, H, alive, next row's state, statistics, pointers ----
+        uint32_t nibs = 0, am = 0;
+        int hmax = SFE_NEG;
+        const int best_before = best;
+        int Hc[RK_C];
+        const bool oob = c0 + RK_C - 1 > g.m;                     // (only the threads at the target's end)
+#pragma unroll
+        for (int k = 0; k < RK_C; k++) {
+            const int F = max(gl[k], Fin - X * k);
+            int H = max(Ht[k], F);
+            if (oob && c0 + k > g.m) H = SFE_NEG;
+            const bool alive = H >= T;                             // R5
+            if (TB) {
+                nibs = __funnelshift_l((uint32_t)(M[k] - H), nibs, 1);           // H not from M
+                nibs = __funnelshift_l((uint32_t)(E[k] - H), nibs, 1);           // H not from E
+                nibs = __funnelshift_l((uint32_t)(Hu[k] - E[k]), nibs, 1);       // E extended (open wins ties)
+                nibs = __funnelshift_l((uint32_t)(H - O - F), nibs, 1);          // next column's F extends this F: F - X > H - (O+X)
+            }
+            Hu[k] = alive ? H - OX : SFE_NEG;
+            Eu[k] = E[k];
+            Hc[k] = H;
+            hmax = max(hmax, H);
+            if (alive) am |= 1u << k;
+        }
+        best = max(best, hmax);
+        if (best > best_before) {                                  // strict: the first maximum of my cells (R7)
+            int kk = RK_C - 1;
+#pragma unroll
+            for (int k = RK_C - 2; k >= 0; k--) kk = Hc[k] == best ? k : kk;
+            best_i = i; best_j = c0 + kk;
+        }
+        // ---- publish: edge for the next row, lagged statistics, pointers ----
+        if (lane == 31) *(volatile unsigned long long *)&sh.edge[warp] = ((unsigned long long)(unsigned)i << 32) | (unsigned)Hu[RK_C - 1];
+        if (q + RK_C == RK_WIN && (am >> (RK_C - 1))) sh.wide_row = i;            // alive in the window's last column: bail out next row
+        const int wm = __reduce_max_sync(FULL, hmax);
+        const int wlo = __reduce_min_sync(FULL, am ? c0 + __ffs(am) - 1 : 0x7fffffff);
+        const int whi = __reduce_max_sync(FULL, am ? c0 + 31 - __clz(am) : -1);
+        if (lane == 0) { sh.rmax[i & 63][warp] = wm; sh.rlo[i & 63][warp] = wlo; sh.rhi[i & 63][warp] = whi; }
+        if (TB && tb_ok) {
+            p.pool[(size_t)cur_chunk * (SFE_CHUNK_BYTES / 4) + (size_t)(i % RK_CHUNK_ROWS) * RK_ROW_WORDS + tid] = nibs;
+            n_words += RK_ROW_WORDS;
+        }
+    }
+    __syncthreads();
+    // ---- the rows not folded yet (rows 0 .. i-1 were computed) ----
+    const bool failed = sh.fail_row >= 0;
+    if (!failed && !wide && folded < i) {
+        int nlo = last_lo, nhi = -1;
+        fold(i, nlo, nhi);
+    }
+    // ---- first maximum over the threads: key (score desc, i asc, j asc) (R7) ----
+    int bs = best, bi = best_i, bj = best_j;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const int os = __shfl_xor_sync(FULL, bs, o), oi = __shfl_xor_sync(FULL, bi, o), oj = __shfl_xor_sync(FULL, bj, o);
+        if (os > bs || (os == bs && (oi < bi || (oi == bi && oj < bj)))) { bs = os; bi = oi; bj = oj; }
+    }
+    if (lane == 0) { sh.red_s[warp] = bs; sh.red_i[warp] = bi; sh.red_j[warp] = bj; }
+    __syncthreads();
+    bs = sh.red_s[0]; bi = sh.red_i[0]; bj = sh.red_j[0];
+#pragma unroll
+    for (int w = 1; w < RK_NW; w++) {
+        const int os = sh.red_s[w], oi = sh.red_i[w], oj = sh.red_j[w];
+        if (os > bs || (os == bs && (oi < bi || (oi == bi && oj < bj)))) { bs = os; bi = oi; bj = oj; }
+    }
+    out.score = bs; out.end_i = bi; out.end_j = bj; out.cells = cells;
+    out.status = (wide ? SFE_ST_WIDE_PENDING : 0u) | ((TB && !tb_ok) ? SFE_ST_PASS_OVERFLOW : 0u) | SFE_ST_BLOCK |
+                 (limit ? SFE_ST_SCORE_LIMIT : 0u) | (failed ? SFE_ST_INTERNAL : 0u);
+    // n_strips / steps feed the overflow re-run's chunk estimate (queue_kernels.cu): a row costs two 256-byte records
+    out.n_strips = 2 * rows_done; out.n_rec = (int)(n_words >> 6); out.steps = rows_done; out.max_steps = max_width;
+    // ---- a8: warp 0 walks the row records and stages the ops; then the chunks go back to the ring ----
+    if (warp == 0) {
+        if (TB && tb_ok && !wide && !limit && !failed) {
+            // the end cell's row lies in the chunk of ordinal bi / 128; cur_chunk holds the last computed row's (i - 1)
+            int ch = cur_chunk;
+            int o = (i > 0 ? i - 1 : 0) / RK_CHUNK_ROWS;
+            while (ch >= 0 && o > bi / RK_CHUNK_ROWS) { ch = __ldcg(p.chunk_prev + ch); o--; }
+            bool ops_ok = true;
+            __threadfence_block();
+            if (!row_walk(p, sh, bi, bj, ch, lane, out.ops_seg, out.n_ops, ops_ok)) out.status |= SFE_ST_INTERNAL;
+            if (!ops_ok) out.status |= SFE_ST_OPS_OVERFLOW;
+        }
+        if (TB) {
+            __threadfence();
+            __syncwarp();
+            int cc = cur_chunk;
+            while (cc >= 0) { const int prev = __ldcg(p.chunk_prev + cc); chunk_push(p.free_ring, p.ring_state, p.n_chunks, cc, &p.counters[CNT_RING_DROPS], lane); cc = prev; }
+        }
+        unsigned smid, wslot;
+        asm("mov.u32 %0, %%smid;" : "=r"(smid));
+        asm("mov.u32 %0, %%warpid;" : "=r"(wslot));
+        out.cycles = clock64() - clk0; out.smid = smid; out.wslot = wslot;
+        if (lane == 0) {
+            p.halves[hid] = out;
+            atomicAdd(&p.counters[CNT_STEPS], (unsigned long long)rows_done);
+            if (TB) atomicAdd(&p.counters[CNT_TBBYTES], (unsigned long long)n_words * 4ULL);
+            if (TB && !tb_ok) atomicAdd(&p.counters[CNT_OVERFLOW], 1ULL);
+            if (wide) atomicAdd(&p.counters[CNT_WIDE], 1ULL);
+            atomicAdd(&p.counters[CNT_BLOCK_HALVES], 1ULL);
+        }
+    }
+}
+
+// Persistent CTAs: each pulls the next half from the first row_n tickets (the longest: sfe_launch_tickets' order).
+template <bool TB>
+__global__ void __launch_bounds__(RK_THREADS, 1) ydrop_row_kernel(const YdParams p)
+{
+    __shared__ RkShared sh;
+    __shared__ unsigned long long tk_s;
+    const long long n_row = p.row_all ? p.n_tickets : (long long)*((volatile unsigned long long *)&p.counters[CNT_ROW_N]);
+    for (;;) {
+        if (threadIdx.x == 0) tk_s = atomicAdd(&p.counters[CNT_ROW_TICKET], 1ULL);
+        __syncthreads();
+        const long long tk = (long long)tk_s;
+        __syncthreads();
+        if (tk >= n_row) break;
+        row_half<TB>(p, p.tickets[tk], sh);
+        __syncthreads();
+    }
+}
+
+int sfe_launch_ydrop_row(const YdParams &p, bool want_tb, long long grid, cudaStream_t st)
+{
+    if (grid < 1) grid = 1;
+    if (want_tb) SFE_KL ydrop_row_kernel<true><<<(unsigned)grid, RK_THREADS, 0, st>>>(p);
+    else SFE_KL ydrop_row_kernel<false><<<(unsigned)grid, RK_THREADS, 0, st>>>(p);
+    SFE_LAUNCH_CHECK();
+}
