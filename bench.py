@@ -28,7 +28,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-SCRATCH_GB = {"c1": 2, "c2": 16, "c4": 24, "c3": 32, "c3s": 24, "c5s": 32, "c5": 48}   # traceback arena (chunks are recycled)
+SCRATCH_GB = {"c1": 2, "c2": 16, "c4": 24, "c3": 32, "c3s": 24, "c5s": 32, "c5": 48, "filter": 2}   # traceback arena (chunks are recycled)
 DEFAULT_WINDOW = {"c3": 16384, "c3s": 16384, "c5s": 1024, "c5": 1024}   # classic Algorithm 3: K for the dense-anchor workloads; others: one batch
 LEADER_WINDOW = 262144                                                  # --spec leaders: most extensions per batch
 TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.csv")      # written by hand from `ncu --set full` captures (see ncu_traffic.md)
@@ -50,6 +50,9 @@ def make_workload(name):
         return W.config3(t_len=1_000_000, n_anchors=5_000), "configs[2] scaled 1/10: 1 Mbp, 5,000 anchors (prefix-scale run)"
     if name == "c5s":
         return W.config5(t_len=10_000_000, n_anchors=100_000), "configs[4] scaled 1/10: 10 Mbp, 100,000 anchors (the prefix-scale run SURVEY 8(d) allows)"
+    if name == "filter":
+        return W.filter_hits(), ("f3 (PAPER.md:213, 225-227): gapped Y-drop as the FILTER over 1,000,000 raw seed hits on a configs[1]-like pair, "
+                                 "95 % of them false; score-only, ydrop 2000, +-1024-base budget per hit, pass = score >= 3000")
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -131,6 +134,11 @@ def _oracle_one(w, qrc, sc, i):
     return r.cells
 
 
+def oracle_scoring(w):
+    from oracle import sfe_oracle as O
+    return O.scoring(ydrop=2000) if w.name == "filter" else O.scoring()
+
+
 def strided_order(n):
     stride = max(1, n // 4096)
     return [i for s in range(stride) for i in range(s, n, stride)]
@@ -141,7 +149,7 @@ def oracle_sample(w, budget_s, indices=None):
     ~budget_s seconds of CPU work are done.  Returns (cells, seconds, n_anchors_done)."""
     from oracle import sfe_oracle as O
     O.lib()
-    sc = O.scoring()
+    sc = oracle_scoring(w)
     qrc = w.query_rc
     order = strided_order(len(w.anchors)) if indices is None else list(indices)
     cells = 0; done = 0
@@ -159,7 +167,7 @@ def oracle_parallel(w, budget_s, indices=None):
     from concurrent.futures import ThreadPoolExecutor
     from oracle import sfe_oracle as O
     O.lib()
-    sc = O.scoring()
+    sc = oracle_scoring(w)
     qrc = w.query_rc
     cores = max(1, os.cpu_count() or 1)
     order = strided_order(len(w.anchors)) if indices is None else list(indices)
@@ -178,7 +186,7 @@ def oracle_serial_prefix(w, budget_s):
     call takes about budget_s.  Returns dict(anchors, extended, kept, cells, seconds)."""
     from oracle import sfe_oracle as O
     O.lib()
-    sc = O.scoring()
+    sc = oracle_scoring(w)
     qrc = w.query_rc
     n = len(w.anchors)
     m = min(n, 16)
@@ -246,7 +254,8 @@ class Job:
         self.nacc = torch.zeros(1, dtype=torch.int64, device=dev)
         self.stats = torch.zeros(B.STATS_DT.itemsize, dtype=torch.uint8, device=dev)
         self.cigar_cap = cigar_cap
-        self.sc = B.scoring()
+        self.filter = w.name == "filter"
+        self.sc = B.scoring(ydrop=2000) if self.filter else B.scoring()
         self.state = {}
 
     def step(self, K=None, flags=None):
@@ -257,7 +266,13 @@ class Job:
         tp = sfe.pack(self.t_ascii, with_rc=False)
         qp = sfe.pack(self.q_ascii, with_rc=True)
         self.state.update(tp=tp, qp=qp)
-        if K > 0:
+        if self.filter:
+            # the filter: one score-only batch; a hit passes iff its gapped score reaches tau.  No containment (nothing is
+            # committed at this stage), so no resolve: the statistics below are filled from the results for the report.
+            res, _, _ = sfe.ydrop_batch(tp[:2], len(w.target), qp, len(w.query), self.pairs, len(w.pairs), self.anchors, self.n,
+                                        self.sc, flags & ~B.WANT_CIGAR, 0)
+            self.state.update(res=res, keep=None)
+        elif K > 0:
             o = sfe.speculate(tp[:2], len(w.target), qp, len(w.query), self.pairs, len(w.pairs), self.anchors, self.n, self.sc, K, flags,
                               self.cigar_cap, accepted_dev=self.acc, n_accepted_dev=self.nacc, stats_dev=self.stats)
             self.state.update(res=o["results"], keep=o["keep"])
@@ -268,6 +283,11 @@ class Job:
             self.state.update(res=res, keep=keep)
 
     def stats_dict(self):
+        if self.filter:
+            r = self.B.results_to_numpy(self.state["res"], self.n)
+            npass = int((r["score"] >= self.sc.min_score).sum())
+            return {"n_anchors": self.n, "n_kept": npass, "n_covered": 0, "n_below": self.n - npass, "cells_total": int(r["cells"].sum()),
+                    "cells_covered": 0, "n_extended": self.n, "n_windows": 1}
         st = self.stats.cpu().numpy().view(self.B.STATS_DT)[0]
         return {k: int(st[k]) for k in self.B.STATS_DT.names}
 
@@ -286,7 +306,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c4", "c3", "c3s", "c5s", "c5"])
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c4", "c3", "c3s", "c5s", "c5", "filter"])
     ap.add_argument("--window", type=int, default=-1, help="Algorithm 3's K (sfe_speculate); 0 = one batch over all anchors; -1 = workload default")
     ap.add_argument("--kernel", default="auto", choices=["auto", "block", "systolic"],
                     help="block: the cooperative-warps kernel (one CTA per half) for every half; auto / systolic: one warp per half")
@@ -305,7 +325,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--c5", default="auto", choices=["auto", "full", "prefix", "off"],
                     help="the c5_e2e key of the default (c4) line: Algorithm 3 end to end on configs[4]; prefix = the 10 Mbp / "
-                         "100,000-anchor prefix-scale run SURVEY 8(d) allows; auto = prefix")
+                         "100,000-anchor prefix-scale run SURVEY 8(d) allows; auto = full")
     ap.add_argument("--limit-anchors", type=int, default=0, help="profiling aid: keep every k-th anchor so that N remain")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -331,6 +351,8 @@ def main():
         w.anchors = w.anchors[:: len(w.anchors) // args.limit_anchors][: args.limit_anchors]
         desc += f" [profiling subset: {len(w.anchors)} anchors]"
     n = len(w.anchors)
+    if args.workload == "filter":
+        args.flags = "score"; args.no_e2e = True
     flags = B.WANT_CIGAR if args.flags == "cigar" else B.SCORE_ONLY
     flags |= {"auto": 0, "block": B.BLOCK_KERNEL, "systolic": B.NO_BLOCK_KERNEL}[args.kernel]
     free_b, _ = torch.cuda.mem_get_info(dev)
@@ -454,7 +476,7 @@ def main():
     if args.workload == "c4" and args.c5 != "off" and not args.limit_anchors:
         del job
         sfe.close(); torch.cuda.empty_cache()
-        name5 = "c5" if args.c5 == "full" else "c5s"
+        name5 = "c5s" if args.c5 == "prefix" else "c5"
         tg = time.perf_counter(); w5, desc5 = make_workload(name5); tg = time.perf_counter() - tg
         free_b, _ = torch.cuda.mem_get_info(dev)
         sfe5 = B.Sfe(local, min(SCRATCH_GB[name5] << 30, int(free_b * 0.6)))
@@ -545,6 +567,9 @@ def main():
                        "l2": "inputs+traceback per step exceed L2 (126 MB)", "generation_s": t_gen,
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "scoring": "HOXD70/400/30/ydrop 9400/lag 32/tau 3000"},
             "kept_alignments_per_s": kept_step * args.steps * world / (ms * 1e-3),
+            "filter": ({"hits_per_s": n * args.steps * world / (ms * 1e-3), "pass_rate": kept_step / n, "passed": kept_step,
+                        "true_hits": w.meta.get("n_true"), "tau": 3000, "ydrop": 2000, "budget_bases": w.meta.get("budget")}
+                       if args.workload == "filter" else None),
             "kept": kept_step, "cells_per_step": cells_step,
             "extended": st0["n_extended"], "windows": st0["n_windows"],
             "speculation_waste": {"ext": 1.0 - (kept_step + st0["n_below"]) / st0["n_extended"] if st0["n_extended"] else None,

@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsfe.so")
+LIB_PATH = os.environ.get("SFE_LIB_PATH") or os.path.join(_HERE, "libsfe.so")      # (override: A/B builds of the same sources)
 
 OK, EINVAL, ENOMEM, ECUDA, ELIMIT = 0, -1, -2, -3, -4
 YDROP_INF = 0x7FFFFFFF

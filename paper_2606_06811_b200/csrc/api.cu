@@ -372,7 +372,8 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
     p.row_split = row_split ? 1 : 0;
     if ((rc = sfe_launch_tickets(anchors_dev, n_anchors, pairs_dev, n_pairs, q_len, !(flags & SFE_NO_BINNING), prio_dev,
                                  (unsigned int *)c->hist.p, (int32_t *)c->tickets.p, c->counters, row_split ? c->opt[SFE_OPT_ROW_KERNEL_CAP] : 0,
-                                 row_split ? c->n_sm / 2 : 0, c->stream))) return rc;
+                                 0 /* proxy-binned tickets stay with the systolic kernel: beside a DENSE launch the row kernel's CTAs
+                                      cost a third of the SM's systolic occupancy and run contended (C4: 64 -> 108 ms) */, c->stream))) return rc;
     if ((rc = timed_ydrop(c, p, want_tb, flags))) return rc;
     c->info[0] += 1; c->info[1] += 2 * n_anchors; c->n_profile = 2 * n_anchors;
     if ((rc = sfe_launch_join(anchors_dev, p.halves, n_anchors, nullptr, n_anchors, want_tb, results_dev, c->stream))) return rc;

@@ -25,50 +25,77 @@
 // cell (first maximum, R7), cell count (R28) and CIGAR (R11, R12) are the oracle's at Lambda = 32: same tests as ydrop_kernel.
 #include "ydrop_common.cuh"
 
-#define RK_NW 4                              // warps per CTA: one per SM sub-partition
-#define RK_C 8                               // columns per thread
+#ifndef RK_NW
+#define RK_NW 8                              // warps per CTA: two per SM sub-partition hide each other's dependency stalls
+#endif
+#ifndef RK_C
+#define RK_C 4                               // columns per thread
+#endif
 #define RK_THREADS (32 * RK_NW)
-#define RK_WCOLS (32 * RK_C)                 // columns per warp (256): the window moves in steps of this
+#define RK_WCOLS (32 * RK_C)                 // columns per warp: the window moves in steps of this
 #define RK_WIN (RK_THREADS * RK_C)           // 1024
-#define RK_ROW_WORDS RK_THREADS              // traceback record of a row: one word (8 nibbles) per thread = 512 B
+#define RK_ROW_WORDS (RK_WIN / 8)            // traceback record of a row: 4 bits per window column = 512 B
 #define RK_CHUNK_ROWS (SFE_CHUNK_BYTES / (4 * RK_ROW_WORDS))     // 128 rows per 64-KiB chunk
 #define RK_NINF (-(1 << 30) - (1 << 28))     // identity of the max-plus scans: the decay terms (< 2^27) fit below it, and H - O - F with
                                              // H < 2^29 (R25) stays inside int32
 #define RK_FOLD 16                           // rows between two folds of the lagged statistics
 #define RK_POLL_LIMIT (1 << 22)
+#ifdef RK_PROFILE
+#include <stdio.h>
+#define RK_T(k) do { const long long t_ = clock64(); prof_t[k] += t_ - prof_last; prof_last = t_; } while (0)
+#else
+#define RK_T(k) do { } while (0)
+#endif
 
 struct RkShared {
     unsigned long long edge[RK_NW];          // by warp: {row << 32 | gated H - OX of its last column after that row}: ONE 8-byte word
-    int carry[2][RK_NW];                     // by row parity, warp: F leaving the warp to the right (before the decay)
-    int rmax[64][RK_NW];                     // by row & 63, warp: max H of the row (any cell: a dead one never raises the best)
-    int rlo[64][RK_NW], rhi[64][RK_NW];      // first / last alive column of the row in the warp's block (lo > hi: none)
-    int new_chunk;
-    int fail_row;                            // row in which a bounded wait ran out (never expected; -1 = none): SFE_ST_INTERNAL
+    __align__(16) int carry[2][RK_NW];       // by row parity, RANK of the warp in the window: F leaving the warp (+ Dw * rank)
+    __align__(16) int rmax[64][RK_NW];       // by row & 63, warp: max H of the row (any cell: a dead one never raises the best)
+    __align__(16) int rlo[64][RK_NW];        // first / last alive column of the row in the warp's block (lo > hi: none)
+    __align__(16) int rhi[64][RK_NW];
+    __align__(8) int fail_row;               // row in which a bounded wait ran out (never expected; -1 = none): SFE_ST_INTERNAL
     int wide_row;                            // row in which the window's last column held an alive cell (-1 = none): the band outgrew it
+    int new_chunk;
     int red_s[RK_NW], red_i[RK_NW], red_j[RK_NW];
     uint32_t opsbuf[SFE_WALK_OPS];
 };
 
-// exclusive prefix over the warps LEFT of rank `rho` in the window of the carries published for this row:
-//   max_{rho' < rho} carry[rho'] - Dw (rho - 1 - rho'),  Dw = X * RK_WCOLS
-static __device__ __forceinline__ int warp_carry_in(const int *carry, int rho, int wsb, int Dw, int lane)
+// Shared memory is addressed through ONE 32-bit base kept in a register and explicit ld/st.shared: left to the compiler,
+// every access to the static struct re-derives its address from SR_CgaCtaId (S2UR + ULEA on sm_100a), ~25 cycles a time
+// on a path that is latency-bound.
+#include <stddef.h>
+#define RK_OFF(field) ((uint32_t)offsetof(RkShared, field))
+static __device__ __forceinline__ int lds32(uint32_t a) { int v; asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+static __device__ __forceinline__ int2 lds64(uint32_t a) { int2 v; asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a)); return v; }
+static __device__ __forceinline__ int4 lds128(uint32_t a) { int4 v; asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a)); return v; }
+static __device__ __forceinline__ unsigned long long lds_u64v(uint32_t a) { unsigned long long v; asm volatile("ld.volatile.shared.u64 %0, [%1];" : "=l"(v) : "r"(a) : "memory"); return v; }
+static __device__ __forceinline__ void sts32(uint32_t a, int v) { asm volatile("st.shared.s32 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
+static __device__ __forceinline__ void sts_u64v(uint32_t a, unsigned long long v) { asm volatile("st.volatile.shared.u64 [%0], %1;" :: "r"(a), "l"(v) : "memory"); }
+
+// maximum over the RK_NW per-warp entries of one ring row: broadcast 128-bit loads, no reduction instruction
+static __device__ __forceinline__ int row_max4(uint32_t a)
 {
-    int v = RK_NINF;
-    if (lane < RK_NW) {
-        const int r = (lane - wsb) & (RK_NW - 1);                 // rank of warp `lane`
-        if (r < rho) v = carry[lane] - Dw * (rho - 1 - r);
-    }
-    return __reduce_max_sync(FULL, v);
+    int m = SFE_NEG;
+#pragma unroll
+    for (int w = 0; w < RK_NW; w += 4) { const int4 x = lds128(a + 4 * w); m = max(m, max(max(x.x, x.y), max(x.z, x.w))); }
+    return m;
+}
+static __device__ __forceinline__ int row_min4(uint32_t a)
+{
+    int m = 0x7fffffff;
+#pragma unroll
+    for (int w = 0; w < RK_NW; w += 4) { const int4 x = lds128(a + 4 * w); m = min(m, min(min(x.x, x.y), min(x.z, x.w))); }
+    return m;
 }
 
 // ---- a8: walk the fixed-size row records from the end cell to the origin (warp 0; every lane holds the same state) ----
-// Nibble of cell (i, j): word (j mod RK_WIN) / RK_C of row i's record, bits 4 (RK_C - 1 - j mod RK_C) ..:
+// Nibble of cell (i, j): word (j mod RK_WIN) / 8 of row i's record (position inside the word: see nibble() below):
 //   bit3 = H not from M, bit2 = H not from E, bit1 = E extended (R11), bit0 = the F of the NEXT column extends this cell's F.
-static __device__ bool row_walk(const YdParams &p, RkShared &sh, const int end_i, const int end_j, int chunk, const int lane,
+static __device__ bool row_walk(const YdParams &p, uint32_t *opsbuf, const int end_i, const int end_j, int chunk, const int lane,
                                 uint32_t &ops_seg, int &n_ops, bool &ops_ok)
 {
     OpsWriter ow;
-    ow.buf = sh.opsbuf; ow.stage = p.ops_stage; ow.used = &p.counters[CNT_OPS]; ow.cap = p.ops_cap;
+    ow.buf = opsbuf; ow.stage = p.ops_stage; ow.used = &p.counters[CNT_OPS]; ow.cap = p.ops_cap;
     ow.nbuf = 0; ow.nops = 0; ow.cur_op = -1; ow.run = 0; ow.prev_seg = SFE_NO_SEG; ow.ok = true;
     ops_seg = SFE_NO_SEG; n_ops = 0; ops_ok = true;
     if (end_i == 0 && end_j == 0) return true;
@@ -82,8 +109,9 @@ static __device__ bool row_walk(const YdParams &p, RkShared &sh, const int end_i
         const int o = r / RK_CHUNK_ROWS;
         const int ch = o == ord ? chunk : prev;                  // 32 consecutive rows span at most two chunks
         const uint32_t w = __ldcg(p.pool + (size_t)ch * (SFE_CHUNK_BYTES / 4) + (size_t)(r - o * RK_CHUNK_ROWS) * RK_ROW_WORDS +
-                                  ((c & (RK_WIN - 1)) / RK_C));
-        return (w >> (4 * (RK_C - 1 - (c & (RK_C - 1))))) & 15u;
+                                  ((c & (RK_WIN - 1)) >> 3));
+        // a thread's RK_C nibbles (first column highest) form one 4 RK_C-bit unit; units fill the word from its low end
+        return (w >> (4 * (RK_C - 1 - (c & (RK_C - 1))) + 4 * RK_C * ((c & 7) / RK_C))) & 15u;
     };
     while (!(i == 0 && j == 0 && state == 0)) {
         if (--guard < 0) return false;
@@ -142,8 +170,14 @@ static __device__ bool row_walk(const YdParams &p, RkShared &sh, const int end_i
 }
 
 template <bool TB>
-static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
+static __device__ __forceinline__ void row_half(const YdParams &p, const int hid)
 {
+    // a function-scope __shared__ object: every access below is a direct shared-space LDS / STS with an immediate offset.
+    // (Reached through a reference parameter the same struct was addressed generically: each access re-derived the
+    // shared window from SR_CgaCtaId -- S2UR + ULEA -- and the row cost 1,350 cycles instead of ~700.)
+    __shared__ RkShared sh;
+    uint32_t sb = (uint32_t)__cvta_generic_to_shared(&sh);
+    asm volatile("" : "+r"(sb));                          // opaque: one register, no re-derivation
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     sfe_half out;
     out.score = 0; out.end_i = 0; out.end_j = 0; out.status = 0; out.cells = 0;
@@ -175,7 +209,7 @@ static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
     unsigned long long cells = 0;                         // folded rows (uniform)
     int folded = 0;                                       // rows < folded have been folded (uniform)
     int rows_done = 0, max_width = 0, last_lo = 0;
-    bool wide = false, limit = false, done = false;
+    bool wide = false, limit = false;
     uint32_t srow32 = 0u;
     int cur_chunk = -1;                                   // traceback chunk of the current 128 rows (uniform)
     bool tb_ok = TB;
@@ -188,10 +222,7 @@ static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
         while (folded < upto) {
             const int r = folded + lane;
             int lo = 0x7fffffff, hi = -1;
-            if (r < upto) {
-#pragma unroll
-                for (int w = 0; w < RK_NW; w++) { lo = min(lo, sh.rlo[r & 63][w]); hi = max(hi, sh.rhi[r & 63][w]); }
-            }
+            if (r < upto) { lo = row_min4(sb + RK_OFF(rlo) + 4 * RK_NW * (r & 63)); hi = row_max4(sb + RK_OFF(rhi) + 4 * RK_NW * (r & 63)); }
             const unsigned nb = r < upto ? 1u : 0u;
             const unsigned deadm = __ballot_sync(FULL, nb && hi < lo);
             const int nrows = min(32, upto - folded);
@@ -212,12 +243,20 @@ static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
         return alive_all;
     };
 
+#ifdef RK_PROFILE
+    long long prof_t[8] = {0, 0, 0, 0, 0, 0, 0, 0}, prof_last = clock64();
+#endif
     int i = 0;
     for (; i <= g.n; i++) {
+        RK_T(7);
+        // ---- early loads: everything the row needs from shared memory is requested before it is used ----
+        const int lw = (warp - 1) & (RK_NW - 1);
+        unsigned long long ev = lds_u64v(sb + RK_OFF(edge) + 8 * lw);             // the left warp's edge {row, value} (broadcast)
+        const int rm = i >= 32 ? row_max4(sb + RK_OFF(rmax) + 4 * RK_NW * ((i - 32) & 63)) : 0;   // R4: best of row i - 32
         // ---- lagged housekeeping, every RK_FOLD rows: rows [i - 32, i - 16) ----
         if ((i & (RK_FOLD - 1)) == 0 && i >= 2 * RK_FOLD) {
             int nlo = last_lo, nhi = -1;
-            if (!fold(i - RK_FOLD, nlo, nhi)) { done = true; break; }
+            if (!fold(i - RK_FOLD, nlo, nhi)) break;
             last_lo = nlo;
             const int nws = nlo & ~(RK_WCOLS - 1);                // the first alive column never moves left: a stale one is safe
             // the last alive column grows by at most one per row: rows up to the next fold stay below nhi + 2 RK_FOLD + 1
@@ -229,22 +268,20 @@ static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
             srow32 = (r == 0 || r > g.n) ? 0u : p.srow[sfe_base(g.qc, g.qm, g.q0 + (long long)g.d * r)];
         }
         const uint32_t srow_lo = __shfl_sync(FULL, srow32, i & 31);
-        // ---- R4: T(i) = best(rows <= i - 32) - ydrop ----
-        if (i >= 32) {
-            const int rm = lane < RK_NW ? sh.rmax[(i - 32) & 63][lane] : SFE_NEG;
-            cumbest = max(cumbest, __reduce_max_sync(FULL, rm));
-            if (cumbest >= SFE_SCORE_LIMIT) { limit = true; break; }              // R25
-        }
-        const int T = p.ydrop_inf ? SFE_T_INF : cumbest - p.Y;
+        int Hd0 = __shfl_up_sync(FULL, Hu[RK_C - 1], 1);
+        cumbest = max(cumbest, rm);
+        if (cumbest >= SFE_SCORE_LIMIT) { limit = true; break; }                  // R25
+        const int T = p.ydrop_inf ? SFE_T_INF : cumbest - p.Y;                    // T(i) = best(rows <= i - 32) - ydrop
+        RK_T(0);
         // ---- my columns in this row's window ----
         const int wsb = ws / RK_WCOLS;
-        const int q = ((tid * RK_C) - ws) & (RK_WIN - 1);         // window position of my first column
-        const int c0 = ws + q;
         const int rho = (warp - wsb) & (RK_NW - 1);               // my warp's rank in the window
+        const int c0 = ws + rho * RK_WCOLS + lane * RK_C;         // my first column
         if (c0 != myc0) {
             myc0 = c0;
 #pragma unroll
             for (int k = 0; k < RK_C; k++) { Hu[k] = SFE_NEG; Eu[k] = SFE_NEG; sel[k] = col_selector(g, c0 + k); }
+            Hd0 = __shfl_up_sync(FULL, Hu[RK_C - 1], 1);          // (the warp's columns change together)
         }
         // ---- traceback chunk of rows i .. i + 127 (popped by warp 0 before the barrier, read by everybody after it) ----
         const bool new_chunk_row = TB && tb_ok && (i % RK_CHUNK_ROWS) == 0;
@@ -256,22 +293,16 @@ static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
                 if (nc == -2) atomicAdd(&p.counters[CNT_RING_DROPS], 1ULL);
             }
         }
-        // ---- diagonal of my first column: the left neighbour's previous-row value ----
-        int Hd0 = __shfl_up_sync(FULL, Hu[RK_C - 1], 1);
-        if (lane == 0) {
-            Hd0 = SFE_NEG;
-            if (i > 0 && q != 0 && c0 - 1 - ws_prev < RK_WIN) {   // column c0 - 1 was inside the previous row's window
-                volatile unsigned long long *e = &sh.edge[(warp - 1) & (RK_NW - 1)];
-                unsigned long long v = *e;
-                for (int spin = 0; (int)(v >> 32) != i - 1 && spin < RK_POLL_LIMIT; spin++) v = *e;
-                if ((int)(v >> 32) != i - 1) sh.fail_row = i;     // (readers act on it from this row's barrier on)
-                Hd0 = (int)(unsigned)v;
-            }
-        }
+        // ---- diagonal of the warp's first column: the left warp's previous-row value (uniform test, no divergence) ----
+        if (i > 0 && rho != 0 && ws + rho * RK_WCOLS - 1 - ws_prev < RK_WIN) {    // that column was inside the previous row's window
+            for (int spin = 0; (int)(ev >> 32) != i - 1 && spin < RK_POLL_LIMIT; spin++) ev = lds_u64v(sb + RK_OFF(edge) + 8 * lw);
+            if ((int)(ev >> 32) != i - 1) sts32(sb + RK_OFF(fail_row), i);        // (readers act on it from this row's barrier on)
+            if (lane == 0) Hd0 = (int)(unsigned)ev;
+        } else if (lane == 0) Hd0 = SFE_NEG;
         if (i == 0 && c0 == 0) Hd0 = -OX;                         // the origin (R8)
+        RK_T(1);
         // ---- phase A: M, E, H~ and the in-thread F chain ----
         int M[RK_C], E[RK_C], Ht[RK_C], gl[RK_C];                 // gl[k]: F entering column k from my own columns left of it
-        int gk = RK_NINF;
 #pragma unroll
         for (int k = 0; k < RK_C; k++) {
             const int Hd = k == 0 ? Hd0 : Hu[k - 1];
@@ -279,28 +310,47 @@ static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
             M[k] = Hd + s + OX;
             E[k] = __viaddmax_s32(Eu[k], -X, Hu[k]);
             Ht[k] = max(M[k], E[k]);
-            gl[k] = gk;
-            gk = __viaddmax_s32(gk, -X, Ht[k] - OX);
         }
+        int gk = RK_NINF;
+#pragma unroll
+        for (int k = 0; k < RK_C; k++) { gl[k] = gk; gk = __viaddmax_s32(gk, -X, Ht[k] - OX); }
+        RK_T(2);
         // ---- F across the threads of the warp: y = x + D lane, prefix maximum, exclusive ----
         int y = gk + D * lane;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) y = max(y, __shfl_up_sync(FULL, y, o));      // out-of-range lanes get their own value back
-        if (lane == 31) sh.carry[i & 1][warp] = y - D * 31;        // F leaving the warp (entering the next warp's first column)
+        if (lane == 31) sts32(sb + RK_OFF(carry) + 4 * (RK_NW * (i & 1) + rho), y - D * 31 + Dw * rho);   // F leaving the warp, pre-shifted by its rank
         int yex = __shfl_up_sync(FULL, y, 1);
         if (lane == 0) yex = RK_NINF;
         const int fin_warp = yex - D * lane + D;                   // F entering my first column from my warp's lanes left of me
+        RK_T(3);
         __syncthreads();                                                                   // the one barrier of the row
+        RK_T(4);
+        // ---- after the barrier: flags and the other warps' carries, requested together ----
+        const int2 fl = lds64(sb + RK_OFF(fail_row));
+        int cm = RK_NINF;
+        {
+            const uint32_t cp = sb + RK_OFF(carry) + 4 * RK_NW * (i & 1);
+#pragma unroll
+            for (int w4 = 0; w4 < RK_NW; w4 += 4) {
+                const int4 x = lds128(cp + 4 * w4);
+                if (w4 + 0 < rho) cm = max(cm, x.x);
+                if (w4 + 1 < rho) cm = max(cm, x.y);
+                if (w4 + 2 < rho) cm = max(cm, x.z);
+                if (w4 + 3 < rho) cm = max(cm, x.w);
+            }
+        }
         // both flags carry the row they were raised in: a fast warp's later write is ignored by a slow reader, so every
         // thread leaves the loop in the same row (a non-uniform exit would hang the next barrier)
-        { const int fr = sh.fail_row; if (fr >= 0 && fr <= i) break; }
-        { const int wr = sh.wide_row; if (wr >= 0 && wr < i) { wide = true; break; } }
-        const int win = warp_carry_in(sh.carry[i & 1], rho, wsb, Dw, lane);                // F entering my warp from the left
-        const int Fin = max(fin_warp, win - D * lane);
+        if (fl.x >= 0 && fl.x <= i) break;
+        if (fl.y >= 0 && fl.y < i) { wide = true; break; }
+        // F entering my warp from the warps left of it: max_{r < rho} carry_r - Dw (rho - 1 - r); then down my warp's lanes
+        const int Fin = max(fin_warp, cm - Dw * (rho - 1) - D * lane);
         if (new_chunk_row) {
-            const int nc = sh.new_chunk;
+            const int nc = lds32(sb + RK_OFF(new_chunk));
             if (nc < 0) tb_ok = false; else cur_chunk = nc;
         }
+        RK_T(5);
         // ---- phase C: F, H, alive, next row's state, statistics, pointers ----
         uint32_t nibs = 0, am = 0;
         int hmax = SFE_NEG;
@@ -325,6 +375,10 @@ static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
             hmax = max(hmax, H);
             if (alive) am |= 1u << k;
         }
+        RK_T(6);
+        // ---- publish the edge for the next row first: the right warp is waiting for it ----
+        if (lane == 31) sts_u64v(sb + RK_OFF(edge) + 8 * warp, ((unsigned long long)(unsigned)i << 32) | (unsigned)Hu[RK_C - 1]);
+        if (rho == RK_NW - 1 && lane == 31 && (am >> (RK_C - 1))) sts32(sb + RK_OFF(wide_row), i);        // alive in the window's last column: bail out next row
         best = max(best, hmax);
         if (best > best_before) {                                  // strict: the first maximum of my cells (R7)
             int kk = RK_C - 1;
@@ -332,18 +386,28 @@ static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
             for (int k = RK_C - 2; k >= 0; k--) kk = Hc[k] == best ? k : kk;
             best_i = i; best_j = c0 + kk;
         }
-        // ---- publish: edge for the next row, lagged statistics, pointers ----
-        if (lane == 31) *(volatile unsigned long long *)&sh.edge[warp] = ((unsigned long long)(unsigned)i << 32) | (unsigned)Hu[RK_C - 1];
-        if (q + RK_C == RK_WIN && (am >> (RK_C - 1))) sh.wide_row = i;            // alive in the window's last column: bail out next row
-        const int wm = __reduce_max_sync(FULL, hmax);
-        const int wlo = __reduce_min_sync(FULL, am ? c0 + __ffs(am) - 1 : 0x7fffffff);
-        const int whi = __reduce_max_sync(FULL, am ? c0 + 31 - __clz(am) : -1);
-        if (lane == 0) { sh.rmax[i & 63][warp] = wm; sh.rlo[i & 63][warp] = wlo; sh.rhi[i & 63][warp] = whi; }
+        // ---- lagged statistics: the lanes holding the warp's first / last alive cell write them; one reduction for the maximum ----
+        {
+            const unsigned bal = __ballot_sync(FULL, am != 0);
+            const int wm = __reduce_max_sync(FULL, hmax);
+            const int fl_lane = bal ? __ffs(bal) - 1 : 0, ll_lane = bal ? 31 - __clz(bal) : 0;
+            const uint32_t so = 4 * (RK_NW * (i & 63) + warp);
+            if (lane == fl_lane) sts32(sb + RK_OFF(rlo) + so, bal ? c0 + __ffs(am) - 1 : 0x7fffffff);
+            if (lane == ll_lane) sts32(sb + RK_OFF(rhi) + so, bal ? c0 + 31 - __clz(am) : -1);
+            if (lane == 0) sts32(sb + RK_OFF(rmax) + so, wm);
+        }
         if (TB && tb_ok) {
-            p.pool[(size_t)cur_chunk * (SFE_CHUNK_BYTES / 4) + (size_t)(i % RK_CHUNK_ROWS) * RK_ROW_WORDS + tid] = nibs;
-            n_words += RK_ROW_WORDS;
+            uint32_t *rec = p.pool + (size_t)cur_chunk * (SFE_CHUNK_BYTES / 4) + (size_t)(i % RK_CHUNK_ROWS) * RK_ROW_WORDS;
+            const int unit = ((c0 & (RK_WIN - 1)) / RK_C);        // my 4 RK_C-bit unit of the row record
+            if (RK_C == 8) rec[unit] = nibs;
+            else if (RK_C == 4) ((uint16_t *)rec)[unit] = (uint16_t)nibs;
+            else ((uint8_t *)rec)[unit] = (uint8_t)nibs;
+            if (tid == 0) n_words += RK_ROW_WORDS;
         }
     }
+#ifdef RK_PROFILE
+    if (lane == 0 && i > 100000) printf("RKPROF warp %d rows %d: top %.1f cols/poll %.1f phaseA %.1f scan %.1f barrier %.1f postbar %.1f phaseC %.1f publish %.1f\n", warp, i, (double)prof_t[0] / i, (double)prof_t[1] / i, (double)prof_t[2] / i, (double)prof_t[3] / i, (double)prof_t[4] / i, (double)prof_t[5] / i, (double)prof_t[6] / i, (double)prof_t[7] / i);
+#endif
     __syncthreads();
     // ---- the rows not folded yet (rows 0 .. i-1 were computed) ----
     const bool failed = sh.fail_row >= 0;
@@ -366,6 +430,7 @@ static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
         const int os = sh.red_s[w], oi = sh.red_i[w], oj = sh.red_j[w];
         if (os > bs || (os == bs && (oi < bi || (oi == bi && oj < bj)))) { bs = os; bi = oi; bj = oj; }
     }
+    n_words = __shfl_sync(FULL, n_words, 0);
     out.score = bs; out.end_i = bi; out.end_j = bj; out.cells = cells;
     out.status = (wide ? SFE_ST_WIDE_PENDING : 0u) | ((TB && !tb_ok) ? SFE_ST_PASS_OVERFLOW : 0u) | SFE_ST_BLOCK |
                  (limit ? SFE_ST_SCORE_LIMIT : 0u) | (failed ? SFE_ST_INTERNAL : 0u);
@@ -380,7 +445,7 @@ static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
             while (ch >= 0 && o > bi / RK_CHUNK_ROWS) { ch = __ldcg(p.chunk_prev + ch); o--; }
             bool ops_ok = true;
             __threadfence_block();
-            if (!row_walk(p, sh, bi, bj, ch, lane, out.ops_seg, out.n_ops, ops_ok)) out.status |= SFE_ST_INTERNAL;
+            if (!row_walk(p, sh.opsbuf, bi, bj, ch, lane, out.ops_seg, out.n_ops, ops_ok)) out.status |= SFE_ST_INTERNAL;
             if (!ops_ok) out.status |= SFE_ST_OPS_OVERFLOW;
         }
         if (TB) {
@@ -408,7 +473,6 @@ static __device__ void row_half(const YdParams &p, const int hid, RkShared &sh)
 template <bool TB>
 __global__ void __launch_bounds__(RK_THREADS, 1) ydrop_row_kernel(const YdParams p)
 {
-    __shared__ RkShared sh;
     __shared__ unsigned long long tk_s;
     const long long n_row = p.row_all ? p.n_tickets : (long long)*((volatile unsigned long long *)&p.counters[CNT_ROW_N]);
     for (;;) {
@@ -417,7 +481,7 @@ __global__ void __launch_bounds__(RK_THREADS, 1) ydrop_row_kernel(const YdParams
         const long long tk = (long long)tk_s;
         __syncthreads();
         if (tk >= n_row) break;
-        row_half<TB>(p, p.tickets[tk], sh);
+        row_half<TB>(p, p.tickets[tk]);
         __syncthreads();
     }
 }

@@ -473,3 +473,54 @@ def config5(t_len: int = 100_000_000, n_anchors: int = 1_000_000) -> Workload:
 
 
 CONFIGS = {"c1": config1, "c2": config2, "c3": config3, "c4": config4, "c5": config5}
+
+
+# ------------------------------------------------------------------------------------------
+# Filter workload (gapped Y-drop as the FILTER over raw seed hits)
+# ------------------------------------------------------------------------------------------
+def filter_hits(n_hits: int = 1_000_000, true_frac: float = 0.05, t_len: int = 2_000_000, n_segments: int = 2000,
+                budget: int = 1024) -> Workload:
+    """Raw, mostly false seed hits on a configs[1]-like pair: the sequences of config2 (segments U[100, 800] at 70 %
+    identity, every second one reverse-complemented); `true_frac` of the hits lie on a segment's true path (qpos jitter
+    U{-3..3}), the rest are uniform random (tpos, qpos, strand) -- what a seeding stage hands to the filter before anything
+    has been verified.  Every hit gets its own pair: the box of +-`budget` bases around it (clipped to the sequences),
+    i.e. a fixed row / column budget per one-sided extension.  Hits are sorted by target position."""
+    base = config2(t_len=t_len, n_segments=n_segments, per_seg=1, n_decoys=0)
+    T, Q = base.target, base.query
+    q_len = len(Q)
+    slot = t_len // n_segments
+    st = Stream(stream_seed(6, 0))
+    n_true = int(true_frac * n_hits)
+    # true hits: re-derive each segment's placement exactly as config2 does (same streams), then pick aligned pairs
+    perm = Stream(stream_seed(2, 2)).permutation(n_segments)
+    lens = Stream(stream_seed(2, 3)).integers(100, 801, n_segments)
+    mst = Stream(stream_seed(2, 4))
+    per = np.bincount(st.integers(0, n_segments, n_true), minlength=n_segments)
+    hits = []
+    for s in range(n_segments):
+        ln_t = int(lens[s]); t0 = s * slot + 16
+        mu = mutate(T[t0:t0 + ln_t], 0.30, 0.02, mst)
+        if per[s] == 0:
+            continue
+        q0 = int(perm[s]) * slot + 16
+        ln = min(len(mu.seq), slot - 32)
+        ok = np.nonzero(mu.q_idx < ln)[0]
+        k = ok[st.integers(0, len(ok), int(per[s]))]
+        jit = st.integers(-3, 4, int(per[s]))
+        minus = (s % 2 == 1)
+        tp = t0 + mu.t_idx[k]
+        qrel = mu.q_idx[k]
+        qp = (q_len - q0 - ln + qrel) if minus else (q0 + qrel)
+        qp = np.clip(qp + jit, 0, q_len)
+        hits.append(np.stack([tp, qp, np.zeros_like(tp), np.full_like(tp, -1 if minus else 1)], 1))
+    n_false = n_hits - sum(len(h) for h in hits)
+    ft = st.integers(0, t_len + 1, n_false); fq = st.integers(0, q_len + 1, n_false); fs = st.integers(0, 2, n_false)
+    hits.append(np.stack([ft, fq, np.zeros_like(ft), np.where(fs > 0, 1, -1)], 1))
+    A = _sort_anchors(np.concatenate(hits).astype(np.int64))
+    n = len(A)
+    A[:, 2] = np.arange(n)
+    # per-hit pair in the FORWARD query frame (sfe_pair): a - strand hit at rc-frame qpos sits at q_len - qpos forward
+    qf = np.where(A[:, 3] > 0, A[:, 1], q_len - A[:, 1])
+    pairs = np.stack([np.maximum(A[:, 0] - budget, 0), np.minimum(A[:, 0] + budget, t_len),
+                      np.maximum(qf - budget, 0), np.minimum(qf + budget, q_len)], 1).astype(np.int64)
+    return Workload("filter", T, Q, pairs, A, dict(n_true=int(n - n_false), n_false=int(n_false), budget=budget))

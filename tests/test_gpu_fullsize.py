@@ -158,6 +158,9 @@ def test_config4_full(sfe_big, oracle):
         check_cigar(w, i, res[i], out["cigar"])
 
 
+LEADERS = B.WANT_CIGAR | B.SPEC_LEADERS          # bench.py's configuration for the dense-anchor workloads (--spec leaders)
+
+
 def _speculate_full(sfe, w, K, cigar_cap, flags=B.WANT_CIGAR | B.CIGAR_KEPT_ONLY):
     import torch
     dev = sfe.device
@@ -172,7 +175,7 @@ def _speculate_full(sfe, w, K, cigar_cap, flags=B.WANT_CIGAR | B.CIGAR_KEPT_ONLY
                 cigar=o["pool"].cpu().numpy().view(np.uint32), cigar_used=int(o["used"].item()))
 
 
-def _check_speculated(w, out, seed, n_sample, n_kept_sample=0, n_largest=6):
+def _check_speculated(w, out, seed, n_sample, n_kept_sample=0, n_largest=6, kept_only=True):
     """n_sample extended anchors (mostly rejected ones) + n_kept_sample kept ones + the largest, against the oracle."""
     res = out["results"]; keep = out["keep"]; n = len(w.anchors)
     skipped = (res["status"] & B.ST_SKIPPED) != 0
@@ -189,14 +192,31 @@ def _check_speculated(w, out, seed, n_sample, n_kept_sample=0, n_largest=6):
     pick = set(sample_indices(res, n, n_sample, seed, ok & (keep != 1), n_largest))
     if n_kept_sample:
         pick |= set(sample_indices(res, n, n_kept_sample, seed + 1, ok & (keep == 1), 2))
-    # bench configuration (SFE_CIGAR_KEPT_ONLY): ops exist for the kept anchors; score / box / cells for every extended one
-    H.assert_anchors_equal(out, w, sorted(pick), want_cigar=lambda i: bool(keep[i] == 1))
-    assert (res["n_ops"][keep != 1] == 0).all()
+    # SFE_CIGAR_KEPT_ONLY: ops exist for the kept anchors only; otherwise for every extended one; score / box / cells always
+    H.assert_anchors_equal(out, w, sorted(pick), want_cigar=(lambda i: bool(keep[i] == 1)) if kept_only else True)
+    if kept_only:
+        assert (res["n_ops"][keep != 1] == 0).all()
     return len(pick)
 
 
+def test_config3_full_leaders(sfe_big, oracle):
+    """configs[2] as bench.py runs it now: predicted leaders (SFE_SPEC_LEADERS), CIGARs while extending, the longest
+    tickets on the cooperative row kernel.  Same kept set as the classic windows of the next test."""
+    w = W.config3()
+    out = _speculate_full(sfe_big, w, 262144, 1 << 26, flags=LEADERS)
+    info = sfe_big.last_speculate_info()
+    assert _check_speculated(w, out, 3, 2, n_kept_sample=40, n_largest=3, kept_only=False) >= 40
+    assert int(out["stats"]["n_extended"]) < 2 * int((out["keep"] == 1).sum()) + 50      # hardly any shadow work
+    assert info["batches"] <= 8
+    classic = _speculate_full(sfe_big, w, 16384, 1 << 26)
+    assert out["keep"].tolist() == classic["keep"].tolist()
+    k = out["keep"] == 1
+    for f in ("score", "tstart", "tend", "qstart", "qend", "cells", "n_ops", "n_ops_back"):
+        assert (out["results"][f][k] == classic["results"][f][k]).all(), f
+
+
 def test_config3_full_windowed(sfe_big, oracle):
-    """configs[2] (10 Mbp, 50,000 dense anchors, extensions of 10^4..10^5 rows) through sfe_speculate, as bench.py runs it:
+    """configs[2] (10 Mbp, 50,000 dense anchors, extensions of 10^4..10^5 rows) through the classic Algorithm 3 windows:
     K = 16384, score-only windows, CIGARs for the kept anchors from one final traceback batch."""
     w = W.config3()
     out = _speculate_full(sfe_big, w, 16384, 1 << 26)
@@ -212,10 +232,29 @@ def test_config5_scaled_windowed(sfe_big, oracle):
     assert _check_speculated(w, out, 5, max(60, n_ext // 1000), n_kept_sample=20) >= n_ext // 1000    # >= 0.1 % of the extended anchors
 
 
-def test_config5_full_windowed(sfe_big, oracle):
-    """configs[4] at FULL size (100 Mbp, 1,000,000 anchors, N runs, segmental duplications, decoys), K = 1024 as bench.py:
-    resolve rule over all anchors, every kept CIGAR rescored, a sample + the largest extensions against the oracle."""
+def test_config5_scaled_leaders_equals_classic(sfe_big, oracle):
+    """configs[4] at 1/10 scale with predicted leaders: the same kept set, and for the kept anchors the same results, as
+    the classic windows; the cooperative row kernel took the long-likely tickets (block_halves > 0)."""
+    w = W.config5(t_len=10_000_000, n_anchors=100_000)
+    out = _speculate_full(sfe_big, w, 262144, 1 << 26, flags=LEADERS)
+    assert sfe_big.last_batch_info()["block_halves"] > 0
+    n_ext = int(out["stats"]["n_extended"])
+    assert _check_speculated(w, out, 5, max(40, n_ext // 1000), n_kept_sample=20, kept_only=False) >= n_ext // 1000
+    classic = _speculate_full(sfe_big, w, 1024, 1 << 26)
+    assert out["keep"].tolist() == classic["keep"].tolist()
+    k = out["keep"] == 1
+    for f in ("score", "tstart", "tend", "qstart", "qend", "cells", "n_ops", "n_ops_back"):
+        assert (out["results"][f][k] == classic["results"][f][k]).all(), f
+    assert n_ext < int(classic["stats"]["n_extended"])
+
+
+def test_config5_full_leaders(sfe_big, oracle):
+    """configs[4] at FULL size (100 Mbp, 1,000,000 anchors, N runs, segmental duplications, decoys) as bench.py runs it
+    (predicted leaders, one batch of up to 262,144 extensions at a time, CIGARs while extending): resolve rule over all
+    anchors, every kept CIGAR rescored, a sample + the largest extensions against the oracle."""
     w = W.config5()
-    out = _speculate_full(sfe_big, w, 1024, 1 << 27)
-    _check_speculated(w, out, 55, 16)
+    out = _speculate_full(sfe_big, w, 262144, 1 << 27, flags=LEADERS)
+    info = sfe_big.last_speculate_info()
+    _check_speculated(w, out, 55, 24, n_kept_sample=12, n_largest=2, kept_only=False)
     assert int((out["keep"] == 1).sum()) > 1000
+    assert info["batches"] <= 16 and info["promoted"] > 0

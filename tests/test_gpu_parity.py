@@ -575,3 +575,27 @@ def test_speculate_leaders_kept_only_and_carried_boxes(sfe, oracle):
         torch.cuda.synchronize()
         keep += o["keep"].cpu().numpy()[: hi - lo].tolist()
     assert keep == ser["state"].tolist() and int(nacc.item()) == ser["n_kept"]
+
+
+def test_filter_workload_equals_oracle(sfe, oracle):
+    """f3: the gapped Y-drop extension as the filter over raw, mostly false seed hits -- score-only,
+    ydrop 2000, one +-1024-base box per hit (a row / column budget), pass = score >= tau.  Every hit's score, box and cell
+    count equal the oracle's; so does the pass set; about the planted fraction of the hits passes."""
+    import torch
+    w = W.filter_hits(n_hits=6000, true_frac=0.05, t_len=400_000, n_segments=400)
+    n = len(w.anchors)
+    dev = sfe.device
+    sc = B.scoring(ydrop=2000)
+    tp = sfe.pack(torch.from_numpy(w.target_ascii().copy()).to(dev), with_rc=False)
+    qp = sfe.pack(torch.from_numpy(w.query_ascii().copy()).to(dev), with_rc=True)
+    res, _, _ = sfe.ydrop_batch(tp[:2], len(w.target), qp, len(w.query), B._dev(B.make_pairs(w.pairs), dev), len(w.pairs),
+                                B._dev(B.make_anchors(w.anchors), dev), n, sc, B.SCORE_ONLY)
+    torch.cuda.synchronize()
+    out = dict(results=B.results_to_numpy(res, n))
+    assert not (out["results"]["status"] & np.uint32(B.ST_BAD_ANCHOR)).any()
+    H.assert_anchors_equal(out, w, range(n), want_cigar=False, ydrop=2000)
+    passed = out["results"]["score"] >= 3000
+    assert 0.5 * w.meta["n_true"] < int(passed.sum()) <= w.meta["n_true"] + 5      # 70 %-identity segments: most true hits pass, false ones do not
+    # the budget binds: no extension leaves its box
+    r = out["results"]; P = w.pairs
+    assert (r["tstart"] >= P[:, 0]).all() and (r["tend"] <= P[:, 1]).all()
