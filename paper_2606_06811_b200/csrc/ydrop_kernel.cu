@@ -152,6 +152,9 @@ static __device__ __forceinline__ void run_group16(int &upH, int &upE, int2 &pen
                                                    const char *rptr, char *wptr, const uint16_t *selp, const int col0,
                                                    const int m, const int t0)
 {
+#ifdef SFE_SHFL_HANDOFF
+    const bool lane_is0 = sfe_lane() == 0, lane_is31 = sfe_lane() == 31;
+#endif
     typedef RingGeom<RL2> G;
     const int best_in = best;
     int Hk[16];
@@ -179,10 +182,22 @@ static __device__ __forceinline__ void run_group16(int &upH, int &upE, int2 &pen
         if (isdead) dead |= 0x8000u >> k;
         if (k & 1) best = __vimax3_s32(best, Hk[k - 1], H); // one VIMNMX3 per two cells
         const int msgH = isdead ? SFE_NEG : Hg;            // dead cells send NEG on the diagonal / open edge
+#ifdef SFE_SHFL_HANDOFF
+        // A/B variant ("previous thread's values ... via warp shuffle"): lanes 1..31 take the message from the
+        // lane above by shuffle; shared memory only carries the strip-to-strip boundary row (lane 31 writes, lane 0 reads).
+        // Measured slower than the shared-memory exchange on sm_100a (profiles/r2_05): two SHFL per step replace one
+        // STS.64 + LDS.64 pair on the same MIO path and their latency sits on the step's dependency chain.
+        if (lane_is31) *(int2 *)(wptr + off) = make_int2(msgH, E);
+        dg = upH; F = Fn; Hgl = Hg;
+        int2 u;
+        u.x = __shfl_up_sync(FULL, msgH, 1); u.y = __shfl_up_sync(FULL, E, 1);
+        if (lane_is0) u = GLOBAL ? __ldcg((const int2 *)(rptr + off)) : *(const int2 *)(rptr + off);
+#else
         *(int2 *)(wptr + off) = make_int2(msgH, E);
         dg = upH; F = Fn; Hgl = Hg;
         SFE_STEP_FENCE();
         const int2 u = GLOBAL ? __ldcg((const int2 *)(rptr + off)) : *(const int2 *)(rptr + off);
+#endif
         if (SK == 1) { upH = u.x; upE = u.y; }             // the lane above is one column ahead: used in the next step
         else { upH = pend.x; upE = pend.y; pend = u; }     // two columns ahead: used the step after next
     }

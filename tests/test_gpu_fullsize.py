@@ -96,8 +96,8 @@ def sample_indices(res, n, k, seed, mask=None, n_largest=6):
     cells = res["cells"].astype(np.int64).copy()
     if mask is not None:
         cells[~mask] = -1
-    pick.update(np.argsort(-cells)[:n_largest].tolist())     # the largest extensions
-    pick.update(np.argsort(cells + (cells < 0) * (1 << 62))[:3].tolist())   # and the smallest
+    pick.update(np.argsort(-cells)[:min(n_largest, len(pool))].tolist())     # the largest extensions
+    pick.update(np.argsort(cells + (cells < 0) * (1 << 62))[:min(3, len(pool))].tolist())   # and the smallest
     return sorted(pick)
 
 
