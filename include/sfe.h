@@ -203,7 +203,7 @@ enum {
     SFE_OPT_FORCE_CLASS,           /* [0]     testing: 1 = nobody leads, 2 = everybody leads, 3 = second half of the anchors never  */
     SFE_OPT_PROMOTE_REACH,         /* [65536] after a batch, followers within this target distance of an extended anchor that will  
                                               not cover them (it scored below tau, or they lie beyond its box) become leaders       */
-    SFE_OPT_ROW_KERNEL_CAP,        /* [2^20]  most priority tickets (long-likely leaders, known long extensions) a pass hands to the
+    SFE_OPT_ROW_KERNEL_CAP,        /* [0]     most priority tickets (long-likely leaders, known long extensions) a pass hands to the
                                               cooperative row kernel, one CTA per half; 0 = never use it beside the systolic kernel  */
     SFE_OPT_ROW_KERNEL_SCORE_ONLY, /* [0]     1 = also in score-only passes (there the systolic chain is currently the faster one)   */
     SFE_OPT_N

@@ -24,12 +24,12 @@ int sfe_launch_tickets(const sfe_anchor *anchors, long long n_anchors, const sfe
                        long long cap_prio, long long cap_plain, cudaStream_t st);
 int sfe_launch_specl_prepare(const sfe_anchor *anchors, long long n, const uint8_t *t_nmask, long long t_len, const uint8_t *q_nmask,
                              const uint8_t *qrc_nmask, long long q_len, int tol, long long gap, int lookback, int n_break,
-                             uint8_t *cls, uint8_t *ext_state, long long *blkmin, void *state, const sfe_box *accepted,
+                             uint8_t *cls, uint8_t *lead_prio, uint8_t *ext_state, long long *blkmin, void *state, const sfe_box *accepted,
                              const long long *n_accepted, sfe_box *act, cudaStream_t st);
 int sfe_launch_spec_advance(void *state, const sfe_anchor *anchors, long long n, const long long *blkmin, long long K, long long span,
                             int esc_max, int tol, long long gap, int lookback, const uint8_t *cls, uint8_t *ext_state, sfe_box *act, int min_score, sfe_box *accepted,
                             long long accepted_cap, long long *win_idx, sfe_anchor *win_anchors, uint8_t *win_prio, uint8_t *keep,
-                            sfe_result *results, sfe_stats *stats, const int32_t *plist, cudaStream_t st);
+                            sfe_result *results, sfe_stats *stats, const int32_t *plist, const uint8_t *lead_prio, cudaStream_t st);
 int sfe_launch_spec_store(const sfe_result *wres, const long long *win_idx, long long wn, sfe_result *results, uint8_t *ext_state,
                           cudaStream_t st);
 int sfe_launch_specl_finish(const void *state, long long *n_accepted_io, cudaStream_t st);
@@ -77,7 +77,7 @@ struct sfe_ctx {
     unsigned long long *counters_host;  // pinned
     DevBuf halves, tickets, sel, hist, blkmin, act, misc, wide_tickets, wide_ring, ops_stage;
     DevBuf sp_state, sp_idx, sp_anchors, sp_results, sp_local, sp_blkmin, sp_act, sp_kanchors, sp_kidx, sp_kres;   // sfe_speculate
-    DevBuf sp_cls, sp_ext, sp_prio, sp_plist;   // predicted leaders
+    DevBuf sp_cls, sp_ext, sp_prio, sp_plist, sp_lprio;   // predicted leaders
     long long opt[SFE_OPT_N];         // sfe_set_option
     long long spec_info[8];           // sfe_last_speculate_info
     long long *state_host;            // pinned, 16 words
@@ -134,7 +134,7 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
     memset(c->spec_info, 0, sizeof c->spec_info);
     c->opt[SFE_OPT_LEADER_DIAG_TOL] = 48; c->opt[SFE_OPT_LEADER_GAP] = 2000; c->opt[SFE_OPT_LEADER_LOOKBACK] = 64;
     c->opt[SFE_OPT_LEADER_NBREAK] = 64; c->opt[SFE_OPT_SPEC_SPAN] = 1 << 20; c->opt[SFE_OPT_SPEC_ESC_MAX] = 64;
-    c->opt[SFE_OPT_SPARSE_WARPS] = 4; c->opt[SFE_OPT_FORCE_CLASS] = 0; c->opt[SFE_OPT_PROMOTE_REACH] = 65536; c->opt[SFE_OPT_ROW_KERNEL_CAP] = 1 << 20; c->opt[SFE_OPT_ROW_KERNEL_SCORE_ONLY] = 0;
+    c->opt[SFE_OPT_SPARSE_WARPS] = 4; c->opt[SFE_OPT_FORCE_CLASS] = 0; c->opt[SFE_OPT_PROMOTE_REACH] = 65536; c->opt[SFE_OPT_ROW_KERNEL_CAP] = 0; c->opt[SFE_OPT_ROW_KERNEL_SCORE_ONLY] = 0;
     c->ev_pending = false; c->kernel_us = 0.0; c->n_profile = 0;
     if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -170,7 +170,7 @@ extern "C" int sfe_destroy(sfe_ctx *c)
     if (c->state_host) cudaFreeHost(c->state_host);
     cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1); cudaEventDestroy(c->ev_fork); cudaEventDestroy(c->ev_join);
     if (c->aux) { cudaStreamSynchronize(c->aux); cudaStreamDestroy(c->aux); }
-    DevBuf *bufs[] = {&c->sp_cls, &c->sp_ext, &c->sp_prio, &c->sp_plist, &c->sp_kanchors, &c->sp_kidx, &c->sp_kres, &c->sp_state, &c->sp_idx, &c->sp_anchors, &c->sp_results, &c->sp_local, &c->sp_blkmin, &c->sp_act, &c->ops_stage, &c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
+    DevBuf *bufs[] = {&c->sp_cls, &c->sp_ext, &c->sp_prio, &c->sp_plist, &c->sp_lprio, &c->sp_kanchors, &c->sp_kidx, &c->sp_kres, &c->sp_state, &c->sp_idx, &c->sp_anchors, &c->sp_results, &c->sp_local, &c->sp_blkmin, &c->sp_act, &c->ops_stage, &c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
                       &c->h_t2, &c->h_tm, &c->h_q2, &c->h_qm, &c->h_r2, &c->h_rm, &c->h_pairs, &c->h_anchors, &c->h_results,
                       &c->h_keep, &c->h_cigar, &c->h_acc, &c->h_small};
     for (DevBuf *b : bufs) b->release();
@@ -459,7 +459,7 @@ extern "C" int sfe_speculate(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t 
         if (!t_nmask || !q_nmask) return SFE_EINVAL;
         if ((rc = c->sp_state.ensure(128)) || (rc = c->sp_idx.ensure((size_t)K * sizeof(long long))) ||
             (rc = c->sp_anchors.ensure((size_t)K * sizeof(sfe_anchor))) || (rc = c->sp_results.ensure((size_t)K * sizeof(sfe_result))) ||
-            (rc = c->sp_prio.ensure((size_t)K)) || (rc = c->sp_cls.ensure((size_t)n_anchors + 8)) || (rc = c->sp_plist.ensure((size_t)n_anchors * sizeof(int32_t))) || (rc = c->sp_ext.ensure((size_t)n_anchors)) ||
+            (rc = c->sp_prio.ensure((size_t)K)) || (rc = c->sp_cls.ensure((size_t)n_anchors + 8)) || (rc = c->sp_plist.ensure((size_t)n_anchors * sizeof(int32_t))) || (rc = c->sp_lprio.ensure((size_t)n_anchors)) || (rc = c->sp_ext.ensure((size_t)n_anchors)) ||
             (rc = c->sp_blkmin.ensure((size_t)((n_anchors + 31) / 32 + 32) * sizeof(long long))) ||
             (rc = c->sp_act.ensure((size_t)(n_anchors + accepted_cap + 1) * sizeof(sfe_box)))) return rc;
         long long *blkmin = (long long *)c->sp_blkmin.p;
@@ -467,7 +467,7 @@ extern "C" int sfe_speculate(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t 
         uint8_t *cls = (uint8_t *)c->sp_cls.p, *ext = (uint8_t *)c->sp_ext.p;
         if ((rc = sfe_launch_specl_prepare(anchors_dev, n_anchors, t_nmask, t_len, q_nmask, qrc_nmask, q_len, (int)c->opt[SFE_OPT_LEADER_DIAG_TOL],
                                            c->opt[SFE_OPT_LEADER_GAP], (int)c->opt[SFE_OPT_LEADER_LOOKBACK], (int)c->opt[SFE_OPT_LEADER_NBREAK],
-                                           cls, ext, blkmin, c->sp_state.p, accepted_dev, (const long long *)n_accepted_dev, act, c->stream))) return rc;
+                                           cls, (uint8_t *)c->sp_lprio.p, ext, blkmin, c->sp_state.p, accepted_dev, (const long long *)n_accepted_dev, act, c->stream))) return rc;
         if (c->opt[SFE_OPT_FORCE_CLASS] == 1) SFE_CUDA_CHECK(cudaMemsetAsync(cls, 0, (size_t)n_anchors, c->stream));        // testing: nobody leads
         else if (c->opt[SFE_OPT_FORCE_CLASS] == 2) SFE_CUDA_CHECK(cudaMemsetAsync(cls, 1, (size_t)n_anchors, c->stream));   // everybody leads
         else if (c->opt[SFE_OPT_FORCE_CLASS] == 3) SFE_CUDA_CHECK(cudaMemsetAsync(cls + n_anchors / 2, 0, (size_t)(n_anchors - n_anchors / 2), c->stream));
@@ -475,7 +475,7 @@ extern "C" int sfe_speculate(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t 
         for (;;) {
             if ((rc = sfe_launch_spec_advance(c->sp_state.p, anchors_dev, n_anchors, blkmin, K, c->opt[SFE_OPT_SPEC_SPAN], (int)c->opt[SFE_OPT_SPEC_ESC_MAX],
                                               (int)c->opt[SFE_OPT_LEADER_DIAG_TOL], c->opt[SFE_OPT_LEADER_GAP], (int)c->opt[SFE_OPT_LEADER_LOOKBACK], cls, ext, act, sc->min_score, accepted_dev, accepted_cap, (long long *)c->sp_idx.p,
-                                              (sfe_anchor *)c->sp_anchors.p, (uint8_t *)c->sp_prio.p, keep_dev, results_dev, stats_dev, (const int32_t *)c->sp_plist.p, c->stream))) return rc;
+                                              (sfe_anchor *)c->sp_anchors.p, (uint8_t *)c->sp_prio.p, keep_dev, results_dev, stats_dev, (const int32_t *)c->sp_plist.p, (const uint8_t *)c->sp_lprio.p, c->stream))) return rc;
             SFE_CUDA_CHECK(cudaMemcpyAsync(c->state_host, c->sp_state.p, 13 * sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
             SFE_CUDA_CHECK(cudaStreamSynchronize(c->stream));
             const long long cursor = c->state_host[0], wn = c->state_host[1];

@@ -513,7 +513,7 @@ static __device__ long long count_n(const uint8_t *nmask, long long a, long long
 
 __global__ void spec_classify_kernel(const sfe_anchor *anchors, long long n, const uint8_t *t_nmask, long long t_len,
                                      const uint8_t *q_nmask, const uint8_t *qrc_nmask, long long q_len, int tol, long long gap,
-                                     int lookback, int n_break, uint8_t *cls)
+                                     int lookback, int n_break, uint8_t *cls, uint8_t *lead_prio)
 {
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -528,7 +528,7 @@ __global__ void spec_classify_kernel(const sfe_anchor *anchors, long long n, con
         return f && b;
     };
     uint8_t c = CLS_LEADER;
-    if (qm && dead_end(a)) { cls[i] = CLS_LEADER; return; }
+    if (qm && dead_end(a)) { cls[i] = CLS_LEADER; lead_prio[i] = 0; return; }
     const long long diag = a.tpos - a.qpos;
     for (long long j = i - 1; j >= 0 && j >= i - lookback; j--) {
         const sfe_anchor p = anchors[j];
@@ -542,15 +542,27 @@ __global__ void spec_classify_kernel(const sfe_anchor *anchors, long long n, con
         c = CLS_FOLLOWER;
         break;
     }
-    if (c == CLS_LEADER) {                                  // long-likely: a follower-to-be right behind it
-        for (long long j = i + 1; j < n && j <= i + lookback; j++) {
+    uint8_t pr = 0;
+    if (c == CLS_LEADER) {
+        // Long-likely, and how long: follow the anchors that would follow this one (same strand / pair, diagonal within tol of the
+        // LAST one found, no gap wider than `gap`) -- the reach of that chain is a proxy of the alignment's span, which nothing
+        // else knows before the extension has run.  Its log2 becomes the ticket priority (longest first).
+        long long last_t = a.tpos, last_d = diag; int nf = 0;
+        for (long long j = i + 1; j < n && j <= i + (1 << 17); j++) {
             const sfe_anchor p = anchors[j];
-            if (p.tpos - a.tpos > gap || p.tpos < a.tpos) break;
+            if (p.tpos - last_t > gap || p.tpos < a.tpos) break;
             if ((p.strand >= 0 ? 1 : -1) != strand || p.pair != a.pair) continue;
-            const long long dd = (p.tpos - p.qpos) - diag;
-            if (dd <= tol && dd >= -tol) { c = CLS_LEADER_LONG; break; }
+            const long long dd = (p.tpos - p.qpos) - last_d;
+            if (dd <= tol && dd >= -tol) { last_t = p.tpos; last_d = p.tpos - p.qpos; nf++; }
+        }
+        if (nf > 0) {
+            c = CLS_LEADER_LONG;
+            long long span = last_t - a.tpos + 1;
+            if (span > 0x3fffffff) span = 0x3fffffff;
+            pr = (uint8_t)(1 + (31 - __clz((int)span)));
         }
     }
+    lead_prio[i] = pr;
     cls[i] = c;
 }
 
@@ -569,7 +581,7 @@ __global__ void spec_advance_kernel(SpecLState *st, const sfe_anchor *anchors, l
                                     long long span, int esc_max, int tol, long long gap, int lookback, const uint8_t *cls, uint8_t *ext_state, sfe_box *act,
                                     int min_score, sfe_box *accepted, long long accepted_cap, long long *win_idx,
                                     sfe_anchor *win_anchors, uint8_t *win_prio, uint8_t *keep, sfe_result *results, sfe_stats *stats,
-                                    const int32_t *plist)
+                                    const int32_t *plist, const uint8_t *lead_prio)
 {
     const int lane = threadIdx.x & 31;
     long long j = st->cursor, nact = st->nact, nacc = st->nacc;
@@ -762,7 +774,7 @@ __global__ void spec_advance_kernel(SpecLState *st, const sfe_anchor *anchors, l
             }
             if ((m >> lane) & 1u) {
                 const long long d = wn + __popc(m & ((1u << lane) - 1));
-                win_idx[d] = i; win_anchors[d] = an; win_prio[d] = c == CLS_LEADER_LONG ? 1 : 0; ext_state[i] = 2;
+                win_idx[d] = i; win_anchors[d] = an; win_prio[d] = c == CLS_LEADER_LONG ? lead_prio[i] : 0; ext_state[i] = 2;
             }
             wn += __popc(m);
             p = next_p;
@@ -838,14 +850,14 @@ __global__ void specl_finish_kernel(const SpecLState *st, long long *n_accepted_
 
 int sfe_launch_specl_prepare(const sfe_anchor *anchors, long long n, const uint8_t *t_nmask, long long t_len, const uint8_t *q_nmask,
                              const uint8_t *qrc_nmask, long long q_len, int tol, long long gap, int lookback, int n_break,
-                             uint8_t *cls, uint8_t *ext_state, long long *blkmin, void *state, const sfe_box *accepted,
+                             uint8_t *cls, uint8_t *lead_prio, uint8_t *ext_state, long long *blkmin, void *state, const sfe_box *accepted,
                              const long long *n_accepted, sfe_box *act, cudaStream_t st)
 {
     const int bs = 256;
     const unsigned nb = (unsigned)((n + bs - 1) / bs);
     SFE_KL block_min_kernel<<<nb, bs, 0, st>>>(anchors, n, blkmin);
     SFE_KL suffix_min_kernel<<<1, 32, 0, st>>>(blkmin, (n + 31) >> 5);
-    SFE_KL spec_classify_kernel<<<nb, bs, 0, st>>>(anchors, n, t_nmask, t_len, q_nmask, qrc_nmask, q_len, tol, gap, lookback, n_break, cls);
+    SFE_KL spec_classify_kernel<<<nb, bs, 0, st>>>(anchors, n, t_nmask, t_len, q_nmask, qrc_nmask, q_len, tol, gap, lookback, n_break, cls, lead_prio);
     if (cudaMemsetAsync(ext_state, 0, (size_t)n, st) != cudaSuccess) return SFE_ECUDA;
     SFE_KL specl_init_kernel<<<1, 32, 0, st>>>((SpecLState *)state, accepted, n_accepted, act);
     SFE_LAUNCH_CHECK();
@@ -854,10 +866,10 @@ int sfe_launch_specl_prepare(const sfe_anchor *anchors, long long n, const uint8
 int sfe_launch_spec_advance(void *state, const sfe_anchor *anchors, long long n, const long long *blkmin, long long K, long long span,
                             int esc_max, int tol, long long gap, int lookback, const uint8_t *cls, uint8_t *ext_state, sfe_box *act, int min_score, sfe_box *accepted,
                             long long accepted_cap, long long *win_idx, sfe_anchor *win_anchors, uint8_t *win_prio, uint8_t *keep,
-                            sfe_result *results, sfe_stats *stats, const int32_t *plist, cudaStream_t st)
+                            sfe_result *results, sfe_stats *stats, const int32_t *plist, const uint8_t *lead_prio, cudaStream_t st)
 {
     SFE_KL spec_advance_kernel<<<1, 32, 0, st>>>((SpecLState *)state, anchors, n, blkmin, K, span, esc_max, tol, gap, lookback, cls, ext_state, act, min_score,
-                                                 accepted, accepted_cap, win_idx, win_anchors, win_prio, keep, results, stats, plist);
+                                                 accepted, accepted_cap, win_idx, win_anchors, win_prio, keep, results, stats, plist, lead_prio);
     SFE_LAUNCH_CHECK();
 }
 

@@ -43,8 +43,8 @@ template <int RL2> struct RingGeom {
 
 // ---- traceback arena --------------------------------------------------------------------------
 // Record = 32 lanes x two 32-bit words (16 cells x 4 bits) = 256 B, written coalesced (one 8-byte
-// store per lane) by one warp per group of 16 steps; lane l owns words 2l (steps 0-7) and 2l+1
-// (steps 8-15).  Records live in 64 KiB chunks handed out by an atomic counter; a half's chunks
+// store per lane) by one warp per group of 16 steps; lane l owns words 2l (bit planes 3 and 2 of its
+// 16 cells: plane 3 in the upper half, step k at bit 15 - k) and 2l+1 (planes 1 and 0).  Records live in 64 KiB chunks handed out by an atomic counter; a half's chunks
 // form a backward-linked list (chunk_prev).
 // Chunks are recycled: a lock-free ring of free chunk ids (SfeFreeRing) hands them out and takes them
 // back as soon as the warp that filled them has walked its traceback, so the arena only has to hold

@@ -102,7 +102,9 @@ struct TbWriter {
             ptr = pool + (size_t)c * SFE_CHUNK_RECS * SFE_REC_WORDS + 2 * lane;
             left = SFE_CHUNK_RECS;
         }
+#ifndef SFE_EXP_NOSTORE
         *(uint2 *)ptr = make_uint2(w0, w1);
+#endif
         ptr += SFE_REC_WORDS; left--; nrec++;
     }
     // give every chunk of this half back (after the walk, or when the half is abandoned)
@@ -137,8 +139,10 @@ static __device__ __forceinline__ uint32_t shift_in_sign(uint32_t acc, int x) { 
 // (alive gate, R5/R6), 4 x (subtract + funnel shift) for the traceback nibble, half a VIMNMX3 (best), and
 // the message STS.64 / LDS.64.  The kernel is issue-bound (profiles/r1_02), so what counts is the
 // number of instructions, not the pipe they run on; the subtractions stay on the FMA pipe (IMAD).
-// Traceback nibble of step k sits at bits 4(7-(k&7)).. of acc0 (k < 8) / acc1 (k >= 8):
-//   bit3 = H not from M, bit2 = H not from E, bit1 = E extended, bit0 = F extended (R11).
+// Traceback: four bit PLANES per lane per group, step k at bit 15-k of each (acc0 = plane3 << 16 | plane2 ... see below):
+//   plane 3 = H not from M, plane 2 = H not from E, plane 1 = E extended, plane 0 = F extended (R11).
+// One accumulator per plane: four independent shift chains of one SHF per step instead of one chain of four (the
+// pointer bits of a long half are a second loop-carried dependency next to the DP's own).
 // dead: bit 15-k set iff the cell of step k is dead.
 // The position of a new lane-local best (strict '>', R7) is found after the group, only by the
 // lanes whose best rose: the first k with H_k == best is the last strict increase.
@@ -157,6 +161,7 @@ static __device__ __forceinline__ void run_group16(int &upH, int &upE, int2 &pen
 #endif
     typedef RingGeom<RL2> G;
     const int best_in = best;
+    uint32_t pl3 = 0, pl2 = 0, pl1 = 0, pl0 = 0;
     int Hk[16];
 #pragma unroll
     for (int k = 0; k < 16; k++) {
@@ -172,13 +177,14 @@ static __device__ __forceinline__ void run_group16(int &upH, int &upE, int2 &pen
         Hk[k] = H;
         const bool isdead = H < T;                         // R5: alive <=> H >= T
         const int Hg = H - OX;
+#ifndef SFE_EXP_NOBITS
         if (TB) {
-            uint32_t &acc = k < 8 ? acc0 : acc1;
-            acc = shift_in_sign(acc, fma_sub(M, H));       // M < H  <=> H not from M
-            acc = shift_in_sign(acc, fma_sub(E, H));       // E < H  <=> H not from E
-            acc = shift_in_sign(acc, fma_sub(upH, E));     // upH < E <=> E extended (open wins ties)
-            acc = shift_in_sign(acc, fma_sub(Hgl, Fn));    // Hgl < F <=> F extended
+            pl3 = shift_in_sign(pl3, fma_sub(M, H));       // M < H  <=> H not from M
+            pl2 = shift_in_sign(pl2, fma_sub(E, H));       // E < H  <=> H not from E
+            pl1 = shift_in_sign(pl1, fma_sub(upH, E));     // upH < E <=> E extended (open wins ties)
+            pl0 = shift_in_sign(pl0, fma_sub(Hgl, Fn));    // Hgl < F <=> F extended
         }
+#endif
         if (isdead) dead |= 0x8000u >> k;
         if (k & 1) best = __vimax3_s32(best, Hk[k - 1], H); // one VIMNMX3 per two cells
         const int msgH = isdead ? SFE_NEG : Hg;            // dead cells send NEG on the diagonal / open edge
@@ -201,6 +207,7 @@ static __device__ __forceinline__ void run_group16(int &upH, int &upE, int2 &pen
         if (SK == 1) { upH = u.x; upE = u.y; }             // the lane above is one column ahead: used in the next step
         else { upH = pend.x; upE = pend.y; pend = u; }     // two columns ahead: used the step after next
     }
+    if (TB) { acc0 = __byte_perm(pl2, pl3, 0x5410); acc1 = __byte_perm(pl0, pl1, 0x5410); }   // plane3:plane2, plane1:plane0
     if (best > best_in) {
         int kk = 15;
 #pragma unroll
@@ -219,13 +226,20 @@ static __device__ __forceinline__ void run_group16(int &upH, int &upE, int2 &pen
 struct TbReader {                       // random access to this half's records; all lanes hold the same cursor
     const uint32_t *pool; const int32_t *chunk_prev;
     int chunk, ord, last_chunk, last_ord, nrec;
+    int up_chunk, up_ord;               // the chunk one above the cursor (ordinal ord + 1), -1 if not known
     bool bad;                           // an index outside the half's records was asked for (never expected)
     __device__ __forceinline__ const uint32_t *rec(int ridx)
     {
         if (ridx < 0 || ridx >= nrec) { bad = true; ridx = 0; }
         const int o = ridx / SFE_CHUNK_RECS;
-        if (o > ord) { chunk = last_chunk; ord = last_ord; }   // rare: the indices are visited in decreasing order
-        while (ord > o) { chunk = __ldcg(chunk_prev + chunk); ord--; }
+        // The walk visits records in (mostly) decreasing order, but a strip's header may sit in the chunk below the
+        // strip's records: going back UP one chunk must not restart from the end of the chain (a half of 5 * 10^5 rows has
+        // ~300 chunks: that restart cost 28,000 cycles per strip, a third of the whole traceback pass, until round 2).
+        if (o > ord) {
+            if (o == up_ord && up_chunk >= 0) { chunk = up_chunk; ord = up_ord; up_chunk = -1; }
+            else { chunk = last_chunk; ord = last_ord; up_chunk = -1; }
+        }
+        while (ord > o) { up_chunk = chunk; up_ord = ord; chunk = __ldcg(chunk_prev + chunk); ord--; }
         return pool + ((size_t)chunk * SFE_CHUNK_RECS + (ridx - o * SFE_CHUNK_RECS)) * SFE_REC_WORDS;
     }
 };
@@ -245,15 +259,18 @@ static __device__ bool walk_traceback(const YdParams &p, TbReader &rd, const int
     __syncwarp();                                        // the records of this half, written lane by lane, are visible
     int i = end_i, j = end_j, state = 0;
     const uint32_t *hr = rd.rec(hdr);
-    int cs = (int)__ldcg(hr), prev_hdr = (int)__ldcg(hr + 1);
-    while (strip > (i >> 5)) { hdr = prev_hdr; strip--; hr = rd.rec(hdr); cs = (int)__ldcg(hr); prev_hdr = (int)__ldcg(hr + 1); }
+    uint2 hv = __ldcg((const uint2 *)hr);
+    int cs = (int)hv.x, prev_hdr = (int)hv.y;
+    while (strip > (i >> 5)) { hdr = prev_hdr; strip--; hr = rd.rec(hdr); hv = __ldcg((const uint2 *)hr); cs = (int)hv.x; prev_hdr = (int)hv.y; }
     int win_lo = 0, win_hi = -1;                         // record groups of this strip held in win[]
+    int pre_idx = -1; uint2 pre_hv = make_uint2(0u, 0u); // header of the strip above, loaded ahead
     long long guard = 3LL * ((long long)end_i + end_j) + 4LL * (strip + 1) + 64;
     while (!(i == 0 && j == 0 && state == 0)) {
         if (--guard < 0 || rd.bad) return false;
         if ((i >> 5) < strip) {                          // crossed into the strip above
             hdr = prev_hdr; strip--;
-            hr = rd.rec(hdr); cs = (int)__ldcg(hr); prev_hdr = (int)__ldcg(hr + 1);
+            if (pre_idx == hdr) hv = pre_hv; else { hr = rd.rec(hdr); hv = __ldcg((const uint2 *)hr); }
+            cs = (int)hv.x; prev_hdr = (int)hv.y;
             win_hi = -1;
         }
         const int L = i & 31;
@@ -262,10 +279,24 @@ static __device__ bool walk_traceback(const YdParams &p, TbReader &rd, const int
         if (g > win_hi || g < win_lo) {                  // (re)load the window: groups g-7 .. g
             __syncwarp();
             win_hi = g; win_lo = max(0, g - (SFE_WALK_WIN_RECS - 1));
-            for (int x = win_hi; x >= win_lo; x--) {
-                const uint2 v = __ldcg((const uint2 *)(rd.rec(hdr + 1 + x) + 2 * lane));
-                *(uint2 *)(win + (x - win_lo) * SFE_REC_WORDS + 2 * lane) = v;
+            // The window's records are consecutive and span at most two chunks: resolve the two chunk bases first, then the
+            // loads are plain address arithmetic and independent of one another -- one memory latency per window, not one
+            // per record (the records of a long half were written long ago: they come from HBM, ~800 cycles each).
+            const int r_hi = hdr + 1 + win_hi, r_lo = hdr + 1 + win_lo;
+            const int o_hi = r_hi / SFE_CHUNK_RECS;
+            const uint32_t *b_hi = rd.rec(r_hi) - (size_t)(r_hi - o_hi * SFE_CHUNK_RECS) * SFE_REC_WORDS;
+            const uint32_t *b_lo = rd.rec(r_lo) - (size_t)(r_lo - (r_lo / SFE_CHUNK_RECS) * SFE_CHUNK_RECS) * SFE_REC_WORDS;
+            if (prev_hdr >= 0 && pre_idx != prev_hdr) { pre_idx = prev_hdr; pre_hv = __ldcg((const uint2 *)rd.rec(prev_hdr)); }   // next strip's header, early
+            uint2 wv[SFE_WALK_WIN_RECS];
+#pragma unroll
+            for (int y = 0; y < SFE_WALK_WIN_RECS; y++) {
+                const int r = r_lo + y;
+                const int o = r / SFE_CHUNK_RECS;
+                const uint32_t *src = (o == o_hi ? b_hi : b_lo) + (size_t)(r - o * SFE_CHUNK_RECS) * SFE_REC_WORDS + 2 * lane;
+                wv[y] = r <= r_hi ? __ldcg((const uint2 *)src) : make_uint2(0u, 0u);
             }
+#pragma unroll
+            for (int y = 0; y < SFE_WALK_WIN_RECS; y++) *(uint2 *)(win + y * SFE_REC_WORDS + 2 * lane) = wv[y];
             __syncwarp();
         }
         // lane k examines the k-th cell from (i, j) in the direction of the current state
@@ -274,7 +305,11 @@ static __device__ bool walk_traceback(const YdParams &p, TbReader &rd, const int
         const int tk = t - lane * (SK * di + dj);
         const bool valid = Lk >= 0 && tk >= 0 && (tk >> 4) >= win_lo;
         uint32_t nib = 0;
-        if (valid) nib = (win[((tk >> 4) - win_lo) * SFE_REC_WORDS + 2 * Lk + ((tk >> 3) & 1)] >> ((7 - (tk & 7)) * 4)) & 15u;
+        if (valid) {
+            const uint2 w = *(const uint2 *)(win + ((tk >> 4) - win_lo) * SFE_REC_WORDS + 2 * Lk);    // planes 3:2, 1:0 of that lane and group
+            const int sft = 15 - (tk & 15);
+            nib = (((w.x >> (16 + sft)) & 1u) << 3) | (((w.x >> sft) & 1u) << 2) | (((w.y >> (16 + sft)) & 1u) << 1) | ((w.y >> sft) & 1u);
+        }
         // nib: bit3 = H not from M, bit2 = H not from E, bit1 = E extended, bit0 = F extended
         const bool cont = state == 0 ? !(nib & 8u) : (state == 1 ? (nib & 2u) != 0 : (nib & 1u) != 0);
         const bool origin = i == lane * di && j == lane * dj;   // the walk ends at (0,0), whose own nibble says "from M"
@@ -471,10 +506,14 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
     out.status = (wide ? (GLOBAL ? (SFE_ST_WIDE | SFE_ST_BAND_LIMIT) : SFE_ST_WIDE_PENDING) : (GLOBAL ? SFE_ST_WIDE : 0u)) |
                  ((TB && !tb.ok) ? SFE_ST_PASS_OVERFLOW : 0u) | (limit ? SFE_ST_SCORE_LIMIT : 0u) | mode_bits;
     out.n_strips = n_strips; out.n_rec = tb.nrec;
+#ifdef SFE_EXP_NOWALK
+    if (false) {
+#else
     if (TB && tb.ok && !wide && !limit) {                             // a8: walk the pointers now, stage the run-length ops
+#endif
         TbReader rd;
         rd.pool = p.pool; rd.chunk_prev = p.chunk_prev; rd.chunk = tb.cur_chunk; rd.ord = (tb.nrec - 1) / SFE_CHUNK_RECS;
-        rd.last_chunk = rd.chunk; rd.last_ord = rd.ord; rd.nrec = tb.nrec; rd.bad = false;
+        rd.last_chunk = rd.chunk; rd.last_ord = rd.ord; rd.nrec = tb.nrec; rd.bad = false; rd.up_chunk = -1; rd.up_ord = -1;
         bool ops_ok = true;
         if (!walk_traceback<SK>(p, rd, bi, bj, last_hdr, n_strips - 1, wk, lane, out.ops_seg, out.n_ops, ops_ok))
             out.status |= SFE_ST_INTERNAL;

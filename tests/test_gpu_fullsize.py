@@ -234,9 +234,14 @@ def test_config5_scaled_windowed(sfe_big, oracle):
 
 def test_config5_scaled_leaders_equals_classic(sfe_big, oracle):
     """configs[4] at 1/10 scale with predicted leaders: the same kept set, and for the kept anchors the same results, as
-    the classic windows; the cooperative row kernel took the long-likely tickets (block_halves > 0)."""
+    the classic windows; here with the cooperative row kernel taking the long-likely tickets (block_halves > 0; by default
+    they stay on the systolic kernel, which test_config5_full_leaders covers)."""
     w = W.config5(t_len=10_000_000, n_anchors=100_000)
-    out = _speculate_full(sfe_big, w, 262144, 1 << 26, flags=LEADERS)
+    sfe_big.set_option(B.OPT_ROW_KERNEL_CAP, 1 << 20)      # the long-likely tickets on the cooperative row kernel, beside the systolic one
+    try:
+        out = _speculate_full(sfe_big, w, 262144, 1 << 26, flags=LEADERS)
+    finally:
+        sfe_big.set_option(B.OPT_ROW_KERNEL_CAP, 0)
     assert sfe_big.last_batch_info()["block_halves"] > 0
     n_ext = int(out["stats"]["n_extended"])
     assert _check_speculated(w, out, 5, max(40, n_ext // 1000), n_kept_sample=20, kept_only=False) >= n_ext // 1000
