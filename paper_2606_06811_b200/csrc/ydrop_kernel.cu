@@ -102,9 +102,7 @@ struct TbWriter {
             ptr = pool + (size_t)c * SFE_CHUNK_RECS * SFE_REC_WORDS + 2 * lane;
             left = SFE_CHUNK_RECS;
         }
-#ifndef SFE_EXP_NOSTORE
         *(uint2 *)ptr = make_uint2(w0, w1);
-#endif
         ptr += SFE_REC_WORDS; left--; nrec++;
     }
     // give every chunk of this half back (after the walk, or when the half is abandoned)
@@ -177,14 +175,12 @@ static __device__ __forceinline__ void run_group16(int &upH, int &upE, int2 &pen
         Hk[k] = H;
         const bool isdead = H < T;                         // R5: alive <=> H >= T
         const int Hg = H - OX;
-#ifndef SFE_EXP_NOBITS
         if (TB) {
             pl3 = shift_in_sign(pl3, fma_sub(M, H));       // M < H  <=> H not from M
             pl2 = shift_in_sign(pl2, fma_sub(E, H));       // E < H  <=> H not from E
             pl1 = shift_in_sign(pl1, fma_sub(upH, E));     // upH < E <=> E extended (open wins ties)
             pl0 = shift_in_sign(pl0, fma_sub(Hgl, Fn));    // Hgl < F <=> F extended
         }
-#endif
         if (isdead) dead |= 0x8000u >> k;
         if (k & 1) best = __vimax3_s32(best, Hk[k - 1], H); // one VIMNMX3 per two cells
         const int msgH = isdead ? SFE_NEG : Hg;            // dead cells send NEG on the diagonal / open edge
@@ -506,11 +502,7 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
     out.status = (wide ? (GLOBAL ? (SFE_ST_WIDE | SFE_ST_BAND_LIMIT) : SFE_ST_WIDE_PENDING) : (GLOBAL ? SFE_ST_WIDE : 0u)) |
                  ((TB && !tb.ok) ? SFE_ST_PASS_OVERFLOW : 0u) | (limit ? SFE_ST_SCORE_LIMIT : 0u) | mode_bits;
     out.n_strips = n_strips; out.n_rec = tb.nrec;
-#ifdef SFE_EXP_NOWALK
-    if (false) {
-#else
     if (TB && tb.ok && !wide && !limit) {                             // a8: walk the pointers now, stage the run-length ops
-#endif
         TbReader rd;
         rd.pool = p.pool; rd.chunk_prev = p.chunk_prev; rd.chunk = tb.cur_chunk; rd.ord = (tb.nrec - 1) / SFE_CHUNK_RECS;
         rd.last_chunk = rd.chunk; rd.last_ord = rd.ord; rd.nrec = tb.nrec; rd.bad = false; rd.up_chunk = -1; rd.up_ord = -1;
