@@ -326,6 +326,8 @@ def main():
     ap.add_argument("--c5", default="auto", choices=["auto", "full", "prefix", "off"],
                     help="the c5_e2e key of the default (c4) line: Algorithm 3 end to end on configs[4]; prefix = the 10 Mbp / "
                          "100,000-anchor prefix-scale run SURVEY 8(d) allows; auto = full")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="sfe_set_option, e.g. SPEC_SPAN=262144, SPARSE_WARPS=8, ROW_KERNEL_CAP=1048576 (binding.OPT_* names)")
     ap.add_argument("--limit-anchors", type=int, default=0, help="profiling aid: keep every k-th anchor so that N remain")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -358,6 +360,10 @@ def main():
     free_b, _ = torch.cuda.mem_get_info(dev)
     scratch = min(SCRATCH_GB[args.workload] << 30, int(free_b * 0.6))
     sfe = B.Sfe(local, scratch)
+    opts = {}
+    for kv in args.opt:
+        k, v = kv.split("=")
+        sfe.set_option(getattr(B, "OPT_" + k.upper()), int(v)); opts[k.upper()] = int(v)
 
     window = DEFAULT_WINDOW.get(args.workload, 0) if args.window < 0 else args.window
     if args.window < 0 and window > 0 and args.spec == "leaders":
@@ -563,7 +569,7 @@ def main():
     line = {"metric": "ydrop_gcups", "value": gcups, "unit": "GCUPS", "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "window_k": window, "kernel": args.kernel, "spec": (args.spec if window > 0 else None), "cigar_for": "kept" if kept_only else ("all" if args.flags == "cigar" else "none"),
+            "config": {"workload": f"{args.workload}: {desc}", "anchors": n, "flags": args.flags, "window_k": window, "kernel": args.kernel, "spec": (args.spec if window > 0 else None), "options": opts or None, "cigar_for": "kept" if kept_only else ("all" if args.flags == "cigar" else "none"),
                        "l2": "inputs+traceback per step exceed L2 (126 MB)", "generation_s": t_gen,
                        "parallelism": "replicas only" if world > 1 else "1 GPU", "scoring": "HOXD70/400/30/ydrop 9400/lag 32/tau 3000"},
             "kept_alignments_per_s": kept_step * args.steps * world / (ms * 1e-3),
