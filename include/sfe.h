@@ -47,8 +47,8 @@ enum {
 #define SFE_SCORE_ONLY 0u             /* scores, boxes and cell counts only                      */
 #define SFE_NO_BINNING 2u             /* tickets in anchor order (default: longest-first bins)   */
 #define SFE_BLOCK_KERNEL 4u           /* every half on a cooperative-warps kernel (one CTA per half, rows in order, prefix
-                                         maximum for F; same results).  By default only the longest
-                                         tickets of a pass go there, beside the warp-systolic kernel                       */
+                                         maximum for F; same results).  SFE_OPT_ROW_KERNEL_CAP > 0
+                                         instead hands only a pass's priority tickets to it, beside the systolic kernel   */
 #define SFE_NO_BLOCK_KERNEL 8u        /* warp-systolic kernel only (overrides SFE_BLOCK_KERNEL and the default split)     */
 #define SFE_CIGAR_KEPT_ONLY 16u       /* sfe_speculate with SFE_WANT_CIGAR: windows run score-only (the commit rule needs
                                          score and box only); CIGARs are produced for the KEPT anchors in one

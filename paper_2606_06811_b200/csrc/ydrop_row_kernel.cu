@@ -2,11 +2,14 @@
 // per anchor-half ... kernel wall time / 3.3"), for the LONG halves whose serial chain bounds a pass.
 //
 // Why a second kernel.  With the row-lagged threshold (R4, Lambda = 32) at most 32 rows of one extension can be in flight:
-// the warp-systolic kernel turns a half of n rows into ~ n/32 (W + 62) dependent wavefront steps, measured 1,016 cycles per
-// row score-only and 2,270 with traceback on a 580 k-row half of configs[4] (profiles/r2_*), whatever else the GPU does.
+// the warp-systolic kernel turns a half of n rows into ~ n/32 (W + 62) dependent wavefront steps, measured 1,030 cycles per
+// row score-only and 1,450 with traceback on a 580 k-row half of configs[4] (profiles/r2_03), whatever else the GPU does.
 // The parallelism that is left is ALONG a row: one CTA per half, rows strictly in order, every thread owns RK_C consecutive
 // columns of a 1024-column window.  The first cooperative kernel (ydrop_block_kernel.cu, kept for Lambda = 0) spent ~700
-// instructions per thread per row and two block barriers on that and was slower than the chain it should replace.  Here:
+// instructions per thread per row and two block barriers on that (2,256 cycles per row).  This one: 1,250 score-only /
+// 1,680 with traceback -- still latency-bound (~250 instructions per warp per row at ~5 cycles each, profiles/r2_04) and,
+// since the systolic kernel's traceback walk was repaired, no longer ahead of it: opt-in (SFE_BLOCK_KERNEL, or
+// SFE_OPT_ROW_KERNEL_CAP for the priority tickets of a pass).  Design:
 //   * ONE block barrier per row (the exchange of the warps' F carries); the diagonal hand-off between neighbouring warps
 //     is an 8-byte {value, row} word that the reader polls (it is there by the time it is needed);
 //   * F(i,j) = max_{j'<j} (H~(i,j') - O - X (j - j')), H~ = max(M, E): a sequential max-plus chain over the thread's own
