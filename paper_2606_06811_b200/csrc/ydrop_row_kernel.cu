@@ -73,6 +73,10 @@ static __device__ __forceinline__ int2 lds64(uint32_t a) { int2 v; asm volatile(
 static __device__ __forceinline__ int4 lds128(uint32_t a) { int4 v; asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a)); return v; }
 static __device__ __forceinline__ unsigned long long lds_u64v(uint32_t a) { unsigned long long v; asm volatile("ld.volatile.shared.u64 %0, [%1];" : "=l"(v) : "r"(a) : "memory"); return v; }
 static __device__ __forceinline__ void sts32(uint32_t a, int v) { asm volatile("st.shared.s32 [%0], %1;" :: "r"(a), "r"(v) : "memory"); }
+static __device__ __forceinline__ void sts32_if(bool c, uint32_t a, int v)
+{
+    asm volatile("{ .reg .pred p; setp.ne.u32 p, %0, 0; @p st.shared.s32 [%1], %2; }" :: "r"((unsigned)c), "r"(a), "r"(v) : "memory");
+}
 static __device__ __forceinline__ void sts_u64v(uint32_t a, unsigned long long v) { asm volatile("st.volatile.shared.u64 [%0], %1;" :: "r"(a), "l"(v) : "memory"); }
 
 // maximum over the RK_NW per-warp entries of one ring row: broadcast 128-bit loads, no reduction instruction
@@ -201,7 +205,7 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
     if (tid == 0) { sh.fail_row = -1; sh.wide_row = -1; sh.new_chunk = -1; }
     __syncthreads();
 
-    int ws = 0, ws_prev = 0;                              // window start of this / the previous row (multiples of RK_WCOLS)
+    int ws = 0;                                           // window start (a multiple of RK_WCOLS); moves only at a fold
     int myc0 = -1;                                        // first of my RK_C columns
     int Hu[RK_C], Eu[RK_C];                               // previous row of my columns: gated H - OX, E
     uint32_t sel[RK_C];
@@ -249,59 +253,128 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
 #ifdef RK_PROFILE
     long long prof_t[8] = {0, 0, 0, 0, 0, 0, 0, 0}, prof_last = clock64();
 #endif
-    int i = 0;
-    for (; i <= g.n; i++) {
-        RK_T(7);
-        // ---- early loads: everything the row needs from shared memory is requested before it is used ----
-        const int lw = (warp - 1) & (RK_NW - 1);
-        unsigned long long ev = lds_u64v(sb + RK_OFF(edge) + 8 * lw);             // the left warp's edge {row, value} (broadcast)
-        const int rm = i >= 32 ? row_max4(sb + RK_OFF(rmax) + 4 * RK_NW * ((i - 32) & 63)) : 0;   // R4: best of row i - 32
-        // ---- lagged housekeeping, every RK_FOLD rows: rows [i - 32, i - 16) ----
-        if ((i & (RK_FOLD - 1)) == 0 && i >= 2 * RK_FOLD) {
-            int nlo = last_lo, nhi = -1;
-            if (!fold(i - RK_FOLD, nlo, nhi)) break;
-            last_lo = nlo;
-            const int nws = nlo & ~(RK_WCOLS - 1);                // the first alive column never moves left: a stale one is safe
-            // the last alive column grows by at most one per row: rows up to the next fold stay below nhi + 2 RK_FOLD + 1
-            if (nhi + 2 * RK_FOLD + 2 >= nws + RK_WIN) { wide = true; break; }
-            ws_prev = ws; ws = nws;
-        } else ws_prev = ws;
-        if ((i & 31) == 0) {
-            const int r = i + lane;
-            srow32 = (r == 0 || r > g.n) ? 0u : p.srow[sfe_base(g.qc, g.qm, g.q0 + (long long)g.d * r)];
-        }
-        const uint32_t srow_lo = __shfl_sync(FULL, srow32, i & 31);
-        int Hd0 = __shfl_up_sync(FULL, Hu[RK_C - 1], 1);
-        cumbest = max(cumbest, rm);
-        if (cumbest >= SFE_SCORE_LIMIT) { limit = true; break; }                  // R25
-        const int T = p.ydrop_inf ? SFE_T_INF : cumbest - p.Y;                    // T(i) = best(rows <= i - 32) - ydrop
-        RK_T(0);
-        // ---- my columns in this row's window ----
-        const int wsb = ws / RK_WCOLS;
-        const int rho = (warp - wsb) & (RK_NW - 1);               // my warp's rank in the window
-        const int c0 = ws + rho * RK_WCOLS + lane * RK_C;         // my first column
-        if (c0 != myc0) {
+    // Everything that depends only on the window position is computed when the window moves (at a fold), not per row: the
+    // warp's rank, the thread's columns, the constants of the carry exchange.  A thread's columns are fixed modulo RK_WIN.
+    int rho = warp, c0 = tid * RK_C;                      // my warp's rank in the window; my first column
+    int k1 = 0, carry_add = 0;                            // Dw (rho - 1) + D lane;  Dw rho - 31 D
+    bool oob = false, need_edge = false;
+    const int lw = (warp - 1) & (RK_NW - 1);
+    auto set_window = [&](const int nws, const int ows) {
+        rho = (warp - nws / RK_WCOLS) & (RK_NW - 1);
+        c0 = nws + rho * RK_WCOLS + lane * RK_C;
+        if (c0 != myc0) {                                 // (the warp's columns change together)
             myc0 = c0;
 #pragma unroll
             for (int k = 0; k < RK_C; k++) { Hu[k] = SFE_NEG; Eu[k] = SFE_NEG; sel[k] = col_selector(g, c0 + k); }
-            Hd0 = __shfl_up_sync(FULL, Hu[RK_C - 1], 1);          // (the warp's columns change together)
         }
-        // ---- traceback chunk of rows i .. i + 127 (popped by warp 0 before the barrier, read by everybody after it) ----
-        const bool new_chunk_row = TB && tb_ok && (i % RK_CHUNK_ROWS) == 0;
-        if (new_chunk_row && warp == 0) {
+        oob = c0 + RK_C - 1 > g.m;                        // (only the threads at the target's end)
+        k1 = Dw * (rho - 1) + D * lane;
+        carry_add = Dw * rho - D * 31;
+        // the diagonal of the warp's first column comes from the left warp iff that column was inside the previous window
+        need_edge = rho != 0 && nws + rho * RK_WCOLS - 1 - ows < RK_WIN;
+    };
+    set_window(0, 0);
+    need_edge = false;                                    // row 0 has no row above it
+    int Tvec = p.ydrop_inf ? SFE_T_INF : -p.Y;            // lane k: T of row (i & ~15) + k
+    unsigned char *rec_ptr = nullptr;                     // my RK_C-cell unit (RK_C / 2 bytes) of the current row's traceback record
+    int pend_chunk = -1;                                  // warp 0: the chunk popped ahead for the next 128 rows, not adopted yet
+    int tb_rows = 0;                                      // rows with a traceback record
+    uint32_t am_p = 0; int hmax_p = SFE_NEG, c0_p = 0;    // the previous row's alive mask / maximum / first column: published one row late
+
+    // The statistics of a row are published while the NEXT row's scan is in flight (branch-free, so the scheduler can put
+    // them into the shuffles' latency); the fold reads rows >= 16 barriers old, so one row of delay costs nothing.
+    auto publish_prev = [&](const int row) {
+        // lowest / highest set bit of the RK_C-bit mask from two packed tables (plain ALU; FLO sits on the slow pipe)
+        static_assert(RK_C <= 4, "the packed bit-position tables cover 4-bit masks");
+        const int lo_v = am_p ? c0_p + (int)((0x12131210u >> (2 * am_p)) & 3u) : 0x7fffffff;     // 2 bits per mask value 0 .. 15
+        const int hi_v = am_p ? c0_p + (int)((0xffffaa50u >> (2 * am_p)) & 3u) : -1;
+        const int wlo = __reduce_min_sync(FULL, lo_v), whi = __reduce_max_sync(FULL, hi_v), wm = __reduce_max_sync(FULL, hmax_p);
+        const uint32_t so = sb + 4 * (RK_NW * (row & 63) + warp);
+        const int v = lane == 0 ? wlo : lane == 1 ? whi : wm;
+        const uint32_t off = lane == 0 ? RK_OFF(rlo) : lane == 1 ? RK_OFF(rhi) : RK_OFF(rmax);
+        sts32_if(lane < 3, so + off, v);
+    };
+
+    if (TB) {                                             // the chunk of rows 0 .. 127
+        if (warp == 0) {
             const int nc = chunk_pop(p.free_ring, p.ring_state, p.n_chunks, lane);
             if (lane == 0) {
                 sh.new_chunk = nc;
-                if (nc >= 0) p.chunk_prev[nc] = cur_chunk;
+                if (nc >= 0) p.chunk_prev[nc] = -1;
                 if (nc == -2) atomicAdd(&p.counters[CNT_RING_DROPS], 1ULL);
             }
         }
-        // ---- diagonal of the warp's first column: the left warp's previous-row value (uniform test, no divergence) ----
-        if (i > 0 && rho != 0 && ws + rho * RK_WCOLS - 1 - ws_prev < RK_WIN) {    // that column was inside the previous row's window
+        __syncthreads();
+        const int nc = lds32(sb + RK_OFF(new_chunk));
+        if (nc < 0) tb_ok = false;
+        else { cur_chunk = nc; rec_ptr = (unsigned char *)(p.pool + (size_t)nc * (SFE_CHUNK_BYTES / 4)) + tid * (RK_C / 2); }
+        __syncthreads();
+    }
+
+    int i = 0;
+    for (; i <= g.n; i++) {
+        RK_T(7);
+        // ---- early load: the left warp's edge {row, value} (broadcast), used after the housekeeping ----
+        unsigned long long ev = lds_u64v(sb + RK_OFF(edge) + 8 * lw);
+        // ---- everything periodic sits behind ONE test per row (a branch costs ~15-20 cycles here, taken or not) ----
+        if ((i & (RK_FOLD - 1)) == 0) {
+            if (i >= 2 * RK_FOLD) {
+                // thresholds of rows i .. i + 15 (R4): T(r) = best(rows <= r - 32) - ydrop; rows i - 32 .. i - 17 were
+                // published >= 16 barriers ago.  Lane k < 16 ends with the running best through row i - 32 + k.
+                int v = lane < RK_FOLD ? row_max4(sb + RK_OFF(rmax) + 4 * RK_NW * ((i - 32 + lane) & 63)) : SFE_NEG;
+#pragma unroll
+                for (int o = 1; o < RK_FOLD; o <<= 1) v = max(v, __shfl_up_sync(FULL, v, o));
+                v = max(v, cumbest);
+                cumbest = __shfl_sync(FULL, v, RK_FOLD - 1);
+                if (cumbest >= SFE_SCORE_LIMIT) { limit = true; break; }              // R25
+                Tvec = p.ydrop_inf ? SFE_T_INF : v - p.Y;
+                // statistics of rows [i - 32, i - 16): cells, termination, the window
+                int nlo = last_lo, nhi = -1;
+                if (!fold(i - RK_FOLD, nlo, nhi)) break;
+                last_lo = nlo;
+                const int nws = nlo & ~(RK_WCOLS - 1);            // the first alive column never moves left: a stale one is safe
+                // the last alive column grows by at most one per row: rows up to the next fold stay below nhi + 2 RK_FOLD + 1
+                if (nhi + 2 * RK_FOLD + 2 >= nws + RK_WIN) { wide = true; break; }
+                if (nws != ws) { set_window(nws, ws); ws = nws; }
+            }
+            if ((i & 31) == 0) {
+                const int r = i + lane;
+                srow32 = (r == 0 || r > g.n) ? 0u : p.srow[sfe_base(g.qc, g.qm, g.q0 + (long long)g.d * r)];
+            }
+            if (TB && tb_ok) {
+                // the traceback chunk of the next 128 rows is popped by warp 0 one fold ahead and adopted by everybody at the
+                // chunk's first row: 16 barriers lie between the two, and no row pays for a test of its own
+                const int ph = i & (RK_CHUNK_ROWS - 1);
+                if (ph == RK_CHUNK_ROWS - RK_FOLD && warp == 0) {
+                    const int nc = chunk_pop(p.free_ring, p.ring_state, p.n_chunks, lane);
+                    pend_chunk = nc;
+                    if (lane == 0) {
+                        sh.new_chunk = nc;
+                        if (nc >= 0) p.chunk_prev[nc] = cur_chunk;
+                        if (nc == -2) atomicAdd(&p.counters[CNT_RING_DROPS], 1ULL);
+                    }
+                }
+                if (ph == 0 && i > 0) {
+                    const int nc = lds32(sb + RK_OFF(new_chunk));
+                    pend_chunk = -1;
+                    if (nc < 0) tb_ok = false;
+                    else { cur_chunk = nc; rec_ptr = (unsigned char *)(p.pool + (size_t)nc * (SFE_CHUNK_BYTES / 4)) + tid * (RK_C / 2); }
+                }
+            }
+        }
+        const uint32_t srow_lo = __shfl_sync(FULL, srow32, i & 31);
+        const int T = __shfl_sync(FULL, Tvec, i & (RK_FOLD - 1));
+        int Hd0 = __shfl_up_sync(FULL, Hu[RK_C - 1], 1);
+        publish_prev(i - 1);                                       // (independent of this row: its reductions run under the loads above)
+        RK_T(0);
+        // ---- diagonal of the warp's first column: the left warp's previous-row value.  The edge is normally there already;
+        // the (uniform) slow path polls for it ----
+        if (need_edge && (int)(ev >> 32) != i - 1) {
             for (int spin = 0; (int)(ev >> 32) != i - 1 && spin < RK_POLL_LIMIT; spin++) ev = lds_u64v(sb + RK_OFF(edge) + 8 * lw);
             if ((int)(ev >> 32) != i - 1) sts32(sb + RK_OFF(fail_row), i);        // (readers act on it from this row's barrier on)
-            if (lane == 0) Hd0 = (int)(unsigned)ev;
-        } else if (lane == 0) Hd0 = SFE_NEG;
+        }
+        if (lane == 0) Hd0 = need_edge ? (int)(unsigned)ev : SFE_NEG;
+        need_edge = rho != 0;                                     // (rows after the first one of a window)
         if (i == 0 && c0 == 0) Hd0 = -OX;                         // the origin (R8)
         RK_T(1);
         // ---- phase A: M, E, H~ and the in-thread F chain ----
@@ -322,7 +395,7 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
         int y = gk + D * lane;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) y = max(y, __shfl_up_sync(FULL, y, o));      // out-of-range lanes get their own value back
-        if (lane == 31) sts32(sb + RK_OFF(carry) + 4 * (RK_NW * (i & 1) + rho), y - D * 31 + Dw * rho);   // F leaving the warp, pre-shifted by its rank
+        sts32_if(lane == 31, sb + RK_OFF(carry) + 4 * (RK_NW * (i & 1) + rho), y + carry_add);   // F leaving the warp, pre-shifted by its rank
         int yex = __shfl_up_sync(FULL, y, 1);
         if (lane == 0) yex = RK_NINF;
         const int fin_warp = yex - D * lane + D;                   // F entering my first column from my warp's lanes left of me
@@ -343,23 +416,20 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
                 if (w4 + 3 < rho) cm = max(cm, x.w);
             }
         }
-        // both flags carry the row they were raised in: a fast warp's later write is ignored by a slow reader, so every
-        // thread leaves the loop in the same row (a non-uniform exit would hang the next barrier)
-        if (fl.x >= 0 && fl.x <= i) break;
-        if (fl.y >= 0 && fl.y < i) { wide = true; break; }
-        // F entering my warp from the warps left of it: max_{r < rho} carry_r - Dw (rho - 1 - r); then down my warp's lanes
-        const int Fin = max(fin_warp, cm - Dw * (rho - 1) - D * lane);
-        if (new_chunk_row) {
-            const int nc = lds32(sb + RK_OFF(new_chunk));
-            if (nc < 0) tb_ok = false; else cur_chunk = nc;
+        // both flags carry the row they were raised in (-1: not raised): a fast warp's later write is ignored by a slow
+        // reader, so every thread leaves the loop in the same row (a non-uniform exit would hang the next barrier)
+        if ((unsigned)fl.x <= (unsigned)i || (unsigned)fl.y < (unsigned)i) {
+            if (!((unsigned)fl.x <= (unsigned)i)) wide = true;
+            break;
         }
+        // F entering my warp from the warps left of it: max_{r < rho} carry_r - Dw (rho - 1 - r); then down my warp's lanes
+        const int Fin = max(fin_warp, cm - k1);
         RK_T(5);
         // ---- phase C: F, H, alive, next row's state, statistics, pointers ----
         uint32_t nibs = 0, am = 0;
         int hmax = SFE_NEG;
         const int best_before = best;
         int Hc[RK_C];
-        const bool oob = c0 + RK_C - 1 > g.m;                     // (only the threads at the target's end)
 #pragma unroll
         for (int k = 0; k < RK_C; k++) {
             const int F = max(gl[k], Fin - X * k);
@@ -381,7 +451,7 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
         RK_T(6);
         // ---- publish the edge for the next row first: the right warp is waiting for it ----
         if (lane == 31) sts_u64v(sb + RK_OFF(edge) + 8 * warp, ((unsigned long long)(unsigned)i << 32) | (unsigned)Hu[RK_C - 1]);
-        if (rho == RK_NW - 1 && lane == 31 && (am >> (RK_C - 1))) sts32(sb + RK_OFF(wide_row), i);        // alive in the window's last column: bail out next row
+        sts32_if(rho == RK_NW - 1 && lane == 31 && (am >> (RK_C - 1)), sb + RK_OFF(wide_row), i);   // alive in the window's last column: bail out next row
         best = max(best, hmax);
         if (best > best_before) {                                  // strict: the first maximum of my cells (R7)
             int kk = RK_C - 1;
@@ -389,25 +459,19 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
             for (int k = RK_C - 2; k >= 0; k--) kk = Hc[k] == best ? k : kk;
             best_i = i; best_j = c0 + kk;
         }
-        // ---- lagged statistics: the lanes holding the warp's first / last alive cell write them; one reduction for the maximum ----
-        {
-            const unsigned bal = __ballot_sync(FULL, am != 0);
-            const int wm = __reduce_max_sync(FULL, hmax);
-            const int fl_lane = bal ? __ffs(bal) - 1 : 0, ll_lane = bal ? 31 - __clz(bal) : 0;
-            const uint32_t so = 4 * (RK_NW * (i & 63) + warp);
-            if (lane == fl_lane) sts32(sb + RK_OFF(rlo) + so, bal ? c0 + __ffs(am) - 1 : 0x7fffffff);
-            if (lane == ll_lane) sts32(sb + RK_OFF(rhi) + so, bal ? c0 + 31 - __clz(am) : -1);
-            if (lane == 0) sts32(sb + RK_OFF(rmax) + so, wm);
-        }
-        if (TB && tb_ok) {
-            uint32_t *rec = p.pool + (size_t)cur_chunk * (SFE_CHUNK_BYTES / 4) + (size_t)(i % RK_CHUNK_ROWS) * RK_ROW_WORDS;
-            const int unit = ((c0 & (RK_WIN - 1)) / RK_C);        // my 4 RK_C-bit unit of the row record
-            if (RK_C == 8) rec[unit] = nibs;
-            else if (RK_C == 4) ((uint16_t *)rec)[unit] = (uint16_t)nibs;
-            else ((uint8_t *)rec)[unit] = (uint8_t)nibs;
-            if (tid == 0) n_words += RK_ROW_WORDS;
+        am_p = am; hmax_p = hmax; c0_p = c0;
+        if (TB) {
+            if (tb_ok) {
+                if (RK_C == 8) *(uint32_t *)rec_ptr = nibs;
+                else if (RK_C == 4) *(uint16_t *)rec_ptr = (uint16_t)nibs;
+                else *rec_ptr = (unsigned char)nibs;
+            }
+            rec_ptr += 4 * RK_ROW_WORDS;
+            tb_rows += tb_ok ? 1 : 0;
         }
     }
+    publish_prev(i - 1);                                           // the last computed row (again, if the loop left after its barrier)
+    n_words = (long long)tb_rows * RK_ROW_WORDS;
 #ifdef RK_PROFILE
     if (lane == 0 && i > 100000) printf("RKPROF warp %d rows %d: top %.1f cols/poll %.1f phaseA %.1f scan %.1f barrier %.1f postbar %.1f phaseC %.1f publish %.1f\n", warp, i, (double)prof_t[0] / i, (double)prof_t[1] / i, (double)prof_t[2] / i, (double)prof_t[3] / i, (double)prof_t[4] / i, (double)prof_t[5] / i, (double)prof_t[6] / i, (double)prof_t[7] / i);
 #endif
@@ -433,7 +497,6 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
         const int os = sh.red_s[w], oi = sh.red_i[w], oj = sh.red_j[w];
         if (os > bs || (os == bs && (oi < bi || (oi == bi && oj < bj)))) { bs = os; bi = oi; bj = oj; }
     }
-    n_words = __shfl_sync(FULL, n_words, 0);
     out.score = bs; out.end_i = bi; out.end_j = bj; out.cells = cells;
     out.status = (wide ? SFE_ST_WIDE_PENDING : 0u) | ((TB && !tb_ok) ? SFE_ST_PASS_OVERFLOW : 0u) | SFE_ST_BLOCK |
                  (limit ? SFE_ST_SCORE_LIMIT : 0u) | (failed ? SFE_ST_INTERNAL : 0u);
@@ -454,7 +517,7 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
         if (TB) {
             __threadfence();
             __syncwarp();
-            int cc = cur_chunk;
+            int cc = pend_chunk >= 0 ? pend_chunk : cur_chunk;          // (a chunk popped ahead is linked in front of the current one)
             while (cc >= 0) { const int prev = __ldcg(p.chunk_prev + cc); chunk_push(p.free_ring, p.ring_state, p.n_chunks, cc, &p.counters[CNT_RING_DROPS], lane); cc = prev; }
         }
         unsigned smid, wslot;
