@@ -257,7 +257,8 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
     // warp's rank, the thread's columns, the constants of the carry exchange.  A thread's columns are fixed modulo RK_WIN.
     int rho = warp, c0 = tid * RK_C;                      // my warp's rank in the window; my first column
     int k1 = 0, carry_add = 0;                            // Dw (rho - 1) + D lane;  Dw rho - 31 D
-    bool oob = false, need_edge = false;
+    bool need_edge = false;
+    int hcap[RK_C];
     const int lw = (warp - 1) & (RK_NW - 1);
     auto set_window = [&](const int nws, const int ows) {
         rho = (warp - nws / RK_WCOLS) & (RK_NW - 1);
@@ -267,7 +268,8 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
 #pragma unroll
             for (int k = 0; k < RK_C; k++) { Hu[k] = SFE_NEG; Eu[k] = SFE_NEG; sel[k] = col_selector(g, c0 + k); }
         }
-        oob = c0 + RK_C - 1 > g.m;                        // (only the threads at the target's end)
+#pragma unroll
+        for (int k = 0; k < RK_C; k++) hcap[k] = c0 + k > g.m ? SFE_NEG : 0x7fffffff;    // (only the threads at the target's end)
         k1 = Dw * (rho - 1) + D * lane;
         carry_add = Dw * rho - D * 31;
         // the diagonal of the warp's first column comes from the left warp iff that column was inside the previous window
@@ -392,30 +394,25 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
         for (int k = 0; k < RK_C; k++) { gl[k] = gk; gk = __viaddmax_s32(gk, -X, Ht[k] - OX); }
         RK_T(2);
         // ---- F across the threads of the warp: y = x + D lane, prefix maximum, exclusive ----
+        // Three doubling steps give y3[l] = max over lanes l-7 .. l; the exclusive prefix over all lanes left of l is then the
+        // maximum of y3 at l-1, l-9, l-17, l-25: four INDEPENDENT shuffles (one latency) instead of three more dependent ones.
         int y = gk + D * lane;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) y = max(y, __shfl_up_sync(FULL, y, o));      // out-of-range lanes get their own value back
-        sts32_if(lane == 31, sb + RK_OFF(carry) + 4 * (RK_NW * (i & 1) + rho), y + carry_add);   // F leaving the warp, pre-shifted by its rank
-        int yex = __shfl_up_sync(FULL, y, 1);
-        if (lane == 0) yex = RK_NINF;
+        for (int o = 1; o < 8; o <<= 1) y = max(y, __shfl_up_sync(FULL, y, o));       // out-of-range lanes get their own value back
+        int e0 = __shfl_up_sync(FULL, y, 1), e1 = __shfl_up_sync(FULL, y, 9), e2 = __shfl_up_sync(FULL, y, 17), e3 = __shfl_up_sync(FULL, y, 25);
+        e0 = lane >= 1 ? e0 : RK_NINF; e1 = lane >= 9 ? e1 : RK_NINF; e2 = lane >= 17 ? e2 : RK_NINF; e3 = lane >= 25 ? e3 : RK_NINF;
+        const int yex = max(max(e0, e1), max(e2, e3));
+        // F leaving the warp (inclusive at lane 31), pre-shifted by the warp's rank
+        sts32_if(lane == 31, sb + RK_OFF(carry) + 4 * (RK_NW * (i & 1) + rho), max(yex, y) + carry_add);
         const int fin_warp = yex - D * lane + D;                   // F entering my first column from my warp's lanes left of me
         RK_T(3);
         __syncthreads();                                                                   // the one barrier of the row
         RK_T(4);
         // ---- after the barrier: flags and the other warps' carries, requested together ----
         const int2 fl = lds64(sb + RK_OFF(fail_row));
-        int cm = RK_NINF;
-        {
-            const uint32_t cp = sb + RK_OFF(carry) + 4 * RK_NW * (i & 1);
-#pragma unroll
-            for (int w4 = 0; w4 < RK_NW; w4 += 4) {
-                const int4 x = lds128(cp + 4 * w4);
-                if (w4 + 0 < rho) cm = max(cm, x.x);
-                if (w4 + 1 < rho) cm = max(cm, x.y);
-                if (w4 + 2 < rho) cm = max(cm, x.z);
-                if (w4 + 3 < rho) cm = max(cm, x.w);
-            }
-        }
+        // the carries of the warps left of mine: lane r < rho loads carry[r], one warp reduction (uniform result)
+        const int cv = lane < rho ? lds32(sb + RK_OFF(carry) + 4 * (RK_NW * (i & 1) + (lane & (RK_NW - 1)))) : RK_NINF;
+        const int cm = __reduce_max_sync(FULL, cv);
         // both flags carry the row they were raised in (-1: not raised): a fast warp's later write is ignored by a slow
         // reader, so every thread leaves the loop in the same row (a non-uniform exit would hang the next barrier)
         if ((unsigned)fl.x <= (unsigned)i || (unsigned)fl.y < (unsigned)i) {
@@ -434,7 +431,7 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
         for (int k = 0; k < RK_C; k++) {
             const int F = max(gl[k], Fin - X * k);
             int H = max(Ht[k], F);
-            if (oob && c0 + k > g.m) H = SFE_NEG;
+            H = min(H, hcap[k]);                                   // columns beyond the target (set with the window)
             const bool alive = H >= T;                             // R5
             if (TB) {
                 nibs = __funnelshift_l((uint32_t)(M[k] - H), nibs, 1);           // H not from M
