@@ -166,6 +166,27 @@ int sfe_resolve(sfe_ctx *ctx, const sfe_anchor *anchors_dev, const sfe_result *r
                 int32_t min_score, sfe_box *accepted_dev, int64_t accepted_cap, int64_t *n_accepted_dev,
                 uint8_t *keep_dev, sfe_stats *stats_dev);
 
+/* sfe_resolve without a context and without any allocation (Alg. 3 phase 3; same rule, same kernels,
+ * same outputs as sfe_resolve, byte for byte) -- for callers that cannot call cudaMalloc: code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it.  sfe_create allocates, so this entry point takes the device ordinal and
+ * the stream (NULL = default stream) instead of an sfe_ctx; it calls no cudaMalloc / cudaFree / allocating routine.
+ * Its scratch (block minima of tpos, the active-box list) is a file-scope __device__ array inside libsfe.so:
+ * 2.75 MiB that every GPU which loads the library holds until the process exits.
+ * Limits: n <= SFE_STATIC_MAX_ANCHORS and accepted_cap <= SFE_STATIC_MAX_ACCEPTED, else SFE_ELIMIT (nothing launched,
+ * sfe_last_error_detail says which); larger inputs go through sfe_resolve, or through consecutive calls on slices
+ * of the anchors that carry accepted_dev / n_accepted_dev (R26).  Arguments, layouts, ownership and the meaning of
+ * results_dev == NULL are sfe_resolve's; all pointers are device pointers on `device`.  Asynchronous on the stream.
+ * Every call on a device shares the one scratch array.  No part of it needs to start at zero (each call overwrites
+ * what it reads), so a previous call's leftovers are harmless; but calls that OVERLAP on the GPU -- different streams,
+ * host threads or concurrently replayed graphs -- race on it and must be serialised by the caller.
+ * sfe_resolve_static_limits reports the two limits and the array's size in bytes (any pointer may be NULL). */
+#define SFE_STATIC_MAX_ANCHORS  (1 << 20)
+#define SFE_STATIC_MAX_ACCEPTED (1 << 16)
+int sfe_resolve_static(int device, void *cuda_stream, const sfe_anchor *anchors_dev, const sfe_result *results_dev,
+                       int64_t n, int32_t min_score, sfe_box *accepted_dev, int64_t accepted_cap,
+                       int64_t *n_accepted_dev, uint8_t *keep_dev, sfe_stats *stats_dev);
+int sfe_resolve_static_limits(int64_t *max_anchors, int64_t *max_accepted, int64_t *scratch_bytes);
+
 /* Algorithm 3 end to end on device buffers.  Repeats until every anchor is decided:
  *   phase 1  scan forward from the cursor: anchors covered by an accepted box are final (keep 0, result
  *            zeroed with SFE_ST_SKIPPED, never extended); the next window_k uncovered anchors form the window;

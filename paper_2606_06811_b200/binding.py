@@ -28,7 +28,7 @@ ST_SKEW2, ST_SKEW_RETRY, ST_BLOCK = 0x1000, 0x2000, 0x800      # profile-only bi
 
 EXPORTS = ("sfe_create", "sfe_destroy", "sfe_strerror", "sfe_last_error_detail", "sfe_pack", "sfe_ydrop_batch", "sfe_resolve",
            "sfe_speculate", "sfe_extend_host", "sfe_speculate_host", "sfe_probe_int_issue", "sfe_last_batch_info", "sfe_last_half_profile",
-           "sfe_launch_counter", "sfe_set_option", "sfe_last_speculate_info")
+           "sfe_launch_counter", "sfe_set_option", "sfe_last_speculate_info", "sfe_resolve_static", "sfe_resolve_static_limits")
 
 
 class Scoring(C.Structure):
@@ -94,6 +94,8 @@ def lib():
         _lib.sfe_last_batch_info.argtypes = [vp, C.POINTER(i64)]
         _lib.sfe_set_option.argtypes = [vp, C.c_int, i64]
         _lib.sfe_last_speculate_info.argtypes = [vp, C.POINTER(i64)]
+        _lib.sfe_resolve_static.argtypes = [C.c_int, vp, vp, vp, i64, i32, vp, i64, vp, vp, vp]
+        _lib.sfe_resolve_static_limits.argtypes = [C.POINTER(i64), C.POINTER(i64), C.POINTER(i64)]
     return _lib
 
 
@@ -289,6 +291,22 @@ class Sfe:
         _check(lib().sfe_last_batch_info(self.h, a), "sfe_last_batch_info")
         keys = ("launches", "halves", "halves_rerun", "tb_bytes", "steps", "wide", "ydrop_kernel_us", "block_halves", "ring_drops")
         return dict(zip(keys, list(a)))
+
+
+def resolve_static(device: int, stream, anchors_dev, results_dev, n, min_score, accepted_dev, accepted_cap, n_accepted_dev,
+                   keep_dev, stats_dev=None):
+    """sfe_resolve_static: the resolve rule with no context and no allocation (the scratch is a static device array in
+    libsfe.so).  `stream` is a raw cudaStream_t value (0 / None = default stream); keep_dev is the caller's."""
+    _check(lib().sfe_resolve_static(device, C.c_void_p(stream or 0), _ptr(anchors_dev), _ptr(results_dev), n, min_score,
+                                    _ptr(accepted_dev), accepted_cap, _ptr(n_accepted_dev), _ptr(keep_dev), _ptr(stats_dev)),
+           "sfe_resolve_static")
+
+
+def resolve_static_limits():
+    """(max anchors per call, max accepted_cap, bytes of the static scratch array)"""
+    a, b, c = C.c_int64(0), C.c_int64(0), C.c_int64(0)
+    _check(lib().sfe_resolve_static_limits(C.byref(a), C.byref(b), C.byref(c)), "sfe_resolve_static_limits")
+    return int(a.value), int(b.value), int(c.value)
 
 
 def launch_counter() -> int:

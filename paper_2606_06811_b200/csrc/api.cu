@@ -98,6 +98,7 @@ void sfe_note_cuda_error(cudaError_t e, const char *file, int line)
     snprintf(g_err_detail, sizeof g_err_detail, "%s:%d: %s", file, line, cudaGetErrorString(e));
     cudaGetLastError();
 }
+void sfe_note_error_text(const char *msg) { snprintf(g_err_detail, sizeof g_err_detail, "%s", msg); }
 extern "C" const char *sfe_last_error_detail(void) { return g_err_detail; }
 
 static void harvest_kernel_time(sfe_ctx *c);

@@ -136,5 +136,6 @@ extern thread_local long long sfe_tls_launches;
 
 // last CUDA failure of the calling host thread (file:line + runtime message), readable through sfe_last_error_detail()
 void sfe_note_cuda_error(cudaError_t e, const char *file, int line);
+void sfe_note_error_text(const char *msg);                 // the text sfe_last_error_detail returns (calling host thread)
 #define SFE_CUDA_CHECK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { sfe_note_cuda_error(e_, __FILE__, __LINE__); return SFE_ECUDA; } } while (0)
 #define SFE_LAUNCH_CHECK() do { cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) { sfe_note_cuda_error(e_, __FILE__, __LINE__); return SFE_ECUDA; } return SFE_OK; } while (0)
