@@ -227,6 +227,12 @@ enum {
     SFE_OPT_ROW_KERNEL_CAP,        /* [0]     most priority tickets (long-likely leaders, known long extensions) a pass hands to the
                                               cooperative row kernel, one CTA per half; 0 = never use it beside the systolic kernel  */
     SFE_OPT_ROW_KERNEL_SCORE_ONLY, /* [0]     1 = also in score-only passes (there the systolic chain is currently the faster one)   */
+    SFE_OPT_LONG_ROWS,             /* [16384] sfe_speculate's leader batches: a half of the systolic kernel still alive after this many rows
+                                              (then twice, four times ... as many) stops if a CTA of the cooperative row kernel is idle
+                                              and is re-run by it from its start -- its rows are a third shorter and it has its SM to
+                                              itself.  0 = off; rounded up to 32 times a power of two                               */
+    SFE_OPT_LONG_ROWS_DENSE,       /* [0]     the same for sfe_ydrop_batch's dense launch; 0 = off                                   */
+    SFE_OPT_ROW_SLOTS,             /* [64]    CTAs of the row kernel that serve those hand-offs (at most half of the SMs)            */
     SFE_OPT_N
 };
 int sfe_set_option(sfe_ctx *ctx, int key, int64_t value);

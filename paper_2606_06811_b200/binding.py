@@ -20,7 +20,7 @@ YDROP_INF = 0x7FFFFFFF
 PRUNE_LAG = 32
 WANT_CIGAR, SCORE_ONLY, NO_BINNING, BLOCK_KERNEL, NO_BLOCK_KERNEL, CIGAR_KEPT_ONLY, SPEC_LEADERS = 1, 0, 2, 4, 8, 16, 32
 (OPT_LEADER_DIAG_TOL, OPT_LEADER_GAP, OPT_LEADER_LOOKBACK, OPT_LEADER_NBREAK, OPT_SPEC_SPAN, OPT_SPEC_ESC_MAX, OPT_SPARSE_WARPS,
- OPT_FORCE_CLASS, OPT_PROMOTE_REACH, OPT_ROW_KERNEL_CAP, OPT_ROW_KERNEL_SCORE_ONLY) = range(11)
+ OPT_FORCE_CLASS, OPT_PROMOTE_REACH, OPT_ROW_KERNEL_CAP, OPT_ROW_KERNEL_SCORE_ONLY, OPT_LONG_ROWS, OPT_LONG_ROWS_DENSE, OPT_ROW_SLOTS) = range(14)
 ST_TB_OVERFLOW, ST_CIGAR_OVERFLOW, ST_WIDE, ST_SCORE_LIMIT, ST_BAD_ANCHOR, ST_BAND_LIMIT, ST_INTERNAL, ST_SKIPPED = 1, 2, 4, 8, 16, 32, 64, 128
 OP_M, OP_I, OP_D = 0, 1, 2
 INFO_N = 12

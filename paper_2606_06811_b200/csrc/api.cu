@@ -75,7 +75,7 @@ struct sfe_ctx {
     uint32_t *pool; int32_t *chunk_prev; int32_t *free_ring; SfeFreeRing *ring_state; int n_chunks;
     unsigned long long *counters;     // device, CNT_N
     unsigned long long *counters_host;  // pinned
-    DevBuf halves, tickets, sel, hist, blkmin, act, misc, wide_tickets, wide_ring, ops_stage;
+    DevBuf halves, tickets, sel, hist, blkmin, act, misc, wide_tickets, long_tickets, wide_ring, ops_stage;
     DevBuf sp_state, sp_idx, sp_anchors, sp_results, sp_local, sp_blkmin, sp_act, sp_kanchors, sp_kidx, sp_kres;   // sfe_speculate
     DevBuf sp_cls, sp_ext, sp_prio, sp_plist, sp_lprio;   // predicted leaders
     long long opt[SFE_OPT_N];         // sfe_set_option
@@ -135,7 +135,8 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
     memset(c->spec_info, 0, sizeof c->spec_info);
     c->opt[SFE_OPT_LEADER_DIAG_TOL] = 48; c->opt[SFE_OPT_LEADER_GAP] = 2000; c->opt[SFE_OPT_LEADER_LOOKBACK] = 64;
     c->opt[SFE_OPT_LEADER_NBREAK] = 64; c->opt[SFE_OPT_SPEC_SPAN] = 1 << 20; c->opt[SFE_OPT_SPEC_ESC_MAX] = 64;
-    c->opt[SFE_OPT_SPARSE_WARPS] = 4; c->opt[SFE_OPT_FORCE_CLASS] = 0; c->opt[SFE_OPT_PROMOTE_REACH] = 65536; c->opt[SFE_OPT_ROW_KERNEL_CAP] = 0; c->opt[SFE_OPT_ROW_KERNEL_SCORE_ONLY] = 0;
+    c->opt[SFE_OPT_SPARSE_WARPS] = 0; c->opt[SFE_OPT_FORCE_CLASS] = 0; c->opt[SFE_OPT_PROMOTE_REACH] = 65536; c->opt[SFE_OPT_ROW_KERNEL_CAP] = 0; c->opt[SFE_OPT_ROW_KERNEL_SCORE_ONLY] = 0;
+    c->opt[SFE_OPT_LONG_ROWS] = 0; c->opt[SFE_OPT_LONG_ROWS_DENSE] = 0; c->opt[SFE_OPT_ROW_SLOTS] = 64;
     c->ev_pending = false; c->kernel_us = 0.0; c->n_profile = 0;
     if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -171,7 +172,7 @@ extern "C" int sfe_destroy(sfe_ctx *c)
     if (c->state_host) cudaFreeHost(c->state_host);
     cudaEventDestroy(c->ev0); cudaEventDestroy(c->ev1); cudaEventDestroy(c->ev_fork); cudaEventDestroy(c->ev_join);
     if (c->aux) { cudaStreamSynchronize(c->aux); cudaStreamDestroy(c->aux); }
-    DevBuf *bufs[] = {&c->sp_cls, &c->sp_ext, &c->sp_prio, &c->sp_plist, &c->sp_lprio, &c->sp_kanchors, &c->sp_kidx, &c->sp_kres, &c->sp_state, &c->sp_idx, &c->sp_anchors, &c->sp_results, &c->sp_local, &c->sp_blkmin, &c->sp_act, &c->ops_stage, &c->wide_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
+    DevBuf *bufs[] = {&c->sp_cls, &c->sp_ext, &c->sp_prio, &c->sp_plist, &c->sp_lprio, &c->sp_kanchors, &c->sp_kidx, &c->sp_kres, &c->sp_state, &c->sp_idx, &c->sp_anchors, &c->sp_results, &c->sp_local, &c->sp_blkmin, &c->sp_act, &c->ops_stage, &c->wide_tickets, &c->long_tickets, &c->wide_ring, &c->halves, &c->tickets, &c->sel, &c->hist, &c->blkmin, &c->act, &c->misc, &c->h_tascii, &c->h_qascii,
                       &c->h_t2, &c->h_tm, &c->h_q2, &c->h_qm, &c->h_r2, &c->h_rm, &c->h_pairs, &c->h_anchors, &c->h_results,
                       &c->h_keep, &c->h_cigar, &c->h_acc, &c->h_small};
     for (DevBuf *b : bufs) b->release();
@@ -337,6 +338,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
     if ((rc = c->tickets.ensure((size_t)(2 * n_anchors) * sizeof(int32_t)))) return rc;
     if ((rc = c->hist.ensure(128 * sizeof(unsigned int)))) return rc;
     if ((rc = c->wide_tickets.ensure((size_t)(2 * n_anchors) * sizeof(int32_t)))) return rc;
+    if ((rc = c->long_tickets.ensure((size_t)(4 * n_anchors) * sizeof(int32_t)))) return rc;
     if ((rc = c->wide_ring.ensure((size_t)SFE_WIDE_WARPS * RingGeom<SFE_WIDE_RING_LOG2>::WARP_BYTES))) return rc;
     if (want_tb && (rc = c->sel.ensure((size_t)n_anchors * sizeof(long long)))) return rc;
     // ops arena: every staged op ends up in the caller's pool, plus two header words per segment
@@ -354,6 +356,16 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
     p.counters = c->counters; p.halves = (sfe_half *)c->halves.p; p.pool = c->pool; p.chunk_prev = c->chunk_prev; p.free_ring = c->free_ring; p.ring_state = c->ring_state;
     p.n_chunks = want_tb ? c->n_chunks : 0; p.n_pairs = n_pairs; p.max_warps = 0x7fffffff; p.sparse_warps = sparse_warps;
     p.wide_ring = (char *)c->wide_ring.p; p.wide_tickets = (int32_t *)c->wide_tickets.p;
+    {   // hand-off of long halves to the row kernel (Lambda = 32 only; not when the caller pinned the kernel choice or the
+        // priority tickets already go to the row kernel)
+        const long long lr = c->opt[first_of_series ? SFE_OPT_LONG_ROWS_DENSE : SFE_OPT_LONG_ROWS];      // (a batch of sfe_speculate is never the first of a series)
+        const bool on = lr > 0 && c->opt[SFE_OPT_ROW_SLOTS] > 0 && !(flags & (SFE_BLOCK_KERNEL | SFE_NO_BLOCK_KERNEL)) &&
+                        sc->prune_lag == SFE_PRUNE_LAG && c->opt[SFE_OPT_ROW_KERNEL_CAP] == 0;
+        p.long_strips = 0;
+        if (on) { long long st = 1; while (st * 32 < lr && st < (1 << 24)) st *= 2; p.long_strips = (int)st; }     // strips, a power of two
+        p.row_slots = (int)(c->opt[SFE_OPT_ROW_SLOTS] < 1024 ? c->opt[SFE_OPT_ROW_SLOTS] : 1024);
+        p.long_tickets = (int32_t *)c->long_tickets.p;
+    }
     p.ops_stage = (uint32_t *)c->ops_stage.p; p.ops_cap = ops_cap;
     p.OX = sc->gap_open + sc->gap_extend; p.X = sc->gap_extend;
     p.lag0 = sc->prune_lag == 0;

@@ -12,6 +12,7 @@
 #define SFE_ST_OPS_OVERFLOW 0x400u    // internal: the ops arena ran out; reported as SFE_ST_CIGAR_OVERFLOW
 #define SFE_ST_BLOCK 0x800u           // internal: computed by the row-synchronous block kernel
 #define SFE_ST_SKEW2 0x1000u          // internal (profile only): the half ran with the lane skew of 2 (reserved ticket)
+#define SFE_ST_LONG_PENDING 0x4000u  // internal: a systolic half reached long_strips strips and was handed to the row kernel (re-run there)
 #define SFE_ST_SKEW_RETRY 0x2000u     // internal (profile only): a skew-2 strip outgrew the window; re-run with skew 1
 // R25: scores stay below 2^29 (inactive-row threshold, SFE_T_INF, the out-of-bounds score and SFE_NEG arithmetic all rely on
 // it).  The running best is tested once per strip / per row; it can rise by at most 32 rows x 127 between two tests.
@@ -80,7 +81,12 @@ struct sfe_half {                 // result of one one-sided extension (a7)
 };
 
 enum { CNT_TICKET = 0, CNT_RING_DROPS, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT_WIDE, CNT_RERUN, CNT_WIDE_N, CNT_WIDE_TICKET, CNT_OPS, CNT_MAXNEED, CNT_CLASS0, CNT_CLASS1, CNT_CLASS2, CNT_CLASS3, CNT_BLOCK_HALVES,
-       CNT_ROW_N, CNT_ROW_TICKET, CNT_N = 24 };
+       CNT_ROW_N, CNT_ROW_TICKET,
+       CNT_LONG_N, CNT_LONG_TICKET,  // hand-off queue (long_tickets): entries pushed by the systolic kernel / positions drawn by idle row CTAs
+       CNT_ROW_FREE, CNT_SYS_DONE,   // row CTAs idle and not yet claimed (signed) / systolic warps that have left their kernel
+       CNT_LONG_LEFT,                // hand-offs nobody served (safety net, normally 0): re-run after the two kernels
+       CNT_ROW_BUSY = 24,            // + (smid & 255): row-kernel CTAs at work on that SM (the systolic warps there wait: see ydrop_kernel)
+       CNT_N = 24 + 256 };
 
 struct SfeFreeRing {              // persistent across launches: every half returns its chunks before it ends
     unsigned long long head;      // pops issued
@@ -105,7 +111,12 @@ struct YdParams {
     SfeFreeRing *ring_state;
     int32_t n_chunks;
     int32_t max_warps;            // warps of the normal kernel allowed to work in this pass
-    int32_t row_all;              // row kernel: 1 = every ticket, 0 = the first counters[CNT_ROW_N] (the longest)
+    int32_t row_all;              // row kernel: 1 = every ticket; 0 = the first counters[CNT_ROW_N] (the longest); 2 = serve the hand-off queue
+                                  // while the systolic kernel runs; 3 = long_tickets[n_tickets .. + counters[CNT_LONG_LEFT]) (leftovers)
+    int32_t long_strips;          // systolic kernel: > 0 = hand-off check-points at long_strips, 2 long_strips, 4 long_strips ... 32-row strips
+    int32_t row_slots;            // CTAs of the row kernel serving the queue (reserve rule of the check-points)
+    int32_t sys_warps;            // warps of the systolic kernel of this pass (the serving CTAs leave when all of them have)
+    int32_t *long_tickets;        // [2 n_tickets]: the hand-off queue (-1 = not written yet), then the leftovers
     int32_t row_split;            // systolic kernel: 1 = skip the first counters[CNT_ROW_N] tickets (the row kernel takes them)
     int32_t n_classes;            // reserved ticket segments in use (set by sfe_launch_ydrop: 4, or fewer in a sparse launch)
     int32_t sparse_warps;         // > 0: resident warps per SM for a chain-bound pass (blocks of 4 warps), see sfe_launch_ydrop

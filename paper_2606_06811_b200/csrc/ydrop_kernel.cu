@@ -338,6 +338,25 @@ static __device__ bool walk_traceback(const YdParams &p, TbReader &rd, const int
     return true;
 }
 
+// A check-point of a long half: take one of the idle row-kernel CTAs if the rule allows it.  A hand-off restarts the half, so
+// it pays only early in the half's life: there are four check-points (long_strips x 1, 2, 4, 8 strips; a restart at the last
+// one costs 8 long_strips strips of the row kernel at most if the half was about to end).  The early ones leave a reserve for
+// halves with more evidence of being long: more than 3/4, 1/2, 1/4 of the CTAs must be idle, the last one takes any.
+// Every successful claim is matched by exactly one push to the hand-off queue.
+static __device__ __forceinline__ bool claim_row_cta(unsigned long long *counters, int slots, int level, int lane)
+{
+    int got = 0;
+    if (lane == 0) {
+        const long long reserve = level >= 3 ? 0 : (long long)slots * (3 - level) / 4;
+        if ((long long)*((volatile unsigned long long *)&counters[CNT_ROW_FREE]) > reserve) {
+            const long long f = (long long)atomicAdd(&counters[CNT_ROW_FREE], ~0ULL);       // FREE--, returns the old value
+            if (f > reserve) got = 1;
+            else atomicAdd(&counters[CNT_ROW_FREE], 1ULL);
+        }
+    }
+    return __shfl_sync(FULL, got, 0) != 0;
+}
+
 template <bool TB, int RL2, bool GLOBAL, int SK>
 // Returns false only when SK == 2 and a strip outgrew the shared-memory window (skew 2 needs 31 more steps per strip):
 // nothing has been published then, and the caller runs the half again with SK == 1.
@@ -370,11 +389,18 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
     int bnd_valid = 0;                         // boundary ring holds row (r0-1) for columns < bnd_valid
     int sel_hi = -32 * SK;                     // selector ring is filled for columns < sel_hi (lane 31 starts at column -31 SK)
     int total_steps = 0, max_steps = 0, last_hdr = -1, n_strips = 0;
-    bool wide = false, limit = false;
+    bool wide = false, limit = false, lng = false;
+    // hand-off: a half still alive at a check-point (long_strips, 2 long_strips, 4 long_strips ... strips) is one of the pass's
+    // long serial chains.  If a CTA of the cooperative row kernel is idle it stops here, queues itself, and that CTA re-runs it
+    // from its start: a row costs the CTA a third less, and it has its SM to itself (ydrop_row_kernel.cu, sfe_launch_ydrop).
+    // (long_strips is a power of two, so the check-points are the powers of two >= it: no state is carried through the loop)
 
     for (int s = 0;; s++) {
         const int r0 = s * 32;
         if (r0 > g.n) break;
+        if (!GLOBAL && s >= p.long_strips && (s & (s - 1)) == 0 && p.long_strips > 0 && s <= 8 * p.long_strips) {
+            if (claim_row_cta(p.counters, p.row_slots, __clz(p.long_strips) - __clz(s), lane)) { lng = true; break; }
+        }
         const int r = r0 + lane;
         const bool active = r <= g.n;
         // R4: T(r) = best over rows <= r - 32, minus ydrop.  Rows <= r - 32 are: every row of
@@ -500,9 +526,9 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
     out.score = bs; out.end_i = bi; out.end_j = bj; out.cells = cells;
     // normal kernel: a bail-out is re-run by the wide kernel; wide kernel: a bail-out is final (band limit)
     out.status = (wide ? (GLOBAL ? (SFE_ST_WIDE | SFE_ST_BAND_LIMIT) : SFE_ST_WIDE_PENDING) : (GLOBAL ? SFE_ST_WIDE : 0u)) |
-                 ((TB && !tb.ok) ? SFE_ST_PASS_OVERFLOW : 0u) | (limit ? SFE_ST_SCORE_LIMIT : 0u) | mode_bits;
+                 ((TB && !tb.ok && !lng) ? SFE_ST_PASS_OVERFLOW : 0u) | (limit ? SFE_ST_SCORE_LIMIT : 0u) | (lng ? SFE_ST_LONG_PENDING : 0u) | mode_bits;
     out.n_strips = n_strips; out.n_rec = tb.nrec;
-    if (TB && tb.ok && !wide && !limit) {                             // a8: walk the pointers now, stage the run-length ops
+    if (TB && tb.ok && !wide && !limit && !lng) {                             // a8: walk the pointers now, stage the run-length ops
         TbReader rd;
         rd.pool = p.pool; rd.chunk_prev = p.chunk_prev; rd.chunk = tb.cur_chunk; rd.ord = (tb.nrec - 1) / SFE_CHUNK_RECS;
         rd.last_chunk = rd.chunk; rd.last_ord = rd.ord; rd.nrec = tb.nrec; rd.bad = false; rd.up_chunk = -1; rd.up_ord = -1;
@@ -523,14 +549,30 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
         p.halves[hid] = out;
         atomicAdd(&p.counters[CNT_STEPS], (unsigned long long)total_steps);
         if (TB) atomicAdd(&p.counters[CNT_TBBYTES], (unsigned long long)tb.nrec * (unsigned long long)SFE_REC_BYTES);
-        if (TB && !tb.ok) atomicAdd(&p.counters[CNT_OVERFLOW], 1ULL);
+        if (TB && !tb.ok && !lng) atomicAdd(&p.counters[CNT_OVERFLOW], 1ULL);
         if (TB && !tb.ok && tb.left < 0) atomicAdd(&p.counters[CNT_RING_DROPS], 1ULL);
         if (wide && !GLOBAL) atomicAdd(&p.counters[CNT_WIDE], 1ULL);
+        if (lng) {                                            // (the result above and the returned chunks are visible before the ticket is)
+            __threadfence();
+            const unsigned long long pos = atomicAdd(&p.counters[CNT_LONG_N], 1ULL);
+            *((volatile int32_t *)&p.long_tickets[pos]) = hid;
+        }
     }
     return true;
 }
 
 // Persistent kernel: every warp pulls anchor-half tickets from one atomic counter (a3).
+// While a row-kernel CTA works on this SM (row_split passes) the systolic warps here take no new ticket: they sleep, the
+// other SMs' warps drain the queue, and the CTA's serial chain of rows -- the pass's critical path -- has the schedulers to
+// itself.  The CTA never waits for a systolic warp, so this cannot deadlock; it ends when the CTA has no ticket left.
+static __device__ __noinline__ void wait_row_cta(const unsigned long long *counters)
+{
+    unsigned smid;
+    asm("mov.u32 %0, %%smid;" : "=r"(smid));
+    const volatile unsigned long long *busy = counters + CNT_ROW_BUSY + (smid & 255u);
+    while (*busy != 0ULL) __nanosleep(20000);
+}
+
 template <bool TB>
 __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kernel(const YdParams p)
 {
@@ -562,6 +604,7 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kerne
         const long long hi = phase == 1 ? p.n_tickets : (lo + seg < p.n_tickets ? lo + seg : p.n_tickets);
         unsigned long long *cnt = &p.counters[phase == 1 ? CNT_TICKET : CNT_CLASS0 + k];
         for (;;) {
+            if (p.row_split || p.long_strips > 0) wait_row_cta(p.counters);
             unsigned long long tk = 0;
             if (lane == 0) tk = atomicAdd(cnt, 1ULL);
             tk = __shfl_sync(FULL, tk, 0);
@@ -574,6 +617,15 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kerne
             __syncwarp();
         }
     }
+}
+
+// Runs in stream order right after the systolic kernel of a hand-off pass: tells the row-kernel CTAs serving the queue on the
+// other stream that no more entries will come.  (Counting the leaving warps inside ydrop_kernel itself cost its hot loop
+// registers: spills, +20 % on C4.)
+__global__ void mark_sys_done_kernel(unsigned long long *counters, unsigned long long n)
+{
+    __threadfence();
+    *((volatile unsigned long long *)&counters[CNT_SYS_DONE]) = n;
 }
 
 // Halves whose strip outgrew the shared-memory window (status SFE_ST_WIDE_PENDING) are collected ...
@@ -604,6 +656,7 @@ __global__ void __launch_bounds__(32) ydrop_wide_kernel(const YdParams p)
     }
 }
 
+int sfe_launch_long_left(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st);
 int sfe_launch_ydrop_block(const YdParams &p, bool want_tb, int n_sm, cudaStream_t st);
 int sfe_launch_ydrop_row(const YdParams &p, bool want_tb, long long grid, cudaStream_t st);
 
@@ -634,14 +687,6 @@ int sfe_launch_ydrop(const YdParams &p_in, bool want_tb, bool use_block, int n_s
         else { p.row_all = 1; rc = sfe_launch_ydrop_row(p, want_tb, p.n_tickets < 2LL * n_sm ? p.n_tickets : 2LL * n_sm, st); }
         if (rc) return rc;
     } else {
-        if (split) {                                              // launched FIRST so that its CTAs get their SM resources
-            SFE_CUDA_CHECK(cudaEventRecord(ev_fork, st));
-            SFE_CUDA_CHECK(cudaStreamWaitEvent(aux, ev_fork, 0));
-            p.row_all = 0;
-            const int rc = sfe_launch_ydrop_row(p, want_tb, p.n_tickets < (long long)n_sm ? p.n_tickets : (long long)n_sm, aux);
-            if (rc) return rc;
-            SFE_CUDA_CHECK(cudaEventRecord(ev_join, aux));
-        }
         int warps_per_block = SFE_BLOCK_THREADS / 32;
         size_t smem = (size_t)warps_per_block * SFE_WARP_SMEM;
         int bps = 0;
@@ -669,9 +714,33 @@ int sfe_launch_ydrop(const YdParams &p_in, bool want_tb, bool use_block, int n_s
         const long long need = (p.n_tickets + warps_per_block - 1) / warps_per_block;
         if (blocks > need) blocks = need;
         if (blocks < 1) blocks = 1;
+        // hand-off of long halves: row-kernel CTAs serve a queue beside this kernel (never all SMs: the systolic blocks must
+        // always find room, the serving CTAs wait for them to finish)
+        const bool handoff = !split && p.long_strips > 0 && aux != nullptr && p.row_slots > 0 && p.max_warps == 0x7fffffff;
+        if (!handoff) p.long_strips = 0;
+        if (handoff) {
+            if (p.row_slots > n_sm / 2) p.row_slots = n_sm / 2;
+            p.sys_warps = (int)(blocks * warps_per_block);
+            SFE_CUDA_CHECK(cudaMemsetAsync(p.long_tickets, 0xff, (size_t)p.n_tickets * sizeof(int32_t), st));
+        }
+        if (split || handoff) {                                   // launched FIRST so that its CTAs get their SM resources
+            SFE_CUDA_CHECK(cudaEventRecord(ev_fork, st));
+            SFE_CUDA_CHECK(cudaStreamWaitEvent(aux, ev_fork, 0));
+            YdParams pr = p;
+            pr.row_all = handoff ? 2 : 0;
+            const long long grid = handoff ? (long long)p.row_slots : (p.n_tickets < (long long)n_sm ? p.n_tickets : (long long)n_sm);
+            const int rc = sfe_launch_ydrop_row(pr, want_tb, grid, aux);
+            if (rc) return rc;
+            SFE_CUDA_CHECK(cudaEventRecord(ev_join, aux));
+        }
         if (want_tb) SFE_KL ydrop_kernel<true><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
         else SFE_KL ydrop_kernel<false><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
-        if (split) SFE_CUDA_CHECK(cudaStreamWaitEvent(st, ev_join, 0));
+        if (handoff) SFE_KL mark_sys_done_kernel<<<1, 1, 0, st>>>(p.counters, (unsigned long long)p.sys_warps);
+        if (split || handoff) SFE_CUDA_CHECK(cudaStreamWaitEvent(st, ev_join, 0));
+        if (handoff) {
+            const int rc = sfe_launch_long_left(p, want_tb, n_sm, st);
+            if (rc) return rc;
+        }
     }
     const int bs = 256;
     SFE_KL select_wide_kernel<<<(unsigned)((p.n_tickets + bs - 1) / bs), bs, 0, st>>>(p);

@@ -532,21 +532,89 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
     }
 }
 
-// Persistent CTAs: each pulls the next half from the first row_n tickets (the longest: sfe_launch_tickets' order).
+// Persistent CTAs.  row_all 1 / 0 / 3: each pulls the next half from a fixed list (every ticket / the first CNT_ROW_N tickets,
+// the longest: sfe_launch_tickets' order / the leftovers of the hand-off queue).
+// row_all 2: the CTAs SERVE THE HAND-OFF QUEUE while the systolic kernel runs beside them (sfe_launch_ydrop).  An idle CTA
+// announces itself (CNT_ROW_FREE++), draws the next queue position and sleeps until that entry is written; a systolic warp
+// whose half is still alive at a check-point takes one idle CTA (CNT_ROW_FREE--) and writes exactly one entry, so every entry
+// has a CTA waiting for it.  The CTA leaves when every systolic warp has left and its entry is still empty.  The wait is
+// bounded (a systolic kernel that never started must not hang the GPU): a CTA that gives up withdraws its announcement, and
+// the launcher's leftover pass re-runs whatever was queued but not served.
 template <bool TB>
 __global__ void __launch_bounds__(RK_THREADS, 1) ydrop_row_kernel(const YdParams p)
 {
-    __shared__ unsigned long long tk_s;
-    const long long n_row = p.row_all ? p.n_tickets : (long long)*((volatile unsigned long long *)&p.counters[CNT_ROW_N]);
+    __shared__ long long tk_s;
+    unsigned smid;
+    asm("mov.u32 %0, %%smid;" : "=r"(smid));
+    if (p.row_all == 2) {
+        for (;;) {
+            if (threadIdx.x == 0) {
+                atomicAdd(&p.counters[CNT_ROW_FREE], 1ULL);
+                const unsigned long long idx = atomicAdd(&p.counters[CNT_LONG_TICKET], 1ULL);
+                volatile int32_t *slot = p.long_tickets + idx;
+                int t = -1;
+                for (long long spin = 0; spin < (1LL << 24); spin++) {           // ~ 1 minute at most
+                    t = *slot;
+                    if (t >= 0) break;
+                    if ((long long)*((volatile unsigned long long *)&p.counters[CNT_SYS_DONE]) >= (long long)p.sys_warps) {
+                        __threadfence();
+                        t = *slot;                                              // pushed just before the last warp left?
+                        break;
+                    }
+                    __nanosleep(4000);
+                }
+                if (t < 0) atomicAdd(&p.counters[CNT_ROW_FREE], ~0ULL);          // withdraw (a late claim is caught by the leftover pass)
+                tk_s = t;
+            }
+            __syncthreads();
+            const int hid = (int)tk_s;
+            __syncthreads();
+            if (hid < 0) break;
+            __threadfence();                                                    // (the systolic warp's result and returned chunks)
+            if (threadIdx.x == 0) atomicAdd(&p.counters[CNT_ROW_BUSY + (smid & 255u)], 1ULL);      // the SM is mine while I work
+            row_half<TB>(p, hid);
+            __syncthreads();
+            if (threadIdx.x == 0) atomicAdd(&p.counters[CNT_ROW_BUSY + (smid & 255u)], ~0ULL);
+        }
+        return;
+    }
+    const long long n_row = p.row_all == 1 ? p.n_tickets : (long long)*((volatile unsigned long long *)&p.counters[p.row_all == 3 ? CNT_LONG_LEFT : CNT_ROW_N]);
+    const int32_t *tickets = p.row_all == 3 ? p.long_tickets + p.n_tickets : p.tickets;
     for (;;) {
-        if (threadIdx.x == 0) tk_s = atomicAdd(&p.counters[CNT_ROW_TICKET], 1ULL);
+        if (threadIdx.x == 0) tk_s = (long long)atomicAdd(&p.counters[CNT_ROW_TICKET], 1ULL);
         __syncthreads();
-        const long long tk = (long long)tk_s;
+        const long long tk = tk_s;
         __syncthreads();
         if (tk >= n_row) break;
-        row_half<TB>(p, p.tickets[tk]);
+        // beside the systolic kernel (row_split) the CTA claims its SM while it works: a half on this kernel is one serial
+        // chain of rows, and every other warp on the SM's schedulers stretches it (the systolic warps there sleep meanwhile)
+        if (p.row_all == 0 && threadIdx.x == 0) atomicAdd(&p.counters[CNT_ROW_BUSY + (smid & 255u)], 1ULL);
+        row_half<TB>(p, tickets[tk]);
         __syncthreads();
+        if (p.row_all == 0 && threadIdx.x == 0) atomicAdd(&p.counters[CNT_ROW_BUSY + (smid & 255u)], ~0ULL);
     }
+}
+
+// Hand-offs that were queued but not served (a serving CTA gave up, or the systolic kernel outlived them): normally none.
+__global__ void select_long_left_kernel(const YdParams p)
+{
+    const long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const long long n = (long long)*((volatile unsigned long long *)&p.counters[CNT_LONG_N]);
+    if (x >= n) return;
+    const int hid = p.long_tickets[x];
+    if (hid >= 0 && (p.halves[hid].status & SFE_ST_LONG_PENDING))
+        p.long_tickets[p.n_tickets + (long long)atomicAdd(&p.counters[CNT_LONG_LEFT], 1ULL)] = hid;
+}
+
+int sfe_launch_long_left(const YdParams &p_in, bool want_tb, int n_sm, cudaStream_t st)
+{
+    YdParams p = p_in;
+    p.row_all = 3; p.row_split = 0;
+    const int bs = 256;
+    SFE_KL select_long_left_kernel<<<(unsigned)((p.n_tickets + bs - 1) / bs), bs, 0, st>>>(p);
+    if (want_tb) SFE_KL ydrop_row_kernel<true><<<(unsigned)n_sm, RK_THREADS, 0, st>>>(p);
+    else SFE_KL ydrop_row_kernel<false><<<(unsigned)n_sm, RK_THREADS, 0, st>>>(p);
+    SFE_LAUNCH_CHECK();
 }
 
 int sfe_launch_ydrop_row(const YdParams &p, bool want_tb, long long grid, cudaStream_t st)

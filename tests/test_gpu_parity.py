@@ -577,6 +577,35 @@ def test_speculate_leaders_kept_only_and_carried_boxes(sfe, oracle):
     assert keep == ser["state"].tolist() and int(nacc.item()) == ser["n_kept"]
 
 
+@pytest.mark.parametrize("slots", [1, 64])
+def test_long_half_handoff_equals_oracle(sfe, oracle, slots):
+    """SFE_OPT_LONG_ROWS / SFE_OPT_LONG_ROWS_DENSE: systolic halves still alive at a check-point (here 64, 128, 256, 512 rows,
+    so that most halves meet one) stop, queue themselves and are re-run from their start by row-kernel CTAs that serve the
+    queue beside the systolic kernel.  Nothing may change: kept set = serial loop, every extended anchor bit-exact against
+    the oracle (score, box, cells, CIGAR), with one serving CTA (almost every check-point finds it busy) and with 64."""
+    w = W.config2(t_len=60_000, n_segments=30, per_seg=8, n_decoys=40, min_len=150, max_len=700)
+    ser = oracle.serial_loop(w.target, w.query, w.query_rc, w.pairs, w.anchors, oracle.scoring(), want_results=False)
+    sfe.set_option(B.OPT_LONG_ROWS, 64); sfe.set_option(B.OPT_LONG_ROWS_DENSE, 64); sfe.set_option(B.OPT_ROW_SLOTS, slots)
+    try:
+        for flags in (B.WANT_CIGAR | B.SPEC_LEADERS, B.SCORE_ONLY | B.SPEC_LEADERS):
+            out = _speculate(sfe, w, 64, flags=flags)
+            if flags & B.WANT_CIGAR:
+                assert sfe.last_batch_info()["block_halves"] > 0                   # halves were handed over
+            assert out["keep"].tolist() == ser["state"].tolist()
+            skipped = (out["results"]["status"] & B.ST_SKIPPED) != 0
+            H.assert_anchors_equal(out, w, np.nonzero(~skipped)[0][:: max(1, int((~skipped).sum()) // 80)], want_cigar=bool(flags & B.WANT_CIGAR))
+        # the dense launch of sfe_ydrop_batch + sfe_resolve
+        full = H.gpu_run(sfe, w)
+        assert sfe.last_batch_info()["block_halves"] > 0
+        H.assert_resolve_equal(full, w)
+        H.assert_anchors_equal(full, w, np.arange(0, len(w.anchors), max(1, len(w.anchors) // 80)))
+        so = H.gpu_run(sfe, w, flags=B.SCORE_ONLY)
+        for f in ("score", "tstart", "tend", "qstart", "qend", "cells"):
+            assert (so["results"][f] == full["results"][f]).all(), f
+    finally:
+        sfe.set_option(B.OPT_LONG_ROWS, 0); sfe.set_option(B.OPT_LONG_ROWS_DENSE, 0); sfe.set_option(B.OPT_ROW_SLOTS, 64)
+
+
 def test_filter_workload_equals_oracle(sfe, oracle):
     """f3: the gapped Y-drop extension as the filter over raw, mostly false seed hits -- score-only,
     ydrop 2000, one +-1024-base box per hit (a row / column budget), pass = score >= tau.  Every hit's score, box and cell
