@@ -28,7 +28,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-SCRATCH_GB = {"c1": 2, "c2": 16, "c4": 24, "c3": 32, "c3s": 24, "c5s": 32, "c5": 48, "filter": 2}   # traceback arena (chunks are recycled)
+SCRATCH_GB = {"c1": 2, "c2": 16, "c4": 24, "c3": 32, "c3s": 24, "c5s": 32, "c5": 96, "filter": 2}   # traceback arena (chunks are recycled)
 DEFAULT_WINDOW = {"c3": 16384, "c3s": 16384, "c5s": 1024, "c5": 1024}   # classic Algorithm 3: K for the dense-anchor workloads; others: one batch
 LEADER_WINDOW = 262144                                                  # --spec leaders: most extensions per batch
 TRAFFIC_FILE = os.path.join(ROOT, "profiles", "ncu_traffic.csv")      # written by hand from `ncu --set full` captures (see ncu_traffic.md)

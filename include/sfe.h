@@ -220,13 +220,14 @@ enum {
     SFE_OPT_SPEC_SPAN,             /* [2^20]  look-ahead, in anchors beyond the commit cursor, in which leaders are extended        */
     SFE_OPT_SPEC_ESC_MAX,          /* [64]    cap of the doubling number of anchors force-extended after repeated commit stops;
                                               1 = exactly one anchor per stop, no cold-diagonal sweep either                        */
-    SFE_OPT_SPARSE_WARPS,          /* [4]     resident warps per SM for sfe_speculate's leader batches (0 = the dense launch)       */
+    SFE_OPT_SPARSE_WARPS,          /* [0]     resident warps per SM for sfe_speculate's leader batches (0 = the dense launch)       */
     SFE_OPT_FORCE_CLASS,           /* [0]     testing: 1 = nobody leads, 2 = everybody leads, 3 = second half of the anchors never  */
     SFE_OPT_PROMOTE_REACH,         /* [65536] after a batch, followers within this target distance of an extended anchor that will  
                                               not cover them (it scored below tau, or they lie beyond its box) become leaders       */
-    SFE_OPT_ROW_KERNEL_CAP,        /* [0]     most priority tickets (long-likely leaders, known long extensions) a pass hands to the
-                                              cooperative row kernel, one CTA per half; 0 = never use it beside the systolic kernel  */
-    SFE_OPT_ROW_KERNEL_SCORE_ONLY, /* [0]     1 = also in score-only passes (there the systolic chain is currently the faster one)   */
+    SFE_OPT_ROW_KERNEL_CAP,        /* [#SMs]  most priority tickets (leaders predicted long, known long extensions: the longest first) a pass
+                                              hands to the cooperative row kernel, one CTA per half, beside the systolic kernel; the CTA
+                                              claims its SM while it works.  0 = never.  Plain sfe_ydrop_batch has no priorities         */
+    SFE_OPT_ROW_KERNEL_SCORE_ONLY, /* [1]     1 = also in score-only passes                                                              */
     SFE_OPT_LONG_ROWS,             /* [16384] sfe_speculate's leader batches: a half of the systolic kernel still alive after this many rows
                                               (then twice, four times ... as many) stops if a CTA of the cooperative row kernel is idle
                                               and is re-run by it from its start -- its rows are a third shorter and it has its SM to

@@ -278,6 +278,10 @@ class Sfe:
         _check(lib().sfe_last_half_profile(self.h, n_halves, C.c_void_p(out.ctypes.data)), "sfe_last_half_profile")
         return out[:n_halves]
 
+    def n_sm(self) -> int:
+        """SM count of the context's device (the default of OPT_ROW_KERNEL_CAP)"""
+        return int(_torch().cuda.get_device_properties(self.device).multi_processor_count)
+
     def set_option(self, key: int, value: int):
         _check(lib().sfe_set_option(self.h, key, value), "sfe_set_option")
 

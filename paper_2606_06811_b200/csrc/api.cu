@@ -135,7 +135,7 @@ extern "C" int sfe_create(sfe_ctx **out, int device, void *cuda_stream, size_t s
     memset(c->spec_info, 0, sizeof c->spec_info);
     c->opt[SFE_OPT_LEADER_DIAG_TOL] = 48; c->opt[SFE_OPT_LEADER_GAP] = 2000; c->opt[SFE_OPT_LEADER_LOOKBACK] = 64;
     c->opt[SFE_OPT_LEADER_NBREAK] = 64; c->opt[SFE_OPT_SPEC_SPAN] = 1 << 20; c->opt[SFE_OPT_SPEC_ESC_MAX] = 64;
-    c->opt[SFE_OPT_SPARSE_WARPS] = 0; c->opt[SFE_OPT_FORCE_CLASS] = 0; c->opt[SFE_OPT_PROMOTE_REACH] = 65536; c->opt[SFE_OPT_ROW_KERNEL_CAP] = 0; c->opt[SFE_OPT_ROW_KERNEL_SCORE_ONLY] = 0;
+    c->opt[SFE_OPT_SPARSE_WARPS] = 0; c->opt[SFE_OPT_FORCE_CLASS] = 0; c->opt[SFE_OPT_PROMOTE_REACH] = 65536; c->opt[SFE_OPT_ROW_KERNEL_CAP] = c->n_sm; c->opt[SFE_OPT_ROW_KERNEL_SCORE_ONLY] = 1;
     c->opt[SFE_OPT_LONG_ROWS] = 0; c->opt[SFE_OPT_LONG_ROWS_DENSE] = 0; c->opt[SFE_OPT_ROW_SLOTS] = 64;
     c->ev_pending = false; c->kernel_us = 0.0; c->n_profile = 0;
     if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess ||
@@ -360,7 +360,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
         // priority tickets already go to the row kernel)
         const long long lr = c->opt[first_of_series ? SFE_OPT_LONG_ROWS_DENSE : SFE_OPT_LONG_ROWS];      // (a batch of sfe_speculate is never the first of a series)
         const bool on = lr > 0 && c->opt[SFE_OPT_ROW_SLOTS] > 0 && !(flags & (SFE_BLOCK_KERNEL | SFE_NO_BLOCK_KERNEL)) &&
-                        sc->prune_lag == SFE_PRUNE_LAG && c->opt[SFE_OPT_ROW_KERNEL_CAP] == 0;
+                        sc->prune_lag == SFE_PRUNE_LAG && !(c->opt[SFE_OPT_ROW_KERNEL_CAP] > 0 && prio_dev != nullptr);
         p.long_strips = 0;
         if (on) { long long st = 1; while (st * 32 < lr && st < (1 << 24)) st *= 2; p.long_strips = (int)st; }     // strips, a power of two
         p.row_slots = (int)(c->opt[SFE_OPT_ROW_SLOTS] < 1024 ? c->opt[SFE_OPT_ROW_SLOTS] : 1024);
@@ -381,7 +381,7 @@ static int ydrop_batch_impl(sfe_ctx *c, const uint8_t *t_codes2, const uint8_t *
     SFE_CUDA_CHECK(cudaMemsetAsync(c->counters, 0, CNT_N * sizeof(unsigned long long), c->stream));
     // the longest tickets go to the cooperative row kernel (one CTA per half) unless the caller pinned the kernel choice
     const bool row_split = !(flags & (SFE_BLOCK_KERNEL | SFE_NO_BLOCK_KERNEL | SFE_NO_BINNING)) && sc->prune_lag == SFE_PRUNE_LAG &&
-                           c->opt[SFE_OPT_ROW_KERNEL_CAP] > 0 && (want_tb || c->opt[SFE_OPT_ROW_KERNEL_SCORE_ONLY]);
+                           c->opt[SFE_OPT_ROW_KERNEL_CAP] > 0 && prio_dev != nullptr && (want_tb || c->opt[SFE_OPT_ROW_KERNEL_SCORE_ONLY]);
     p.row_split = row_split ? 1 : 0;
     if ((rc = sfe_launch_tickets(anchors_dev, n_anchors, pairs_dev, n_pairs, q_len, !(flags & SFE_NO_BINNING), prio_dev,
                                  (unsigned int *)c->hist.p, (int32_t *)c->tickets.p, c->counters, row_split ? c->opt[SFE_OPT_ROW_KERNEL_CAP] : 0,

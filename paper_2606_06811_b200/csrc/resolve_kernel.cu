@@ -528,9 +528,12 @@ __global__ void spec_classify_kernel(const sfe_anchor *anchors, long long n, con
         return f && b;
     };
     uint8_t c = CLS_LEADER;
-    if (qm && dead_end(a)) { cls[i] = CLS_LEADER; lead_prio[i] = 0; return; }
+    // an anchor inside an N run leads (nobody covers it before it has been extended).  Its extension is usually empty -- but
+    // within ydrop / |n_score| bases of the run's edge it climbs out and runs the full length of what lies beyond (measured on
+    // configs[4]: the longest halves of a batch started there), so its reach is estimated like everybody's below.
+    const bool inside_n = qm && dead_end(a);
     const long long diag = a.tpos - a.qpos;
-    for (long long j = i - 1; j >= 0 && j >= i - lookback; j--) {
+    for (long long j = i - 1; !inside_n && j >= 0 && j >= i - lookback; j--) {
         const sfe_anchor p = anchors[j];
         if (a.tpos - p.tpos > gap) break;                   // anchors are in target order (any other order: everybody leads)
         if (a.tpos < p.tpos) break;
@@ -544,20 +547,37 @@ __global__ void spec_classify_kernel(const sfe_anchor *anchors, long long n, con
     }
     uint8_t pr = 0;
     if (c == CLS_LEADER) {
-        // Long-likely, and how long: follow the anchors that would follow this one (same strand / pair, diagonal within tol of the
-        // LAST one found, no gap wider than `gap`) -- the reach of that chain is a proxy of the alignment's span, which nothing
-        // else knows before the extension has run.  Its log2 becomes the ticket priority (longest first).
-        long long last_t = a.tpos, last_d = diag; int nf = 0;
-        for (long long j = i + 1; j < n && j <= i + (1 << 17); j++) {
-            const sfe_anchor p = anchors[j];
-            if (p.tpos - last_t > gap || p.tpos < a.tpos) break;
-            if ((p.strand >= 0 ? 1 : -1) != strand || p.pair != a.pair) continue;
-            const long long dd = (p.tpos - p.qpos) - last_d;
-            if (dd <= tol && dd >= -tol) { last_t = p.tpos; last_d = p.tpos - p.qpos; nf++; }
+        // Long-likely, and how long: follow the anchors on this one's diagonal in both directions (same strand / pair, diagonal
+        // within tol of the LAST one found, no gap wider than `gap`, no long N run in between) -- the reach of that chain is a
+        // proxy of the alignment's span, which nothing else knows before the extension has run.  Forward it is the anchors that
+        // would follow this one; backward it is ground an earlier leader is expected to cover, but this anchor's LEFT half runs
+        // over it all the same when that leader's extension stopped short of it (measured on configs[4]: the longest halves
+        // of a batch were such left halves).  The log2 of the longer reach is the priority of both tickets (longest first).
+        // (Priority only: an N run shorter than n_cross can be bridged by two gaps within ydrop, so it does not end the reach;
+        // N bases add up over consecutive hops until a hop has none.)
+        const int n_cross = 2 * n_break + n_break / 2;
+        long long span = 0; int nf = 0;
+#pragma unroll 1
+        for (int dir = 1; dir >= -1; dir -= 2) {
+            long long last_t = a.tpos, last_d = diag, n_acc = 0;                 // n_acc: N bases since the last hop without any
+            for (long long j = i + dir; j >= 0 && j < n && j <= i + (1 << 17) && j >= i - (1 << 17); j += dir) {
+                const sfe_anchor p = anchors[j];
+                const long long dt = dir > 0 ? p.tpos - last_t : last_t - p.tpos;
+                if (dt > gap || (dir > 0 ? p.tpos < a.tpos : p.tpos > a.tpos)) break;
+                if ((p.strand >= 0 ? 1 : -1) != strand || p.pair != a.pair) continue;
+                const long long dd = (p.tpos - p.qpos) - last_d;
+                if (dd <= tol && dd >= -tol) {
+                    const long long cn = count_n(t_nmask, dir > 0 ? last_t : p.tpos, dir > 0 ? p.tpos : last_t);
+                    n_acc = cn ? n_acc + cn : 0;
+                    if (n_acc >= n_cross) break;
+                    last_t = p.tpos; last_d = p.tpos - p.qpos; nf++;
+                }
+            }
+            const long long sp = (dir > 0 ? last_t - a.tpos : a.tpos - last_t) + 1;
+            if (sp > span) span = sp;
         }
         if (nf > 0) {
             c = CLS_LEADER_LONG;
-            long long span = last_t - a.tpos + 1;
             if (span > 0x3fffffff) span = 0x3fffffff;
             pr = (uint8_t)(1 + (31 - __clz((int)span)));
         }

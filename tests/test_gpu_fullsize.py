@@ -234,15 +234,15 @@ def test_config5_scaled_windowed(sfe_big, oracle):
 
 def test_config5_scaled_leaders_equals_classic(sfe_big, oracle):
     """configs[4] at 1/10 scale with predicted leaders: the same kept set, and for the kept anchors the same results, as
-    the classic windows; here with the cooperative row kernel taking the long-likely tickets (block_halves > 0; by default
-    they stay on the systolic kernel, which test_config5_full_leaders covers)."""
+    the classic windows; here with every ticket on the systolic kernel (block_halves == 0; by default the cooperative row
+    kernel takes the longest-predicted tickets, which test_config5_full_leaders and test_config3_full_leaders cover)."""
     w = W.config5(t_len=10_000_000, n_anchors=100_000)
-    sfe_big.set_option(B.OPT_ROW_KERNEL_CAP, 1 << 20)      # the long-likely tickets on the cooperative row kernel, beside the systolic one
+    sfe_big.set_option(B.OPT_ROW_KERNEL_CAP, 0)
     try:
         out = _speculate_full(sfe_big, w, 262144, 1 << 26, flags=LEADERS)
+        assert sfe_big.last_batch_info()["block_halves"] == 0
     finally:
-        sfe_big.set_option(B.OPT_ROW_KERNEL_CAP, 0)
-    assert sfe_big.last_batch_info()["block_halves"] > 0
+        sfe_big.set_option(B.OPT_ROW_KERNEL_CAP, sfe_big.n_sm())
     n_ext = int(out["stats"]["n_extended"])
     assert _check_speculated(w, out, 5, max(40, n_ext // 1000), n_kept_sample=20, kept_only=False) >= n_ext // 1000
     classic = _speculate_full(sfe_big, w, 1024, 1 << 26)

@@ -586,6 +586,7 @@ def test_long_half_handoff_equals_oracle(sfe, oracle, slots):
     w = W.config2(t_len=60_000, n_segments=30, per_seg=8, n_decoys=40, min_len=150, max_len=700)
     ser = oracle.serial_loop(w.target, w.query, w.query_rc, w.pairs, w.anchors, oracle.scoring(), want_results=False)
     sfe.set_option(B.OPT_LONG_ROWS, 64); sfe.set_option(B.OPT_LONG_ROWS_DENSE, 64); sfe.set_option(B.OPT_ROW_SLOTS, slots)
+    cap0 = sfe.n_sm(); sfe.set_option(B.OPT_ROW_KERNEL_CAP, 0)      # (the priority split and the hand-off exclude each other)
     try:
         for flags in (B.WANT_CIGAR | B.SPEC_LEADERS, B.SCORE_ONLY | B.SPEC_LEADERS):
             out = _speculate(sfe, w, 64, flags=flags)
@@ -604,6 +605,7 @@ def test_long_half_handoff_equals_oracle(sfe, oracle, slots):
             assert (so["results"][f] == full["results"][f]).all(), f
     finally:
         sfe.set_option(B.OPT_LONG_ROWS, 0); sfe.set_option(B.OPT_LONG_ROWS_DENSE, 0); sfe.set_option(B.OPT_ROW_SLOTS, 64)
+        sfe.set_option(B.OPT_ROW_KERNEL_CAP, cap0)
 
 
 def test_filter_workload_equals_oracle(sfe, oracle):
