@@ -357,7 +357,9 @@ static __device__ __forceinline__ bool claim_row_cta(unsigned long long *counter
     return __shfl_sync(FULL, got, 0) != 0;
 }
 
-template <bool TB, int RL2, bool GLOBAL, int SK>
+template <bool TB, int RL2, bool GLOBAL, int SK, bool COOP = false>
+// COOP: the variant with the hand-off check-points (a second instantiation: the plain one's code must not carry them,
+// C4 was 3 % slower with them compiled in).
 // Returns false only when SK == 2 and a strip outgrew the shared-memory window (skew 2 needs 31 more steps per strip):
 // nothing has been published then, and the caller runs the half again with SK == 1.
 static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, char *wk, const int lane, const uint32_t mode_bits)
@@ -398,7 +400,7 @@ static __device__ bool extend_half(const YdParams &p, const int hid, char *wsm, 
     for (int s = 0;; s++) {
         const int r0 = s * 32;
         if (r0 > g.n) break;
-        if (!GLOBAL && s >= p.long_strips && (s & (s - 1)) == 0 && p.long_strips > 0 && s <= 8 * p.long_strips) {
+        if (COOP && !GLOBAL && s >= p.long_strips && (s & (s - 1)) == 0 && p.long_strips > 0 && s <= 8 * p.long_strips) {
             if (claim_row_cta(p.counters, p.row_slots, __clz(p.long_strips) - __clz(s), lane)) { lng = true; break; }
         }
         const int r = r0 + lane;
@@ -573,7 +575,7 @@ static __device__ __noinline__ void wait_row_cta(const unsigned long long *count
     while (*busy != 0ULL) __nanosleep(20000);
 }
 
-template <bool TB>
+template <bool TB, bool COOP>
 __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kernel(const YdParams p)
 {
     extern __shared__ __align__(16) char smem[];
@@ -604,7 +606,7 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kerne
         const long long hi = phase == 1 ? p.n_tickets : (lo + seg < p.n_tickets ? lo + seg : p.n_tickets);
         unsigned long long *cnt = &p.counters[phase == 1 ? CNT_TICKET : CNT_CLASS0 + k];
         for (;;) {
-            if (p.row_split || p.long_strips > 0) wait_row_cta(p.counters);
+            if (COOP) wait_row_cta(p.counters);
             unsigned long long tk = 0;
             if (lane == 0) tk = atomicAdd(cnt, 1ULL);
             tk = __shfl_sync(FULL, tk, 0);
@@ -612,8 +614,8 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kerne
             // the reserved (longest) tickets run with a lane skew of 2: a shorter dependent step, a few more idle steps
             bool done = false;
             const bool long_skew = phase == 0 && SFE_LONG_SKEW == 2;
-            if (long_skew) done = extend_half<TB, SFE_RING_LOG2, false, SFE_LONG_SKEW>(p, p.tickets[lo + tk], wsm, wsm, lane, SFE_ST_SKEW2);
-            if (!done) extend_half<TB, SFE_RING_LOG2, false, 1>(p, p.tickets[lo + tk], wsm, wsm, lane, long_skew ? SFE_ST_SKEW_RETRY : 0u);
+            if (long_skew) done = extend_half<TB, SFE_RING_LOG2, false, SFE_LONG_SKEW, COOP>(p, p.tickets[lo + tk], wsm, wsm, lane, SFE_ST_SKEW2);
+            if (!done) extend_half<TB, SFE_RING_LOG2, false, 1, COOP>(p, p.tickets[lo + tk], wsm, wsm, lane, long_skew ? SFE_ST_SKEW_RETRY : 0u);
             __syncwarp();
         }
     }
@@ -664,8 +666,10 @@ int sfe_launch_ydrop_row(const YdParams &p, bool want_tb, long long grid, cudaSt
 int sfe_ydrop_init_device(void)
 {
     const int smem = (SFE_BLOCK_THREADS / 32) * SFE_WARP_SMEM;
-    SFE_CUDA_CHECK(cudaFuncSetAttribute(ydrop_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    SFE_CUDA_CHECK(cudaFuncSetAttribute(ydrop_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    SFE_CUDA_CHECK(cudaFuncSetAttribute(ydrop_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    SFE_CUDA_CHECK(cudaFuncSetAttribute(ydrop_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    SFE_CUDA_CHECK(cudaFuncSetAttribute(ydrop_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    SFE_CUDA_CHECK(cudaFuncSetAttribute(ydrop_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     return SFE_OK;
 }
 
@@ -690,8 +694,8 @@ int sfe_launch_ydrop(const YdParams &p_in, bool want_tb, bool use_block, int n_s
         int warps_per_block = SFE_BLOCK_THREADS / 32;
         size_t smem = (size_t)warps_per_block * SFE_WARP_SMEM;
         int bps = 0;
-        if (want_tb) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<true>, SFE_BLOCK_THREADS, smem);
-        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<false>, SFE_BLOCK_THREADS, smem);
+        if (want_tb) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<true, false>, SFE_BLOCK_THREADS, smem);
+        else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, ydrop_kernel<false, false>, SFE_BLOCK_THREADS, smem);
         if (bps < 1) return SFE_ECUDA;
         long long blocks;
         if (p.sparse_warps > 0) {
@@ -733,8 +737,13 @@ int sfe_launch_ydrop(const YdParams &p_in, bool want_tb, bool use_block, int n_s
             if (rc) return rc;
             SFE_CUDA_CHECK(cudaEventRecord(ev_join, aux));
         }
-        if (want_tb) SFE_KL ydrop_kernel<true><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
-        else SFE_KL ydrop_kernel<false><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
+        if (split || handoff) {                                   // the variant that waits for / hands over to the row kernel's CTAs
+            if (want_tb) SFE_KL ydrop_kernel<true, true><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
+            else SFE_KL ydrop_kernel<false, true><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
+        } else {
+            if (want_tb) SFE_KL ydrop_kernel<true, false><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
+            else SFE_KL ydrop_kernel<false, false><<<(unsigned)blocks, warps_per_block * 32, smem, st>>>(p);
+        }
         if (handoff) SFE_KL mark_sys_done_kernel<<<1, 1, 0, st>>>(p.counters, (unsigned long long)p.sys_warps);
         if (split || handoff) SFE_CUDA_CHECK(cudaStreamWaitEvent(st, ev_join, 0));
         if (handoff) {

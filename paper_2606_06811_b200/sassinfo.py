@@ -43,7 +43,7 @@ def _sass(kernel_substr: str) -> list[tuple[int, str, str]]:
 
 def hot_loop(traceback: bool = True) -> dict:
     """Returns dict(per_cell=I, alu=, fma=, lsu=, other=, hist=Counter) for the 16-step block."""
-    name = "ydrop_kernelILb1EE" if traceback else "ydrop_kernelILb0EE"
+    name = "ydrop_kernelILb1ELb0EE" if traceback else "ydrop_kernelILb0ELb0EE"      # <TB, COOP = false>: the plain instantiation
     ins = _sass(name)
     if not ins:
         raise RuntimeError(f"kernel {name} not found in {LIB}")
