@@ -228,10 +228,12 @@ enum {
                                               hands to the cooperative row kernel, one CTA per half, beside the systolic kernel; the CTA
                                               claims its SM while it works.  0 = never.  Plain sfe_ydrop_batch has no priorities         */
     SFE_OPT_ROW_KERNEL_SCORE_ONLY, /* [1]     1 = also in score-only passes                                                              */
-    SFE_OPT_LONG_ROWS,             /* [16384] sfe_speculate's leader batches: a half of the systolic kernel still alive after this many rows
-                                              (then twice, four times ... as many) stops if a CTA of the cooperative row kernel is idle
-                                              and is re-run by it from its start -- its rows are a third shorter and it has its SM to
-                                              itself.  0 = off; rounded up to 32 times a power of two                               */
+    SFE_OPT_LONG_ROWS,             /* [0]     hand-off (off by default): in sfe_speculate's batches a half of the systolic kernel still alive
+                                              after this many rows (and after 2, 4, 8 times as many) stops if a CTA of the row kernel is
+                                              idle (early check-points leave a reserve) and is re-run by that CTA from its start.  For
+                                              passes whose priorities are missing or wrong; not combined with the priority split (it
+                                              applies to passes without priorities, or with ROW_KERNEL_CAP = 0).  Rounded up to 32 times
+                                              a power of two.  Measured: DESIGN.md section 6                                              */
     SFE_OPT_LONG_ROWS_DENSE,       /* [0]     the same for sfe_ydrop_batch's dense launch; 0 = off                                   */
     SFE_OPT_ROW_SLOTS,             /* [64]    CTAs of the row kernel that serve those hand-offs (at most half of the SMs)            */
     SFE_OPT_N

@@ -6,17 +6,21 @@
 // row score-only and 1,450 with traceback on a 580 k-row half of configs[4] (profiles/r2_03), whatever else the GPU does.
 // The parallelism that is left is ALONG a row: one CTA per half, rows strictly in order, every thread owns RK_C consecutive
 // columns of a 1024-column window.  The first cooperative kernel (ydrop_block_kernel.cu, kept for Lambda = 0) spent ~700
-// instructions per thread per row and two block barriers on that (2,256 cycles per row).  This one: 1,250 score-only /
-// 1,680 with traceback -- still latency-bound (~250 instructions per warp per row at ~5 cycles each, profiles/r2_04) and,
-// since the systolic kernel's traceback walk was repaired, no longer ahead of it: opt-in (SFE_BLOCK_KERNEL, or
-// SFE_OPT_ROW_KERNEL_CAP for the priority tickets of a pass).  Design:
+// instructions per thread per row and two block barriers on that (2,256 cycles per row).  This one: 780 score-only /
+// 1,030 with traceback on the same half (profiles/r2_04) -- a quarter / 30 % less than the systolic chain.  It takes the
+// tickets a pass predicts longest (SFE_OPT_ROW_KERNEL_CAP, default: one per SM, beside the systolic kernel; the CTA claims
+// its SM while it works), every ticket with SFE_BLOCK_KERNEL, and the halves handed over by SFE_OPT_LONG_ROWS.  Design:
 //   * ONE block barrier per row (the exchange of the warps' F carries); the diagonal hand-off between neighbouring warps
 //     is an 8-byte {value, row} word that the reader polls (it is there by the time it is needed);
 //   * F(i,j) = max_{j'<j} (H~(i,j') - O - X (j - j')), H~ = max(M, E): a sequential max-plus chain over the thread's own
 //     columns (DPX VIADDMNMX), one shuffle scan per warp (shfl_up returns the caller's own value out of range, so a max
 //     scan needs no predicate), one 4-entry combine across warps;
 //   * everything that is not needed for the next row is LAGGED: per-row maxima (for T of row i + 32), alive bounds (cell
-//     count, end of the half, window position) go to shared-memory rings and are folded every 16 rows;
+//     count, end of the half, window position) go to shared-memory rings -- written one row late, under the next row's
+//     scan -- and are folded every 16 rows, where the thresholds of the next 16 rows are computed at once;
+//   * whatever depends only on the window position (the warp's rank, the thread's columns, the constants of the carry
+//     exchange, the target-end caps) is set when the window moves, and everything periodic (fold, query bases, traceback
+//     chunk: popped one fold ahead) sits behind ONE test per row: a branch costs this loop 15-20 cycles, taken or not;
 //   * the column -> (warp, lane, slot) map is fixed modulo the window, so a traceback row is a fixed 512-byte record the
 //     walk can address without any directory, and a thread's 8 nibbles are exactly one coalesced 32-bit store;
 //   * the "F extended" bit is stored with the cell the gap run CONTINUES FROM (F(i,j) - X > H(i,j) - (O+X): the cell's own
