@@ -124,3 +124,22 @@ def test_hot_loop_codegen_guard(built):
     for b in blocks:
         if b.startswith("_Z12ydrop_kernelILb"):
             assert "STACK:0" in b.replace(" ", ""), b[:300]
+
+
+def test_resolve_static_limits_and_argument_checks(built):
+    """sfe_resolve_static's host logic needs no GPU: the limits are reported, sizes beyond them are refused with a message
+    that names the limit before any CUDA call, n == 0 is a no-op, negative sizes / a device ordinal out of range are invalid."""
+    import ctypes as C
+    L = B.lib()
+    max_n, max_acc, nbytes = B.resolve_static_limits()
+    assert (max_n, max_acc) == (1 << 20, 1 << 16) and nbytes == 262400 + ((65537 * 40 + 255) // 256) * 256
+    one = C.c_void_p(64)                                    # never dereferenced: the checks come first
+    assert L.sfe_resolve_static(0, None, one, None, max_n + 1, 0, one, 1, one, one, None) == B.ELIMIT
+    assert b"SFE_STATIC_MAX_ANCHORS" in L.sfe_last_error_detail()
+    assert L.sfe_resolve_static(0, None, one, None, 1, 0, one, max_acc + 1, one, one, None) == B.ELIMIT
+    assert b"SFE_STATIC_MAX_ACCEPTED" in L.sfe_last_error_detail()
+    assert L.sfe_resolve_static(0, None, None, None, 0, 0, None, 0, None, None, None) == B.OK
+    assert L.sfe_resolve_static(0, None, one, None, -1, 0, one, 1, one, one, None) == B.EINVAL
+    assert L.sfe_resolve_static(-1, None, one, None, 1, 0, one, 1, one, one, None) == B.EINVAL
+    assert L.sfe_resolve_static(64, None, one, None, 1, 0, one, 1, one, one, None) == B.EINVAL
+
