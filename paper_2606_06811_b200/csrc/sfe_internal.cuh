@@ -85,6 +85,7 @@ enum { CNT_TICKET = 0, CNT_RING_DROPS, CNT_OVERFLOW, CNT_TBBYTES, CNT_STEPS, CNT
        CNT_LONG_N, CNT_LONG_TICKET,  // hand-off queue (long_tickets): entries pushed by the systolic kernel / positions drawn by idle row CTAs
        CNT_ROW_FREE, CNT_SYS_DONE,   // row CTAs idle and not yet claimed (signed) / systolic warps that have left their kernel
        CNT_LONG_LEFT,                // hand-offs nobody served (safety net, normally 0): re-run after the two kernels
+       CNT_ROW_STARTED,              // CTAs of the row kernel beside the systolic one that have started (the systolic kernel's start gate)
        CNT_ROW_BUSY = 24,            // + (smid & 255): row-kernel CTAs at work on that SM (the systolic warps there wait: see ydrop_kernel)
        CNT_N = 24 + 256 };
 
@@ -116,6 +117,7 @@ struct YdParams {
     int32_t long_strips;          // systolic kernel: > 0 = hand-off check-points at long_strips, 2 long_strips, 4 long_strips ... 32-row strips
     int32_t row_slots;            // CTAs of the row kernel serving the queue (reserve rule of the check-points)
     int32_t sys_warps;            // warps of the systolic kernel of this pass (the serving CTAs leave when all of them have)
+    int32_t row_grid;             // CTAs of the row kernel launched beside the systolic kernel (its start gate waits for them)
     int32_t *long_tickets;        // [2 n_tickets]: the hand-off queue (-1 = not written yet), then the leftovers
     int32_t row_split;            // systolic kernel: 1 = skip the first counters[CNT_ROW_N] tickets (the row kernel takes them)
     int32_t n_classes;            // reserved ticket segments in use (set by sfe_launch_ydrop: 4, or fewer in a sparse launch)

@@ -583,6 +583,13 @@ __global__ void __launch_bounds__(SFE_BLOCK_THREADS, SFE_MIN_BLOCKS) ydrop_kerne
     char *wsm = smem + (threadIdx.x >> 5) * SFE_WARP_SMEM;
     // re-run passes after a traceback-arena overflow admit only as many warps as the arena can serve
     if ((int)(blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) >= p.max_warps) return;
+    if (COOP) {
+        // start gate: the row kernel's CTAs were launched on another stream and must be RESIDENT before this kernel's
+        // persistent blocks take the SMs (else they start when these blocks leave: the two kernels run one after the other).
+        // This launch leaves room for them (2 blocks per SM), so they always arrive; the wait is bounded all the same.
+        const volatile unsigned long long *started = &p.counters[CNT_ROW_STARTED];
+        for (int spin = 0; spin < 20000 && *started < (unsigned long long)p.row_grid; spin++) __nanosleep(1000);
+    }
     // Ticket queue (a3): tickets are sorted longest bin first and every warp takes the next one (LPT order).
     // One extension is a serial chain of wavefront steps (R4 allows only 32 rows in flight), so the longest
     // halves decide when the kernel ends -- and the SM's schedulers strongly favour the lowest hardware warp
@@ -715,6 +722,10 @@ int sfe_launch_ydrop(const YdParams &p_in, bool want_tb, bool use_block, int n_s
             if (bps > 2 && p.n_tickets <= (long long)n_sm * bps * warps_per_block) bps = 2;
             blocks = (long long)n_sm * bps;
         }
+        if ((split || (p.long_strips > 0 && aux != nullptr && p.row_slots > 0)) && p.sparse_warps == 0 && bps > 2) {
+            bps = 2;                                              // beside the row kernel: 2 blocks + one row CTA fill an SM's registers
+            blocks = (long long)n_sm * bps;
+        }
         const long long need = (p.n_tickets + warps_per_block - 1) / warps_per_block;
         if (blocks > need) blocks = need;
         if (blocks < 1) blocks = 1;
@@ -733,6 +744,7 @@ int sfe_launch_ydrop(const YdParams &p_in, bool want_tb, bool use_block, int n_s
             YdParams pr = p;
             pr.row_all = handoff ? 2 : 0;
             const long long grid = handoff ? (long long)p.row_slots : (p.n_tickets < (long long)n_sm ? p.n_tickets : (long long)n_sm);
+            p.row_grid = pr.row_grid = (int)grid;
             const int rc = sfe_launch_ydrop_row(pr, want_tb, grid, aux);
             if (rc) return rc;
             SFE_CUDA_CHECK(cudaEventRecord(ev_join, aux));

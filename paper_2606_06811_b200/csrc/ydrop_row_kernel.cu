@@ -545,11 +545,13 @@ static __device__ __forceinline__ void row_half(const YdParams &p, const int hid
 // bounded (a systolic kernel that never started must not hang the GPU): a CTA that gives up withdraws its announcement, and
 // the launcher's leftover pass re-runs whatever was queued but not served.
 template <bool TB>
-__global__ void __launch_bounds__(RK_THREADS, 1) ydrop_row_kernel(const YdParams p)
+__global__ void __maxnreg__(112) ydrop_row_kernel(const YdParams p)   // 112: one CTA + two systolic blocks fill an SM's registers exactly
 {
     __shared__ long long tk_s;
     unsigned smid;
     asm("mov.u32 %0, %%smid;" : "=r"(smid));
+    // beside the systolic kernel: tell its start gate that this CTA is resident (sfe_launch_ydrop)
+    if ((p.row_all == 0 || p.row_all == 2) && threadIdx.x == 0) atomicAdd(&p.counters[CNT_ROW_STARTED], 1ULL);
     if (p.row_all == 2) {
         for (;;) {
             if (threadIdx.x == 0) {
